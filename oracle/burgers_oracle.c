@@ -1,0 +1,366 @@
+/*
+ * burgers_oracle.c -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, scalar fp64 restatement of what the hot path of
+ * arxiv 2601.12204 computes: time-stepping the 1D viscous Burgers equation
+ *     u_t + u u_x = nu u_xx                              (Eq.1)
+ * with first-order upwind convection (Eq.3 + upwind rule) and
+ * second-order central diffusion (Eq.4), explicit (forward Euler,
+ * PAPER.md:216 Eq.21; classical RK4, Eq.22) and implicit
+ * (BTCS, Eq.23, in the lagged-coefficient reading of
+ * DESIGN.md "Readings" Q4), plus the CFL time step (Eq.7-8,
+ * :287 Eq.24).
+ *
+ * Rules this file obeys:
+ *   - only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ *     --impl reference leg may load it; the product path never does;
+ *   - it shares no code, header, table or helper with the CUDA path;
+ *   - always fp64, compiled -O2 -ffp-contract=off (no FMA contraction), no
+ *     blocking, fusion or reordering beyond what each definition states;
+ *   - OpenMP only over independent trajectories (and over space for the
+ *     Jacobi-style explicit update of a single long grid, which is
+ *     order-independent by definition: all of u^{n+1} comes from u^n).
+ *
+ * Parity pins (tests/test_oracle_*.py): worked 4-node example done in exact
+ * rational arithmetic (G1,G4), Cole-Hopf closed form (R1/G2), exact Fourier
+ * amplification factors (R2/G3), dense Gaussian elimination for N<=16 (R3),
+ * CFL limit closed form (R4/G5), invariants (G6), textbook special cases (G7),
+ * travelling viscous shock (G8).  No function here is "parity unpinned".
+ *
+ * Notation follows the paper / SURVEY.md 8(c): c_i = u_i dt/dx, r = nu dt/dx^2.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+enum { BC_PERIODIC = 0, BC_DIRICHLET = 1 };
+enum { SCHEME_EULER = 0, SCHEME_RK4 = 1 };
+
+/* D1: grid spacing.  Periodic: N distinct nodes, dx = L/N (node N == node 0,
+ * PAPER.md:181 Eq.18).  Dirichlet: N nodes including both ends, dx = L/(N-1)
+ * (Eq.16-17). */
+static double grid_dx(int64_t N, double L, int bc)
+{
+    return (bc == BC_PERIODIC) ? L / (double)N : L / (double)(N - 1);
+}
+
+/* D2: semi-discrete operator F(u) (Eq.3-4, upwind rule :89,
+ * assembled form :216 Eq.21).  Dirichlet end nodes get F = 0 (they never move).
+ * Test hook: if use_adv, the constant `adv` replaces the multiplying u_i and the
+ * sign test (linear advection-diffusion, used only by the Fourier pin R2). */
+static void rhs_F(const double *u, double *F, int64_t N, double dx, double nu,
+                  int bc, int use_adv, double adv)
+{
+    int64_t lo = 0, hi = N;
+    if (bc == BC_DIRICHLET) {
+        F[0] = 0.0;
+        F[N - 1] = 0.0;
+        lo = 1;
+        hi = N - 1;
+    }
+    for (int64_t i = lo; i < hi; ++i) {
+        int64_t im = (i == 0) ? N - 1 : i - 1;     /* periodic wrap, D1 */
+        int64_t ip = (i == N - 1) ? 0 : i + 1;
+        double ui = u[i];
+        double dm = ui - u[im];                    /* backward difference, Eq.3 */
+        double dp = u[ip] - ui;                    /* forward difference, :89   */
+        double a = use_adv ? adv : ui;
+        double g = (a > 0.0) ? dm : dp;            /* upwind rule, :89 (Q3: 0 -> dp) */
+        double conv = a * g / dx;
+        double diff = nu * (dp - dm) / (dx * dx);  /* Eq.4 */
+        F[i] = -conv + diff;
+    }
+}
+
+/* Exposed for the worked-example pin G1. */
+void oracle_rhs(const double *u, double *F, int64_t N, double L, double nu,
+                int bc, int use_adv, double adv)
+{
+    rhs_F(u, F, N, grid_dx(N, L, bc), nu, bc, use_adv, adv);
+}
+
+/* D3: one trajectory, n_steps explicit steps with fixed dt.
+ * Euler: u^{n+1} = u^n + dt F(u^n)                               (Eq.21)
+ * RK4 : k1=F(u), k2=F(u+dt/2 k1), k3=F(u+dt/2 k2), k4=F(u+dt k3),
+ *       u^{n+1} = u + dt/6 (k1+2k2+2k3+k4)                       (Eq.22)
+ * Jacobi-style: all of u^{n+1} from u^n. */
+static void explicit_one(double *u, int64_t N, double dx, double nu, double dt,
+                         int64_t n_steps, int bc, int scheme, int use_adv,
+                         double adv, double *wk /* 5N doubles */)
+{
+    double *k1 = wk, *k2 = wk + N, *k3 = wk + 2 * N, *k4 = wk + 3 * N,
+           *y = wk + 4 * N;
+    for (int64_t n = 0; n < n_steps; ++n) {
+        if (scheme == SCHEME_EULER) {
+            rhs_F(u, k1, N, dx, nu, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) u[i] = u[i] + dt * k1[i];
+        } else {
+            rhs_F(u, k1, N, dx, nu, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y[i] = u[i] + 0.5 * dt * k1[i];
+            rhs_F(y, k2, N, dx, nu, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y[i] = u[i] + 0.5 * dt * k2[i];
+            rhs_F(y, k3, N, dx, nu, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y[i] = u[i] + dt * k3[i];
+            rhs_F(y, k4, N, dx, nu, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i)
+                u[i] = u[i] + dt / 6.0 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+        }
+    }
+}
+
+/* Explicit time stepping of B independent trajectories, u is [B][N] row-major,
+ * updated in place; nu[b], dt[b] per trajectory.  Returns 0, or -1 on bad args /
+ * allocation failure. */
+int oracle_explicit(double *u, int64_t B, int64_t N, double L, const double *nu,
+                    const double *dt, int64_t n_steps, int bc, int scheme,
+                    int use_adv, double adv, int nthreads)
+{
+    if (!u || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    if (scheme != SCHEME_EULER && scheme != SCHEME_RK4) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel num_threads(nthreads)
+    {
+        double *wk = (double *)malloc((size_t)5 * (size_t)N * sizeof(double));
+        if (!wk) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t b = 0; b < B; ++b)
+                explicit_one(u + b * N, N, dx, nu[b], dt[b], n_steps, bc, scheme,
+                             use_adv, adv, wk);
+            free(wk);
+        }
+    }
+    return fail ? -1 : 0;
+}
+
+/* Single long grid (B = 1), forward Euler only: same arithmetic as
+ * explicit_one, the spatial loop split over threads (the update is Jacobi-style,
+ * so the result does not depend on the split).  Used for timing/parity of the
+ * long-grid config; results are bitwise equal to oracle_explicit. */
+int oracle_explicit_long(double *u, int64_t N, double L, double nu, double dt,
+                         int64_t n_steps, int bc, int nthreads)
+{
+    if (!u || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    double *v = (double *)malloc((size_t)N * sizeof(double));
+    if (!v) return -1;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+    double *src = u, *dst = v;
+    for (int64_t n = 0; n < n_steps; ++n) {
+#pragma omp parallel for num_threads(nthreads) schedule(static)
+        for (int64_t i = 0; i < N; ++i) {
+            if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) {
+                dst[i] = src[i];
+                continue;
+            }
+            int64_t im = (i == 0) ? N - 1 : i - 1;
+            int64_t ip = (i == N - 1) ? 0 : i + 1;
+            double ui = src[i];
+            double dm = ui - src[im];
+            double dp = src[ip] - ui;
+            double g = (ui > 0.0) ? dm : dp;
+            double conv = ui * g / dx;
+            double diff = nu * (dp - dm) / (dx * dx);
+            double Fi = -conv + diff;
+            dst[i] = ui + dt * Fi;
+        }
+        double *t = src; src = dst; dst = t;
+    }
+    if (src != u) memcpy(u, src, (size_t)N * sizeof(double));
+    free(v);
+    return 0;
+}
+
+/* D4: BTCS rows from the lagged state u^n (Q4).  With c_i = a_i dt/dx
+ * (a_i = u_i^n, or the constant adv under the test hook), r = nu dt/dx^2:
+ *   sub_i  = -r - max(c_i,0)   (multiplies u_{i-1}^{n+1})
+ *   diag_i = 1 + 2r + |c_i|
+ *   sup_i  = -r + min(c_i,0)   (multiplies u_{i+1}^{n+1})
+ *   rhs_i  = u_i^n
+ * i.e. (u_i^{n+1}-u_i^n)/dt + u_i^n * upwind_x(u^{n+1}) = nu * central_xx(u^{n+1}).
+ */
+static void btcs_rows(const double *u, int64_t N, double dx, double nu, double dt,
+                      int use_adv, double adv, double *sub, double *diag,
+                      double *sup, double *rhs)
+{
+    double r = nu * dt / (dx * dx);
+    for (int64_t i = 0; i < N; ++i) {
+        double a = use_adv ? adv : u[i];
+        double c = a * dt / dx;
+        double cpos = (c > 0.0) ? c : 0.0;
+        double cneg = (c > 0.0) ? 0.0 : c;
+        sub[i] = -r - cpos;
+        diag[i] = 1.0 + 2.0 * r + fabs(c);
+        sup[i] = -r + cneg;
+        rhs[i] = u[i];
+    }
+}
+
+/* Exposed for the row-value pin G4. */
+void oracle_btcs_rows(const double *u, int64_t N, double L, double nu, double dt,
+                      int bc, int use_adv, double adv, double *sub, double *diag,
+                      double *sup, double *rhs)
+{
+    btcs_rows(u, N, grid_dx(N, L, bc), nu, dt, use_adv, adv, sub, diag, sup, rhs);
+}
+
+/* D7: Thomas algorithm, rows 0..n-1 (sub[0] and sup[n-1] are not referenced).
+ * cp, dp: scratch of n doubles each.  No pivoting (D4: strictly diagonally
+ * dominant). */
+static void thomas(int64_t n, const double *sub, const double *diag,
+                   const double *sup, const double *rhs, double *x, double *cp,
+                   double *dp)
+{
+    cp[0] = sup[0] / diag[0];
+    dp[0] = rhs[0] / diag[0];
+    for (int64_t i = 1; i < n; ++i) {
+        double m = diag[i] - sub[i] * cp[i - 1];
+        cp[i] = sup[i] / m;
+        dp[i] = (rhs[i] - sub[i] * dp[i - 1]) / m;
+    }
+    x[n - 1] = dp[n - 1];
+    for (int64_t i = n - 2; i >= 0; --i) x[i] = dp[i] - cp[i] * x[i + 1];
+}
+
+/* Exposed for the dense-elimination pin R3.  Returns -1 on allocation failure. */
+int oracle_thomas(int64_t n, const double *sub, const double *diag,
+                  const double *sup, const double *rhs, double *x)
+{
+    double *wk = (double *)malloc((size_t)2 * (size_t)n * sizeof(double));
+    if (!wk) return -1;
+    thomas(n, sub, diag, sup, rhs, x, wk, wk + n);
+    free(wk);
+    return 0;
+}
+
+/* D6: cyclic tridiagonal solve by Sherman-Morrison.  M = tridiag(sub,diag,sup)
+ * plus corners M[0][n-1] = sub[0], M[n-1][0] = sup[n-1].  gamma = -diag[0];
+ * T = tridiagonal part with diag'[0] = diag[0]-gamma,
+ * diag'[n-1] = diag[n-1] - sub[0]*sup[n-1]/gamma; w = (gamma,0,..,0,sup[n-1])^T,
+ * v = (1,0,..,0,sub[0]/gamma)^T, M = T + w v^T.  Solve T y = rhs, T q = w;
+ * x = y - q (v.y)/(1 + v.q).   wk: 6n doubles. */
+static void cyclic_sm(int64_t n, const double *sub, const double *diag,
+                      const double *sup, const double *rhs, double *x, double *wk)
+{
+    double *dmod = wk, *w = wk + n, *y = wk + 2 * n, *q = wk + 3 * n,
+           *cp = wk + 4 * n, *dp = wk + 5 * n;
+    double gamma = -diag[0];
+    double alpha = sub[0];      /* corner M[0][n-1]   */
+    double beta = sup[n - 1];   /* corner M[n-1][0]   */
+    for (int64_t i = 0; i < n; ++i) {
+        dmod[i] = diag[i];
+        w[i] = 0.0;
+    }
+    dmod[0] = diag[0] - gamma;
+    dmod[n - 1] = diag[n - 1] - alpha * beta / gamma;
+    w[0] = gamma;
+    w[n - 1] = beta;
+    thomas(n, sub, dmod, sup, rhs, y, cp, dp);
+    thomas(n, sub, dmod, sup, w, q, cp, dp);
+    double vy = y[0] + alpha / gamma * y[n - 1];
+    double vq = q[0] + alpha / gamma * q[n - 1];
+    double fact = vy / (1.0 + vq);
+    for (int64_t i = 0; i < n; ++i) x[i] = y[i] - fact * q[i];
+}
+
+/* Exposed for the dense-elimination pin R3. */
+int oracle_cyclic(int64_t n, const double *sub, const double *diag,
+                  const double *sup, const double *rhs, double *x)
+{
+    double *wk = (double *)malloc((size_t)6 * (size_t)n * sizeof(double));
+    if (!wk) return -1;
+    cyclic_sm(n, sub, diag, sup, rhs, x, wk);
+    free(wk);
+    return 0;
+}
+
+/* One trajectory, n_steps BTCS steps.  Periodic: D6 on all N rows.  Dirichlet
+ * (D5): unknowns i = 1..N-2, rhs_1 -= sub_1 u_0, rhs_{N-2} -= sup_{N-2} u_{N-1},
+ * end nodes untouched.  wk: 10N doubles + N for the new state. */
+static void btcs_one(double *u, int64_t N, double dx, double nu, double dt,
+                     int64_t n_steps, int bc, int use_adv, double adv, double *wk)
+{
+    double *sub = wk, *diag = wk + N, *sup = wk + 2 * N, *rhs = wk + 3 * N,
+           *x = wk + 4 * N, *wk2 = wk + 5 * N; /* 6N */
+    for (int64_t n = 0; n < n_steps; ++n) {
+        btcs_rows(u, N, dx, nu, dt, use_adv, adv, sub, diag, sup, rhs);
+        if (bc == BC_PERIODIC) {
+            cyclic_sm(N, sub, diag, sup, rhs, x, wk2);
+            for (int64_t i = 0; i < N; ++i) u[i] = x[i];
+        } else {
+            int64_t m = N - 2;
+            rhs[1] = rhs[1] - sub[1] * u[0];
+            rhs[N - 2] = rhs[N - 2] - sup[N - 2] * u[N - 1];
+            thomas(m, sub + 1, diag + 1, sup + 1, rhs + 1, x + 1, wk2, wk2 + N);
+            for (int64_t i = 1; i <= N - 2; ++i) u[i] = x[i];
+        }
+    }
+}
+
+int oracle_btcs(double *u, int64_t B, int64_t N, double L, const double *nu,
+                const double *dt, int64_t n_steps, int bc, int use_adv, double adv,
+                int nthreads)
+{
+    if (!u || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel num_threads(nthreads)
+    {
+        double *wk = (double *)malloc((size_t)11 * (size_t)N * sizeof(double));
+        if (!wk) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t b = 0; b < B; ++b)
+                btcs_one(u + b * N, N, dx, nu[b], dt[b], n_steps, bc, use_adv, adv, wk);
+            free(wk);
+        }
+    }
+    return fail ? -1 : 0;
+}
+
+/* D8: dt_b = C * min(dx / max_i |u_b,i|, dx^2 / (2 nu_b)), x/0 = +inf
+ * (PAPER.md:116-118 Eq.7-8, :287 Eq.24).  Max over all N stored nodes. */
+int oracle_dt_from_cfl(const double *u, int64_t B, int64_t N, double L,
+                       const double *nu, double C, int bc, double *dt_out)
+{
+    if (!u || !nu || !dt_out || B < 1 || N < 3 || !(L > 0.0) || !(C > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    for (int64_t b = 0; b < B; ++b) {
+        double m = 0.0;
+        for (int64_t i = 0; i < N; ++i) {
+            double a = fabs(u[b * N + i]);
+            if (a > m) m = a;
+        }
+        double conv = (m > 0.0) ? dx / m : INFINITY;
+        double diff = (nu[b] > 0.0) ? dx * dx / (2.0 * nu[b]) : INFINITY;
+        dt_out[b] = C * ((conv < diff) ? conv : diff);
+    }
+    return 0;
+}
+
+int oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
