@@ -1,0 +1,176 @@
+/*
+ * burgers.h -- C ABI of libburgers: time stepping of the 1D viscous Burgers
+ * equation  u_t + u u_x = nu u_xx  (Eq.1) on B200 (sm_100a).
+ *
+ * Spatial discretisation (Eq.3-4; upwind rule PAPER.md:89):
+ * first-order upwind convection, second-order central diffusion.
+ * Time discretisation: forward Euler (Eq.21), classical RK4 of the
+ * same semi-discrete operator (Eq.22), and BTCS
+ * (Eq.23) in the lagged-coefficient reading of
+ * DESIGN.md (Q4): per step one (cyclic) tridiagonal solve.
+ * Time-step limit (PAPER.md:116-118 Eq.7-8, :287 Eq.24).
+ *
+ * Conventions common to every call
+ * --------------------------------
+ *  - Status: 0 = BURGERS_OK, <0 = error.  Nothing throws, nothing aborts.
+ *    Argument errors are returned synchronously BEFORE anything is enqueued.
+ *  - Device entry points (no `_host` suffix): `u`, `nu`, `dt`, `dt_out`, `ws` are
+ *    CUDA DEVICE pointers owned by the caller; `stream` is a cudaStream_t passed
+ *    as void* (NULL = default stream).  Calls only enqueue work on `stream` and
+ *    return; no device synchronisation inside.  The library allocates nothing
+ *    persistent and keeps no global mutable state (re-entrant; concurrent calls
+ *    on different streams with disjoint buffers are legal).
+ *  - `_host` entry points: every pointer is a HOST pointer (pinned or pageable);
+ *    the call allocates device buffers, copies in, runs the same device path,
+ *    copies out, frees, and returns after the result is in host memory.
+ *  - Layout: `u` is [B][N] row-major (trajectory-contiguous), base 16-byte
+ *    aligned; `nu`, `dt`, `dt_out` have length B (one value per trajectory).
+ *    `u` is updated IN PLACE: after the call (stream-ordered) it holds the state
+ *    after `n_steps` steps.  n_steps = 0 is a valid no-op.
+ *  - Grid (readings Q6/Q8 of DESIGN.md).  Periodic: N distinct nodes,
+ *    dx = L/N, node i at i dx, neighbours wrap mod N (Eq.18).
+ *    Dirichlet: N nodes including both ends, dx = L/(N-1); the boundary values
+ *    are u[b][0] and u[b][N-1] AS FOUND IN THE INPUT and are never modified
+ *    (Eq.16-17).
+ *  - Errors: NULL pointer -> BURGERS_ERR_NULL; B<1, N<3, n_steps<0 ->
+ *    BURGERS_ERR_SHAPE; unknown bc/scheme/plan/op -> BURGERS_ERR_ENUM; L<=0, C<=0
+ *    or non-finite -> BURGERS_ERR_VALUE; workspace too small (or NULL when a
+ *    non-zero size is required) -> BURGERS_ERR_WORKSPACE; a CUDA launch/runtime
+ *    failure -> BURGERS_ERR_CUDA; a plan that cannot run this shape ->
+ *    BURGERS_ERR_PLAN.  Device-side values (nu<0, dt<=0, NaN in u) are not
+ *    checked; NaN/Inf propagate per IEEE.
+ *  - Scratch comes from `ws` (size from burgers_workspace_bytes, 256-byte aligned
+ *    base recommended, 16-byte required).  Its content is undefined on return.
+ */
+#ifndef BURGERS_H
+#define BURGERS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BURGERS_VERSION 100 /* 0.1.0 */
+
+enum {
+    BURGERS_OK = 0,
+    BURGERS_ERR_NULL = -1,
+    BURGERS_ERR_SHAPE = -2,
+    BURGERS_ERR_ENUM = -3,
+    BURGERS_ERR_VALUE = -4,
+    BURGERS_ERR_WORKSPACE = -5,
+    BURGERS_ERR_CUDA = -6,
+    BURGERS_ERR_PLAN = -7
+};
+enum { BURGERS_BC_PERIODIC = 0, BURGERS_BC_DIRICHLET = 1 };
+enum { BURGERS_SCHEME_EULER = 0, BURGERS_SCHEME_RK4 = 1 };
+enum { BURGERS_OP_EXPLICIT = 0, BURGERS_OP_BTCS = 1, BURGERS_OP_CFL = 2 };
+
+/* Kernel plans.  AUTO picks by shape; the others force one
+ * plan (tests use this for cross-plan agreement, G10) and return
+ * BURGERS_ERR_PLAN when the shape does not fit it. */
+enum {
+    BURGERS_PLAN_AUTO = 0,
+    /* explicit: */
+    BURGERS_PLAN_RESIDENT = 1, /* whole trajectory on chip for all n_steps      */
+    BURGERS_PLAN_TILED = 2,    /* overlapped tiles, k steps per HBM round trip  */
+    /* BTCS: */
+    BURGERS_PLAN_THOMAS = 3,   /* one thread per system, interleaved [N][B] ws  */
+    BURGERS_PLAN_HYBRID = 4,   /* one CTA per system: partitions + PCR, resident*/
+    BURGERS_PLAN_LONG = 5      /* one system across many CTAs (partition tree)  */
+};
+
+/* ---- explicit time stepping (PAPER.md:216 Eq.21; :224-229 Eq.22) --------------
+ * n_steps steps of  u^{n+1} = u^n + dt F(u^n)  (Euler) or classical RK4 of F,
+ * F_i = -u_i g_i/dx + nu (u_{i+1} - 2u_i + u_{i-1})/dx^2,
+ * g_i = u_i - u_{i-1} if u_i > 0 else u_{i+1} - u_i.
+ * dt[b] is held fixed over the call.  RK4: the upwind direction is re-decided from
+ * each stage value; Dirichlet end nodes have k = 0 in every stage.
+ * fp32: the state is carried as a two-term sum on chip (compensated
+ * accumulation), rounded to fp32 once when written back. */
+int burgers_explicit_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                         const float *dt, int64_t n_steps, int bc, int scheme,
+                         void *ws, size_t ws_bytes, void *stream);
+int burgers_explicit_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                         const double *dt, int64_t n_steps, int bc, int scheme,
+                         void *ws, size_t ws_bytes, void *stream);
+/* Same, forcing a plan.  `tblock` = steps per HBM round trip of the TILED plan
+ * (0 = library default; ignored by RESIDENT); `ppt` = grid points held per thread
+ * (0 = library default; else one of 1,2,4,8,16,32 -- BURGERS_ERR_PLAN if the shape
+ * does not fit it). */
+int burgers_explicit_plan_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                              const float *dt, int64_t n_steps, int bc, int scheme,
+                              int plan, int tblock, int ppt, void *ws, size_t ws_bytes,
+                              void *stream);
+int burgers_explicit_plan_f64(double *u, int64_t B, int64_t N, double L,
+                              const double *nu, const double *dt, int64_t n_steps,
+                              int bc, int scheme, int plan, int tblock, int ppt,
+                              void *ws, size_t ws_bytes, void *stream);
+
+/* ---- BTCS (Eq.23; D4-D7) ----------------------
+ * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:
+ *   sub_i = -r - max(c_i,0),  diag_i = 1 + 2r + |c_i|,  sup_i = -r + min(c_i,0).
+ * Dirichlet: unknowns i = 1..N-2, known end values moved to the right-hand side.
+ * Periodic: cyclic system (corner terms; Sherman-Morrison in the THOMAS plan,
+ * cyclic reduction of the interface system in HYBRID/LONG -- same solution up to
+ * rounding).  The matrix is strictly diagonally dominant: no pivoting. */
+int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                     const float *dt, int64_t n_steps, int bc, void *ws,
+                     size_t ws_bytes, void *stream);
+int burgers_btcs_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                     const double *dt, int64_t n_steps, int bc, void *ws,
+                     size_t ws_bytes, void *stream);
+int burgers_btcs_plan_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                          const float *dt, int64_t n_steps, int bc, int plan, void *ws,
+                          size_t ws_bytes, void *stream);
+int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                          const double *dt, int64_t n_steps, int bc, int plan, void *ws,
+                          size_t ws_bytes, void *stream);
+
+/* ---- CFL time step (PAPER.md:116-118 Eq.7-8, :287 Eq.24) -----------------------
+ * dt_out[b] = C * min(dx / max_i |u[b][i]|, dx^2 / (2 nu[b])), with x/0 = +inf
+ * (u == 0 gives the diffusive bound, nu == 0 the convective one, both: +inf).
+ * The max runs over all N stored nodes (Dirichlet: end nodes included).
+ * dt_out doubles as the reduction scratch (no workspace). */
+int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float *nu,
+                    double C, int bc, float *dt_out, void *stream);
+int dt_from_cfl_f64(const double *u, int64_t B, int64_t N, double L, const double *nu,
+                    double C, int bc, double *dt_out, void *stream);
+
+/* ---- host-buffer variants (end-to-end path; all pointers HOST) ----------------- */
+int burgers_explicit_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                              const float *dt, int64_t n_steps, int bc, int scheme);
+int burgers_explicit_host_f64(double *u, int64_t B, int64_t N, double L,
+                              const double *nu, const double *dt, int64_t n_steps,
+                              int bc, int scheme);
+int burgers_btcs_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
+                          const float *dt, int64_t n_steps, int bc);
+int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                          const double *dt, int64_t n_steps, int bc);
+int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu,
+                         double C, int bc, float *dt_out);
+int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L,
+                         const double *nu, double C, int bc, double *dt_out);
+
+/* ---- queries (pure functions of the shape; no device work) -------------------- */
+/* Scratch bytes needed by op (BURGERS_OP_*) with `plan` (BURGERS_PLAN_AUTO allowed).
+ * `scheme` is ignored for BTCS/CFL.  Returns 0 when none is needed or when the
+ * arguments are invalid (the op call itself reports the error). */
+size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
+                               int scheme, int plan);
+/* The plan AUTO resolves to for this shape (BURGERS_PLAN_*), or <0 on bad args.
+ * Needs a CUDA device only for the resident-fit check of the explicit op. */
+int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
+                       int scheme);
+/* Number of kernel launches (memset/memcpy nodes excluded) the op enqueues. */
+int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
+                             int scheme, int plan, int tblock, int64_t n_steps);
+const char *burgers_strerror(int status); /* static strings */
+int burgers_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BURGERS_H */

@@ -1,0 +1,252 @@
+"""Thin ctypes binding of libburgers.so (include/burgers.h) -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the library; this module only turns
+torch tensors / numpy arrays into pointers and sizes.  There is NO CPU fallback: if the
+library has not been built (``python -m paper_2601_12204_b200.build``) importing this module
+raises, and calling a device entry point with a non-CUDA tensor raises.
+
+Device calls take torch CUDA tensors (``u`` [B][N] contiguous, ``nu``/``dt`` [B]) and enqueue on
+the current torch stream; ``*_host`` calls take numpy arrays (host memory) and return when the
+result is back in host memory.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libburgers.so")
+
+OK = 0
+ERR_NULL, ERR_SHAPE, ERR_ENUM, ERR_VALUE, ERR_WORKSPACE, ERR_CUDA, ERR_PLAN = -1, -2, -3, -4, -5, -6, -7
+BC_PERIODIC, BC_DIRICHLET = 0, 1
+SCHEME_EULER, SCHEME_RK4 = 0, 1
+OP_EXPLICIT, OP_BTCS, OP_CFL = 0, 1, 2
+PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG = 0, 1, 2, 3, 4, 5
+
+EXPORTS = [
+    "burgers_explicit_f32", "burgers_explicit_f64", "burgers_explicit_plan_f32",
+    "burgers_explicit_plan_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
+    "burgers_btcs_plan_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
+    "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
+    "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
+    "burgers_launch_count", "burgers_strerror", "burgers_version",
+]
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_2601_12204_b200.build` "
+        "(there is no CPU fallback)")
+
+_lib = ctypes.CDLL(LIB_PATH)
+
+_p, _i64, _f64, _int, _sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int, ctypes.c_size_t
+for _sfx in ("f32", "f64"):
+    getattr(_lib, f"burgers_explicit_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _p, _sz, _p]
+    getattr(_lib, f"burgers_explicit_plan_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _int, _int, _int, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_plan_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _p, _sz, _p]
+    getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
+    getattr(_lib, f"burgers_explicit_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int]
+    getattr(_lib, f"burgers_btcs_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int]
+    getattr(_lib, f"dt_from_cfl_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p]
+    for _n in ("burgers_explicit_", "burgers_explicit_plan_", "burgers_btcs_", "burgers_btcs_plan_",
+               "dt_from_cfl_", "burgers_explicit_host_", "burgers_btcs_host_", "dt_from_cfl_host_"):
+        getattr(_lib, _n + _sfx).restype = _int
+_lib.burgers_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _int, _int, _int]
+_lib.burgers_workspace_bytes.restype = _sz
+_lib.burgers_plan_query.argtypes = [_int, _int, _i64, _i64, _int, _int]
+_lib.burgers_plan_query.restype = _int
+_lib.burgers_launch_count.argtypes = [_int, _int, _i64, _i64, _int, _int, _int, _int, _i64]
+_lib.burgers_launch_count.restype = _i64
+_lib.burgers_strerror.argtypes = [_int]
+_lib.burgers_strerror.restype = ctypes.c_char_p
+_lib.burgers_version.argtypes = []
+_lib.burgers_version.restype = _int
+
+
+class BurgersError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {strerror(status)} (status {status})")
+
+
+def raw():
+    """The ctypes library handle (tests of the raw C ABI: error codes, symbols)."""
+    return _lib
+
+
+def strerror(status: int) -> str:
+    return _lib.burgers_strerror(int(status)).decode()
+
+
+def version() -> int:
+    return int(_lib.burgers_version())
+
+
+def workspace_bytes(op, is_f64, B, N, bc, scheme=0, plan=PLAN_AUTO) -> int:
+    return int(_lib.burgers_workspace_bytes(op, int(bool(is_f64)), B, N, bc, scheme, plan))
+
+
+def plan_query(op, is_f64, B, N, bc, scheme=0) -> int:
+    return int(_lib.burgers_plan_query(op, int(bool(is_f64)), B, N, bc, scheme))
+
+
+def launch_count(op, is_f64, B, N, bc, scheme=0, plan=PLAN_AUTO, tblock=0, n_steps=0) -> int:
+    return int(_lib.burgers_launch_count(op, int(bool(is_f64)), B, N, bc, scheme, plan, tblock, n_steps))
+
+
+def _check(st, where):
+    if st != OK:
+        raise BurgersError(st, where)
+
+
+# ------------------------------------------------------------------ device (torch) entry points
+def _dev(t, name, dtype=None):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA torch tensor (no CPU fallback)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name} must have dtype {dtype}")
+    return t
+
+
+def _sfx(t):
+    import torch
+    if t.dtype == torch.float32:
+        return "f32"
+    if t.dtype == torch.float64:
+        return "f64"
+    raise TypeError("u must be float32 or float64")
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _shape(u):
+    if u.dim() == 1:
+        return 1, u.shape[0]
+    if u.dim() != 2:
+        raise ValueError("u must be [B][N] or [N]")
+    return u.shape[0], u.shape[1]
+
+
+def _ws(ws, need, device):
+    import torch
+    if need == 0:
+        return None, 0, ws
+    if ws is None:
+        ws = torch.empty(need, dtype=torch.uint8, device=device)
+    _dev(ws, "ws")
+    return ctypes.c_void_p(ws.data_ptr()), ws.numel() * ws.element_size(), ws
+
+
+def alloc_workspace(op, u, bc, scheme=0, plan=PLAN_AUTO):
+    """A uint8 CUDA tensor big enough for `op` on `u` (None when no scratch is needed)."""
+    import torch
+    B, N = _shape(u)
+    need = workspace_bytes(op, u.dtype == torch.float64, B, N, bc, scheme, plan)
+    return torch.empty(need, dtype=torch.uint8, device=u.device) if need else None
+
+
+def burgers_explicit(u, L, nu, dt, n_steps, bc, scheme, ws=None, plan=PLAN_AUTO, tblock=0, ppt=0):
+    """In-place explicit time stepping of u [B][N] (include/burgers.h: burgers_explicit_*)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    if nu.numel() != B or dt.numel() != B:
+        raise ValueError("nu and dt must have length B")
+    need = workspace_bytes(OP_EXPLICIT, u.dtype == torch.float64, B, N, bc, scheme, plan)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    fn = getattr(_lib, f"burgers_explicit_plan_{sfx}")
+    st = fn(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(), int(n_steps), int(bc),
+            int(scheme), int(plan), int(tblock), int(ppt), wsp, wsb, _stream())
+    _check(st, f"burgers_explicit_{sfx}")
+    return u
+
+
+def burgers_btcs(u, L, nu, dt, n_steps, bc, ws=None, plan=PLAN_AUTO):
+    """In-place BTCS time stepping of u [B][N] (include/burgers.h: burgers_btcs_*)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    if nu.numel() != B or dt.numel() != B:
+        raise ValueError("nu and dt must have length B")
+    need = workspace_bytes(OP_BTCS, u.dtype == torch.float64, B, N, bc, 0, plan)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    fn = getattr(_lib, f"burgers_btcs_plan_{sfx}")
+    st = fn(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(), int(n_steps), int(bc),
+            int(plan), wsp, wsb, _stream())
+    _check(st, f"burgers_btcs_{sfx}")
+    return u
+
+
+def dt_from_cfl(u, L, nu, C, bc, out=None):
+    """dt[b] = C min(dx/max|u_b|, dx^2/(2 nu_b)) (include/burgers.h: dt_from_cfl_*)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype)
+    B, N = _shape(u)
+    if nu.numel() != B:
+        raise ValueError("nu must have length B")
+    if out is None:
+        out = torch.empty(B, dtype=u.dtype, device=u.device)
+    _dev(out, "out", u.dtype)
+    st = getattr(_lib, f"dt_from_cfl_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), float(C),
+                                             int(bc), out.data_ptr(), _stream())
+    _check(st, f"dt_from_cfl_{sfx}")
+    return out
+
+
+# ------------------------------------------------------------------ host (numpy) entry points
+def _host(a, name, dtype=None):
+    if not isinstance(a, np.ndarray) or not a.flags.c_contiguous:
+        raise TypeError(f"{name} must be a C-contiguous numpy array")
+    if dtype is not None and a.dtype != dtype:
+        raise TypeError(f"{name} must have dtype {dtype}")
+    return a
+
+
+def _hsfx(a):
+    if a.dtype == np.float32:
+        return "f32"
+    if a.dtype == np.float64:
+        return "f64"
+    raise TypeError("u must be float32 or float64")
+
+
+def burgers_explicit_host(u, L, nu, dt, n_steps, bc, scheme):
+    """Host-buffer explicit stepping: u (numpy, [B][N]) is updated in place."""
+    _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    st = getattr(_lib, f"burgers_explicit_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data,
+                                                       dt.ctypes.data, int(n_steps), int(bc), int(scheme))
+    _check(st, f"burgers_explicit_host_{sfx}")
+    return u
+
+
+def burgers_btcs_host(u, L, nu, dt, n_steps, bc):
+    _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    st = getattr(_lib, f"burgers_btcs_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data,
+                                                   dt.ctypes.data, int(n_steps), int(bc))
+    _check(st, f"burgers_btcs_host_{sfx}")
+    return u
+
+
+def dt_from_cfl_host(u, L, nu, C, bc):
+    _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype)
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    out = np.empty(B, dtype=u.dtype)
+    st = getattr(_lib, f"dt_from_cfl_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, float(C),
+                                                  int(bc), out.ctypes.data)
+    _check(st, f"dt_from_cfl_host_{sfx}")
+    return out

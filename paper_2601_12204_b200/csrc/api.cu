@@ -1,0 +1,296 @@
+// api.cu -- the C ABI of include/burgers.h: argument validation, plan selection, dispatch,
+// and the host-buffer (end-to-end) variants.  No arithmetic of the method lives here.
+#include <cmath>
+
+#include "common.cuh"
+
+using namespace burgers;
+
+namespace {
+
+int check_common(const void *u, const void *nu, const void *dt, int64_t B, int64_t N, double L,
+                 int64_t n_steps, int bc) {
+    if (!u || !nu || !dt) return BURGERS_ERR_NULL;
+    if (B < 1 || N < 3 || n_steps < 0) return BURGERS_ERR_SHAPE;
+    if (bc != BURGERS_BC_PERIODIC && bc != BURGERS_BC_DIRICHLET) return BURGERS_ERR_ENUM;
+    if (!(L > 0.0) || !std::isfinite(L)) return BURGERS_ERR_VALUE;
+    return BURGERS_OK;
+}
+
+bool scheme_ok(int scheme) { return scheme == BURGERS_SCHEME_EULER || scheme == BURGERS_SCHEME_RK4; }
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// AUTO plan of the BTCS op: one long system -> LONG; a system that fits one
+// CTA -> HYBRID; anything else -> THOMAS.
+int btcs_auto_plan(int is_f64, int64_t B, int64_t N, int bc) {
+    if (btcs_hybrid_fits(is_f64, N, bc) && B < 200000) return BURGERS_PLAN_HYBRID;
+    if (btcs_long_fits(N, bc) && B * 1024 <= N) return BURGERS_PLAN_LONG;
+    return BURGERS_PLAN_THOMAS;
+}
+
+template <typename T>
+int explicit_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
+                  int bc, int scheme, int plan, int tblock, int ppt, void *ws, size_t ws_bytes,
+                  void *stream) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!scheme_ok(scheme)) return BURGERS_ERR_ENUM;
+    if (plan != BURGERS_PLAN_AUTO && plan != BURGERS_PLAN_RESIDENT && plan != BURGERS_PLAN_TILED)
+        return BURGERS_ERR_ENUM;
+    ExplicitGeom g;
+    st = explicit_geometry(sizeof(T) == 8, B, N, bc, scheme, plan, tblock, ppt, &g);
+    if (st != BURGERS_OK) return st;
+    if (g.plan == BURGERS_PLAN_TILED) {
+        const size_t need = (size_t)B * (size_t)N * sizeof(T);
+        if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
+    }
+    return launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, scheme, g, (T *)ws,
+                              (cudaStream_t)stream);
+}
+
+template <typename T>
+int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
+              int plan, void *ws, size_t ws_bytes, void *stream) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    const int is_f64 = sizeof(T) == 8;
+    if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(is_f64, B, N, bc);
+    const double dx = grid_dx(N, L, bc);
+    cudaStream_t s = (cudaStream_t)stream;
+    switch (plan) {
+        case BURGERS_PLAN_THOMAS: {
+            const size_t need = btcs_thomas_ws_elems(B, N, bc) * sizeof(T);
+            if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
+            return launch_btcs_thomas<T>(u, B, N, dx, nu, dt, n_steps, bc, (T *)ws, s);
+        }
+        case BURGERS_PLAN_HYBRID:
+            if (!btcs_hybrid_fits(is_f64, N, bc)) return BURGERS_ERR_PLAN;
+            return launch_btcs_hybrid<T>(u, B, N, dx, nu, dt, n_steps, bc, s);
+        case BURGERS_PLAN_LONG: {
+            if (!btcs_long_fits(N, bc)) return BURGERS_ERR_PLAN;
+            const size_t need = btcs_long_ws_elems(B, N, bc) * sizeof(T);
+            if (need && (!ws || ws_bytes < need)) return BURGERS_ERR_WORKSPACE;
+            return launch_btcs_long<T>(u, B, N, dx, nu, dt, n_steps, bc, (T *)ws, s);
+        }
+    }
+    return BURGERS_ERR_ENUM;
+}
+
+template <typename T>
+int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out,
+             void *stream) {
+    if (!u || !nu || !dt_out) return BURGERS_ERR_NULL;
+    if (B < 1 || N < 3) return BURGERS_ERR_SHAPE;
+    if (bc != BURGERS_BC_PERIODIC && bc != BURGERS_BC_DIRICHLET) return BURGERS_ERR_ENUM;
+    if (!(L > 0.0) || !std::isfinite(L) || !(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
+    return launch_cfl<T>(u, B, N, grid_dx(N, L, bc), nu, C, dt_out, (cudaStream_t)stream);
+}
+
+// ---- host-buffer path: allocate, copy in, run the device path, copy out, free ---------------
+struct DevBuf {
+    void *p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    bool alloc(size_t bytes) { return bytes == 0 || cudaMalloc(&p, bytes) == cudaSuccess; }
+};
+
+template <typename T, typename F>
+int host_step(T *u, int64_t B, int64_t N, const T *nu, const T *dt, size_t ws_bytes, F run) {
+    const size_t ub = (size_t)B * (size_t)N * sizeof(T), vb = (size_t)B * sizeof(T);
+    DevBuf du, dnu, ddt, dws;
+    if (!du.alloc(ub) || !dnu.alloc(vb) || !ddt.alloc(vb) || !dws.alloc(ws_bytes)) return BURGERS_ERR_CUDA;
+    cudaStream_t s = nullptr;
+    if (cudaMemcpyAsync(du.p, u, ub, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    if (cudaMemcpyAsync(dnu.p, nu, vb, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    if (cudaMemcpyAsync(ddt.p, dt, vb, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    int st = run((T *)du.p, (const T *)dnu.p, (const T *)ddt.p, dws.p);
+    if (st != BURGERS_OK) { cudaStreamSynchronize(s); return st; }
+    if (cudaMemcpyAsync(u, du.p, ub, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    return cuda_status(cudaStreamSynchronize(s));
+}
+
+template <typename T>
+int explicit_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
+                  int bc, int scheme) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!scheme_ok(scheme)) return BURGERS_ERR_ENUM;
+    const size_t wsb = burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc, scheme,
+                                               BURGERS_PLAN_AUTO);
+    return host_step<T>(u, B, N, nu, dt, wsb, [&](T *du, const T *dnu, const T *ddt, void *ws) {
+        return explicit_call<T>(du, B, N, L, dnu, ddt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws,
+                                wsb, nullptr);
+    });
+}
+
+template <typename T>
+int btcs_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    const size_t wsb = burgers_workspace_bytes(BURGERS_OP_BTCS, sizeof(T) == 8, B, N, bc, 0,
+                                               BURGERS_PLAN_AUTO);
+    return host_step<T>(u, B, N, nu, dt, wsb, [&](T *du, const T *dnu, const T *ddt, void *ws) {
+        return btcs_call<T>(du, B, N, L, dnu, ddt, n_steps, bc, BURGERS_PLAN_AUTO, ws, wsb, nullptr);
+    });
+}
+
+template <typename T>
+int cfl_host(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out) {
+    if (!u || !nu || !dt_out) return BURGERS_ERR_NULL;
+    if (B < 1 || N < 3) return BURGERS_ERR_SHAPE;
+    const size_t ub = (size_t)B * (size_t)N * sizeof(T), vb = (size_t)B * sizeof(T);
+    DevBuf du, dnu, ddt;
+    if (!du.alloc(ub) || !dnu.alloc(vb) || !ddt.alloc(vb)) return BURGERS_ERR_CUDA;
+    cudaStream_t s = nullptr;
+    if (cudaMemcpyAsync(du.p, u, ub, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    if (cudaMemcpyAsync(dnu.p, nu, vb, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    int st = cfl_call<T>((const T *)du.p, B, N, L, (const T *)dnu.p, C, bc, (T *)ddt.p, nullptr);
+    if (st != BURGERS_OK) { cudaStreamSynchronize(s); return st; }
+    if (cudaMemcpyAsync(dt_out, ddt.p, vb, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    return cuda_status(cudaStreamSynchronize(s));
+}
+
+}  // namespace
+
+extern "C" {
+
+int burgers_explicit_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                         int64_t n_steps, int bc, int scheme, void *ws, size_t ws_bytes, void *stream) {
+    return explicit_call<float>(u, B, N, L, nu, dt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes, stream);
+}
+int burgers_explicit_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                         int64_t n_steps, int bc, int scheme, void *ws, size_t ws_bytes, void *stream) {
+    return explicit_call<double>(u, B, N, L, nu, dt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes, stream);
+}
+int burgers_explicit_plan_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                              int64_t n_steps, int bc, int scheme, int plan, int tblock, int ppt,
+                              void *ws, size_t ws_bytes, void *stream) {
+    return explicit_call<float>(u, B, N, L, nu, dt, n_steps, bc, scheme, plan, tblock, ppt, ws, ws_bytes, stream);
+}
+int burgers_explicit_plan_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                              const double *dt, int64_t n_steps, int bc, int scheme, int plan,
+                              int tblock, int ppt, void *ws, size_t ws_bytes, void *stream) {
+    return explicit_call<double>(u, B, N, L, nu, dt, n_steps, bc, scheme, plan, tblock, ppt, ws, ws_bytes, stream);
+}
+
+int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                     int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
+    return btcs_call<float>(u, B, N, L, nu, dt, n_steps, bc, BURGERS_PLAN_AUTO, ws, ws_bytes, stream);
+}
+int burgers_btcs_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                     int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
+    return btcs_call<double>(u, B, N, L, nu, dt, n_steps, bc, BURGERS_PLAN_AUTO, ws, ws_bytes, stream);
+}
+int burgers_btcs_plan_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                          int64_t n_steps, int bc, int plan, void *ws, size_t ws_bytes, void *stream) {
+    return btcs_call<float>(u, B, N, L, nu, dt, n_steps, bc, plan, ws, ws_bytes, stream);
+}
+int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                          int64_t n_steps, int bc, int plan, void *ws, size_t ws_bytes, void *stream) {
+    return btcs_call<double>(u, B, N, L, nu, dt, n_steps, bc, plan, ws, ws_bytes, stream);
+}
+
+int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C, int bc,
+                    float *dt_out, void *stream) {
+    return cfl_call<float>(u, B, N, L, nu, C, bc, dt_out, stream);
+}
+int dt_from_cfl_f64(const double *u, int64_t B, int64_t N, double L, const double *nu, double C, int bc,
+                    double *dt_out, void *stream) {
+    return cfl_call<double>(u, B, N, L, nu, C, bc, dt_out, stream);
+}
+
+int burgers_explicit_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                              int64_t n_steps, int bc, int scheme) {
+    return explicit_host<float>(u, B, N, L, nu, dt, n_steps, bc, scheme);
+}
+int burgers_explicit_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                              const double *dt, int64_t n_steps, int bc, int scheme) {
+    return explicit_host<double>(u, B, N, L, nu, dt, n_steps, bc, scheme);
+}
+int burgers_btcs_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                          int64_t n_steps, int bc) {
+    return btcs_host<float>(u, B, N, L, nu, dt, n_steps, bc);
+}
+int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                          int64_t n_steps, int bc) {
+    return btcs_host<double>(u, B, N, L, nu, dt, n_steps, bc);
+}
+int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C,
+                         int bc, float *dt_out) {
+    if (bc != BURGERS_BC_PERIODIC && bc != BURGERS_BC_DIRICHLET) return BURGERS_ERR_ENUM;
+    if (!(L > 0.0) || !std::isfinite(L) || !(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
+    return cfl_host<float>(u, B, N, L, nu, C, bc, dt_out);
+}
+int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L, const double *nu, double C,
+                         int bc, double *dt_out) {
+    if (bc != BURGERS_BC_PERIODIC && bc != BURGERS_BC_DIRICHLET) return BURGERS_ERR_ENUM;
+    if (!(L > 0.0) || !std::isfinite(L) || !(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
+    return cfl_host<double>(u, B, N, L, nu, C, bc, dt_out);
+}
+
+size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, int scheme,
+                               int plan) {
+    if (B < 1 || N < 3) return 0;
+    const size_t esz = dtype_is_f64 ? 8 : 4;
+    if (op == BURGERS_OP_EXPLICIT) {
+        ExplicitGeom g;
+        if (explicit_geometry(dtype_is_f64, B, N, bc, scheme, plan, 0, 0, &g) != BURGERS_OK) return 0;
+        return g.plan == BURGERS_PLAN_TILED ? align_up((size_t)B * (size_t)N * esz, 256) : 0;
+    }
+    if (op == BURGERS_OP_BTCS) {
+        if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
+        if (plan == BURGERS_PLAN_THOMAS) return align_up(btcs_thomas_ws_elems(B, N, bc) * esz, 256);
+        if (plan == BURGERS_PLAN_LONG) return align_up(btcs_long_ws_elems(B, N, bc) * esz, 256);
+        return 0;
+    }
+    return 0;
+}
+
+int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, int scheme) {
+    if (B < 1 || N < 3) return BURGERS_ERR_SHAPE;
+    if (op == BURGERS_OP_EXPLICIT) {
+        ExplicitGeom g;
+        int st = explicit_geometry(dtype_is_f64, B, N, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, &g);
+        return st == BURGERS_OK ? g.plan : st;
+    }
+    if (op == BURGERS_OP_BTCS) return btcs_auto_plan(dtype_is_f64, B, N, bc);
+    if (op == BURGERS_OP_CFL) return BURGERS_PLAN_AUTO;
+    return BURGERS_ERR_ENUM;
+}
+
+int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, int scheme,
+                             int plan, int tblock, int64_t n_steps) {
+    if (B < 1 || N < 3 || n_steps < 0) return 0;
+    if (op == BURGERS_OP_CFL) return cfl_launch_count(dtype_is_f64, B, N);
+    if (n_steps == 0) return 0;
+    if (op == BURGERS_OP_EXPLICIT) {
+        ExplicitGeom g;
+        if (explicit_geometry(dtype_is_f64, B, N, bc, scheme, plan, tblock, 0, &g) != BURGERS_OK) return 0;
+        return g.plan == BURGERS_PLAN_RESIDENT ? 1 : (n_steps + g.tblock - 1) / g.tblock;
+    }
+    if (op == BURGERS_OP_BTCS) {
+        if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
+        if (plan == BURGERS_PLAN_THOMAS) return btcs_thomas_launch_count(n_steps);
+        if (plan == BURGERS_PLAN_HYBRID) return 1;
+        if (plan == BURGERS_PLAN_LONG) return btcs_long_launch_count(B, N, n_steps);
+    }
+    return 0;
+}
+
+const char *burgers_strerror(int status) {
+    switch (status) {
+        case BURGERS_OK: return "ok";
+        case BURGERS_ERR_NULL: return "null pointer argument";
+        case BURGERS_ERR_SHAPE: return "bad shape (need B>=1, N>=3, n_steps>=0, grid within limits)";
+        case BURGERS_ERR_ENUM: return "unknown bc / scheme / plan / op";
+        case BURGERS_ERR_VALUE: return "bad value (need finite L>0, C>0)";
+        case BURGERS_ERR_WORKSPACE: return "workspace missing or too small (see burgers_workspace_bytes)";
+        case BURGERS_ERR_CUDA: return "CUDA runtime / launch failure";
+        case BURGERS_ERR_PLAN: return "requested plan cannot run this shape";
+    }
+    return "unknown status";
+}
+
+int burgers_version(void) { return BURGERS_VERSION; }
+
+}  // extern "C"

@@ -1,0 +1,70 @@
+// common.cuh -- internal declarations shared by the translation units of libburgers.
+// (Product code only; the CPU oracle under oracle/ shares nothing with this.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/burgers.h"
+
+namespace burgers {
+
+constexpr int kWarp = 32;
+
+// Grid spacing (D1): periodic dx = L/N (node N == node 0),
+// Dirichlet dx = L/(N-1).
+inline double grid_dx(int64_t N, double L, int bc) {
+    return bc == BURGERS_BC_PERIODIC ? L / (double)N : L / (double)(N - 1);
+}
+
+inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? BURGERS_OK : BURGERS_ERR_CUDA; }
+inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
+
+// ---------------------------------------------------------------- CFL (cfl.cu)
+template <typename T>
+int launch_cfl(const T *u, int64_t B, int64_t N, double dx, const T *nu, double C, T *dt_out,
+               cudaStream_t s);
+int64_t cfl_launch_count(int is_f64, int64_t B, int64_t N);
+
+// ---------------------------------------------------------------- explicit (explicit_*.cu)
+// Geometry of one explicit launch plan, decided on the host (explicit_plan.cu).
+struct ExplicitGeom {
+    int plan;        // BURGERS_PLAN_RESIDENT / BURGERS_PLAN_TILED
+    int P;           // grid points per thread
+    int nth;         // active threads per CTA (CTA holds nth*P points)
+    int block;       // launched threads per CTA (nth rounded up to a warp multiple)
+    int tblock;      // steps per launch (TILED), unused for RESIDENT
+    int halo;        // halo points per side (TILED) = tblock*radius rounded up
+    int64_t W;       // valid outputs per tile (TILED)
+    int64_t tiles;   // tiles per trajectory (TILED)
+};
+// Fills `g` for (dtype, N, bc, scheme) under `plan` (AUTO allowed) with optional overrides
+// (tblock/ppt = 0 -> defaults).  Returns BURGERS_OK or BURGERS_ERR_PLAN.
+int explicit_geometry(int is_f64, int64_t B, int64_t N, int bc, int scheme, int plan, int tblock,
+                      int ppt, ExplicitGeom *g);
+template <typename T>
+int launch_explicit(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                    int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
+                    cudaStream_t s);
+// max threads per CTA the explicit kernel <T,P,scheme> may be launched with (register limit)
+int explicit_max_threads(int is_f64, int P, int scheme);
+
+// ---------------------------------------------------------------- BTCS (btcs_*.cu)
+template <typename T>
+int launch_btcs_thomas(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                       int64_t n_steps, int bc, T *ws, cudaStream_t s);
+size_t btcs_thomas_ws_elems(int64_t B, int64_t N, int bc);
+int64_t btcs_thomas_launch_count(int64_t n_steps);
+
+template <typename T>
+int launch_btcs_hybrid(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                       int64_t n_steps, int bc, cudaStream_t s);
+bool btcs_hybrid_fits(int is_f64, int64_t N, int bc);
+
+template <typename T>
+int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                     int64_t n_steps, int bc, T *ws, cudaStream_t s);
+size_t btcs_long_ws_elems(int64_t B, int64_t N, int bc);
+int64_t btcs_long_launch_count(int64_t B, int64_t N, int64_t n_steps);
+bool btcs_long_fits(int64_t N, int bc);
+
+}  // namespace burgers

@@ -1,0 +1,84 @@
+// explicit_plan.cu -- host-side geometry of the explicit plans (no device code).
+#include "common.cuh"
+
+namespace burgers {
+
+// must mirror expl::max_threads_for (explicit_impl.cuh)
+int explicit_max_threads(int is_f64, int P, int scheme) {
+    const int bytes = is_f64 ? 8 : 4;
+    const int arrays = (scheme == BURGERS_SCHEME_RK4) ? 3 : (bytes == 4 ? 3 : 1);
+    const int regs = P * (bytes / 4) * arrays + 40;
+    int t = 1024;
+    while (t > 32 && t * regs > 65536) t /= 2;
+    return t;
+}
+
+static bool valid_ppt(int p) { return p == 1 || p == 2 || p == 4 || p == 8 || p == 16 || p == 32; }
+
+static bool resident_fit(int is_f64, int64_t N, int scheme, int P, ExplicitGeom *g) {
+    if (N % P) return false;
+    const int64_t nth = N / P;
+    if (nth > explicit_max_threads(is_f64, P, scheme)) return false;
+    g->plan = BURGERS_PLAN_RESIDENT;
+    g->P = P;
+    g->nth = (int)nth;
+    g->block = (int)((nth + 31) / 32 * 32);
+    g->tblock = 0; g->halo = 0; g->W = N; g->tiles = 1;
+    return true;
+}
+
+static bool resident_geometry(int is_f64, int64_t N, int scheme, int ppt, ExplicitGeom *g) {
+    if (ppt) return resident_fit(is_f64, N, scheme, ppt, g);
+    // prefer many points per thread (few halo exchanges per update) while keeping >= 2 warps
+    for (int P = 32; P >= 1; P /= 2)
+        if (N / P >= 64 && resident_fit(is_f64, N, scheme, P, g)) return true;
+    for (int P = 1; P <= 32; P *= 2)
+        if (resident_fit(is_f64, N, scheme, P, g)) return true;
+    return false;
+}
+
+static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock, int ppt,
+                           ExplicitGeom *g) {
+    const int V = is_f64 ? 2 : 4;
+    const int radius = (scheme == BURGERS_SCHEME_RK4) ? 4 : 1;
+    int P = ppt ? ppt : 16;
+    // Dirichlet: the frozen end nodes must be the first / last point of a thread
+    if (bc == BURGERS_BC_DIRICHLET) {
+        if (ppt && N % P) return false;
+        while (N % P) P /= 2;
+    }
+    int nth = 256;
+    const int maxt = explicit_max_threads(is_f64, P, scheme);
+    if (nth > maxt) nth = maxt;
+    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 4 : 16;
+    const int64_t Wt = (int64_t)nth * P;
+    const int q = P > V ? P : V;
+    int halo = 0;
+    for (;;) {
+        halo = (tblock * radius + q - 1) / q * q;
+        if (Wt - 2 * halo >= Wt / 4 && Wt - 2 * halo >= 1) break;
+        if (tblock == 1) return false;
+        tblock /= 2;
+    }
+    g->plan = BURGERS_PLAN_TILED;
+    g->P = P; g->nth = nth; g->block = nth;
+    g->tblock = tblock; g->halo = halo; g->W = Wt - 2 * halo;
+    g->tiles = (N + g->W - 1) / g->W;
+    return true;
+}
+
+int explicit_geometry(int is_f64, int64_t B, int64_t N, int bc, int scheme, int plan, int tblock,
+                      int ppt, ExplicitGeom *g) {
+    (void)B;
+    if (ppt && !valid_ppt(ppt)) return BURGERS_ERR_PLAN;
+    if (tblock < 0) return BURGERS_ERR_PLAN;
+    if (plan == BURGERS_PLAN_AUTO || plan == BURGERS_PLAN_RESIDENT) {
+        if (resident_geometry(is_f64, N, scheme, ppt, g)) return BURGERS_OK;
+        if (plan == BURGERS_PLAN_RESIDENT) return BURGERS_ERR_PLAN;
+    }
+    if (plan == BURGERS_PLAN_AUTO || plan == BURGERS_PLAN_TILED)
+        return tiled_geometry(is_f64, N, bc, scheme, tblock, ppt, g) ? BURGERS_OK : BURGERS_ERR_PLAN;
+    return BURGERS_ERR_ENUM;
+}
+
+}  // namespace burgers

@@ -1,0 +1,120 @@
+"""C-ABI checks that need no GPU: the library builds, loads, exports every symbol that
+include/burgers.h declares, rejects bad arguments synchronously (before any CUDA call), and
+its pure shape queries behave."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "burgers.h")
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_12204_b200 import build
+    build.build()
+    from paper_2601_12204_b200 import binding
+    return binding
+
+
+def _declared():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b((?:burgers|dt_from_cfl)_\w+)\s*\(", src)))
+
+
+def test_header_symbols_exported(B):
+    names = _declared()
+    assert len(names) >= 21
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in burgers.h but not exported"
+    assert sorted(B.EXPORTS) == names
+
+
+def test_version_and_strerror(B):
+    assert B.version() == 100
+    assert B.strerror(0) == "ok"
+    for st in range(-7, 0):
+        assert B.strerror(st) not in ("ok", "unknown status")
+    assert B.strerror(-99) == "unknown status"
+
+
+def test_argument_errors_are_synchronous(B):
+    lib = B.raw()
+    one = ctypes.c_void_p(16)  # never dereferenced: every call below fails validation first
+    f = lib.burgers_explicit_f64
+    assert f(None, 1, 8, 1.0, one, one, 1, 0, 0, None, 0, None) == B.ERR_NULL
+    assert f(one, 1, 8, 1.0, None, one, 1, 0, 0, None, 0, None) == B.ERR_NULL
+    assert f(one, 0, 8, 1.0, one, one, 1, 0, 0, None, 0, None) == B.ERR_SHAPE
+    assert f(one, 1, 2, 1.0, one, one, 1, 0, 0, None, 0, None) == B.ERR_SHAPE
+    assert f(one, 1, 8, 1.0, one, one, -1, 0, 0, None, 0, None) == B.ERR_SHAPE
+    assert f(one, 1, 8, 1.0, one, one, 1, 2, 0, None, 0, None) == B.ERR_ENUM
+    assert f(one, 1, 8, 1.0, one, one, 1, 0, 5, None, 0, None) == B.ERR_ENUM
+    assert f(one, 1, 8, 0.0, one, one, 1, 0, 0, None, 0, None) == B.ERR_VALUE
+    assert f(one, 1, 8, float("nan"), one, one, 1, 0, 0, None, 0, None) == B.ERR_VALUE
+    assert f(one, 1, 8, float("inf"), one, one, 1, 0, 0, None, 0, None) == B.ERR_VALUE
+    g = lib.burgers_explicit_plan_f32
+    assert g(one, 1, 8, 1.0, one, one, 1, 0, 0, 9, 0, 0, None, 0, None) == B.ERR_ENUM
+    assert g(one, 1, 8, 1.0, one, one, 1, 0, 0, B.PLAN_RESIDENT, 0, 3, None, 0, None) == B.ERR_PLAN
+    assert g(one, 1, 7, 1.0, one, one, 1, 0, 0, B.PLAN_RESIDENT, 0, 2, None, 0, None) == B.ERR_PLAN
+    # TILED needs a workspace
+    assert g(one, 1, 1 << 20, 1.0, one, one, 1, 0, 0, B.PLAN_TILED, 0, 0, None, 0, None) == B.ERR_WORKSPACE
+    h = lib.burgers_btcs_f64
+    assert h(None, 1, 8, 1.0, one, one, 1, 0, None, 0, None) == B.ERR_NULL
+    assert h(one, 1, 8, 1.0, one, one, 1, 7, None, 0, None) == B.ERR_ENUM
+    assert h(one, 1, 8, -1.0, one, one, 1, 0, None, 0, None) == B.ERR_VALUE
+    hp = lib.burgers_btcs_plan_f64
+    assert hp(one, 1, 8, 1.0, one, one, 1, 0, B.PLAN_THOMAS, None, 0, None) == B.ERR_WORKSPACE
+    assert hp(one, 1, 8, 1.0, one, one, 1, 0, B.PLAN_RESIDENT, None, 0, None) == B.ERR_ENUM
+    c = lib.dt_from_cfl_f32
+    assert c(None, 1, 8, 1.0, one, 0.4, 0, one, None) == B.ERR_NULL
+    assert c(one, 1, 8, 1.0, one, 0.0, 0, one, None) == B.ERR_VALUE
+    assert c(one, 1, 8, 1.0, one, 0.4, 3, one, None) == B.ERR_ENUM
+    assert c(one, 1, 1, 1.0, one, 0.4, 0, one, None) == B.ERR_SHAPE
+    # host variants validate the same way
+    assert lib.burgers_explicit_host_f32(None, 1, 8, 1.0, one, one, 1, 0, 0) == B.ERR_NULL
+    assert lib.burgers_btcs_host_f64(one, 1, 8, 1.0, one, one, -2, 0) == B.ERR_SHAPE
+    assert lib.dt_from_cfl_host_f64(one, 1, 8, 1.0, one, -1.0, 0, one) == B.ERR_VALUE
+
+
+def test_plan_queries(B):
+    # configs of BASELINE.json: C2 and C5 are resident, C4a is tiled
+    assert B.plan_query(B.OP_EXPLICIT, False, 1024, 4096, B.BC_DIRICHLET, B.SCHEME_EULER) == B.PLAN_RESIDENT
+    assert B.plan_query(B.OP_EXPLICIT, True, 1024, 4096, B.BC_DIRICHLET, B.SCHEME_EULER) == B.PLAN_RESIDENT
+    assert B.plan_query(B.OP_EXPLICIT, False, 65536, 1024, B.BC_PERIODIC, B.SCHEME_RK4) == B.PLAN_RESIDENT
+    assert B.plan_query(B.OP_EXPLICIT, False, 1, 1 << 24, B.BC_PERIODIC, B.SCHEME_EULER) == B.PLAN_TILED
+    assert B.plan_query(B.OP_EXPLICIT, True, 1, 3001, B.BC_PERIODIC, B.SCHEME_EULER) == B.PLAN_TILED
+    assert B.workspace_bytes(B.OP_EXPLICIT, False, 1024, 4096, B.BC_DIRICHLET, 0) == 0
+    assert B.workspace_bytes(B.OP_EXPLICIT, False, 1, 1 << 24, B.BC_PERIODIC, 0) == 4 << 24
+    assert B.workspace_bytes(B.OP_BTCS, True, 8, 100, B.BC_PERIODIC, 0, B.PLAN_THOMAS) >= 4 * 8 * 100 * 8
+    assert B.workspace_bytes(B.OP_BTCS, True, 8, 100, B.BC_DIRICHLET, 0, B.PLAN_THOMAS) >= 3 * 8 * 100 * 8
+    assert B.launch_count(B.OP_EXPLICIT, False, 1024, 4096, 1, 0, n_steps=10000) == 1
+    assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=2000, tblock=16) == 125
+    assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=0) == 0
+    assert B.launch_count(B.OP_CFL, False, 1024, 4096, 1) == 1
+    assert B.launch_count(B.OP_CFL, False, 1, 1 << 24, 0) == 2
+
+
+def test_device_entry_points_refuse_cpu_tensors(B):
+    import torch
+    u = torch.zeros(2, 8, dtype=torch.float64)
+    v = torch.ones(2, dtype=torch.float64)
+    with pytest.raises(TypeError):
+        B.burgers_explicit(u, 1.0, v, v, 1, B.BC_PERIODIC, B.SCHEME_EULER)
+    with pytest.raises(TypeError):
+        B.burgers_btcs(u, 1.0, v, v, 1, B.BC_PERIODIC)
+    with pytest.raises(TypeError):
+        B.dt_from_cfl(u, 1.0, v, 0.4, B.BC_PERIODIC)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2601_12204_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
+                assert "burgers_oracle" not in txt and "liboracle" not in txt, f

@@ -1,0 +1,261 @@
+"""GPU parity tests: the CUDA path (called through the C ABI) against the CPU oracle, element by
+element, on the seeded synthetic workloads of DESIGN.md / BASELINE.json at sizes the oracle
+finishes in seconds (several tiles / CTAs and ragged tails), plus cross-plan agreement (G10),
+edge cases and API semantics.  Full-size configs: tests/test_gpu_fullsize.py."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from parity import TOL, oracle_dt, rel_err, to_dev
+from paper_2601_12204_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_12204_b200 import binding
+    return binding
+
+
+def run_explicit(B, u0, L, nu, dt, n, bc, scheme, **kw):
+    u = to_dev(u0.copy())
+    B.burgers_explicit(u, L, to_dev(nu), to_dev(dt), n, bc, scheme, **kw)
+    return u.cpu().numpy()
+
+
+def run_btcs(B, u0, L, nu, dt, n, bc, **kw):
+    u = to_dev(u0.copy())
+    B.burgers_btcs(u, L, to_dev(nu), to_dev(dt), n, bc, **kw)
+    return u.cpu().numpy()
+
+
+def check_explicit(B, w, n, scheme, cfl=None, tol_scale=1.0, **kw):
+    dt = oracle_dt(w.u0, w.L, w.nu, cfl or w.cfl, w.bc, w.dtype)
+    ref = oracle.explicit(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64),
+                          dt.astype(np.float64), n, w.bc, scheme)
+    got = run_explicit(B, w.u0, w.L, w.nu, dt, n, w.bc, scheme, **kw)
+    e = rel_err(got, ref, w.u0)
+    assert e <= TOL[w.dtype] * tol_scale, (w.name, scheme, kw, e)
+    return e
+
+
+def check_btcs(B, w, n, cfl=None, **kw):
+    dt = oracle_dt(w.u0, w.L, w.nu, cfl or w.cfl, w.bc, w.dtype)
+    ref = oracle.btcs(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64), dt.astype(np.float64),
+                      n, w.bc)
+    got = run_btcs(B, w.u0, w.L, w.nu, dt, n, w.bc, **kw)
+    e = rel_err(got, ref, w.u0)
+    assert e <= TOL[w.dtype], (w.name, kw, e)
+    return e
+
+
+# ------------------------------------------------------------------ dt_from_cfl (a1)
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(1, 3), (5, 17), (7, 256), (3, 4099), (2, 70001), (1, 1 << 20), (300, 1024)])
+def test_dt_from_cfl_matches_oracle(B, dtype, shape):
+    rng = np.random.default_rng(7)
+    Bn, N = shape
+    u0 = (rng.standard_normal(shape) * 3).astype(dtype)
+    nu = np.exp(rng.uniform(math.log(1e-4), math.log(1.0), Bn)).astype(dtype)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        ref = oracle.dt_from_cfl(u0.astype(np.float64), L, nu.astype(np.float64), 0.4, bc).astype(dtype)
+        got = B.dt_from_cfl(to_dev(u0), L, to_dev(nu), 0.4, bc).cpu().numpy()
+        # same fp64 formula on the same inputs, rounded once: allow 2 ulp
+        assert np.all(np.abs(got - ref) <= 2 * np.spacing(np.abs(ref))), (shape, bc)
+
+
+def test_dt_from_cfl_zero_cases(B):
+    u0 = np.zeros((3, 64)); u0[1, 5] = -2.0; u0[2, 63] = 4.0
+    nu = np.array([0.1, 0.0, 0.0])
+    got = B.dt_from_cfl(to_dev(u0), 64.0, to_dev(nu), 0.5, B.BC_PERIODIC).cpu().numpy()
+    assert got[0] == 0.5 * 1.0 / (2 * 0.1)          # u == 0: diffusive bound
+    assert got[1] == 0.5 * 1.0 / 2.0                # nu == 0: convective bound, |u| max = 2
+    assert got[2] == 0.5 * 1.0 / 4.0                # Dirichlet-style end node counts too
+    z = B.dt_from_cfl(to_dev(np.zeros((1, 8))), 1.0, to_dev(np.zeros(1)), 0.5, B.BC_PERIODIC).cpu().numpy()
+    assert np.isinf(z[0]) and z[0] > 0
+
+
+# ------------------------------------------------------------------ config 1 (worked on the GPU too)
+def test_c1_sine_euler_rk4_btcs_vs_oracle_and_colehopf(B):
+    from refs import colehopf_sin
+    w = W.c1_sine()
+    x = np.arange(w.N) * (w.L / w.N)
+    exact = colehopf_sin(x, 1.0, 0.05)
+    for scheme, C, name in ((B.SCHEME_EULER, 0.4, "euler"), (B.SCHEME_RK4, 0.8, "rk4"), (None, 4.0, "btcs")):
+        dtc = oracle.dt_from_cfl(w.u0, w.L, w.nu, C, w.bc)[0]
+        n, dt = W.steps_for_final_time(dtc, 1.0)
+        dta = np.array([dt])
+        if scheme is None:
+            ref = oracle.btcs(w.u0, w.L, w.nu, dta, n, w.bc)
+            got = run_btcs(B, w.u0, w.L, w.nu, dta, n, w.bc)
+        else:
+            ref = oracle.explicit(w.u0, w.L, w.nu, dta, n, w.bc, scheme)
+            got = run_explicit(B, w.u0, w.L, w.nu, dta, n, w.bc, scheme)
+        assert rel_err(got, ref, w.u0) <= 1e-10, name
+        rms = math.sqrt(np.mean((got[0] - exact) ** 2))
+        assert rms < 2.5e-2, (name, rms)        # first-order schemes at N=256 (G2: ~1.1e-2 / 1.8e-2)
+    assert (n, name) == (42, "btcs")
+
+
+def test_worked_example_4node_on_gpu(B):
+    from refs import read_golden
+    G = read_golden("worked_example_4node.txt")
+    u4 = np.array([[1.0, 2.0, -1.0, 0.0]])
+    nu = np.array([0.1]); dt = np.array([0.1])
+    for plan in (B.PLAN_RESIDENT, B.PLAN_TILED):
+        got = run_explicit(B, u4, 4.0, nu, dt, 1, B.BC_PERIODIC, B.SCHEME_EULER, plan=plan)
+        np.testing.assert_allclose(got[0], G["euler_periodic"], atol=1e-14)
+        got = run_explicit(B, u4, 4.0, nu, dt, 2, B.BC_PERIODIC, B.SCHEME_EULER, plan=plan)
+        np.testing.assert_allclose(got[0], G["euler2_periodic"], atol=1e-14)
+        got = run_explicit(B, u4, 4.0, nu, dt, 1, B.BC_PERIODIC, B.SCHEME_RK4, plan=plan)
+        np.testing.assert_allclose(got[0], G["rk4_periodic"], atol=1e-14)
+        got = run_explicit(B, u4, 3.0, nu, dt, 1, B.BC_DIRICHLET, B.SCHEME_EULER, plan=plan)
+        np.testing.assert_allclose(got[0], G["euler_dirichlet"], atol=1e-14)
+        got = run_explicit(B, u4, 3.0, nu, dt, 1, B.BC_DIRICHLET, B.SCHEME_RK4, plan=plan)
+        np.testing.assert_allclose(got[0], G["rk4_dirichlet"], atol=1e-14)
+    for plan in (B.PLAN_AUTO, B.PLAN_THOMAS):
+        got = run_btcs(B, u4, 4.0, nu, dt, 1, B.BC_PERIODIC, plan=plan)
+        np.testing.assert_allclose(got[0], G["btcs_periodic"], atol=1e-14)
+        got = run_btcs(B, u4, 3.0, nu, dt, 1, B.BC_DIRICHLET, plan=plan)
+        np.testing.assert_allclose(got[0], G["btcs_dirichlet"], atol=1e-14)
+
+
+# ------------------------------------------------------------------ config 2 (reduced): Dirichlet Euler
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_c2_reduced_resident(B, dtype):
+    w = W.c2_dirichlet_batch(B=24, N=4096, dtype=dtype)
+    check_explicit(B, w, 3000, B.SCHEME_EULER)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("ppt", [1, 2, 4, 8, 16, 32])
+def test_c2_reduced_every_points_per_thread(B, dtype, ppt):
+    w = W.c2_dirichlet_batch(B=5, N=512, dtype=dtype)
+    check_explicit(B, w, 700, B.SCHEME_EULER, plan=B.PLAN_RESIDENT, ppt=ppt)
+    check_explicit(B, w, 150, B.SCHEME_RK4, cfl=0.8, plan=B.PLAN_RESIDENT, ppt=ppt)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_c2_reduced_tiled_matches(B, dtype):
+    # same workload through the temporally blocked plan: several tiles, ragged last block of steps
+    w = W.c2_dirichlet_batch(B=3, N=4096 * 3, dtype=dtype)
+    check_explicit(B, w, 333, B.SCHEME_EULER, plan=B.PLAN_TILED)
+    check_explicit(B, w, 50, B.SCHEME_RK4, cfl=0.8, plan=B.PLAN_TILED)
+    check_explicit(B, w, 100, B.SCHEME_EULER, plan=B.PLAN_TILED, tblock=7, ppt=8)
+
+
+# ------------------------------------------------------------------ config 5 (reduced): periodic RK4
+def test_c5_reduced_rk4(B):
+    w = W.c5_rk4_ensemble(n_steps=600, rows=np.arange(0, 65536, 2048))
+    check_explicit(B, w, 600, B.SCHEME_RK4)
+    check_explicit(B, w, 600, B.SCHEME_RK4, plan=B.PLAN_RESIDENT, ppt=32)   # one warp per trajectory
+    check_explicit(B, w, 600, B.SCHEME_RK4, plan=B.PLAN_RESIDENT, ppt=8)
+    w64 = W.c5_rk4_ensemble(n_steps=200, rows=np.arange(0, 65536, 8192), dtype=np.float64)
+    check_explicit(B, w64, 200, B.SCHEME_RK4)
+    check_explicit(B, w64, 200, B.SCHEME_EULER, cfl=0.4)
+
+
+# ------------------------------------------------------------------ config 4a (reduced): long periodic grid
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_c4a_reduced_long_grid_tiled(B, dtype):
+    w = W.c4a_long_explicit(N=(1 << 16) + 40, n_steps=500, dtype=dtype)   # ragged last tile
+    assert B.plan_query(B.OP_EXPLICIT, dtype == np.float64, 1, w.N, w.bc, 0) == B.PLAN_TILED
+    check_explicit(B, w, 500, B.SCHEME_EULER)
+    check_explicit(B, w, 37, B.SCHEME_RK4, cfl=0.8)
+    w2 = W.c4a_long_explicit(N=50021, n_steps=100, dtype=dtype)          # prime N: scalar loads
+    check_explicit(B, w2, 100, B.SCHEME_EULER)
+
+
+def test_odd_sizes_and_signs(B):
+    rng = np.random.default_rng(11)
+    for N in (3, 4, 5, 31, 33, 100, 201, 1000, 1023, 3001):
+        for bc, L in ((B.BC_PERIODIC, 2.0), (B.BC_DIRICHLET, 1.0)):
+            u0 = rng.uniform(-2, 2, (3, N))
+            nu = rng.uniform(0.01, 0.1, 3)
+            dt = oracle.dt_from_cfl(u0, L, nu, 0.4, bc)
+            for scheme in (B.SCHEME_EULER, B.SCHEME_RK4):
+                ref = oracle.explicit(u0, L, nu, dt, 25, bc, scheme)
+                got = run_explicit(B, u0, L, nu, dt, 25, bc, scheme)
+                assert rel_err(got, ref, u0) <= 1e-12, (N, bc, scheme)
+                got = run_explicit(B, u0, L, nu, dt, 25, bc, scheme, plan=B.PLAN_TILED, tblock=4)
+                assert rel_err(got, ref, u0) <= 1e-12, (N, bc, scheme, "tiled")
+            ref = oracle.btcs(u0, L, nu, 10 * dt, 9, bc)
+            got = run_btcs(B, u0, L, nu, 10 * dt, 9, bc, plan=B.PLAN_THOMAS)
+            assert rel_err(got, ref, u0) <= 1e-12, (N, bc, "btcs-thomas")
+            got = run_btcs(B, u0, L, nu, 10 * dt, 9, bc)
+            assert rel_err(got, ref, u0) <= 1e-12, (N, bc, "btcs-auto")
+
+
+# ------------------------------------------------------------------ config 3 (reduced): periodic BTCS
+def test_c3_reduced_btcs_periodic(B):
+    w = W.c3_periodic_btcs(B=40, N=2048, n_steps=60)
+    check_btcs(B, w, 60)
+    check_btcs(B, w, 60, plan=B.PLAN_THOMAS)
+
+
+def test_btcs_dirichlet_and_fp32(B):
+    w = W.c2_dirichlet_batch(B=9, N=1000, dtype=np.float64)
+    check_btcs(B, w, 40, cfl=10.0)
+    check_btcs(B, w, 40, cfl=10.0, plan=B.PLAN_THOMAS)
+    w32 = W.c3_periodic_btcs(B=6, N=512, n_steps=50, dtype=np.float32)
+    check_btcs(B, w32, 50)
+    w32d = W.c2_dirichlet_batch(B=6, N=512, dtype=np.float32)
+    check_btcs(B, w32d, 50, cfl=10.0)
+
+
+def test_c4b_reduced_long_btcs(B):
+    w = W.c4b_long_btcs(N=1 << 16, n_steps=12)
+    check_btcs(B, w, 12)
+    check_btcs(B, w, 12, plan=B.PLAN_THOMAS)
+
+
+# ------------------------------------------------------------------ semantics
+def test_zero_steps_and_step_splitting(B):
+    w = W.c5_rk4_ensemble(n_steps=0, rows=np.arange(4), dtype=np.float64)
+    dt = oracle_dt(w.u0, w.L, w.nu, 0.4, w.bc, w.dtype)
+    same = run_explicit(B, w.u0, w.L, w.nu, dt, 0, w.bc, B.SCHEME_EULER)
+    np.testing.assert_array_equal(same, w.u0)
+    a = run_explicit(B, w.u0, w.L, w.nu, dt, 30, w.bc, B.SCHEME_EULER)
+    b = run_explicit(B, run_explicit(B, w.u0, w.L, w.nu, dt, 11, w.bc, B.SCHEME_EULER), w.L, w.nu, dt, 19,
+                     w.bc, B.SCHEME_EULER)
+    np.testing.assert_array_equal(a, b)          # fp64: p then q steps == p+q steps, bitwise
+    c = run_btcs(B, w.u0, w.L, w.nu, dt * 10, 6, w.bc)
+    d = run_btcs(B, run_btcs(B, w.u0, w.L, w.nu, dt * 10, 2, w.bc), w.L, w.nu, dt * 10, 4, w.bc)
+    np.testing.assert_array_equal(c, d)
+
+
+def test_dirichlet_ends_never_move_and_max_principle(B):
+    w = W.c2_dirichlet_batch(B=4, N=1024, dtype=np.float64)
+    u0 = w.u0.copy(); u0[:, 0] = 0.75; u0[:, -1] = -0.5
+    dt = oracle_dt(u0, w.L, w.nu, 0.4, w.bc, w.dtype)
+    for got in (run_explicit(B, u0, w.L, w.nu, dt, 500, w.bc, B.SCHEME_EULER),
+                run_explicit(B, u0, w.L, w.nu, dt, 100, w.bc, B.SCHEME_RK4),
+                run_btcs(B, u0, w.L, w.nu, dt * 25, 20, w.bc)):
+        np.testing.assert_array_equal(got[:, 0], u0[:, 0])
+        np.testing.assert_array_equal(got[:, -1], u0[:, -1])
+        assert np.all(got.max(axis=1) <= u0.max(axis=1) + 1e-12)
+        assert np.all(got.min(axis=1) >= u0.min(axis=1) - 1e-12)
+
+
+def test_host_entry_points_match_device_path(B):
+    w = W.c2_dirichlet_batch(B=6, N=2048, dtype=np.float32)
+    dt_h = B.dt_from_cfl_host(w.u0, w.L, w.nu, 0.4, w.bc)
+    dt_d = B.dt_from_cfl(to_dev(w.u0), w.L, to_dev(w.nu), 0.4, w.bc).cpu().numpy()
+    np.testing.assert_array_equal(dt_h, dt_d)
+    uh = w.u0.copy()
+    B.burgers_explicit_host(uh, w.L, w.nu, dt_h, 200, w.bc, B.SCHEME_EULER)
+    ud = run_explicit(B, w.u0, w.L, w.nu, dt_h, 200, w.bc, B.SCHEME_EULER)
+    np.testing.assert_array_equal(uh, ud)
+    w3 = W.c3_periodic_btcs(B=5, N=256, n_steps=10)
+    dt3 = B.dt_from_cfl_host(w3.u0, w3.L, w3.nu, 10.0, w3.bc)
+    uh = w3.u0.copy()
+    B.burgers_btcs_host(uh, w3.L, w3.nu, dt3, 10, w3.bc)
+    np.testing.assert_array_equal(uh, run_btcs(B, w3.u0, w3.L, w3.nu, dt3, 10, w3.bc))
+
+
+def test_library_is_loaded_in_this_process(B):
+    maps = open("/proc/self/maps").read()
+    assert "libburgers.so" in maps
