@@ -1,0 +1,414 @@
+#!/usr/bin/env python
+"""bench.py -- grid-point updates/s of the Burgers hot path on B200 (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload c2_f32|c2_f64|c3|c4a|c4b|c5] [--no-extras]
+
+A "step" is ONE pass of the hot path over one batch of the seeded synthetic workload:
+dt_from_cfl (CFL reduction) followed by the time-stepping call (all n_steps of the config).
+Headline workload at N=1: BASELINE.json configs[1] (C2: B=1024 Dirichlet trajectories, N=4096,
+10,000 forward-Euler steps, fp32).  `value` = grid-point updates/s (B*N*n_steps per step) with
+the inputs resident in HBM; `e2e` = the same through the host-buffer C-ABI calls (H2D + D2H inside
+the timed region); `roofline` = the dominant kernel against its bound;
+`cpu_baseline` = the fp64 CPU oracle timed on this box's cores on a bounded sample; `schemes` =
+the other configs (one line each, fewer repetitions).  N>1: every rank runs its own shard of an
+N-times larger batch (trajectories are independent: no collective on the data path; weak scaling).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+SM_COUNT = 148
+FP32_LANES, FP64_LANES = 128, 64
+# algorithmic instruction counts per update
+I_EULER, I_RK4, I_BTCS = 8, 36, 38
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return {"hbm_gbs": float(p["hbm_gbs"]), "sm_max_mhz": float(p.get("sm_max_mhz", 1965.0)),
+                "source": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "source": "fallback"}
+
+
+# ------------------------------------------------------------------------------- workloads
+def make_workload(name, rank=0, world=1, reduced=False):
+    """(workload, spec) -- spec: op, scheme, plan label, algorithmic instr/update, pipe lanes."""
+    from paper_2601_12204_b200 import workloads as W
+    if name in ("c2_f32", "c2_f64"):
+        dtype = np.float32 if name == "c2_f32" else np.float64
+        Bg = 1024 * world
+        w = W.c2_dirichlet_batch(B=Bg, dtype=dtype, rows=W.shard_rows(Bg, rank, world),
+                                 n_steps=1000 if reduced else 10000)
+        return w, dict(op="explicit", scheme=0, instr=I_EULER if dtype == np.float32 else 6,
+                       lanes=FP32_LANES if dtype == np.float32 else FP64_LANES)
+    if name == "c3":
+        Bg = 4096 * world
+        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
+        return w, dict(op="btcs", scheme=None, instr=I_BTCS, lanes=FP64_LANES)
+    if name == "c4a":
+        w = W.c4a_long_explicit(n_steps=200 if reduced else 2000)
+        return w, dict(op="explicit", scheme=0, instr=I_EULER, lanes=FP32_LANES)
+    if name == "c4b":
+        w = W.c4b_long_btcs(n_steps=20 if reduced else 200)
+        return w, dict(op="btcs", scheme=None, instr=I_BTCS, lanes=FP64_LANES)
+    if name == "c5":
+        Bg = 65536 * world
+        w = W.c5_rk4_ensemble(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=500 if reduced else 5000)
+        return w, dict(op="explicit", scheme=1, instr=I_RK4, lanes=FP32_LANES)
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                clk, smax = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                sm.append(clk)
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": smax,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def cpu_info():
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return model
+
+
+# ------------------------------------------------------------------------------- oracle leg
+def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
+    """Times the CPU oracle (as it stands) on a bounded sample of workload `w`: whole trajectories
+    (all n_steps) for batched configs, a shortened step count for the single long grids.
+    Returns (updates, seconds, threads, description)."""
+    import oracle
+    threads = oracle.default_threads()
+    u0 = w.u0.astype(np.float64)
+    nu = w.nu.astype(np.float64)
+    dt = oracle.dt_from_cfl(u0, w.L, nu, w.cfl, w.bc).astype(w.dtype).astype(np.float64)
+
+    def run(rows, n):
+        t0 = time.perf_counter()
+        if spec["op"] == "btcs":
+            oracle.btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+        elif w.B == 1:
+            oracle.explicit_long(u0[0], w.L, nu[0], dt[0], n, w.bc, threads=threads)
+        else:
+            oracle.explicit(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, spec["scheme"], threads=threads)
+        return time.perf_counter() - t0
+
+    if w.B == 1:      # long grid: calibrate on 2 steps, then as many steps as fit the budget
+        rows = np.arange(1)
+        t = run(rows, 2) / 2
+        n = int(max(2, min(w.n_steps, target_s / max(t, 1e-9))))
+        sec = run(rows, n)
+        return w.N * n, sec, threads, f"{n} of {w.n_steps} steps of the full N={w.N} grid"
+    nb = min(w.B, threads)
+    ncal = max(1, min(w.n_steps, 200))
+    t = run(np.arange(nb), ncal) / (nb * ncal)                 # seconds per trajectory-step (all threads busy)
+    want = int(target_s / max(t * w.n_steps, 1e-12))
+    nb = int(max(threads, min(w.B, want // threads * threads)))
+    nb = min(nb, w.B)
+    sec = run(np.arange(nb), w.n_steps)
+    return nb * w.N * w.n_steps, sec, threads, f"first {nb} of {w.B} trajectories, all {w.n_steps} steps"
+
+
+# ------------------------------------------------------------------------------- GPU legs
+class GpuRunner:
+    def __init__(self, w, spec, device):
+        import torch
+        from paper_2601_12204_b200 import binding as B
+        self.torch, self.B, self.w, self.spec = torch, B, w, spec
+        self.dev = device
+        self.u0 = torch.from_numpy(w.u0).to(device)
+        self.nu = torch.from_numpy(w.nu).to(device)
+        self.u = torch.empty_like(self.u0)
+        self.dt = torch.empty_like(self.nu)
+        is64 = w.dtype == np.float64
+        if spec["op"] == "explicit":
+            self.plan = B.plan_query(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
+            need = B.workspace_bytes(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
+            self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
+        else:
+            self.plan = B.plan_query(B.OP_BTCS, is64, w.B, w.N, w.bc)
+            need = B.workspace_bytes(B.OP_BTCS, is64, w.B, w.N, w.bc)
+            self.launches = B.launch_count(B.OP_BTCS, is64, w.B, w.N, w.bc, n_steps=w.n_steps)
+        self.launches += B.launch_count(B.OP_CFL, is64, w.B, w.N, w.bc)
+        self.ws = torch.empty(need, dtype=torch.uint8, device=device) if need else None
+        self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
+
+    def reset(self):
+        self.u.copy_(self.u0)
+        self.flush.zero_()          # L2 flush between timed iterations (outside the event pairs)
+
+    def cfl(self):
+        self.B.dt_from_cfl(self.u, self.w.L, self.nu, self.w.cfl, self.w.bc, out=self.dt)
+
+    def op(self):
+        w, B = self.w, self.B
+        if self.spec["op"] == "explicit":
+            B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
+        else:
+            B.burgers_btcs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
+
+    def timed(self, steps, warmup):
+        """Returns (list of step ms, list of op-only ms) from CUDA events on the launching stream."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.reset(); self.cfl(); self.op()
+        torch.cuda.synchronize()
+        step_ms, op_ms = [], []
+        for _ in range(steps):
+            self.reset()
+            e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            e0.record(); self.cfl(); e1.record(); self.op(); e2.record()
+            e2.synchronize()
+            step_ms.append(e0.elapsed_time(e2)); op_ms.append(e1.elapsed_time(e2))
+        return step_ms, op_ms
+
+    def e2e(self, steps, warmup):
+        """Same step through the host-buffer C-ABI calls: pinned host arrays in, result read back."""
+        torch, B, w = self.torch, self.B, self.w
+        hu0 = torch.from_numpy(w.u0).pin_memory()
+        hnu = torch.from_numpy(w.nu).pin_memory()
+        hu = torch.empty_like(hu0).pin_memory()
+        u_np, nu_np = hu.numpy(), hnu.numpy()
+        ms = []
+        for i in range(warmup + steps):
+            hu.copy_(hu0)
+            self.flush.zero_(); torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            dt = B.dt_from_cfl_host(u_np, w.L, nu_np, w.cfl, w.bc)
+            if self.spec["op"] == "explicit":
+                B.burgers_explicit_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc, self.spec["scheme"])
+            else:
+                B.burgers_btcs_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc)
+            t1 = time.perf_counter()
+            if i >= warmup:
+                ms.append((t1 - t0) * 1e3)
+        esz = w.u0.dtype.itemsize
+        h2d = 2 * w.B * w.N * esz + 3 * w.B * esz      # cfl: u, nu; step: u, nu, dt
+        d2h = w.B * w.N * esz + w.B * esz              # cfl: dt; step: u
+        return ms, h2d, d2h
+
+
+def roofline(spec, w, op_ms, pk):
+    """Dominant kernel = the time-stepping kernel(s) of the op call."""
+    sec = statistics.mean(op_ms) * 1e-3
+    ups = w.updates / sec
+    peak = SM_COUNT * spec["lanes"] * pk["sm_max_mhz"] * 1e6 / 1e9        # G lane-instr/s
+    ach = ups * spec["instr"] / 1e9
+    esz = w.u0.dtype.itemsize
+    return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Ginst/s", "frac": ach / peak,
+            "traffic": None,
+            "note": (f"{spec['instr']} algorithmic {'fp64' if spec['lanes'] == FP64_LANES else 'fp32'}-pipe "
+                     f"instr/update x updates / kernel time; peak = {SM_COUNT} SMs x {spec['lanes']} lanes x "
+                     f"{pk['sm_max_mhz']:.0f} MHz (nominal unit counts, max clock)"),
+            "hbm_accounting_frac": ups * 2 * esz / (pk["hbm_gbs"] * 1e9),
+            "hbm_peak_source": pk["source"]}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", 0)); world = int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback; see --impl reference)")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2601_12204_b200 import build as _b
+    if rank == 0:
+        _b.build()
+    if world > 1:
+        dist.barrier()
+    pk = peaks()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    w, spec = make_workload(args.workload, rank, world, args.reduced)
+    r = GpuRunner(w, spec, device)
+    sampler = ClockSampler(local)
+    barrier()
+    r.timed(0, args.warmup)
+    barrier()
+    sampler.start(); t0 = time.time()
+    step_ms, op_ms = r.timed(args.steps, 0)
+    barrier()
+    t1 = time.time()
+    clocks = sampler.stop(t0, t1)
+    ms = max_over_ranks(statistics.mean(step_ms))
+    total_updates = w.updates * world
+    value = total_updates / (ms * 1e-3)
+    out = {
+        "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
+        else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else "grid-point updates/s (B*N*steps/s), BTCS"),
+        "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {w.name}, {w.n_steps} time steps per bench step, "
+                               f"bc={'periodic' if w.bc == 0 else 'dirichlet'}, CFL {w.cfl}",
+                   "B_per_gpu": w.B, "N": w.N, "n_steps": w.n_steps, "plan": int(r.plan),
+                   "parallelism": f"batch-sharded x{world} (no collective)" if world > 1 else "single GPU",
+                   "l2": "flushed between timed steps (512 MiB memset outside the event pairs)",
+                   "input_sha256": w.sha256()[:16]},
+        "gpu_launches": int(r.launches * args.steps),
+        "clocks": clocks,
+    }
+    if rank == 0:
+        out["roofline"] = roofline(spec, w, op_ms, pk)
+        e_ms, h2d, d2h = r.e2e(max(1, min(args.steps, 3)), 1)
+        out["e2e"] = {"value": w.updates * world / (statistics.mean(e_ms) * 1e-3), "unit": "updates/s",
+                      "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                      "ms_per_step": statistics.mean(e_ms),
+                      "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
+    if world == 1 and not args.no_extras:
+        extras = {}
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5"):
+            if name == args.workload:
+                continue
+            try:
+                w2, spec2 = make_workload(name, 0, 1, args.reduced)
+                r2 = GpuRunner(w2, spec2, device)
+                if spec2["op"] == "btcs" and w2.B == 1 and r2.plan == r2.B.PLAN_THOMAS:
+                    raise RuntimeError("single long system would run on one thread (LONG plan unavailable)")
+                s_ms, o_ms = r2.timed(2, 1)
+                rf = roofline(spec2, w2, o_ms, pk)
+                extras[name] = {"workload": w2.name, "n_steps": w2.n_steps, "plan": int(r2.plan),
+                                "updates_per_s": w2.updates / (statistics.mean(s_ms) * 1e-3),
+                                "ms_per_step": statistics.mean(s_ms), "alu_frac": rf["frac"],
+                                "hbm_accounting_frac": rf["hbm_accounting_frac"],
+                                "dtype": "f32" if w2.dtype == np.float32 else "f64"}
+                del r2
+                torch.cuda.empty_cache()
+            except Exception as ex:  # a missing plan must not hide the headline number
+                extras[name] = {"error": f"{type(ex).__name__}: {ex}"}
+        out["schemes"] = extras
+    if rank == 0 and world == 1 and not args.no_cpu:
+        upd, sec, threads, desc = oracle_sample_run(w, spec)
+        out["cpu_baseline"] = {"value": upd / sec, "unit": "updates/s", "cores": threads, "kind": "oracle",
+                               "sample": desc, "cpu": cpu_info(), "seconds": sec}
+    if rank == 0:
+        print(json.dumps(out), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The reference arm of this tier is the CPU oracle, as it stands, on the host cores."""
+    if int(os.environ.get("RANK", 0)) != 0:
+        return
+    import oracle
+    oracle.build()
+    w, spec = make_workload(args.workload, 0, 1, args.reduced)
+    per = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, desc, threads = [], "", 1
+    for i in range(args.warmup + args.steps):
+        upd, sec, threads, desc = oracle_sample_run(w, spec, target_s=per)
+        if i >= args.warmup:
+            vals.append((upd, sec))
+    upd = sum(v[0] for v in vals); sec = sum(v[1] for v in vals)
+    value = upd / sec
+    out = {"impl": "reference",
+           "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
+           else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else "grid-point updates/s (B*N*steps/s), BTCS"),
+           "value": value, "unit": "updates/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": sec / max(1, len(vals)) * 1e3, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"{args.workload}: {w.name} (bounded sample per step: {desc})",
+                      "N": w.N, "n_steps": w.n_steps},
+           "cpu_baseline": {"value": value, "unit": "updates/s", "cores": threads, "kind": "oracle",
+                            "sample": desc, "cpu": cpu_info()},
+           "e2e": {"value": value, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5"])
+    ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -83,30 +83,42 @@ def c1_sine(N: int = 256, nu: float = 0.05, scheme: int = EULER, cfl: float = 0.
 
 
 def c2_dirichlet_batch(B: int = 1024, N: int = 4096, n_steps: int = 10000,
-                       dtype=np.float32, seed: int = SEED_BASE + 2) -> Workload:
-    """Config 2: B Dirichlet trajectories on [0,1], 8 sine modes, nu log-uniform."""
+                       dtype=np.float32, seed: int = SEED_BASE + 2, rows=None) -> Workload:
+    """Config 2: B Dirichlet trajectories on [0,1], 8 sine modes, nu log-uniform.
+
+    ``rows``: optional index array -- only those trajectories of the B-trajectory batch (all
+    random draws are made for the whole batch first, so a subset / shard is bit-identical to
+    the same rows of the full workload)."""
     rng = np.random.default_rng(seed)
     Z = rng.standard_normal((B, 8))
     k = np.arange(1, 9, dtype=np.float64)
     A = Z / np.sqrt(k)[None, :]                       # amplitudes ~ N(0, 1/k) (variance)
     lognu = rng.uniform(math.log(1e-3), math.log(1e-1), B)
     nu = np.exp(lognu)
+    if rows is not None:
+        rows = np.asarray(rows)
+        A, nu = A[rows], nu[rows]
     x = np.arange(N, dtype=np.float64) / (N - 1)
-    u0 = np.zeros((B, N))
+    u0 = np.zeros((len(nu), N))
     for m in range(8):
         u0 += A[:, m:m + 1] * np.sin(k[m] * math.pi * x)[None, :]
     u0[:, 0] = 0.0
     u0[:, -1] = 0.0
-    return _finish(f"C2-dirichlet-B{B}-N{N}", u0, nu, 1.0, DIRICHLET, EULER, 0.4,
+    return _finish(f"C2-dirichlet-B{len(nu)}of{B}-N{N}", u0, nu, 1.0, DIRICHLET, EULER, 0.4,
                    n_steps, dtype)
 
 
 def c3_periodic_btcs(B: int = 4096, N: int = 2048, n_steps: int = 1000,
-                     dtype=np.float64, seed: int = SEED_BASE + 3) -> Workload:
-    """Config 3: B periodic trajectories, 1 + 0.5 sum of 4 random-phase modes k<=16."""
+                     dtype=np.float64, seed: int = SEED_BASE + 3, rows=None) -> Workload:
+    """Config 3: B periodic trajectories, 1 + 0.5 sum of 4 random-phase modes k<=16.
+    ``rows`` as in :func:`c2_dirichlet_batch`."""
     rng = np.random.default_rng(seed)
     ks = np.stack([rng.permutation(16)[:4] + 1 for _ in range(B)]).astype(np.float64)
     phi = rng.uniform(0.0, 2.0 * math.pi, (B, 4))
+    if rows is not None:
+        rows = np.asarray(rows)
+        ks, phi = ks[rows], phi[rows]
+    B = len(ks)
     L = 2.0 * math.pi
     x = np.arange(N, dtype=np.float64) * (L / N)
     u0 = np.ones((B, N))
@@ -161,3 +173,13 @@ def c5_rk4_ensemble(B: int = 65536, N: int = 1024, n_steps: int = 5000,
     u0 = amp[:, None] * np.exp(-0.5 * (d / wid[:, None]) ** 2)
     return _finish(f"C5-rk4-B{len(amp)}of{B}-N{N}", u0, nu, L, PERIODIC, RK4, 0.8,
                    n_steps, dtype)
+
+
+def shard_rows(B_global: int, rank: int, world: int) -> np.ndarray:
+    """Rows of a B_global-trajectory batch owned by `rank` of `world` (contiguous, balanced to
+    within one row).  Trajectories are independent: sharding needs no collective."""
+    if not (0 <= rank < world) or B_global < 0:
+        raise ValueError("bad shard request")
+    base, rem = divmod(B_global, world)
+    lo = rank * base + min(rank, rem)
+    return np.arange(lo, lo + base + (1 if rank < rem else 0))
