@@ -192,8 +192,26 @@ def test_odd_sizes_and_signs(B):
 # ------------------------------------------------------------------ config 3 (reduced): periodic BTCS
 def test_c3_reduced_btcs_periodic(B):
     w = W.c3_periodic_btcs(B=40, N=2048, n_steps=60)
+    assert B.plan_query(B.OP_BTCS, True, w.B, w.N, w.bc) == B.PLAN_HYBRID
     check_btcs(B, w, 60)
+    check_btcs(B, w, 60, plan=B.PLAN_HYBRID)
     check_btcs(B, w, 60, plan=B.PLAN_THOMAS)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("N", [8, 16, 64, 128, 512, 1024, 4096])
+def test_btcs_hybrid_sizes_and_time_steps(B, dtype, N):
+    """HYBRID plan over its whole size range (P = 4, 8, 16; 2..256 threads), both boundary types,
+    from tiny to huge diffusion numbers (PCR early exit and the full-depth 2x2 ending)."""
+    rng = np.random.default_rng(N)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        u0 = rng.uniform(-1.5, 2.5, (3, N)).astype(dtype)
+        nu = rng.uniform(0.01, 0.1, 3).astype(dtype)
+        for C in (0.05, 10.0, 3000.0):
+            dt = oracle_dt(u0, L, nu, C, bc, dtype)
+            ref = oracle.btcs(u0.astype(np.float64), L, nu.astype(np.float64), dt.astype(np.float64), 7, bc)
+            got = run_btcs(B, u0, L, nu, dt, 7, bc, plan=B.PLAN_HYBRID)
+            assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (N, bc, C)
 
 
 def test_btcs_dirichlet_and_fp32(B):
