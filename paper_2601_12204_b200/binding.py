@@ -24,7 +24,7 @@ ERR_NULL, ERR_SHAPE, ERR_ENUM, ERR_VALUE, ERR_WORKSPACE, ERR_CUDA, ERR_PLAN = -1
 BC_PERIODIC, BC_DIRICHLET = 0, 1
 SCHEME_EULER, SCHEME_RK4 = 0, 1
 OP_EXPLICIT, OP_BTCS, OP_CFL = 0, 1, 2
-PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG = 0, 1, 2, 3, 4, 5
+PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG, PLAN_LONG_GENERAL = 0, 1, 2, 3, 4, 5, 6
 
 EXPORTS = [
     "burgers_explicit_f32", "burgers_explicit_f64", "burgers_explicit_plan_f32",

@@ -1,0 +1,141 @@
+// btcs_common.cuh -- device helpers shared by the BTCS kernels (btcs_hybrid.cu, btcs_long.cu):
+// kernel (2) "fused BTCS assembly" and the per-thread partition elimination of kernel (4).
+//
+// BTCS rows (D4; Eq.23 with the convective coefficient lagged
+// at u^n): with c = u dt/dx, r = nu dt/dx^2,
+//     sub a = -r - max(c,0),   diag b = 1 + 2r + |c|,   sup e = -r + min(c,0),   rhs d = u.
+// All three coefficients are functions of the ONE loaded value u_i^n: they are recomputed in
+// registers and never stored.  b - |a| - |e| = 1 for every dt, nu >= 0 and u (strict diagonal
+// dominance), so no elimination below needs pivoting.
+//
+// Partition elimination (one thread owns P consecutive rows 0..P-1 of its system):
+//   forward  (rows 1..P-1):  f_j x_0 + x_j + c_j x_{j+1} = q_j          [normalised, diag = 1]
+//   backward (rows P-3..1, scalars only):  row 1 as  F x_0 + x_1 + G x_{P-1} = R, which turns the
+//   thread's row 0 into an equation in (x_{-1}, x_0, x_{P-1}).  The thread's two INTERFACE rows
+//       first:  A x_{-1} + x_0 + C x_{P-1} = D         last:  f x_0 + x_{P-1} + c x_P = q
+//   (x_{-1} / x_P = last / first unknown of the neighbouring threads) form, over all threads, a
+//   tridiagonal system of 2 rows per thread that the callers solve by parallel cyclic reduction.
+//   Back substitution, once x_0 and x_{P-1} are known:  x_j = q_j - f_j x_0 - c_j x_{j+1}.
+#pragma once
+#include "common.cuh"
+
+namespace burgers {
+namespace btcs {
+
+// PCR early-exit threshold: once every off-diagonal of the (normalised) reduced rows is below
+// this, the remaining levels cannot change a bit of the answer.
+template <typename T> struct Lim;
+template <> struct Lim<double> { static __device__ __forceinline__ double tiny() { return 8.470329472543003e-22; } };  // 2^-70
+template <> struct Lim<float> { static __device__ __forceinline__ float tiny() { return 9.094947e-13f; } };          // 2^-40
+
+template <typename T> __device__ __forceinline__ T t_abs(T x);
+template <> __device__ __forceinline__ float t_abs<float>(float x) { return fabsf(x); }
+template <> __device__ __forceinline__ double t_abs<double>(double x) { return fabs(x); }
+template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
+template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
+template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
+
+template <typename T> __device__ __forceinline__ T rcp(T x) { return T(1) / x; }
+
+template <typename T>
+struct Coef {
+    T r, cx, b0;  // b0 = 1 + 2r
+    __device__ __forceinline__ void init(T nu, T dt, double inv_dx) {
+        const double dtb = (double)dt;
+        cx = (T)(dtb * inv_dx);
+        r = (T)((double)nu * dtb * inv_dx * inv_dx);
+        b0 = T(1) + T(2) * r;
+    }
+    __device__ __forceinline__ void at(T u, T &a, T &b, T &e) const {
+        const T c = u * cx;
+        const bool pos = c > T(0);
+        const T cpos = pos ? c : T(0);
+        const T cneg = pos ? T(0) : c;
+        a = -r - cpos;
+        b = b0 + t_abs(c);
+        e = -r + cneg;
+    }
+};
+
+// One interface row  A x_prev + x + C x_next = D  (normalised).
+template <typename T> struct Row { T A, C, D; };
+
+// Assembly + partition elimination of P rows held in v[].  ident(j) == true makes row j the
+// identity row x_j = v_j (Dirichlet end nodes, D5 written as part of the system; out-of-domain
+// padding).  Outputs the forward-elimination coefficients f, c, q (entries 1..P-1) and the two
+// interface rows.
+template <typename T, int P, typename Ident>
+__device__ __forceinline__ void eliminate(const T (&v)[P], const Coef<T> &co, Ident ident,
+                                          T (&f)[P], T (&c)[P], T (&q)[P], Row<T> &first,
+                                          Row<T> &last) {
+    static_assert(P >= 3, "a partition needs at least 3 rows");
+    T a0, b0, e0;
+    co.at(v[0], a0, b0, e0);
+    if (ident(0)) { a0 = T(0); b0 = T(1); e0 = T(0); }
+    {
+        T a, b, e;
+        co.at(v[1], a, b, e);
+        if (ident(1)) { a = T(0); b = T(1); e = T(0); }
+        const T m = rcp(b);
+        f[1] = a * m; c[1] = e * m; q[1] = v[1] * m;
+    }
+#pragma unroll
+    for (int j = 2; j < P; ++j) {
+        T a, b, e;
+        co.at(v[j], a, b, e);
+        if (ident(j)) { a = T(0); b = T(1); e = T(0); }
+        const T m = rcp(t_fma(-a, c[j - 1], b));
+        const T am = a * m;
+        f[j] = -am * f[j - 1];
+        c[j] = e * m;
+        q[j] = t_fma(-am, q[j - 1], v[j] * m);
+    }
+    // backward recurrence (scalars): row 1 as F x_0 + x_1 + G x_{P-1} = R
+    T F = f[P - 2], G = c[P - 2], R = q[P - 2];
+#pragma unroll
+    for (int j = P - 3; j >= 1; --j) {
+        F = t_fma(-c[j], F, f[j]);
+        G = -c[j] * G;
+        R = t_fma(-c[j], R, q[j]);
+    }
+    const T m = rcp(t_fma(-e0, F, b0));
+    first.A = a0 * m;
+    first.C = -e0 * G * m;
+    first.D = t_fma(-e0, R, v[0]) * m;
+    last.A = f[P - 1];
+    last.C = c[P - 1];
+    last.D = q[P - 1];
+}
+
+// Back substitution into v[] given the partition's end unknowns x0 = x_0, xl = x_{P-1}.
+template <typename T, int P>
+__device__ __forceinline__ void back_substitute(T (&v)[P], const T (&f)[P], const T (&c)[P],
+                                                const T (&q)[P], T x0, T xl) {
+    v[0] = x0; v[P - 1] = xl;
+    T xn = xl;
+#pragma unroll
+    for (int j = P - 2; j >= 1; --j) {
+        xn = t_fma(-c[j], xn, t_fma(-f[j], x0, q[j]));
+        v[j] = xn;
+    }
+}
+
+// One PCR combination: row k with its neighbours km (k - s) and kp (k + s), all normalised.
+template <typename T>
+__device__ __forceinline__ Row<T> pcr_combine(const Row<T> &k, const Row<T> &km, const Row<T> &kp) {
+    const T m = rcp(t_fma(-k.A, km.C, t_fma(-k.C, kp.A, T(1))));
+    Row<T> n;
+    n.A = -k.A * km.A * m;
+    n.C = -k.C * kp.C * m;
+    n.D = t_fma(-k.A, km.D, t_fma(-k.C, kp.D, k.D)) * m;
+    return n;
+}
+
+constexpr int max_threads_for_regs(int regs) {
+    int t = 1024;
+    while (t > 32 && t * regs > 65536) t /= 2;
+    return t;
+}
+
+}  // namespace btcs
+}  // namespace burgers

@@ -22,37 +22,12 @@
 //  4. back substitution inside each thread: x_j = q_j - f_j x_0 - c_j x_{j+1}, j = P-2..1.
 // Periodic systems are solved directly as cyclic systems (no Sherman-Morrison second right-hand
 // side); the result equals D6's up to rounding.
-#include "common.cuh"
+#include "btcs_common.cuh"
 
 namespace burgers {
 namespace {
 
-template <typename T> struct Lim;
-template <> struct Lim<double> { static __device__ __forceinline__ double tiny() { return 8.470329472543003e-22; } };  // 2^-70
-template <> struct Lim<float> { static __device__ __forceinline__ float tiny() { return 9.094947e-13f; } };          // 2^-40
-
-template <typename T> __device__ __forceinline__ T t_abs(T x);
-template <> __device__ __forceinline__ float t_abs<float>(float x) { return fabsf(x); }
-template <> __device__ __forceinline__ double t_abs<double>(double x) { return fabs(x); }
-template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
-template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
-template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
-
-template <typename T> __device__ __forceinline__ T rcp(T x) { return T(1) / x; }
-
-template <typename T>
-struct Coef {
-    T r, cx, b0;  // b0 = 1 + 2r
-    __device__ __forceinline__ void at(T u, T &a, T &b, T &e) const {
-        const T c = u * cx;
-        const bool pos = c > T(0);
-        const T cpos = pos ? c : T(0);
-        const T cneg = pos ? T(0) : c;
-        a = -r - cpos;
-        b = b0 + t_abs(c);
-        e = -r + cneg;
-    }
-};
+using namespace btcs;
 
 constexpr int hybrid_max_threads(int bytes, int P) {
     int regs = P * (bytes / 4) * 4 + 48;
@@ -73,11 +48,8 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
     T *sD = sC + 2 * M;
     T *row = u + (int64_t)blockIdx.x * N + (int64_t)t * P;
 
-    const double dtb = (double)dt[blockIdx.x];
     Coef<T> co;
-    co.cx = (T)(dtb * inv_dx);
-    co.r = (T)((double)nu[blockIdx.x] * dtb * inv_dx * inv_dx);
-    co.b0 = T(1) + T(2) * co.r;
+    co.init(nu[blockIdx.x], dt[blockIdx.x], inv_dx);
     const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
     const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
 
@@ -93,43 +65,15 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
     int cur = 0;
     for (int64_t n = 0; n < n_steps; ++n) {
         T f[P], c[P], q[P];
-        // ---- assembly + forward elimination
-        T a0, b0, e0;
-        co.at(v[0], a0, b0, e0);
-        const T d0 = v[0];
-        if (fixL) { a0 = T(0); b0 = T(1); e0 = T(0); }
+        // ---- assembly + partition elimination; interface rows -> shared memory, buffer cur^1
         {
-            T a, b, e;
-            co.at(v[1], a, b, e);
-            const T m = rcp(b);
-            f[1] = a * m; c[1] = e * m; q[1] = v[1] * m;
-        }
-#pragma unroll
-        for (int j = 2; j < P; ++j) {
-            T a, b, e;
-            co.at(v[j], a, b, e);
-            if (j == P - 1 && fixR) { a = T(0); b = T(1); e = T(0); }
-            const T m = rcp(t_fma(-a, c[j - 1], b));
-            const T am = a * m;
-            f[j] = -am * f[j - 1];
-            c[j] = e * m;
-            q[j] = t_fma(-am, q[j - 1], v[j] * m);
-        }
-        // ---- backward recurrence (scalars): row 1 as F x_0 + x_1 + G x_{P-1} = R
-        T F = f[P - 2], G = c[P - 2], R = q[P - 2];
-#pragma unroll
-        for (int j = P - 3; j >= 1; --j) {
-            F = t_fma(-c[j], F, f[j]);
-            G = -c[j] * G;
-            R = t_fma(-c[j], R, q[j]);
-        }
-        // ---- interface rows (normalised) -> shared memory, buffer cur^1
-        {
-            const T m = rcp(t_fma(-e0, F, b0));
+            Row<T> first, last;
+            eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
+                            f, c, q, first, last);
             const int o = (cur ^ 1) * M + 2 * t;
-            sA[o] = a0 * m;           sA[o + 1] = f[P - 1];
-            sC[o] = -e0 * G * m;      sC[o + 1] = c[P - 1];
-            sD[o] = t_fma(-e0, R, d0) * m;  sD[o + 1] = q[P - 1];
+            sA[o] = first.A; sA[o + 1] = last.A;
+            sC[o] = first.C; sC[o + 1] = last.C;
+            sD[o] = first.D; sD[o + 1] = last.D;
         }
         __syncthreads();
         cur ^= 1;
@@ -167,14 +111,7 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
             cur ^= 1;
         }
         // ---- back substitution
-        const T x0 = sD[cur * M + 2 * t], xl = sD[cur * M + 2 * t + 1];
-        v[0] = x0; v[P - 1] = xl;
-        T xn = xl;
-#pragma unroll
-        for (int j = P - 2; j >= 1; --j) {
-            xn = t_fma(-c[j], xn, t_fma(-f[j], x0, q[j]));
-            v[j] = xn;
-        }
+        back_substitute<T, P>(v, f, c, q, sD[cur * M + 2 * t], sD[cur * M + 2 * t + 1]);
     }
 
 #pragma unroll

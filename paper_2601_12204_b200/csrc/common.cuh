@@ -60,11 +60,14 @@ int launch_btcs_hybrid(T *u, int64_t B, int64_t N, double dx, const T *nu, const
                        int64_t n_steps, int bc, cudaStream_t s);
 bool btcs_hybrid_fits(int is_f64, int64_t N, int bc);
 
+// LONG: one system across many CTAs.  `ws` holds the ping-pong state, the global interface rows
+// and the status word (btcs_long_ws_bytes).  general_only != 0 runs the cooperative GENERAL
+// kernel alone (BURGERS_PLAN_LONG_GENERAL).
 template <typename T>
 int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
-                     int64_t n_steps, int bc, T *ws, cudaStream_t s);
-size_t btcs_long_ws_elems(int64_t B, int64_t N, int bc);
-int64_t btcs_long_launch_count(int64_t B, int64_t N, int64_t n_steps);
+                     int64_t n_steps, int bc, void *ws, int general_only, cudaStream_t s);
+size_t btcs_long_ws_bytes(int esz, int64_t B, int64_t N);
+int64_t btcs_long_launch_count(int64_t n_steps, int general_only);
 bool btcs_long_fits(int64_t N, int bc);
 
 }  // namespace burgers

@@ -69,6 +69,9 @@ def test_argument_errors_are_synchronous(B):
     hp = lib.burgers_btcs_plan_f64
     assert hp(one, 1, 8, 1.0, one, one, 1, 0, B.PLAN_THOMAS, None, 0, None) == B.ERR_WORKSPACE
     assert hp(one, 1, 8, 1.0, one, one, 1, 0, B.PLAN_RESIDENT, None, 0, None) == B.ERR_ENUM
+    assert hp(one, 1, 1000, 1.0, one, one, 1, 0, B.PLAN_LONG, None, 0, None) == B.ERR_PLAN
+    assert hp(one, 1, 1 << 16, 1.0, one, one, 1, 0, B.PLAN_LONG, None, 0, None) == B.ERR_WORKSPACE
+    assert hp(one, 1, 1 << 16, 1.0, one, one, 1, 0, B.PLAN_LONG_GENERAL, None, 0, None) == B.ERR_WORKSPACE
     c = lib.dt_from_cfl_f32
     assert c(None, 1, 8, 1.0, one, 0.4, 0, one, None) == B.ERR_NULL
     assert c(one, 1, 8, 1.0, one, 0.0, 0, one, None) == B.ERR_VALUE
@@ -94,6 +97,16 @@ def test_plan_queries(B):
     assert B.launch_count(B.OP_EXPLICIT, False, 1024, 4096, 1, 0, n_steps=10000) == 1
     assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=2000, tblock=16) == 125
     assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=0) == 0
+    # BTCS: C3 fits one CTA per system (HYBRID); C4b is one long system across CTAs (LONG);
+    # shapes neither fits fall back to the thread-per-system Thomas plan
+    assert B.plan_query(B.OP_BTCS, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
+    assert B.plan_query(B.OP_BTCS, True, 1, 1 << 22, B.BC_PERIODIC) == B.PLAN_LONG
+    assert B.plan_query(B.OP_BTCS, True, 3, 3001, B.BC_PERIODIC) == B.PLAN_THOMAS
+    assert B.launch_count(B.OP_BTCS, True, 4096, 2048, 0, n_steps=1000) == 1
+    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=200) == 202
+    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, plan=B.PLAN_LONG_GENERAL, n_steps=200) == 1
+    assert B.workspace_bytes(B.OP_BTCS, True, 1, 1 << 22, 0) >= int(2.5 * 8 * (1 << 22))
+    assert B.workspace_bytes(B.OP_BTCS, True, 1, 1000, 0, 0, B.PLAN_LONG) == 0      # does not fit
     assert B.launch_count(B.OP_CFL, False, 1024, 4096, 1) == 1
     assert B.launch_count(B.OP_CFL, False, 1, 1 << 24, 0) == 2
 

@@ -225,9 +225,55 @@ def test_btcs_dirichlet_and_fp32(B):
 
 
 def test_c4b_reduced_long_btcs(B):
+    """One long cyclic system across many CTAs (a7): the AUTO plan is LONG; its two device paths
+    (overlapped tiles with the checked truncated PCR; cooperative global PCR) and the
+    thread-per-system Thomas plan all agree with the oracle (G10)."""
     w = W.c4b_long_btcs(N=1 << 16, n_steps=12)
+    assert B.plan_query(B.OP_BTCS, True, w.B, w.N, w.bc) == B.PLAN_LONG
     check_btcs(B, w, 12)
+    check_btcs(B, w, 12, plan=B.PLAN_LONG)
+    check_btcs(B, w, 12, plan=B.PLAN_LONG_GENERAL)
     check_btcs(B, w, 12, plan=B.PLAN_THOMAS)
+    check_btcs(B, w, 5, plan=B.PLAN_LONG)             # odd step count: result ends in the workspace
+    w2 = W.c4b_long_btcs(N=1 << 18, n_steps=7)
+    check_btcs(B, w2, 7)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("C", [0.05, 10.0, 40.0, 3000.0])
+def test_btcs_long_batches_boundaries_and_fallback(B, dtype, C):
+    """LONG plan on small batches of long systems, both boundary types, mixed-sign data, from tiny
+    to huge diffusion numbers.  C = 10 is BASELINE's "10x the explicit limit"; at C = 40 and 3000
+    the couplings decay too slowly for the 128-point halo, so the tiled kernels must detect it
+    (status word) and the cooperative kernel must take over from the failing step."""
+    rng = np.random.default_rng(int(C * 100) + 1)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        N = 1 << 14
+        x = np.arange(N) / N
+        u0 = np.stack([a * np.sin(2 * math.pi * k * x + p) + m for a, k, p, m in
+                       zip(rng.uniform(0.5, 2, 3), (1, 3, 7), rng.uniform(0, 6, 3), (-0.4, 0.0, 1.0))]).astype(dtype)
+        nu = rng.uniform(0.01, 0.1, 3).astype(dtype)
+        dt = oracle_dt(u0, L, nu, C, bc, dtype)
+        ref = oracle.btcs(u0.astype(np.float64), L, nu.astype(np.float64), dt.astype(np.float64), 6, bc)
+        for plan in (B.PLAN_LONG, B.PLAN_LONG_GENERAL):
+            got = run_btcs(B, u0, L, nu, dt, 6, bc, plan=plan)
+            assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (bc, C, plan)
+
+
+def test_btcs_long_convection_dominated_and_step_split(B):
+    """nu tiny: the matrix is one-sided (|sub| ~ c, |sup| ~ 0 where u > 0), the slowest-decaying
+    case for a given Courant number; and p then q steps == p+q steps bitwise (G6-v)."""
+    N = 1 << 15
+    x = np.arange(N) * (2 * math.pi / N)
+    u0 = (1.0 + 0.8 * np.sin(x) * np.cos(3 * x))[None, :]
+    nu = np.array([1e-7]); L = 2 * math.pi
+    for C in (2.0, 10.0):
+        dt = oracle_dt(u0, L, nu, C, B.BC_PERIODIC, np.float64)
+        ref = oracle.btcs(u0, L, nu, dt, 9, B.BC_PERIODIC)
+        a = run_btcs(B, u0, L, nu, dt, 9, B.BC_PERIODIC)
+        assert rel_err(a, ref, u0) <= 1e-10, C
+        b = run_btcs(B, run_btcs(B, u0, L, nu, dt, 4, B.BC_PERIODIC), L, nu, dt, 5, B.BC_PERIODIC)
+        np.testing.assert_array_equal(a, b)
 
 
 # ------------------------------------------------------------------ semantics
