@@ -35,7 +35,27 @@ template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
 template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
 template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
 
-template <typename T> __device__ __forceinline__ T rcp(T x) { return T(1) / x; }
+// Reciprocal of a pivot.  Every pivot of the eliminations here lies in a benign range (partition
+// pivots are >= 1 by diagonal dominance, PCR pivots in (0, 1]), so the IEEE division's special-case
+// handling (denormals, overflow: ~25 SASS instructions with a slow-path branch in fp64) buys
+// nothing: hardware approximation (MUFU.RCP64H / MUFU.RCP) + Newton steps, error <= ~1 ulp.
+// NaN / Inf still propagate.
+template <typename T> __device__ __forceinline__ T rcp(T x);
+template <> __device__ __forceinline__ double rcp<double>(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));   // ~20 good bits
+    double e = fma(-x, y, 1.0);
+    e = fma(e, e, e);
+    y = fma(y, e, y);                                        // cubic step: ~60 bits
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);                                     // rounding-limited
+}
+template <> __device__ __forceinline__ float rcp<float>(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    const float e = fmaf(-x, y, 1.0f);
+    return fmaf(y, e, y);
+}
 
 template <typename T>
 struct Coef {

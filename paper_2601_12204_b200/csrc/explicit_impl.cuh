@@ -14,9 +14,15 @@
 // neighbouring threads by warp shuffle (CTA of one warp) or through a double-buffered shared
 // memory edge array with ONE barrier per exchange (several warps).
 //
-// Arithmetic per point (D2, scaled by dt): with cx = dt/dx, rr = nu dt/dx^2, l/c/r the left,
-// centre and right values and w = (c > 0 ? l : r) the upwind neighbour,
-//   dt*F = rr*(l + r - 2c) - cx*|c|*(c - w)          [ u*g == |u|*(u - w) for either sign ]
+// Arithmetic per point (D2, scaled by dt): with hcx = dt/(2 dx), rr = nu dt/dx^2 and l/c/r the
+// left, centre and right values, the sign-switched upwind difference of PAPER.md:89 is written in
+// its branch-free "central difference + numerical diffusion" form
+//   u_i g_i = u_i (u_{i+1} - u_{i-1})/2 - |u_i| (u_{i+1} - 2u_i + u_{i-1})/2     (either sign of u_i)
+// so that
+//   dt*F = (rr + hcx*|c|) * (l + r - 2c) - hcx*c*(r - l)
+// which is 7 FMA-pipe instructions and no compare/select (the select form costs 7 + 2): the
+// kernels are issue-bound, so instructions per update are what matters.
+// It equals D2 up to rounding, keeps constants exactly fixed and keeps odd symmetry exact.
 // fp32 Euler carries the state as base + s (two fp32 terms; increments are accumulated into the
 // small term s, so they are not lost against ulp(u)) -- the stencil reads the
 // rounded sum v = fl(base + s).
@@ -49,13 +55,20 @@ template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
 template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
 template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
 
-// dt*F at one point (D2).  7 FP instructions + compare/select.
+// dt*F at one point (D2) added to `acc`:  acc + (rr + hcx|c|) lap - hcx c (r - l).  7 FP instructions.
 template <typename T>
-__device__ __forceinline__ T dtF(T l, T c, T r, T cx, T rr) {
-    const T w = (c > T(0)) ? l : r;              // upwind neighbour (0 -> forward, Q3)
+__device__ __forceinline__ T add_dtF(T acc, T l, T c, T r, T hcx, T rr) {
     const T lap = t_fma(T(-2), c, l + r);        // u_{i+1} - 2u_i + u_{i-1}   (Eq.4)
-    const T a = cx * t_abs(c);
-    return t_fma(-a, c - w, rr * lap);
+    const T k = t_fma(hcx, t_abs(c), rr);        // diffusion number + upwind numerical diffusion
+    const T e = hcx * c;
+    return t_fma(-e, r - l, t_fma(k, lap, acc));
+}
+template <typename T>
+__device__ __forceinline__ T dtF(T l, T c, T r, T hcx, T rr) {
+    const T lap = t_fma(T(-2), c, l + r);
+    const T k = t_fma(hcx, t_abs(c), rr);
+    const T e = hcx * c;
+    return t_fma(-e, r - l, k * lap);
 }
 
 // Halo exchange: every thread publishes its first and last point and receives the last point
@@ -109,7 +122,7 @@ explicit_kernel(const Params<T> p) {
 
     // per-trajectory constants, evaluated in fp64 and rounded once
     const double dtb = (double)p.dt[b];
-    const T cx = (T)(dtb * p.inv_dx);
+    const T hcx = (T)(0.5 * dtb * p.inv_dx);
     const T rr = (T)((double)p.nu[b] * dtb * p.inv_dx * p.inv_dx);
 
     // ---------------- load
@@ -176,16 +189,12 @@ explicit_kernel(const Params<T> p) {
                 const T r = (j + 1 < P) ? v[j + 1] : right;
                 const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
                 if (SPLIT) {
-                    const T w = (c > T(0)) ? l : r;
-                    const T lap = t_fma(T(-2), c, l + r);
-                    const T a = cx * t_abs(c);
-                    T sn = t_fma(rr, lap, s[j]);
-                    sn = t_fma(-a, c - w, sn);
+                    const T sn = add_dtF<T>(s[j], l, c, r, hcx, rr);
                     s[j] = frozen ? s[j] : sn;
                     v[j] = base[j] + s[j];
                 } else {
-                    const T inc = dtF<T>(l, c, r, cx, rr);
-                    v[j] = frozen ? c : c + inc;
+                    const T vn = add_dtF<T>(c, l, c, r, hcx, rr);
+                    v[j] = frozen ? c : vn;
                 }
                 l = c;
             }
@@ -211,7 +220,7 @@ explicit_kernel(const Params<T> p) {
                     const T c = (stage == 0) ? v[j] : y[j];
                     const T r = (j + 1 < P) ? ((stage == 0) ? v[j + 1] : y[j + 1]) : right;
                     const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
-                    T K = dtF<T>(l, c, r, cx, rr);
+                    T K = dtF<T>(l, c, r, hcx, rr);
                     K = frozen ? T(0) : K;
                     if (stage == 0) { acc[j] = K; y[j] = t_fma(T(0.5), K, v[j]); }
                     else if (stage == 1) { acc[j] = t_fma(T(2), K, acc[j]); y[j] = t_fma(T(0.5), K, v[j]); }
