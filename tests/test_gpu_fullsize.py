@@ -1,0 +1,162 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (AUTO plan,
+dt from the library's own dt_from_cfl, one call for all n_steps).
+
+The oracle cannot run the full configs in seconds, so it checks SAMPLED outputs it can compute one
+by one, exactly:
+  - batched configs (C2, C3, C5): trajectories are independent, so the oracle runs a seeded sample
+    of whole trajectories (all steps) and every point of those is compared;
+  - single long grids (C4a, C4b): the oracle runs WINDOWS of the grid.  Explicit Euler has a
+    numerical domain of dependence of exactly one cell per step, so the central part of a window
+    with a margin of n_steps cells is exact whatever is done at the window ends.  BTCS couples all
+    points, but the influence of a point decays per cell like lam = ((1+2r) - sqrt(1+4r)) / (2r)
+    per step (Green's function of the diffusion part; convection only strengthens the diagonal):
+    at r = 5, lam = 0.642, i.e. < 1e-12 beyond 63 cells per step, so a margin of 64*n_steps cells
+    makes the window's centre exact to far below the 1e-10 tolerance;
+plus properties that hold at any size, checked on ALL outputs: finiteness, the discrete maximum
+principle (D4 / D9), frozen Dirichlet ends, and for BTCS the defining residual
+A(u^n) u^{n+1} = u^n of the last step evaluated in fp64 numpy over the whole grid.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from parity import TOL, rel_err, to_dev
+from paper_2601_12204_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_12204_b200 import binding
+    return binding
+
+
+def _gpu_pass(B, w, scheme):
+    """One bench.py pass: dt_from_cfl then the time-stepping call (AUTO plan).  Returns (u, dt)."""
+    u, nu = to_dev(w.u0.copy()), to_dev(w.nu)
+    dt = B.dt_from_cfl(u, w.L, nu, w.cfl, w.bc)
+    if scheme is None:
+        B.burgers_btcs(u, w.L, nu, dt, w.n_steps, w.bc)
+    else:
+        B.burgers_explicit(u, w.L, nu, dt, w.n_steps, w.bc, scheme)
+    return u.cpu().numpy(), dt.cpu().numpy()
+
+
+def _check_dt(w, dt):
+    ref = oracle.dt_from_cfl(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64), w.cfl, w.bc).astype(w.dtype)
+    assert np.all(np.abs(dt - ref) <= 2 * np.spacing(np.abs(ref)))
+
+
+def _max_principle(got, u0, slack):
+    assert np.all(np.isfinite(got))
+    hi, lo = u0.max(axis=1).astype(np.float64), u0.min(axis=1).astype(np.float64)
+    s = slack * np.abs(u0).max(axis=1).astype(np.float64)
+    assert np.all(got.max(axis=1) <= hi + s) and np.all(got.min(axis=1) >= lo - s)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_c2_full(B, dtype):
+    w = W.c2_dirichlet_batch(dtype=dtype)                          # B=1024, N=4096, 10 000 steps
+    assert B.plan_query(B.OP_EXPLICIT, dtype == np.float64, w.B, w.N, w.bc, 0) == B.PLAN_RESIDENT
+    got, dt = _gpu_pass(B, w, B.SCHEME_EULER)
+    _check_dt(w, dt)
+    rows = np.sort(np.random.default_rng(2).choice(w.B, 24, replace=False))
+    rows[0], rows[-1] = 0, w.B - 1
+    ref = oracle.explicit(w.u0[rows].astype(np.float64), w.L, w.nu[rows].astype(np.float64),
+                          dt[rows].astype(np.float64), w.n_steps, w.bc, oracle.EULER)
+    assert rel_err(got[rows], ref, w.u0[rows]) <= TOL[np.dtype(dtype)]
+    np.testing.assert_array_equal(got[:, 0], w.u0[:, 0])
+    np.testing.assert_array_equal(got[:, -1], w.u0[:, -1])
+    _max_principle(got, w.u0, 1e-5 if dtype == np.float32 else 1e-12)   # |c| + 2r <= 0.8: monotone
+
+
+def test_c3_full(B):
+    w = W.c3_periodic_btcs()                                       # B=4096, N=2048, 1 000 steps
+    assert B.plan_query(B.OP_BTCS, True, w.B, w.N, w.bc) == B.PLAN_HYBRID
+    got, dt = _gpu_pass(B, w, None)
+    _check_dt(w, dt)
+    rows = np.sort(np.random.default_rng(3).choice(w.B, 24, replace=False))
+    rows[0], rows[-1] = 0, w.B - 1
+    ref = oracle.btcs(w.u0[rows], w.L, w.nu[rows], dt[rows], w.n_steps, w.bc)
+    assert rel_err(got[rows], ref, w.u0[rows]) <= 1e-10
+    _max_principle(got, w.u0, 1e-12)                               # M-matrix: any dt
+
+
+def test_c5_full(B):
+    w = W.c5_rk4_ensemble()                                        # B=65536, N=1024, 5 000 RK4 steps
+    assert B.plan_query(B.OP_EXPLICIT, False, w.B, w.N, w.bc, 1) == B.PLAN_RESIDENT
+    got, dt = _gpu_pass(B, w, B.SCHEME_RK4)
+    _check_dt(w, dt)
+    rows = np.arange(0, w.B, 4096)                                 # 16 trajectories
+    rows[-1] = w.B - 1
+    ref = oracle.explicit(w.u0[rows].astype(np.float64), w.L, w.nu[rows].astype(np.float64),
+                          dt[rows].astype(np.float64), w.n_steps, w.bc, oracle.RK4)
+    assert rel_err(got[rows], ref, w.u0[rows]) <= 1e-4
+    assert np.all(np.isfinite(got))
+    # RK4 is not monotone, but these pulses only decay: bounded by the initial range (+ rounding)
+    _max_principle(got, w.u0, 1e-3)
+
+
+def _window(u0_row, start, width):
+    idx = (start + np.arange(width)) % u0_row.shape[0]
+    return idx, u0_row[idx]
+
+
+def test_c4a_full_windows(B):
+    w = W.c4a_long_explicit()                                      # N=2^24, 2 000 Euler steps, fp32
+    assert B.plan_query(B.OP_EXPLICIT, False, 1, w.N, w.bc, 0) == B.PLAN_TILED
+    got, dt = _gpu_pass(B, w, B.SCHEME_EULER)
+    _check_dt(w, dt)
+    n, N = w.n_steps, w.N
+    margin, width = n + 8, 1 << 16
+    # the grid wrap, both smoothed steps, a tile boundary region and a flat part
+    for start in (N - width // 2, N // 4 - width // 2, 3 * N // 4 - width // 2, 5 * 4064 * 100 - 77, N // 2):
+        idx, win = _window(w.u0[0], start, width)
+        # same dx as the full grid: Dirichlet window of `width` nodes has dx = Lw/(width-1)
+        Lw = (w.L / N) * (width - 1)
+        ref = oracle.explicit(win[None, :].astype(np.float64), Lw, w.nu.astype(np.float64),
+                              dt.astype(np.float64), n, oracle.DIRICHLET, oracle.EULER)[0]
+        c = slice(margin, width - margin)
+        err = np.abs(got[0, idx[c]].astype(np.float64) - ref[c]).max() / np.abs(w.u0).max()
+        assert err <= 1e-4, (start, err)
+    _max_principle(got, w.u0, 1e-5)
+
+
+def test_c4b_full_windows_and_residual(B):
+    w = W.c4b_long_btcs()                                          # N=2^22, 200 BTCS steps, fp64
+    assert B.plan_query(B.OP_BTCS, True, 1, w.N, w.bc) == B.PLAN_LONG
+    u, nu = to_dev(w.u0.copy()), to_dev(w.nu)
+    dt_d = B.dt_from_cfl(u, w.L, nu, w.cfl, w.bc)
+    B.burgers_btcs(u, w.L, nu, dt_d, w.n_steps - 1, w.bc)
+    prev = u.cpu().numpy()[0].copy()
+    B.burgers_btcs(u, w.L, nu, dt_d, 1, w.bc)
+    got = u.cpu().numpy()
+    dt = dt_d.cpu().numpy()
+    _check_dt(w, dt)
+    # in one call too (the bench configuration): p then q steps == p+q steps, bitwise
+    one, _ = _gpu_pass(B, w, None)
+    np.testing.assert_array_equal(one, got)
+    # residual of the last step over the whole grid, fp64 numpy (D4 written out)
+    N = w.N
+    dx = w.L / N
+    c = prev * dt[0] / dx
+    r = w.nu[0] * dt[0] / dx ** 2
+    x = got[0]
+    res = (-r - np.maximum(c, 0)) * np.roll(x, 1) + (1 + 2 * r + np.abs(c)) * x + (-r + np.minimum(c, 0)) * np.roll(x, -1) - prev
+    assert np.abs(res).max() <= 1e-13 * (1 + 4 * r), np.abs(res).max()
+    # windows against the oracle (margin: 64 cells per step, see the module docstring)
+    lam = ((1 + 2 * r) - math.sqrt(1 + 4 * r)) / (2 * r)
+    assert lam ** 64 < 1e-12
+    n = w.n_steps
+    margin, width = 64 * n, 1 << 16
+    for start in (N - width // 2, N // 4 - width // 2, 3 * N // 4 - width // 2):
+        idx, win = _window(w.u0[0], start, width)
+        Lw = dx * (width - 1)
+        ref = oracle.btcs(win[None, :], Lw, w.nu, dt, n, oracle.DIRICHLET)[0]
+        cc = slice(margin, width - margin)
+        err = np.abs(got[0, idx[cc]] - ref[cc]).max() / np.abs(w.u0).max()
+        assert err <= 1e-10, (start, err)
+    _max_principle(got, w.u0, 1e-12)

@@ -1,0 +1,96 @@
+"""N>1 host logic on CPU: two `gloo` ranks (world_size 2) shard a batched workload the way
+`bench.py --gpus 2` does (contiguous trajectory slices, no data-path
+collective), and the pieces are checked against the unsharded batch:
+  - every rank's shard is bit-identical to the same rows of the full workload,
+  - the shards tile the batch exactly (no row lost or duplicated),
+  - stepping the shards independently (here: with the CPU oracle, the only stepper that runs
+    without a GPU) and concatenating equals stepping the whole batch -- i.e. sharding needs no
+    exchange,
+  - the max-over-ranks reduction bench.py uses for its timing returns the slowest rank's value.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+from paper_2601_12204_b200 import workloads as W
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _rank_main(rank, world, port, Bg, out):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import oracle
+        rows = W.shard_rows(Bg, rank, world)
+        results = {}
+        for name, make, stepper in (
+            ("c2", lambda r: W.c2_dirichlet_batch(B=Bg, N=128, dtype=np.float64, rows=r),
+             lambda w, dt: oracle.explicit(w.u0, w.L, w.nu, dt, 40, w.bc, oracle.EULER, threads=1)),
+            ("c3", lambda r: W.c3_periodic_btcs(B=Bg, N=64, rows=r),
+             lambda w, dt: oracle.btcs(w.u0, w.L, w.nu, dt, 5, w.bc, threads=1)),
+            ("c5", lambda r: W.c5_rk4_ensemble(B=Bg, N=64, dtype=np.float64, rows=r),
+             lambda w, dt: oracle.explicit(w.u0, w.L, w.nu, dt, 20, w.bc, oracle.RK4, threads=1)),
+        ):
+            w = make(rows)
+            dt = oracle.dt_from_cfl(w.u0, w.L, w.nu, w.cfl, w.bc)      # per trajectory: no all-reduce
+            u = stepper(w, dt)
+            # gather (rows, u0, dt, u) on every rank -- test plumbing only, not the data path
+            gathered = [None] * world
+            dist.all_gather_object(gathered, (rows, w.u0, dt, u))
+            results[name] = gathered
+        # bench.py's timing reduction: max over ranks
+        t = torch.tensor([10.0 + rank], dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        results["max_ms"] = float(t.item())
+        dist.barrier()
+        if rank == 0:
+            torch.save(results, out)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+def test_two_rank_batch_sharding_matches_full_batch(tmp_path):
+    import oracle
+    oracle.build()
+    world, Bg = 2, 7                      # odd batch: ragged shards (4 + 3)
+    out = str(tmp_path / "res.pt")
+    mp.spawn(_rank_main, args=(world, _free_port(), Bg, out), nprocs=world, join=True)
+    res = torch.load(out, weights_only=False)
+    assert res["max_ms"] == 11.0
+    full = {
+        "c2": (W.c2_dirichlet_batch(B=Bg, N=128, dtype=np.float64),
+               lambda w, dt: oracle.explicit(w.u0, w.L, w.nu, dt, 40, w.bc, oracle.EULER)),
+        "c3": (W.c3_periodic_btcs(B=Bg, N=64), lambda w, dt: oracle.btcs(w.u0, w.L, w.nu, dt, 5, w.bc)),
+        "c5": (W.c5_rk4_ensemble(B=Bg, N=64, dtype=np.float64),
+               lambda w, dt: oracle.explicit(w.u0, w.L, w.nu, dt, 20, w.bc, oracle.RK4)),
+    }
+    for name, (w, stepper) in full.items():
+        parts = res[name]
+        rows = np.concatenate([p[0] for p in parts])
+        np.testing.assert_array_equal(rows, np.arange(Bg))                      # exact tiling
+        np.testing.assert_array_equal(np.concatenate([p[1] for p in parts]), w.u0)   # same inputs
+        dt = oracle.dt_from_cfl(w.u0, w.L, w.nu, w.cfl, w.bc)
+        np.testing.assert_array_equal(np.concatenate([p[2] for p in parts]), dt)
+        np.testing.assert_array_equal(np.concatenate([p[3] for p in parts]), stepper(w, dt))
+
+
+def test_shard_rows_properties():
+    for Bg in (0, 1, 5, 1024, 65536 + 3):
+        for world in (1, 2, 3, 8):
+            parts = [W.shard_rows(Bg, r, world) for r in range(world)]
+            np.testing.assert_array_equal(np.concatenate(parts), np.arange(Bg))
+            sizes = [len(p) for p in parts]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        W.shard_rows(8, 2, 2)
