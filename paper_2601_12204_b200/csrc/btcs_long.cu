@@ -5,16 +5,18 @@
 // is solved exactly (to rounding) by partition elimination + parallel cyclic reduction, as in
 // btcs_hybrid.cu, with the interface system now spanning CTAs.  Two device paths:
 //
-//  TILED (fast path, one launch per time step, ping-pong u <-> ws): every CTA owns W consecutive
-//    points of one system and loads them with a halo of Hp points per side.  Its threads eliminate
-//    their P-row partitions, and the CTA runs PCR on its 2*Tn interface rows as an OPEN chain (the
-//    couplings leaving the tile are dropped).  The wrong rows at the two tile ends contaminate,
-//    after j PCR levels, only the 2^j outermost rows; the matrix is strictly diagonally dominant,
-//    so the off-diagonals of the reduced rows decay (quadratically per level) and the owned rows
-//    are normally finished (all |A|,|C| < 2^-70 fp64 / 2^-40 fp32: x_k = D_k to the last bit)
-//    before the contamination has crossed the halo.  The CTA CHECKS this: if after the J levels
-//    the halo allows some owned row is not finished, it records the failing step in the status
-//    word and every later TILED launch returns at once, leaving u^n of the failing step intact.
+//  TILED (fast path, one launch per time step, ping-pong u <-> ws): every tile of kW consecutive
+//    points of one system is loaded with a halo of kHaloL / kHaloR threads (x kTP points) per side.
+//    Its threads eliminate their kTP-row partitions, one in-CTA cyclic-reduction step leaves ONE
+//    reduced row per thread, and the CTA runs PCR on these rows as an OPEN chain (the couplings
+//    leaving the tile are dropped).  The wrong rows at the two tile ends contaminate, after j PCR
+//    levels, only the 2^j outermost threads; the matrix is strictly diagonally dominant, so the
+//    off-diagonals of the reduced rows decay (quadratically per level) and the owned rows are
+//    normally finished (all |A|,|C| < 2^-70 fp64 / 2^-40 fp32) before the contamination has
+//    crossed the halo.  The CTA CHECKS this: if after the kLevels levels the halo allows some
+//    needed row is not finished, it records the failing step in the status word and every later
+//    TILED launch returns at once, leaving u^n of the failing step intact.  The kernel is
+//    persistent within a step (grid = SMs x resident CTAs) and software-pipelined with cp.async.
 //  GENERAL (cooperative persistent kernel, exact for any coefficients): partitions eliminated by
 //    all threads of the grid, interface rows in global memory (L2 resident), global PCR with one
 //    grid-wide barrier per level and early exit as soon as every off-diagonal is below the
@@ -33,14 +35,20 @@ namespace {
 using namespace btcs;
 
 // ---- geometry (host + device agree through these constants) ---------------------------------
-constexpr int kP = 8;          // rows per thread partition
-constexpr int kTn = 256;       // threads per CTA of the TILED kernel (tile = kTn*kP points)
-constexpr int kHaloT = 16;     // halo threads per side  (halo = kHaloT*kP = 128 points)
-constexpr int kLevels = 5;     // PCR levels the halo allows: 2^kLevels == 2*kHaloT rows
-constexpr int kW = (kTn - 2 * kHaloT) * kP;   // owned points per tile
+constexpr int kP = 8;          // rows per thread partition of the GENERAL kernel
+// TILED kernel: kTP rows per thread, kTn threads per CTA (tile = kTn*kTP points).  After the in-CTA
+// cyclic-reduction step every thread holds ONE reduced row (coupling ~ lambda^kTP between
+// neighbours); kLevels PCR levels follow, which contaminate 2^kLevels threads from each open tile
+// end.  The left halo is one thread wider because x_0 of a partition is recovered from the
+// reduced unknown of its LEFT neighbour.
+constexpr int kTP = 16;
+constexpr int kTn = 128;
+constexpr int kLevels = 3;
+constexpr int kHaloR = 1 << kLevels;          // threads
+constexpr int kHaloL = kHaloR + 1;
+constexpr int kW = (kTn - kHaloL - kHaloR) * kTP;   // owned points per tile
 constexpr int kGenThreads = 256;
 constexpr int kStatusBytes = 1024;            // status word + 2 x 64 level flags
-static_assert((1 << kLevels) == 2 * kHaloT, "levels must match the halo");
 
 __device__ __forceinline__ int64_t wrap(int64_t g, int64_t N) {
     g %= N;
@@ -48,122 +56,196 @@ __device__ __forceinline__ int64_t wrap(int64_t g, int64_t N) {
 }
 
 // ------------------------------------------------------------------------ TILED step kernel
+// Per thread: P-row partition elimination -> two interface rows
+//     first:  A x_L(t-1) + x_0(t) + C x_L(t) = D          last:  f x_0(t) + x_L(t) + c x_0(t+1) = q
+// One cyclic-reduction step removes every x_0 (substituting first(t) and first(t+1) into last(t)):
+//     [-f A] x_L(t-1) + [1 - f C - c A'] x_L(t) + [-c C'] x_L(t+1) = q - f D - c D'     (' = thread t+1)
+// leaving one row per thread in the unknowns x_L, solved by truncated PCR on the open chain; then
+// x_0(t) = D - A x_L(t-1) - C x_L(t) and the partition is back-substituted.
+//
+// The kernel is PERSISTENT within a step: gridDim.x CTAs (a multiple of the SM count) walk over
+// the tiles, and the next tile's points are fetched into a second shared-memory stage with
+// cp.async (LDGSTS, 16 B per thread per request, fully coalesced) while the current tile is being
+// eliminated, so that the global-load latency is hidden behind FP64 work.  The stage is written
+// with an XOR swizzle of the 16-byte chunk index so that thread t can read its own P consecutive
+// points (a 128-byte row in fp64) with conflict-free LDS.128.
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(unsigned dst, const void *src, unsigned bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
 template <typename T>
-__global__ void __launch_bounds__(kTn, 2)
+__global__ void __launch_bounds__(kTn, 4)
 btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *__restrict__ nu,
-                       const T *__restrict__ dt, int64_t N, int64_t tiles, double inv_dx, int bc,
-                       int step, int *__restrict__ status) {
-    constexpr int P = kP, Tn = kTn, M = 2 * kTn;
+                       const T *__restrict__ dt, int64_t N, int tiles, int B, double inv_dx,
+                       int bc, int step, int *__restrict__ status) {
+    constexpr int P = kTP, Tn = kTn;
     constexpr int V = 16 / sizeof(T);
-    __shared__ T sA[2][M], sC[2][M], sD[2][M];
-    __shared__ int s_failed;
-    const int t = threadIdx.x;
-    if (t == 0) s_failed = *reinterpret_cast<volatile int *>(status);
-    __syncthreads();
-    if (s_failed != 0) return;            // an earlier step failed (uniform over the CTA)
-
-    const int64_t b = blockIdx.x / tiles, tile = blockIdx.x % tiles;
+    constexpr int CR = P / V;                 // 16-byte chunks per thread row (8 fp64, 4 fp32)
+    constexpr int SW = 8 / CR;                // rows sharing one 128-byte line
+    constexpr int RB = CR * 16;               // bytes per thread row
+    constexpr int WB = 32 * RB;               // bytes per warp region of a stage
+    __shared__ __align__(128) T stage[2][Tn * P];
+    __shared__ T sA[2][Tn], sC[2][Tn], sD[2][Tn];
+    const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    if (*reinterpret_cast<volatile int *>(status) != 0) return;   // an earlier step failed (uniform)
     const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
-    const int64_t g0 = tile * kW + (int64_t)(t - kHaloT) * P;     // unwrapped index of row 0
-    const T *srow = src + b * N;
-    Coef<T> co;
-    co.init(nu[b], dt[b], inv_dx);
 
-    // ---- load the partition (periodic: wrap; Dirichlet: out-of-domain rows are x = 0)
-    T v[P];
-    const bool inside = (g0 >= 0 && g0 + P <= N);
-    if ((N % V) == 0) {
+    // Warp-private staging: warp w of the CTA owns rows 32w..32w+31 of a tile = WB contiguous bytes
+    // of global memory.  It copies them with CR requests of 512 contiguous bytes each (lane l moves
+    // chunk k*32+l), and every lane later reads / writes its OWN row: only __syncwarp() in between.
+    // Chunk c of row r lives at r*RB + ((c ^ ((r/SW) % CR)) * 16); request k of lane l moves chunk
+    // c = l % CR of row r = k*(32/CR) + l/CR of the warp region.
+    const int fr = lane / CR, fc = lane % CR;                        // row / chunk of request 0
+    auto f_off = [&](int k) {
+        const int r = k * (32 / CR) + fr;
+        return (unsigned)(warp * WB + r * RB + ((fc ^ ((r / SW) % CR)) * 16));
+    };
+    const unsigned r_off = (unsigned)(t * RB) | (unsigned)((((t / SW) % CR)) * 16);   // XOR with c*16 per chunk
+    const unsigned stage0 = smem_u32(&stage[0][0]);
+    constexpr unsigned kStageBytes = Tn * P * sizeof(T);
+
+    auto fetch = [&](int b, int tile, int st) {
+        const int64_t wg0 = (int64_t)tile * kW + (int64_t)(warp * 32 - kHaloL) * P;   // first point of the warp region
+        const bool edge = (wg0 < 0) || (wg0 + 32 * P > N);
+        const T *srow = src + (int64_t)b * N;
+        const unsigned d0 = stage0 + st * kStageBytes;
+        if (!edge) {
+            const T *g = srow + wg0 + lane * V;
 #pragma unroll
-        for (int c = 0; c < P / V; ++c) {
-            int64_t g = g0 + c * V;
-            bool ok = true;
-            if (!inside) {
-                if (dirichlet) ok = (g >= 0 && g < N);
-                else g = wrap(g, N);
+            for (int k = 0; k < CR; ++k) cp_async16(d0 + f_off(k), g + k * 32 * V, 16);
+        } else {
+#pragma unroll
+            for (int k = 0; k < CR; ++k) {
+                int64_t g = wg0 + (int64_t)(k * 32 + lane) * V;
+                unsigned bytes = 16;
+                if (dirichlet) { if (g < 0 || g >= N) { bytes = 0; g = 0; } }
+                else { if (g < 0) g += N; else if (g >= N) g -= N; }
+                cp_async16(d0 + f_off(k), srow + g, bytes);
             }
-            int4 q4 = make_int4(0, 0, 0, 0);
-            if (ok) q4 = *reinterpret_cast<const int4 *>(srow + g);
+        }
+        cp_async_commit();
+    };
+
+    // work items (system b, tile) in order; this CTA takes every gridDim.x-th one
+    int b = (int)(blockIdx.x / (unsigned)tiles), tile = (int)(blockIdx.x % (unsigned)tiles);
+    const int db = (int)(gridDim.x / (unsigned)tiles), dtile = (int)(gridDim.x % (unsigned)tiles);
+    if (b < B) fetch(b, tile, 0);
+    for (int st = 0; b < B; st ^= 1) {
+        int bn = b + db, tn_ = tile + dtile;
+        if (tn_ >= tiles) { tn_ -= tiles; ++bn; }
+        if (bn < B) { fetch(bn, tn_, st ^ 1); cp_async_wait<1>(); }
+        else cp_async_wait<0>();
+        __syncwarp();
+
+        const int64_t g0 = (int64_t)tile * kW + (int64_t)(t - kHaloL) * P;     // unwrapped index of row 0
+        Coef<T> co;
+        co.init(nu[b], dt[b], inv_dx);
+
+        // ---- this thread's partition from the swizzled stage
+        T v[P];
+        const unsigned rbase = stage0 + st * kStageBytes + r_off;
+#pragma unroll
+        for (int c = 0; c < CR; ++c) {
+            int4 q4;
+            asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(q4.x), "=r"(q4.y), "=r"(q4.z), "=r"(q4.w) : "r"(rbase ^ (unsigned)(c * 16)));
             const T *e = reinterpret_cast<const T *>(&q4);
 #pragma unroll
             for (int k = 0; k < V; ++k) v[c * V + k] = e[k];
         }
-    } else {
-#pragma unroll
-        for (int j = 0; j < P; ++j) {
-            int64_t g = g0 + j;
-            bool ok = true;
-            if (!inside) {
-                if (dirichlet) ok = (g >= 0 && g < N);
-                else g = wrap(g, N);
-            }
-            v[j] = ok ? srow[g] : T(0);
+
+        // ---- assembly + partition elimination
+        T f[P], c[P], q[P];
+        Row<T> first, last;
+        if (dirichlet && (g0 <= 0 || g0 + P >= N)) {
+            eliminate<T, P>(v, co, [&](int j) { return g0 + j <= 0 || g0 + j >= N - 1; }, f, c, q, first, last);
+        } else {
+            eliminate<T, P>(v, co, [](int) { return false; }, f, c, q, first, last);
         }
-    }
+        if (t == 0) first.A = T(0);          // open chain: drop the couplings leaving the tile
+        if (t == Tn - 1) last.C = T(0);
 
-    // ---- assembly + partition elimination
-    T f[P], c[P], q[P];
-    Row<T> first, last;
-    if (dirichlet && (g0 <= 0 || g0 + P >= N)) {
-        eliminate<T, P>(v, co, [&](int j) { return g0 + j <= 0 || g0 + j >= N - 1; }, f, c, q, first, last);
-    } else {
-        eliminate<T, P>(v, co, [](int) { return false; }, f, c, q, first, last);
-    }
-    if (t == 0) first.A = T(0);          // open chain: drop the couplings leaving the tile
-    if (t == Tn - 1) last.C = T(0);
-    sA[0][2 * t] = first.A; sA[0][2 * t + 1] = last.A;
-    sC[0][2 * t] = first.C; sC[0][2 * t + 1] = last.C;
-    sD[0][2 * t] = first.D; sD[0][2 * t + 1] = last.D;
-    __syncthreads();
+        // ---- cyclic-reduction step: one row per thread in x_L
+        sA[1][t] = first.A; sC[1][t] = first.C; sD[1][t] = first.D;
+        __syncthreads();
+        Row<T> row;
+        {
+            const int tn = (t + 1 < Tn) ? t + 1 : t;       // t = Tn-1: last.C == 0, values unused
+            const T nA = sA[1][tn], nC = sC[1][tn], nD = sD[1][tn];
+            const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
+            row.A = -last.A * first.A * m;
+            row.C = -last.C * nC * m;
+            row.D = t_fma(-last.A, first.D, t_fma(-last.C, nD, last.D)) * m;
+        }
+        sA[0][t] = row.A; sC[0][t] = row.C; sD[0][t] = row.D;
+        __syncthreads();
 
-    // ---- PCR on the open chain of M interface rows, at most kLevels levels
-    int cur = 0;
-    bool finished = false;
-#pragma unroll 1
-    for (int l = 0; l < kLevels; ++l) {
-        const int s = 1 << l;
-        int flag = 0;
+        // ---- PCR on the open chain of Tn rows, at most kLevels levels.  Rows that must be
+        // finished: the owned threads and the left neighbour of the first owned thread.
+        const bool needed = (t >= kHaloL - 1) && (t < Tn - kHaloR);
+        int cur = 0;
+        bool finished = false;
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int k = t + h * Tn;
-            const int km = k - s, kp = k + s;
-            Row<T> rk, rm, rp;
-            rk.A = sA[cur][k]; rk.C = sC[cur][k]; rk.D = sD[cur][k];
+        for (int l = 0; l < kLevels; ++l) {
+            const int s = 1 << l;
+            const int km = t - s, kp = t + s;
+            Row<T> rm, rp;
             if (km >= 0) { rm.A = sA[cur][km]; rm.C = sC[cur][km]; rm.D = sD[cur][km]; }
             else { rm.A = T(0); rm.C = T(0); rm.D = T(0); }
-            if (kp < M) { rp.A = sA[cur][kp]; rp.C = sC[cur][kp]; rp.D = sD[cur][kp]; }
+            if (kp < Tn) { rp.A = sA[cur][kp]; rp.C = sC[cur][kp]; rp.D = sD[cur][kp]; }
             else { rp.A = T(0); rp.C = T(0); rp.D = T(0); }
-            const Row<T> n = pcr_combine(rk, rm, rp);
-            sA[cur ^ 1][k] = n.A; sC[cur ^ 1][k] = n.C; sD[cur ^ 1][k] = n.D;
-            const bool owned = (k >= 2 * kHaloT) && (k < M - 2 * kHaloT);
-            flag |= owned & ((t_abs(n.A) > Lim<T>::tiny()) | (t_abs(n.C) > Lim<T>::tiny()));
+            row = pcr_combine(row, rm, rp);
+            sA[cur ^ 1][t] = row.A; sC[cur ^ 1][t] = row.C; sD[cur ^ 1][t] = row.D;
+            // NaN-safe: a row that is not provably finished counts as unfinished
+            const int flag = needed & !((t_abs(row.A) <= Lim<T>::tiny()) & (t_abs(row.C) <= Lim<T>::tiny()));
+            const int any = __syncthreads_or(flag);
+            cur ^= 1;
+            if (!any) { finished = true; break; }
         }
-        const int any = __syncthreads_or(flag);
-        cur ^= 1;
-        if (!any) { finished = true; break; }
-    }
-    if (!finished) {                       // the halo was too short for these coefficients
-        if (t == 0) atomicCAS(status, 0, step + 1);
-        return;
-    }
+        if (!finished) {                       // the halo was too short for these coefficients
+            if (t == 0) atomicCAS(status, 0, step + 1);
+            break;                             // uniform over the CTA
+        }
 
-    // ---- back substitution and store of the owned partitions
-    const bool owned = (t >= kHaloT) && (t < Tn - kHaloT) && (g0 < N);
-    if (!owned) return;
-    back_substitute<T, P>(v, f, c, q, sD[cur][2 * t], sD[cur][2 * t + 1]);
-    T *drow = dst + b * N;
-    if ((N % V) == 0) {
+        // ---- recover x_0, back substitution; the warp's rows go back through its stage region so
+        // that the global stores are 512 contiguous bytes per request
+        const bool owned = (t >= kHaloL) && (t < Tn - kHaloR);
+        if (owned) {
+            const T xL = row.D;
+            const T xLprev = sD[cur][t - 1];
+            const T x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
+            back_substitute<T, P>(v, f, c, q, x0, xL);
 #pragma unroll
-        for (int cc = 0; cc < P / V; ++cc) {
-            int4 q4;
-            T *e = reinterpret_cast<T *>(&q4);
+            for (int cc = 0; cc < CR; ++cc) {
+                int4 q4;
+                T *e = reinterpret_cast<T *>(&q4);
 #pragma unroll
-            for (int k = 0; k < V; ++k) e[k] = v[cc * V + k];
-            *reinterpret_cast<int4 *>(drow + g0 + cc * V) = q4;
+                for (int k = 0; k < V; ++k) e[k] = v[cc * V + k];
+                asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(rbase ^ (unsigned)(cc * 16)), "r"(q4.x), "r"(q4.y), "r"(q4.z), "r"(q4.w) : "memory");
+            }
         }
-    } else {
+        __syncwarp();
+        {
+            const int64_t wg0 = (int64_t)tile * kW + (int64_t)(warp * 32 - kHaloL) * P;
+            T *drow = dst + (int64_t)b * N;
+            const unsigned s0 = stage0 + st * kStageBytes;
 #pragma unroll
-        for (int j = 0; j < P; ++j) drow[g0 + j] = v[j];
+            for (int k = 0; k < CR; ++k) {
+                const int rt = warp * 32 + (k * 32 + lane) / CR;            // thread that owns this chunk's row
+                const int64_t g = wg0 + (int64_t)(k * 32 + lane) * V;
+                if (rt >= kHaloL && rt < Tn - kHaloR && g < N) {
+                    int4 q4;
+                    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(q4.x), "=r"(q4.y), "=r"(q4.z), "=r"(q4.w) : "r"(s0 + f_off(k)));
+                    *reinterpret_cast<int4 *>(drow + g) = q4;
+                }
+            }
+        }
+        __syncwarp();      // the stage region is re-filled by this warp's next-but-one fetch
+        b = bn; tile = tn_;
     }
+    cp_async_wait<0>();
 }
 
 // After the TILED launches: move the newest valid state into u when it sits in ws.
@@ -312,7 +394,7 @@ size_t row_elems(int64_t B, int64_t N) { return (size_t)B * (size_t)(2 * (N / kP
 // LONG runs power-of-two grids of at least four tiles (shorter systems fit one CTA: HYBRID).
 bool btcs_long_fits(int64_t N, int bc) {
     (void)bc;
-    return pow2(N) && N >= 4 * (int64_t)kTn * kP;
+    return pow2(N) && N >= 4 * (int64_t)kTn * kTP;
 }
 
 // ws layout (elements of T): [B*N ping-pong state][6 x B*M interface rows] then kStatusBytes.
@@ -346,11 +428,20 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
 
     if (!general_only) {
         const int64_t tiles = (N + kW - 1) / kW;
-        if (B * tiles > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+        const int64_t items = B * tiles;
+        int dev0 = 0, sms0 = 0, occ0 = 0;
+        if (cudaGetDevice(&dev0) != cudaSuccess ||
+            cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, btcs_long_tiled_kernel<T>, kTn, 0) != cudaSuccess ||
+            occ0 < 1)
+            return BURGERS_ERR_CUDA;
+        // persistent grid: every SM gets the same number of CTAs, every CTA about the same number of tiles
+        int64_t grid_t = (int64_t)sms0 * occ0;
+        if (grid_t > items) grid_t = items;
         T *cur = u, *nxt = pong;
         for (int64_t n = 0; n < n_steps; ++n) {
-            btcs_long_tiled_kernel<T><<<(unsigned)(B * tiles), kTn, 0, s>>>(cur, nxt, nu, dt, N, tiles, inv_dx,
-                                                                          bc, (int)n, status);
+            btcs_long_tiled_kernel<T><<<(unsigned)grid_t, kTn, 0, s>>>(cur, nxt, nu, dt, N, (int)tiles, (int)B, inv_dx,
+                                                                     bc, (int)n, status);
             T *tmp = cur; cur = nxt; nxt = tmp;
         }
         int st = last_launch_status();
