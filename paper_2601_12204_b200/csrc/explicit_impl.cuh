@@ -14,17 +14,25 @@
 // neighbouring threads by warp shuffle (CTA of one warp) or through a double-buffered shared
 // memory edge array with ONE barrier per exchange (several warps).
 //
-// Arithmetic per point (D2, scaled by dt): with hcx = dt/(2 dx), rr = nu dt/dx^2 and l/c/r the
-// left, centre and right values, the sign-switched upwind difference of PAPER.md:89 is written in
-// its branch-free "central difference + numerical diffusion" form
-//   u_i g_i = u_i (u_{i+1} - u_{i-1})/2 - |u_i| (u_{i+1} - 2u_i + u_{i-1})/2     (either sign of u_i)
-// so that
-//   dt*F = (rr + hcx*|c|) * (l + r - 2c) - hcx*c*(r - l)
-// which is 7 FMA-pipe instructions and no compare/select (the select form costs 7 + 2): the
-// kernels are issue-bound, so instructions per update are what matters.
-// It equals D2 up to rounding, keeps constants exactly fixed and keeps odd symmetry exact.
+// Arithmetic per point (D2 scaled by dt; cx = dt/dx, rr = nu dt/dx^2).  With the one-sided differences
+// d_j = u_{j+1} - u_j (each shared by two neighbouring points) the update is
+//     lap = d_j - d_{j-1},   g = (u_j > 0) ? d_{j-1} : d_j   (upwind rule PAPER.md:89),
+//     dt*F = rr*lap - cx*u_j*g.
+// The B200 FP32 pipe is limited by REGISTER-OPERAND bandwidth, not by instruction count (measured:
+// FADD with 2 register operands 0.98 warp-instr/cycle/SMSP, FFMA with 3 distinct registers 0.61;
+// DESIGN.md "Kernels"), so the form is chosen to minimise register reads per update:
+//   fp32: the state is carried SCALED, w = cx*u, which folds the convective coefficient into the
+//         state:  dt*F*cx = rr*lap(w) - w*g(w):  FADD, FADD, FSETP+FSEL (ALU pipe), FFMA, FFMA
+//         (+ FADD for the compensated sum) = 7 issue slots / 15 register reads per update (the
+//         select-free |u| form needs 8 / 19).  Scaling happens once at load, unscaling once at
+//         store; Dirichlet end nodes are stored back bit-exactly from the loaded values.
+//   fp64: the FP64 pipe (64 lanes/SM) is the limit, so what counts is DP instructions: unscaled
+//         form, DADD, DADD, DMUL, DFMA, DFMA = 5 per update with the select done on the integer
+//         pipe from the sign of the high word.  Unscaled, so that p then q steps equal p+q steps
+//         bitwise.
+// Both equal D2 up to rounding, keep constants exactly fixed and keep odd symmetry exact.
 // fp32 Euler carries the state as base + s (two fp32 terms; increments are accumulated into the
-// small term s, so they are not lost against ulp(u)) -- the stencil reads the
+// small term s, so they are not lost against ulp(w)) -- the stencil reads the
 // rounded sum v = fl(base + s).
 #pragma once
 #include "common.cuh"
@@ -46,6 +54,10 @@ struct Params {
     int halo;         // TILED: halo points per side
     int64_t W;        // TILED: valid outputs per tile
     int64_t tiles;    // TILED: tiles per trajectory
+    // fp32 carries the state scaled (w = cx*u, see below).  Between the launches of a TILED call the
+    // ping-pong buffers hold w, so only the first launch scales and only the last one unscales.
+    // Frozen Dirichlet end nodes are ALWAYS stored unscaled (their original bits).
+    int in_scaled, out_scaled;
 };
 
 template <typename T> __device__ __forceinline__ T t_abs(T x);
@@ -55,20 +67,32 @@ template <typename T> __device__ __forceinline__ T t_fma(T a, T b, T c);
 template <> __device__ __forceinline__ float t_fma<float>(float a, float b, float c) { return fmaf(a, b, c); }
 template <> __device__ __forceinline__ double t_fma<double>(double a, double b, double c) { return fma(a, b, c); }
 
-// dt*F at one point (D2) added to `acc`:  acc + (rr + hcx|c|) lap - hcx c (r - l).  7 FP instructions.
-template <typename T>
-__device__ __forceinline__ T add_dtF(T acc, T l, T c, T r, T hcx, T rr) {
-    const T lap = t_fma(T(-2), c, l + r);        // u_{i+1} - 2u_i + u_{i-1}   (Eq.4)
-    const T k = t_fma(hcx, t_abs(c), rr);        // diffusion number + upwind numerical diffusion
-    const T e = hcx * c;
-    return t_fma(-e, r - l, t_fma(k, lap, acc));
+// upwind difference: backward difference dm where the value is > 0, else forward dp
+template <typename T> __device__ __forceinline__ T upwind(T c, T dm, T dp);
+template <> __device__ __forceinline__ float upwind<float>(float c, float dm, float dp) { return (c > 0.f) ? dm : dp; }
+template <> __device__ __forceinline__ double upwind<double>(double c, double dm, double dp) {
+    // sign test on the high word (integer pipe; the FP64 pipe is the scarce one).  +-0 and positive
+    // denormals below 2^-1022 take dp: they multiply the difference by (next to) nothing (Q3).
+    return (__double2hiint(c) > 0) ? dm : dp;
 }
-template <typename T>
-__device__ __forceinline__ T dtF(T l, T c, T r, T hcx, T rr) {
-    const T lap = t_fma(T(-2), c, l + r);
-    const T k = t_fma(hcx, t_abs(c), rr);
-    const T e = hcx * c;
-    return t_fma(-e, r - l, k * lap);
+
+// acc + dt*F at one point from its value c and the differences dm = c - left, dp = right - c.
+//   SCALED (state w = cx*u):  acc + rr*(dp - dm) - c*g          k1 = rr, k2 unused
+//   unscaled:                 acc + rr*(dp - dm) - cx*(c*g)     k1 = rr, k2 = cx
+template <typename T, bool SCALED>
+__device__ __forceinline__ T add_dtF(T acc, T c, T dm, T dp, T rr, T cx) {
+    const T lap = dp - dm;                       // u_{i+1} - 2u_i + u_{i-1}   (Eq.4)
+    const T g = upwind<T>(c, dm, dp);
+    if (SCALED) return t_fma(-c, g, t_fma(rr, lap, acc));
+    return t_fma(-cx, c * g, t_fma(rr, lap, acc));
+}
+// dt*F alone (RK4 stages)
+template <typename T, bool SCALED>
+__device__ __forceinline__ T dtF(T c, T dm, T dp, T rr, T cx) {
+    const T lap = dp - dm;
+    const T g = upwind<T>(c, dm, dp);
+    if (SCALED) return t_fma(-c, g, rr * lap);
+    return t_fma(-cx, c * g, rr * lap);
 }
 
 // Halo exchange: every thread publishes its first and last point and receives the last point
@@ -121,9 +145,15 @@ explicit_kernel(const Params<T> p) {
     T *drow = p.dst + b * N;
 
     // per-trajectory constants, evaluated in fp64 and rounded once
+    constexpr bool SCALED = (sizeof(T) == 4);
     const double dtb = (double)p.dt[b];
-    const T hcx = (T)(0.5 * dtb * p.inv_dx);
+    const T cx = (T)(dtb * p.inv_dx);
     const T rr = (T)((double)p.nu[b] * dtb * p.inv_dx * p.inv_dx);
+    // fp32: the state is carried as w = scale*u with scale = cx.  dt == 0 (cx == 0) leaves u
+    // unchanged: no steps, scale 1.
+    const bool degenerate = SCALED && (cx == T(0));
+    const T scale = (SCALED && !degenerate) ? cx : T(1);
+    const int64_t steps = degenerate ? 0 : p.steps;
 
     // ---------------- load
     T v[P];
@@ -138,7 +168,7 @@ explicit_kernel(const Params<T> p) {
                 bool inside = true;
                 if (TILED) {
                     if (dirichlet) inside = (g >= 0 && g < N);
-                    else { g %= N; if (g < 0) g += N; }
+                    else if (g < 0 || g >= N) { g %= N; if (g < 0) g += N; }
                 }
                 if (inside) {
                     int4 q = *reinterpret_cast<const int4 *>(srow + g);
@@ -154,7 +184,7 @@ explicit_kernel(const Params<T> p) {
                 bool inside = true;
                 if (TILED) {
                     if (dirichlet) inside = (g >= 0 && g < N);
-                    else { g %= N; if (g < 0) g += N; }
+                    else if (g < 0 || g >= N) { g %= N; if (g < 0) g += N; }
                 }
                 if (inside) v[j] = srow[g];
             }
@@ -171,32 +201,38 @@ explicit_kernel(const Params<T> p) {
     // j = P-1 of their thread (N % P == 0, tile origin % P == 0).
     const bool fixL = dirichlet && (g0 == 0);
     const bool fixR = dirichlet && (g0 + P - 1 == N - 1);
+    const T keepL = v[0], keepR = v[P - 1];       // stored back bit-exactly when frozen
     int buf = 0;
     T left, right;
 
     if (SCHEME == BURGERS_SCHEME_EULER) {
         T base[SPLIT ? P : 1], s[SPLIT ? P : 1];
-        if (SPLIT) {
+        if (SPLIT) {       // w = scale*u as an exact two-term sum (or w itself from the last launch)
 #pragma unroll
-            for (int j = 0; j < P; ++j) { base[j] = v[j]; s[j] = T(0); }
+            for (int j = 0; j < P; ++j) {
+                const bool raw = !p.in_scaled || (j == 0 && fixL) || (j == P - 1 && fixR);
+                base[j] = raw ? v[j] * scale : v[j];
+                s[j] = raw ? t_fma(v[j], scale, -base[j]) : T(0);
+                v[j] = base[j];
+            }
         }
-        for (int64_t n = 0; n < p.steps; ++n) {
+        for (int64_t n = 0; n < steps; ++n) {
             exchange<T, WARP>(v[0], v[P - 1], left, right, tl, tr, edge, buf);
-            T l = left;
+            T dm = v[0] - left;
 #pragma unroll
             for (int j = 0; j < P; ++j) {
                 const T c = v[j];
-                const T r = (j + 1 < P) ? v[j + 1] : right;
+                const T dp = ((j + 1 < P) ? v[j + 1] : right) - c;
                 const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
                 if (SPLIT) {
-                    const T sn = add_dtF<T>(s[j], l, c, r, hcx, rr);
+                    const T sn = add_dtF<T, SCALED>(s[j], c, dm, dp, rr, cx);
                     s[j] = frozen ? s[j] : sn;
                     v[j] = base[j] + s[j];
                 } else {
-                    const T vn = add_dtF<T>(c, l, c, r, hcx, rr);
+                    const T vn = add_dtF<T, SCALED>(c, c, dm, dp, rr, cx);
                     v[j] = frozen ? c : vn;
                 }
-                l = c;
+                dm = dp;
             }
             if (SPLIT && (n & 63) == 63) {  // renormalise: base <- fl(base+s), s <- exact remainder
 #pragma unroll
@@ -207,29 +243,52 @@ explicit_kernel(const Params<T> p) {
                 }
             }
         }
-    } else {  // classical RK4; K_s = dt*F(y_s)
+        if (SPLIT && !p.out_scaled) {       // u = (base + s)/scale, rounded once
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                const T qn = base[j] / scale;
+                const T rem = t_fma(-qn, scale, base[j]) + s[j];
+                v[j] = qn + rem / scale;
+            }
+        }
+    } else {  // classical RK4; K_s = dt*F(y_s) (times scale)
         T y[P], acc[P];
-        for (int64_t n = 0; n < p.steps; ++n) {
+        if (SCALED) {
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                const bool raw = !p.in_scaled || (j == 0 && fixL) || (j == P - 1 && fixR);
+                v[j] = raw ? v[j] * scale : v[j];
+            }
+        }
+        for (int64_t n = 0; n < steps; ++n) {
 #pragma unroll
             for (int stage = 0; stage < 4; ++stage) {
                 if (stage == 0) exchange<T, WARP>(v[0], v[P - 1], left, right, tl, tr, edge, buf);
                 else exchange<T, WARP>(y[0], y[P - 1], left, right, tl, tr, edge, buf);
-                T l = left;
+                T dm = ((stage == 0) ? v[0] : y[0]) - left;
 #pragma unroll
                 for (int j = 0; j < P; ++j) {
                     const T c = (stage == 0) ? v[j] : y[j];
-                    const T r = (j + 1 < P) ? ((stage == 0) ? v[j + 1] : y[j + 1]) : right;
+                    const T dp = ((j + 1 < P) ? ((stage == 0) ? v[j + 1] : y[j + 1]) : right) - c;
                     const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
-                    T K = dtF<T>(l, c, r, hcx, rr);
+                    T K = dtF<T, SCALED>(c, dm, dp, rr, cx);
                     K = frozen ? T(0) : K;
                     if (stage == 0) { acc[j] = K; y[j] = t_fma(T(0.5), K, v[j]); }
                     else if (stage == 1) { acc[j] = t_fma(T(2), K, acc[j]); y[j] = t_fma(T(0.5), K, v[j]); }
                     else if (stage == 2) { acc[j] = t_fma(T(2), K, acc[j]); y[j] = v[j] + K; }
                     else { acc[j] += K; v[j] = t_fma(acc[j], T(1.0 / 6.0), v[j]); }
-                    l = c;
+                    dm = dp;
                 }
             }
         }
+        if (SCALED && !p.out_scaled) {
+#pragma unroll
+            for (int j = 0; j < P; ++j) v[j] = v[j] / scale;
+        }
+    }
+    if (SCALED) {          // frozen Dirichlet nodes: the loaded bits, not a scale/unscale round trip
+        if (fixL) v[0] = keepL;
+        if (fixR) v[P - 1] = keepR;
     }
 
     // ---------------- store
@@ -304,6 +363,7 @@ int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, con
     Params<T> p;
     p.nu = nu; p.dt = dt; p.N = N; p.inv_dx = 1.0 / dx; p.nth = g.nth; p.bc = bc;
     p.halo = g.halo; p.W = g.W; p.tiles = g.tiles;
+    p.in_scaled = 0; p.out_scaled = 0;
     if (g.plan == BURGERS_PLAN_RESIDENT) {
         p.src = u; p.dst = u; p.steps = n_steps;
         return scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
@@ -316,6 +376,7 @@ int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, con
     while (done < n_steps) {
         const int64_t k = (n_steps - done < g.tblock) ? n_steps - done : g.tblock;
         p.src = cur; p.dst = nxt; p.steps = k;
+        p.in_scaled = (done > 0); p.out_scaled = (done + k < n_steps);
         int st = scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
                                                 : launch_scheme<T, BURGERS_SCHEME_RK4>(p, g, B, s);
         if (st != BURGERS_OK) return st;
