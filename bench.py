@@ -33,8 +33,15 @@ if ROOT not in sys.path:
 
 SM_COUNT = 148
 FP32_LANES, FP64_LANES = 128, 64
-# algorithmic instruction counts per update
-I_EULER, I_RK4, I_BTCS = 8, 36, 38
+# algorithmic instruction counts per update (DESIGN.md "Kernels" / "Rooflines"):
+#   fp32 Euler: 7 issue slots (FADD, FADD, FSETP, FSEL, FFMA, FFMA + FADD of the compensated sum)
+#   fp32 RK4:   4 stages x 8 (FADD, FADD, FSETP, FSEL, FMUL, FFMA + 2 FFMA for accumulator / next stage)
+#   fp64 Euler: 5 FP64-pipe instructions (DADD, DADD, DMUL, DFMA, DFMA; the select runs on the integer pipe)
+#   fp64 BTCS:  FP64-pipe instructions of assembly + partition elimination + interface solve + back substitution
+I_EULER_F32, I_EULER_F64, I_RK4_F32, I_BTCS_HYBRID, I_BTCS_LONG = 7, 5, 32, 26, 22
+# dram__bytes_read.sum + dram__bytes_write.sum of the time-stepping kernel, per launch, from the
+# `ncu --set full` captures summarised in profiles/ (r01_ncu_full_<workload>.txt)
+NCU_TRAFFIC_BYTES = {"c2_f32": 16.8e6, "c2_f64": 33.6e6, "c3": 81.9e6, "c4a": 86.8e6, "c4b": 33.7e6, "c5": 509.8e6}
 
 
 def peaks():
@@ -55,22 +62,22 @@ def make_workload(name, rank=0, world=1, reduced=False):
         Bg = 1024 * world
         w = W.c2_dirichlet_batch(B=Bg, dtype=dtype, rows=W.shard_rows(Bg, rank, world),
                                  n_steps=1000 if reduced else 10000)
-        return w, dict(op="explicit", scheme=0, instr=I_EULER if dtype == np.float32 else 6,
+        return w, dict(op="explicit", scheme=0, instr=I_EULER_F32 if dtype == np.float32 else I_EULER_F64,
                        lanes=FP32_LANES if dtype == np.float32 else FP64_LANES)
     if name == "c3":
         Bg = 4096 * world
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
-        return w, dict(op="btcs", scheme=None, instr=I_BTCS, lanes=FP64_LANES)
+        return w, dict(op="btcs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES)
     if name == "c4a":
         w = W.c4a_long_explicit(n_steps=200 if reduced else 2000)
-        return w, dict(op="explicit", scheme=0, instr=I_EULER, lanes=FP32_LANES)
+        return w, dict(op="explicit", scheme=0, instr=I_EULER_F32, lanes=FP32_LANES)
     if name == "c4b":
         w = W.c4b_long_btcs(n_steps=20 if reduced else 200)
-        return w, dict(op="btcs", scheme=None, instr=I_BTCS, lanes=FP64_LANES)
+        return w, dict(op="btcs", scheme=None, instr=I_BTCS_LONG, lanes=FP64_LANES)
     if name == "c5":
         Bg = 65536 * world
         w = W.c5_rk4_ensemble(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=500 if reduced else 5000)
-        return w, dict(op="explicit", scheme=1, instr=I_RK4, lanes=FP32_LANES)
+        return w, dict(op="explicit", scheme=1, instr=I_RK4_F32, lanes=FP32_LANES)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -87,7 +94,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                 "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
@@ -249,7 +256,7 @@ class GpuRunner:
         return ms, h2d, d2h
 
 
-def roofline(spec, w, op_ms, pk):
+def roofline(spec, w, op_ms, pk, name=None, launches=1):
     """Dominant kernel = the time-stepping kernel(s) of the op call."""
     sec = statistics.mean(op_ms) * 1e-3
     ups = w.updates / sec
@@ -257,7 +264,9 @@ def roofline(spec, w, op_ms, pk):
     ach = ups * spec["instr"] / 1e9
     esz = w.u0.dtype.itemsize
     return {"bound": "alu", "achieved": ach, "peak": peak, "unit": "Ginst/s", "frac": ach / peak,
-            "traffic": None,
+            "traffic": (NCU_TRAFFIC_BYTES[name] if name in NCU_TRAFFIC_BYTES else None),
+            "traffic_unit": "bytes per launch (ncu dram read+write, profiles/)",
+            "launches_per_step": launches,
             "note": (f"{spec['instr']} algorithmic {'fp64' if spec['lanes'] == FP64_LANES else 'fp32'}-pipe "
                      f"instr/update x updates / kernel time; peak = {SM_COUNT} SMs x {spec['lanes']} lanes x "
                      f"{pk['sm_max_mhz']:.0f} MHz (nominal unit counts, max clock)"),
@@ -325,7 +334,7 @@ def run_ours(args):
         "clocks": clocks,
     }
     if rank == 0:
-        out["roofline"] = roofline(spec, w, op_ms, pk)
+        out["roofline"] = roofline(spec, w, op_ms, pk, args.workload, int(r.launches))
         e_ms, h2d, d2h = r.e2e(max(1, min(args.steps, 3)), 1)
         out["e2e"] = {"value": w.updates * world / (statistics.mean(e_ms) * 1e-3), "unit": "updates/s",
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -396,7 +405,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5"])

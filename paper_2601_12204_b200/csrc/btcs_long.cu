@@ -90,6 +90,11 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
     __shared__ __align__(128) T stage[2][Tn * P];
     __shared__ T sA[2][Tn], sC[2][Tn], sD[2][Tn];
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+    // Programmatic dependent launch: let the next step's grid be scheduled while this one runs
+    // (its CTAs become resident as ours retire), and wait here for the previous step's grid to
+    // have completed and flushed before reading anything it wrote.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (*reinterpret_cast<volatile int *>(status) != 0) return;   // an earlier step failed (uniform)
     const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
 
@@ -439,9 +444,16 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
         int64_t grid_t = (int64_t)sms0 * occ0;
         if (grid_t > items) grid_t = items;
         T *cur = u, *nxt = pong;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)grid_t); cfg.blockDim = dim3(kTn); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+        cfg.attrs = attr; cfg.numAttrs = 1;
         for (int64_t n = 0; n < n_steps; ++n) {
-            btcs_long_tiled_kernel<T><<<(unsigned)grid_t, kTn, 0, s>>>(cur, nxt, nu, dt, N, (int)tiles, (int)B, inv_dx,
-                                                                     bc, (int)n, status);
+            if (cudaLaunchKernelEx(&cfg, btcs_long_tiled_kernel<T>, (const T *)cur, nxt, nu, dt, N, (int)tiles, (int)B,
+                                   inv_dx, bc, (int)n, status) != cudaSuccess)
+                return BURGERS_ERR_CUDA;
             T *tmp = cur; cur = nxt; nxt = tmp;
         }
         int st = last_launch_status();

@@ -50,7 +50,7 @@ static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock
     int nth = 256;
     const int maxt = explicit_max_threads(is_f64, P, scheme);
     if (nth > maxt) nth = maxt;
-    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 4 : 16;
+    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 16 : 64;   // measured on C4a: 16 -> 11.9 ms, 64 -> 9.4 ms
     const int64_t Wt = (int64_t)nth * P;
     const int q = P > V ? P : V;
     int halo = 0;
