@@ -13,13 +13,16 @@
 //        first:  A x_{-1} + x_0 + C x_{P-1} = D          last:  f x_0 + x_{P-1} + c x_P = q
 //     (x_{-1} / x_P = last / first unknown of the neighbouring threads; periodic wrap between the
 //     last and the first thread -- the cyclic corner terms need no special treatment here).
-//  3. the 2T interface rows form a CYCLIC tridiagonal system, solved by parallel cyclic reduction
-//     in shared memory (rows kept normalised, diag = 1).  The matrix is strictly diagonally
-//     dominant (D4), so the off-diagonals of the reduced rows shrink quadratically per PCR level;
-//     once every |A|,|C| is below 2^-70 (fp64; 2^-40 fp32) the remaining levels cannot change a
-//     bit of the answer and the loop exits early (block-wide vote).  If it runs to the end, the
-//     last level is the exact 2x2 solve of rows k and k+T.
-//  4. back substitution inside each thread: x_j = q_j - f_j x_0 - c_j x_{j+1}, j = P-2..1.
+//  3. one cyclic-reduction step substitutes the x_0 rows of threads t and t+1 into the last row of
+//     thread t, leaving ONE reduced row per thread in the unknowns x_{P-1}(t); these T rows form a
+//     CYCLIC tridiagonal system, solved by parallel cyclic reduction in shared memory (rows kept
+//     normalised, diag = 1).  The matrix is strictly diagonally dominant (D4), so the off-diagonals
+//     of the reduced rows shrink quadratically per PCR level; once every |A|,|C| is below 2^-70
+//     (fp64; 2^-40 fp32) the remaining levels cannot change a bit of the answer and the loop exits
+//     early (block-wide vote, NaN-safe).  If it runs to the end, the last level is the exact 2x2
+//     solve of rows t and t+T/2.
+//  4. x_0(t) = D - A x_{P-1}(t-1) - C x_{P-1}(t) from the thread's first interface row, then back
+//     substitution inside each thread: x_j = q_j - f_j x_0 - c_j x_{j+1}, j = P-2..1.
 // Periodic systems are solved directly as cyclic systems (no Sherman-Morrison second right-hand
 // side); the result equals D6's up to rounding.
 #include "btcs_common.cuh"
@@ -42,10 +45,13 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
                    double inv_dx, int64_t n_steps, int bc) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int t = threadIdx.x, Tn = blockDim.x, M = 2 * Tn;
-    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][M]
-    T *sC = sA + 2 * M;
-    T *sD = sC + 2 * M;
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (PCR ping-pong)
+    T *sC = sA + 2 * Tn;
+    T *sD = sC + 2 * Tn;
+    T *sFA = sD + 2 * Tn;                     // [Tn] first interface rows (cyclic-reduction step)
+    T *sFC = sFA + Tn;
+    T *sFD = sFC + Tn;
     T *row = u + (int64_t)blockIdx.x * N + (int64_t)t * P;
 
     Coef<T> co;
@@ -62,56 +68,59 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
         for (int k = 0; k < V; ++k) v[c * V + k] = e[k];
     }
 
-    int cur = 0;
     for (int64_t n = 0; n < n_steps; ++n) {
         T f[P], c[P], q[P];
-        // ---- assembly + partition elimination; interface rows -> shared memory, buffer cur^1
-        {
-            Row<T> first, last;
-            eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
-                            f, c, q, first, last);
-            const int o = (cur ^ 1) * M + 2 * t;
-            sA[o] = first.A; sA[o + 1] = last.A;
-            sC[o] = first.C; sC[o + 1] = last.C;
-            sD[o] = first.D; sD[o + 1] = last.D;
-        }
+        // ---- assembly + partition elimination
+        Row<T> first, last;
+        eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
+                        f, c, q, first, last);
+        // ---- cyclic-reduction step: substitute the x_0 rows of threads t and t+1 into the x_L row
+        // of thread t:  [-f A] x_L(t-1) + [1 - f C - c A'] x_L(t) + [-c C'] x_L(t+1) = q - f D - c D'
+        sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
         __syncthreads();
-        cur ^= 1;
-        // ---- parallel cyclic reduction over the M interface rows
+        Row<T> r;
+        {
+            const int tn = (t + 1) & mask;
+            const T nA = sFA[tn], nC = sFC[tn], nD = sFD[tn];
+            const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
+            r.A = -last.A * first.A * m;
+            r.C = -last.C * nC * m;
+            r.D = t_fma(-last.A, first.D, t_fma(-last.C, nD, last.D)) * m;
+        }
+        int cur = 0;
+        sA[t] = r.A; sC[t] = r.C; sD[t] = r.D;
+        __syncthreads();
+        // ---- parallel cyclic reduction over the Tn reduced rows (cyclic chain), early exit
         bool finished = false;
-        for (int s = 1; s < Tn; s <<= 1) {
-            int flag = 0;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int k = t + h * Tn;
-                const int km = (k - s) & (M - 1), kp = (k + s) & (M - 1);
-                const T *pA = sA + cur * M, *pC = sC + cur * M, *pD = sD + cur * M;
-                const T A = pA[k], C = pC[k], D = pD[k];
-                const T m = rcp(t_fma(-A, pC[km], t_fma(-C, pA[kp], T(1))));
-                const T An = -A * pA[km] * m;
-                const T Cn = -C * pC[kp] * m;
-                const T Dn = t_fma(-A, pD[km], t_fma(-C, pD[kp], D)) * m;
-                const int o = (cur ^ 1) * M + k;
-                sA[o] = An; sC[o] = Cn; sD[o] = Dn;
-                flag |= (t_abs(An) > Lim<T>::tiny()) | (t_abs(Cn) > Lim<T>::tiny());
-            }
+        for (int s = 1; s < Tn / 2; s <<= 1) {
+            const int km = (t - s) & mask, kp = (t + s) & mask;
+            const T *pA = sA + cur * Tn, *pC = sC + cur * Tn, *pD = sD + cur * Tn;
+            Row<T> rm, rp;
+            rm.A = pA[km]; rm.C = pC[km]; rm.D = pD[km];
+            rp.A = pA[kp]; rp.C = pC[kp]; rp.D = pD[kp];
+            r = pcr_combine(r, rm, rp);
+            const int o = (cur ^ 1) * Tn + t;
+            sA[o] = r.A; sC[o] = r.C; sD[o] = r.D;
+            const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
             const int any = __syncthreads_or(flag);
             cur ^= 1;
             if (!any) { finished = true; break; }
         }
-        if (!finished) {  // rows k and k+Tn couple only to each other: exact 2x2 solve
-            const T *pA = sA + cur * M, *pC = sC + cur * M, *pD = sD + cur * M;
-            const int k = t, k2 = t + Tn;
-            const T p1 = pA[k] + pC[k], p2 = pA[k2] + pC[k2];
-            const T D1 = pD[k], D2 = pD[k2];
-            const T m = rcp(t_fma(-p1, p2, T(1)));
-            sD[(cur ^ 1) * M + k] = t_fma(-p1, D2, D1) * m;
-            sD[(cur ^ 1) * M + k2] = t_fma(-p2, D1, D2) * m;
+        T xL = r.D, xLprev;
+        if (finished) {
+            xLprev = sD[cur * Tn + ((t - 1) & mask)];
+        } else {  // rows t and t + Tn/2 couple only to each other: exact 2x2 solve
+            const int o = (t + Tn / 2) & mask;
+            const T p1 = r.A + r.C, p2 = sA[cur * Tn + o] + sC[cur * Tn + o];
+            const T D2 = sD[cur * Tn + o];
+            xL = t_fma(-p1, D2, r.D) * rcp(t_fma(-p1, p2, T(1)));
+            sFD[t] = xL;               // sFD is free: its readers passed two barriers ago
             __syncthreads();
-            cur ^= 1;
+            xLprev = sFD[(t - 1) & mask];
         }
-        // ---- back substitution
-        back_substitute<T, P>(v, f, c, q, sD[cur * M + 2 * t], sD[cur * M + 2 * t + 1]);
+        // ---- recover x_0 and back-substitute
+        const T x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
+        back_substitute<T, P>(v, f, c, q, x0, xL);
     }
 
 #pragma unroll
@@ -147,7 +156,7 @@ bool hybrid_geometry(int is_f64, int64_t N, int *P_out, int *T_out) {
 template <typename T, int P>
 int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
              int Tn, cudaStream_t s) {
-    const size_t smem = (size_t)12 * Tn * sizeof(T);
+    const size_t smem = (size_t)9 * Tn * sizeof(T);
     btcs_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
     return last_launch_status();
 }
