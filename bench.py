@@ -393,8 +393,10 @@ def run_reference(args):
            "value": value, "unit": "updates/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": sec / max(1, len(vals)) * 1e3, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"{args.workload}: {w.name} (bounded sample per step: {desc})",
-                      "N": w.N, "n_steps": w.n_steps},
+           "config": {"workload": f"{args.workload}: {w.name}, {w.n_steps} time steps per bench step, "
+                                  f"bc={'periodic' if w.bc == 0 else 'dirichlet'}, CFL {w.cfl}",
+                      "B_per_gpu": w.B, "N": w.N, "n_steps": w.n_steps, "sample": desc,
+                      "input_sha256": w.sha256()[:16]},
            "cpu_baseline": {"value": value, "unit": "updates/s", "cores": threads, "kind": "oracle",
                             "sample": desc, "cpu": cpu_info()},
            "e2e": {"value": value, "unit": "updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},

@@ -90,10 +90,12 @@ int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, 
 }
 
 // ---- host-buffer path: allocate, copy in, run the device path, copy out, free ---------------
+// Stream-ordered allocations from the device's default memory pool (cudaMallocAsync): after the
+// first call the pool serves them without a driver round trip; nothing is kept by the library.
 struct DevBuf {
     void *p = nullptr;
-    ~DevBuf() { if (p) cudaFree(p); }
-    bool alloc(size_t bytes) { return bytes == 0 || cudaMalloc(&p, bytes) == cudaSuccess; }
+    ~DevBuf() { if (p) cudaFreeAsync(p, nullptr); }
+    bool alloc(size_t bytes) { return bytes == 0 || cudaMallocAsync(&p, bytes, nullptr) == cudaSuccess; }
 };
 
 template <typename T, typename F>
