@@ -84,6 +84,50 @@ cfl_reduce_kernel(const T *__restrict__ u, const T *__restrict__ nu, T *__restri
     }
 }
 
+// Short rows (at most kWarpRowVecs 16-byte vectors): ONE WARP PER TRAJECTORY, several trajectories
+// per CTA, no shared memory and no CTA barrier; every lane keeps up to 8 independent 128-bit loads
+// in flight.  (One CTA per 4 KB row, as the chunked kernel would do for config 5, is latency-bound:
+// measured 2.5 TB/s.)
+constexpr int kWarpRowVecs = 1024;   // rows up to 16 KB
+constexpr int kWarpRowWarps = 8;
+
+template <typename T>
+__global__ void __launch_bounds__(kWarpRowWarps * 32)
+cfl_warp_row_kernel(const T *__restrict__ u, const T *__restrict__ nu, T *__restrict__ dt_out,
+                    int64_t B, int64_t N, double dx, double C) {
+    constexpr int V = 16 / sizeof(T);
+    const int lane = threadIdx.x & 31;
+    const int64_t b = (int64_t)blockIdx.x * kWarpRowWarps + (threadIdx.x >> 5);
+    if (b >= B) return;
+    const int4 *row4 = reinterpret_cast<const int4 *>(u + b * N);   // N % V == 0: 16-byte aligned rows
+    const int nv = (int)(N / V);
+    T m = T(0);
+    int i = lane;
+    for (; i + 7 * 32 < nv; i += 8 * 32) {
+        int4 q[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) q[k] = __ldg(row4 + i + k * 32);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const T *e = reinterpret_cast<const T *>(&q[k]);
+#pragma unroll
+            for (int j = 0; j < V; ++j) m = absmax(m, e[j]);
+        }
+    }
+    for (; i < nv; i += 32) {
+        int4 q = __ldg(row4 + i);
+        const T *e = reinterpret_cast<const T *>(&q);
+#pragma unroll
+        for (int j = 0; j < V; ++j) m = absmax(m, e[j]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        T other = __shfl_xor_sync(0xffffffffu, m, o);
+        m = (other > m) ? other : m;
+    }
+    if (lane == 0) dt_out[b] = cfl_dt<T>(m, nu[b], dx, C);
+}
+
 template <typename T>
 __global__ void cfl_finalize_kernel(const T *__restrict__ nu, T *__restrict__ dt_out, int64_t B,
                                     double dx, double C) {
@@ -107,6 +151,12 @@ template <typename T>
 int launch_cfl(const T *u, int64_t B, int64_t N, double dx, const T *nu, double C, T *dt_out,
                cudaStream_t s) {
     const int V = 16 / (int)sizeof(T);
+    if (N % V == 0 && N / V <= kWarpRowVecs && B >= 4 * 148) {    // many short rows: warp per trajectory
+        const int64_t grid = (B + kWarpRowWarps - 1) / kWarpRowWarps;
+        if (grid > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+        cfl_warp_row_kernel<T><<<(unsigned)grid, kWarpRowWarps * 32, 0, s>>>(u, nu, dt_out, B, N, dx, C);
+        return last_launch_status();
+    }
     const int threads = cfl_threads(N, V);
     const int64_t span = (int64_t)threads * kCflItems;
     const int64_t chunks = (N + span - 1) / span;
@@ -125,8 +175,8 @@ int launch_cfl(const T *u, int64_t B, int64_t N, double dx, const T *nu, double 
 }
 
 int64_t cfl_launch_count(int is_f64, int64_t B, int64_t N) {
-    (void)B;
     const int V = is_f64 ? 2 : 4;
+    if (N % V == 0 && N / V <= kWarpRowVecs && B >= 4 * 148) return 1;
     const int64_t span = (int64_t)cfl_threads(N, V) * kCflItems;
     return ((N + span - 1) / span > 1) ? 2 : 1;
 }

@@ -54,7 +54,8 @@ def check_btcs(B, w, n, cfl=None, **kw):
 
 # ------------------------------------------------------------------ dt_from_cfl (a1)
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
-@pytest.mark.parametrize("shape", [(1, 3), (5, 17), (7, 256), (3, 4099), (2, 70001), (1, 1 << 20), (300, 1024)])
+@pytest.mark.parametrize("shape", [(1, 3), (5, 17), (7, 256), (3, 4099), (2, 70001), (1, 1 << 20), (300, 1024),
+                                   (700, 1024), (1000, 36), (600, 4100), (593, 2048)])   # >= 592 short rows: warp per row
 def test_dt_from_cfl_matches_oracle(B, dtype, shape):
     rng = np.random.default_rng(7)
     Bn, N = shape
