@@ -356,6 +356,119 @@ int oracle_dt_from_cfl(const double *u, int64_t B, int64_t N, double L,
     return 0;
 }
 
+/* ---------------------------------------------------------------------------
+ * D11: fully implicit BTCS with CENTRAL convection solved
+ * by Newton-Raphson, as the paper writes it out (Eq.10-15).
+ * Residual (Eq.11), w = iterate for u^{n+1}, h = dt/(2 dx), r = nu dt/dx^2:
+ *   F_i(w) = w_i - u_i^n + h w_i (w_{i+1} - w_{i-1}) - r (w_{i+1} - 2 w_i + w_{i-1})
+ * Jacobian (Eq.14; Eq.15 is garbled in the paper -- reading Q5: differentiate Eq.11):
+ *   J_{i,i-1} = -h w_i - r,  J_{i,i} = 1 + h (w_{i+1} - w_{i-1}) + 2 r,  J_{i,i+1} = h w_i - r
+ * Newton (Eq.12-13): w^0 = u^n; while max_i |F_i(w^k)| >= tol and k < max_iter:
+ *   solve J(w^k) delta = -F(w^k), w^{k+1} = w^k + delta.   (criterion: PAPER.md:245)
+ * Dirichlet: end nodes fixed (F = 0, delta = 0 there); periodic: cyclic system.
+ * Test hook use_adv: the multiplying w_i is replaced by the constant adv (linear
+ * advection-diffusion: J does not depend on w, one iteration is exact).
+ * No pivoting: J is diagonally dominant when the cell Peclet number
+ * |w| dx / nu <= 2 and h (w_{i+1} - w_{i-1}) > -1 (D11).
+ */
+static void newton_residual(const double *w, const double *un, int64_t N, double h,
+                            double r, int bc, int use_adv, double adv, double *F)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) { F[i] = 0.0; continue; }
+        int64_t im = (i == 0) ? N - 1 : i - 1;
+        int64_t ip = (i == N - 1) ? 0 : i + 1;
+        double a = use_adv ? adv : w[i];
+        F[i] = w[i] - un[i] + h * a * (w[ip] - w[im]) - r * (w[ip] - 2.0 * w[i] + w[im]);
+    }
+}
+
+static void newton_jacobian(const double *w, int64_t N, double h, double r, int bc,
+                            int use_adv, double adv, double *sub, double *diag, double *sup)
+{
+    for (int64_t i = 0; i < N; ++i) {
+        if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) { sub[i] = 0.0; diag[i] = 1.0; sup[i] = 0.0; continue; }
+        int64_t im = (i == 0) ? N - 1 : i - 1;
+        int64_t ip = (i == N - 1) ? 0 : i + 1;
+        double a = use_adv ? adv : w[i];
+        sub[i] = -h * a - r;
+        diag[i] = 1.0 + (use_adv ? 0.0 : h * (w[ip] - w[im])) + 2.0 * r;
+        sup[i] = h * a - r;
+    }
+}
+
+/* Exposed for the pins (worked example, finite-difference Jacobian check). */
+void oracle_newton_residual(const double *w, const double *un, int64_t N, double L, double nu,
+                            double dt, int bc, int use_adv, double adv, double *F)
+{
+    double dx = grid_dx(N, L, bc);
+    newton_residual(w, un, N, dt / (2.0 * dx), nu * dt / (dx * dx), bc, use_adv, adv, F);
+}
+void oracle_newton_jacobian(const double *w, int64_t N, double L, double nu, double dt, int bc,
+                            int use_adv, double adv, double *sub, double *diag, double *sup)
+{
+    double dx = grid_dx(N, L, bc);
+    newton_jacobian(w, N, dt / (2.0 * dx), nu * dt / (dx * dx), bc, use_adv, adv, sub, diag, sup);
+}
+
+/* One trajectory; returns the total number of Newton iterations (linear solves).
+ * wk: 13N doubles. */
+static int64_t newton_one(double *u, int64_t N, double dx, double nu, double dt, int64_t n_steps,
+                          int bc, double tol, int max_iter, int use_adv, double adv, double *wk)
+{
+    double *w = wk, *F = wk + N, *sub = wk + 2 * N, *diag = wk + 3 * N, *sup = wk + 4 * N,
+           *rhs = wk + 5 * N, *x = wk + 6 * N, *wk2 = wk + 7 * N; /* 6N */
+    double h = dt / (2.0 * dx), r = nu * dt / (dx * dx);
+    int64_t total = 0;
+    for (int64_t n = 0; n < n_steps; ++n) {
+        for (int64_t i = 0; i < N; ++i) w[i] = u[i];
+        for (int k = 0;; ++k) {
+            newton_residual(w, u, N, h, r, bc, use_adv, adv, F);
+            double m = 0.0;
+            for (int64_t i = 0; i < N; ++i) { double a = fabs(F[i]); if (!(a <= m)) m = a; }
+            if (m < tol || k >= max_iter) break;
+            newton_jacobian(w, N, h, r, bc, use_adv, adv, sub, diag, sup);
+            for (int64_t i = 0; i < N; ++i) rhs[i] = -F[i];
+            if (bc == BC_PERIODIC) cyclic_sm(N, sub, diag, sup, rhs, x, wk2);
+            else thomas(N, sub, diag, sup, rhs, x, wk2, wk2 + N);   /* identity rows at the ends */
+            for (int64_t i = 0; i < N; ++i) w[i] = w[i] + x[i];
+            ++total;
+        }
+        for (int64_t i = 0; i < N; ++i) u[i] = w[i];
+    }
+    return total;
+}
+
+/* B trajectories, in place; iters_out[b] (may be NULL) = Newton iterations summed over the steps. */
+int oracle_newton_btcs(double *u, int64_t B, int64_t N, double L, const double *nu,
+                       const double *dt, int64_t n_steps, int bc, double tol, int max_iter,
+                       int use_adv, double adv, int64_t *iters_out, int nthreads)
+{
+    if (!u || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0) || max_iter < 0) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel num_threads(nthreads)
+    {
+        double *wk = (double *)malloc((size_t)13 * (size_t)N * sizeof(double));
+        if (!wk) {
+#pragma omp atomic write
+            fail = 1;
+        } else {
+#pragma omp for schedule(dynamic, 1)
+            for (int64_t b = 0; b < B; ++b) {
+                int64_t it = newton_one(u + b * N, N, dx, nu[b], dt[b], n_steps, bc, tol, max_iter,
+                                        use_adv, adv, wk);
+                if (iters_out) iters_out[b] = it;
+            }
+            free(wk);
+        }
+    }
+    return fail ? -1 : 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

@@ -92,6 +92,56 @@ def btcs_exact(u, dx, nu, dt, bc):
     return rows, [u[0]] + x + [u[N - 1]]
 
 
+def newton_exact(u, dx, nu, dt, bc, iters):
+    """`iters` Newton iterations on the residual of PAPER.md Eq.11 (central convection, all terms at
+    n+1) from w0 = u^n, with the Jacobian obtained by differentiating Eq.11 (Q5/D11)."""
+    N = len(u)
+    h, r = dt / (2 * dx), nu * dt / dx ** 2
+    idx = list(range(N)) if bc == "periodic" else list(range(1, N - 1))
+    w = list(u)
+    out = []
+    for _ in range(iters):
+        F = {}
+        M = [[Fr(0)] * N for _ in range(N)]
+        for i in idx:
+            wm, wp, wi = w[(i - 1) % N], w[(i + 1) % N], w[i]
+            F[i] = wi - u[i] + h * wi * (wp - wm) - r * (wp - 2 * wi + wm)      # Eq.11
+            M[i][(i - 1) % N] += -h * wi - r
+            M[i][i] += 1 + h * (wp - wm) + 2 * r
+            M[i][(i + 1) % N] += h * wi - r
+        Mi = [[M[i][j] for j in idx] for i in idx]          # frozen end nodes: delta = 0
+        d = solve_exact(Mi, [-F[i] for i in idx])           # Eq.12
+        for i, di in zip(idx, d):
+            w[i] = w[i] + di                                 # Eq.13
+        out.append(list(w))
+    return out
+
+
+def write_newton_example():
+    u = [Fr(1), Fr(2), Fr(-1), Fr(0)]
+    dx, nu, dt = Fr(1), Fr(1, 10), Fr(1, 10)
+    lines = [
+        "# Newton-Raphson on PAPER.md Eq.11 (fully implicit, central convection), 4-node example:",
+        "# u^n=[1,2,-1,0], dx=1, nu=0.1, dt=0.1; iterates w^1, w^2, w^3 from w^0 = u^n in exact rational",
+        "# arithmetic (tests/golden/make_golden.py), rounded once to fp64.  Eq.12-13 PAPER.md:147-151.",
+    ]
+    N = len(u)
+    h, r = dt / (2 * dx), nu * dt / dx ** 2
+    F0 = [u[i] - u[i] + h * u[i] * (u[(i + 1) % N] - u[(i - 1) % N]) - r * (u[(i + 1) % N] - 2 * u[i] + u[(i - 1) % N])
+          for i in range(N)]
+    lines.append("F0_periodic " + fmt(F0))
+    lines.append("J0_sub_periodic " + fmt([-h * u[i] - r for i in range(N)]))
+    lines.append("J0_diag_periodic " + fmt([1 + h * (u[(i + 1) % N] - u[(i - 1) % N]) + 2 * r for i in range(N)]))
+    lines.append("J0_sup_periodic " + fmt([h * u[i] - r for i in range(N)]))
+    for k, w in enumerate(newton_exact(u, dx, nu, dt, "periodic", 3), 1):
+        lines.append(f"newton{k}_periodic " + fmt(w))
+    lines.append("# Dirichlet: same u, L=3 (dx=1), end nodes frozen at 1 and 0")
+    for k, w in enumerate(newton_exact(u, dx, nu, dt, "dirichlet", 3), 1):
+        lines.append(f"newton{k}_dirichlet " + fmt(w))
+    with open(os.path.join(HERE, "newton_4node.txt"), "w") as f:
+        f.write("\n".join(lines) + "\n")
+
+
 def fmt(vals):
     return " ".join(repr(float(v)) for v in vals)
 
@@ -175,5 +225,6 @@ def write_colehopf():
 
 if __name__ == "__main__":
     write_worked_example()
+    write_newton_example()
     write_colehopf()
     print("golden fixtures written to", HERE)
