@@ -80,6 +80,25 @@ int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
 }
 
 template <typename T>
+int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
+                double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
+    const int is_f64 = sizeof(T) == 8;
+    if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
+    if (plan != BURGERS_PLAN_HYBRID && plan != BURGERS_PLAN_THOMAS) return BURGERS_ERR_ENUM;
+    if (plan == BURGERS_PLAN_HYBRID && !newton_hybrid_fits(is_f64, N)) return BURGERS_ERR_PLAN;
+    if (plan == BURGERS_PLAN_THOMAS) {
+        const size_t need = newton_thomas_ws_elems(B, N, bc) * sizeof(T);
+        if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
+    }
+    static_assert(sizeof(long long) == sizeof(int64_t), "iters_out is int64");
+    return launch_newton<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, tol, max_iter,
+                            reinterpret_cast<long long *>(iters_out), plan, (T *)ws, (cudaStream_t)stream);
+}
+
+template <typename T>
 int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out,
              void *stream) {
     if (!u || !nu || !dt_out) return BURGERS_ERR_NULL;
@@ -194,6 +213,17 @@ int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const doubl
     return btcs_call<double>(u, B, N, L, nu, dt, n_steps, bc, plan, ws, ws_bytes, stream);
 }
 
+int burgers_newton_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, int plan,
+                       void *ws, size_t ws_bytes, void *stream) {
+    return newton_call<float>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
+}
+int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, int plan,
+                       void *ws, size_t ws_bytes, void *stream) {
+    return newton_call<double>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
+}
+
 int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C, int bc,
                     float *dt_out, void *stream) {
     return cfl_call<float>(u, B, N, L, nu, C, bc, dt_out, stream);
@@ -241,6 +271,10 @@ size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, i
         if (explicit_geometry(dtype_is_f64, B, N, bc, scheme, plan, 0, 0, &g) != BURGERS_OK) return 0;
         return g.plan == BURGERS_PLAN_TILED ? align_up((size_t)B * (size_t)N * esz, 256) : 0;
     }
+    if (op == BURGERS_OP_NEWTON) {
+        if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
+        return plan == BURGERS_PLAN_THOMAS ? align_up(newton_thomas_ws_elems(B, N, bc) * esz, 256) : 0;
+    }
     if (op == BURGERS_OP_BTCS) {
         if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
         if (plan == BURGERS_PLAN_THOMAS) return align_up(btcs_thomas_ws_elems(B, N, bc) * esz, 256);
@@ -259,6 +293,7 @@ int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, i
         return st == BURGERS_OK ? g.plan : st;
     }
     if (op == BURGERS_OP_BTCS) return btcs_auto_plan(dtype_is_f64, B, N, bc);
+    if (op == BURGERS_OP_NEWTON) return newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
     if (op == BURGERS_OP_CFL) return BURGERS_PLAN_AUTO;
     return BURGERS_ERR_ENUM;
 }
@@ -272,6 +307,10 @@ int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int
         ExplicitGeom g;
         if (explicit_geometry(dtype_is_f64, B, N, bc, scheme, plan, tblock, 0, &g) != BURGERS_OK) return 0;
         return g.plan == BURGERS_PLAN_RESIDENT ? 1 : (n_steps + g.tblock - 1) / g.tblock;
+    }
+    if (op == BURGERS_OP_NEWTON) {
+        if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
+        return plan == BURGERS_PLAN_HYBRID ? 1 : 3;
     }
     if (op == BURGERS_OP_BTCS) {
         if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
@@ -289,7 +328,7 @@ const char *burgers_strerror(int status) {
         case BURGERS_ERR_NULL: return "null pointer argument";
         case BURGERS_ERR_SHAPE: return "bad shape (need B>=1, N>=3, n_steps>=0, grid within limits)";
         case BURGERS_ERR_ENUM: return "unknown bc / scheme / plan / op";
-        case BURGERS_ERR_VALUE: return "bad value (need finite L>0, C>0)";
+        case BURGERS_ERR_VALUE: return "bad value (need finite L>0, C>0, tol>=0, max_iter>=0)";
         case BURGERS_ERR_WORKSPACE: return "workspace missing or too small (see burgers_workspace_bytes)";
         case BURGERS_ERR_CUDA: return "CUDA runtime / launch failure";
         case BURGERS_ERR_PLAN: return "requested plan cannot run this shape";

@@ -129,6 +129,102 @@ __device__ __forceinline__ void eliminate(const T (&v)[P], const Coef<T> &co, Id
     last.D = q[P - 1];
 }
 
+// The same partition elimination for GENERAL rows (newton.cu): rowfn(j, a, b, e) yields sub / diag /
+// sup of row j; q[] holds the right-hand sides on entry and the eliminated ones on exit.
+template <typename T, int P, typename RowFn>
+__device__ __forceinline__ void eliminate_general(RowFn rowfn, T (&q)[P], T (&f)[P], T (&c)[P],
+                                                  Row<T> &first, Row<T> &last) {
+    static_assert(P >= 3, "a partition needs at least 3 rows");
+    T a0, b0, e0;
+    rowfn(0, a0, b0, e0);
+    const T d0 = q[0];
+    {
+        T a, b, e;
+        rowfn(1, a, b, e);
+        const T m = rcp(b);
+        f[1] = a * m; c[1] = e * m; q[1] = q[1] * m;
+    }
+#pragma unroll
+    for (int j = 2; j < P; ++j) {
+        T a, b, e;
+        rowfn(j, a, b, e);
+        const T m = rcp(t_fma(-a, c[j - 1], b));
+        const T am = a * m;
+        f[j] = -am * f[j - 1];
+        c[j] = e * m;
+        q[j] = t_fma(-am, q[j - 1], q[j] * m);
+    }
+    T F = f[P - 2], G = c[P - 2], R = q[P - 2];
+#pragma unroll
+    for (int j = P - 3; j >= 1; --j) {
+        F = t_fma(-c[j], F, f[j]);
+        G = -c[j] * G;
+        R = t_fma(-c[j], R, q[j]);
+    }
+    const T m = rcp(t_fma(-e0, F, b0));
+    first.A = a0 * m;
+    first.C = -e0 * G * m;
+    first.D = t_fma(-e0, R, d0) * m;
+    last.A = f[P - 1];
+    last.C = c[P - 1];
+    last.D = q[P - 1];
+}
+
+// Solve the cyclic interface system of one CTA (Tn = blockDim.x threads, a power of two >= 2) given
+// every thread's two interface rows: one cyclic-reduction step (one reduced row per thread in the
+// unknowns x_L), parallel cyclic reduction with early exit, exact 2x2 ending; returns this thread's
+// x_0 and x_L.  smem: sA, sC, sD of 2*Tn entries each (PCR ping-pong), sF of 3*Tn entries.
+// Contains CTA barriers: call from uniform control flow.
+template <typename T>
+__device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T> &last, T *sA, T *sC, T *sD,
+                                                T *sF, T &x0, T &xL) {
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    T *sFA = sF, *sFC = sF + Tn, *sFD = sF + 2 * Tn;
+    sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
+    __syncthreads();
+    Row<T> r;
+    {
+        const int tn = (t + 1) & mask;
+        const T nA = sFA[tn], nC = sFC[tn], nD = sFD[tn];
+        const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
+        r.A = -last.A * first.A * m;
+        r.C = -last.C * nC * m;
+        r.D = t_fma(-last.A, first.D, t_fma(-last.C, nD, last.D)) * m;
+    }
+    int cur = 0;
+    sA[t] = r.A; sC[t] = r.C; sD[t] = r.D;
+    __syncthreads();
+    bool finished = false;
+    for (int s = 1; s < Tn / 2; s <<= 1) {
+        const int km = (t - s) & mask, kp = (t + s) & mask;
+        const T *pA = sA + cur * Tn, *pC = sC + cur * Tn, *pD = sD + cur * Tn;
+        Row<T> rm, rp;
+        rm.A = pA[km]; rm.C = pC[km]; rm.D = pD[km];
+        rp.A = pA[kp]; rp.C = pC[kp]; rp.D = pD[kp];
+        r = pcr_combine(r, rm, rp);
+        const int o = (cur ^ 1) * Tn + t;
+        sA[o] = r.A; sC[o] = r.C; sD[o] = r.D;
+        const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
+        const int any = __syncthreads_or(flag);
+        cur ^= 1;
+        if (!any) { finished = true; break; }
+    }
+    T xLprev;
+    xL = r.D;
+    if (finished) {
+        xLprev = sD[cur * Tn + ((t - 1) & mask)];
+    } else {  // rows t and t + Tn/2 couple only to each other: exact 2x2 solve
+        const int o = (t + Tn / 2) & mask;
+        const T p1 = r.A + r.C, p2 = sA[cur * Tn + o] + sC[cur * Tn + o];
+        const T D2 = sD[cur * Tn + o];
+        xL = t_fma(-p1, D2, r.D) * rcp(t_fma(-p1, p2, T(1)));
+        sD[(cur ^ 1) * Tn + t] = xL;   // the other PCR buffer is free; the next write to it follows a barrier
+        __syncthreads();
+        xLprev = sD[(cur ^ 1) * Tn + ((t - 1) & mask)];
+    }
+    x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
+}
+
 // Back substitution into v[] given the partition's end unknowns x0 = x_0, xl = x_{P-1}.
 template <typename T, int P>
 __device__ __forceinline__ void back_substitute(T (&v)[P], const T (&f)[P], const T (&c)[P],

@@ -114,9 +114,9 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
             const T p1 = r.A + r.C, p2 = sA[cur * Tn + o] + sC[cur * Tn + o];
             const T D2 = sD[cur * Tn + o];
             xL = t_fma(-p1, D2, r.D) * rcp(t_fma(-p1, p2, T(1)));
-            sFD[t] = xL;               // sFD is free: its readers passed two barriers ago
+            sD[(cur ^ 1) * Tn + t] = xL;   // the other PCR buffer is free; its next write follows a barrier
             __syncthreads();
-            xLprev = sFD[(t - 1) & mask];
+            xLprev = sD[(cur ^ 1) * Tn + ((t - 1) & mask)];
         }
         // ---- recover x_0 and back-substitute
         const T x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));

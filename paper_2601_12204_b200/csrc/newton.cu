@@ -1,0 +1,321 @@
+// newton.cu -- SURVEY 8(f) NEXT-1: fully implicit BTCS with CENTRAL convection solved by
+// Newton-Raphson, the implicit scheme the paper writes out (Eq.10-15).
+//
+// Per time step (D11), w = iterate for u^{n+1}, h = dt/(2 dx), r = nu dt/dx^2:
+//   residual (Eq.11)   F_i = w_i - u_i^n + h w_i (w_{i+1} - w_{i-1}) - r (w_{i+1} - 2 w_i + w_{i-1})
+//   Jacobian (Eq.14; Eq.15 is garbled -- reading Q5: the derivative of Eq.11)
+//                      J_{i,i-1} = -h w_i - r,  J_{i,i} = 1 + h (w_{i+1} - w_{i-1}) + 2r,  J_{i,i+1} = h w_i - r
+//   Newton (Eq.12-13)  w^0 = u^n;  while max_i |F_i(w^k)| >= tol and k < max_iter:
+//                      solve J(w^k) delta = -F(w^k),  w^{k+1} = w^k + delta
+// (stopping rule: "maximum residual falling below 1e-6"; tol is an argument).
+// Dirichlet end nodes are identity rows with zero right-hand side; periodic systems are cyclic.
+// Residual and Jacobian are fused into the solver: nothing but u touches HBM.
+//
+// Two plans:
+//   HYBRID  one CTA per system, w and u^n resident in registers for all n_steps; per Newton iteration
+//           one halo exchange, the residual with a block-wide convergence vote, then the same partition
+//           elimination + cyclic-reduction + PCR interface solve as btcs_hybrid.cu (btcs_common.cuh)
+//           on the Jacobian rows.  No pivoting: J is diagonally dominant when the cell Peclet number
+//           |w| dx / nu <= 2 and h (w_{i+1} - w_{i-1}) > -1.
+//   THOMAS  one thread per system on the interleaved [N][B] workspace layout of btcs_thomas.cu (any
+//           N >= 3), Sherman-Morrison for periodic systems; the general-shape fallback and cross-check.
+#include "btcs_common.cuh"
+
+namespace burgers {
+namespace {
+
+using namespace btcs;
+
+constexpr int newton_max_threads(int bytes, int P) {
+    int regs = P * (bytes / 4) * 5 + 56;
+    int t = 1024;
+    while (t > 32 && t * regs > 65536) t /= 2;
+    return t;
+}
+
+template <typename T, int P>
+__global__ void __launch_bounds__(newton_max_threads(sizeof(T), P))
+newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
+                     double inv_dx, int64_t n_steps, int bc, T tol, int max_iter,
+                     long long *__restrict__ iters_out) {
+    constexpr int V = 16 / sizeof(T);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn]
+    T *sC = sA + 2 * Tn;
+    T *sD = sC + 2 * Tn;
+    T *sF = sD + 2 * Tn;                      // [3][Tn]
+    T *sE = sF + 3 * Tn;                      // [2][Tn] partition edge values of w
+    T *row = u + (int64_t)blockIdx.x * N + (int64_t)t * P;
+
+    const double dtb = (double)dt[blockIdx.x];
+    const T h = (T)(0.5 * dtb * inv_dx);
+    const T r = (T)((double)nu[blockIdx.x] * dtb * inv_dx * inv_dx);
+    const T b0 = T(1) + T(2) * r;
+    const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
+    const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
+
+    T w[P], un[P];
+#pragma unroll
+    for (int c = 0; c < P / V; ++c) {
+        int4 q4 = *reinterpret_cast<const int4 *>(row + c * V);
+        const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+        for (int k = 0; k < V; ++k) w[c * V + k] = e[k];
+    }
+    long long iters = 0;
+    for (int64_t n = 0; n < n_steps; ++n) {
+#pragma unroll
+        for (int j = 0; j < P; ++j) un[j] = w[j];
+        for (int k = 0;; ++k) {
+            // ---- halo exchange of the partition edges
+            sE[t] = w[0]; sE[Tn + t] = w[P - 1];
+            __syncthreads();
+            const T wl = sE[Tn + ((t - 1) & mask)], wr = sE[(t + 1) & mask];
+            // ---- residual (Eq.11); q = -F is the right-hand side of Eq.12
+            T q[P];
+            int big = 0;
+#pragma unroll
+            for (int j = 0; j < P; ++j) {
+                const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
+                const T dc = wp - wm;
+                const T lap = (wp - w[j]) - (w[j] - wm);
+                T F = t_fma(h * w[j], dc, t_fma(-r, lap, w[j] - un[j]));
+                if ((j == 0 && fixL) || (j == P - 1 && fixR)) F = T(0);
+                q[j] = -F;
+                big |= !(t_abs(F) < tol);          // NaN counts as not converged
+            }
+            const int any = __syncthreads_or(big);  // also orders the sE reads before the next writes
+            if (!any || k >= max_iter) break;       // uniform over the CTA
+            // ---- Jacobian rows (Eq.14), partition elimination, interface solve, back substitution
+            T f[P], c[P];
+            Row<T> first, last;
+            eliminate_general<T, P>(
+                [&](int j, T &a, T &b, T &e) {
+                    if ((j == 0 && fixL) || (j == P - 1 && fixR)) { a = T(0); b = T(1); e = T(0); return; }
+                    const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
+                    const T hw = h * w[j];
+                    a = -hw - r;
+                    b = t_fma(h, wp - wm, b0);
+                    e = hw - r;
+                },
+                q, f, c, first, last);
+            T x0, xL;
+            solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL);
+            T d[P];
+#pragma unroll
+            for (int j = 0; j < P; ++j) d[j] = T(0);
+            back_substitute<T, P>(d, f, c, q, x0, xL);
+#pragma unroll
+            for (int j = 0; j < P; ++j) w[j] += d[j];      // Eq.13
+            ++iters;
+        }
+    }
+    if (iters_out && t == 0) iters_out[blockIdx.x] = iters;
+
+#pragma unroll
+    for (int c = 0; c < P / V; ++c) {
+        int4 q4;
+        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+        for (int k = 0; k < V; ++k) e[k] = w[c * V + k];
+        *reinterpret_cast<int4 *>(row + c * V) = q4;
+    }
+}
+
+bool pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
+
+bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out) {
+    const int bytes = is_f64 ? 8 : 4;
+    const int cand[3] = {8, 16, 4};           // 8 first: five arrays of P values live in registers
+    int bestP = 0;
+    for (int i = 0; i < 3; ++i) {
+        const int P = cand[i];
+        if (N % P) continue;
+        const int64_t Tn = N / P;
+        if (!pow2(Tn) || Tn < 2 || Tn > newton_max_threads(bytes, P)) continue;
+        if (Tn >= 32) { bestP = P; break; }
+        if (!bestP || P < bestP) bestP = P;
+    }
+    if (!bestP) return false;
+    *P_out = bestP; *T_out = (int)(N / bestP);
+    return true;
+}
+
+template <typename T, int P>
+int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                    double tol, int max_iter, long long *iters_out, int Tn, cudaStream_t s) {
+    const size_t smem = (size_t)11 * Tn * sizeof(T);
+    newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)tol,
+                                                            max_iter, iters_out);
+    return last_launch_status();
+}
+
+// ------------------------------------------------------------------ thread-per-system plan
+template <typename T>
+__global__ void newton_transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int64_t rows, int64_t cols) {
+    __shared__ T tile[32][33];
+    const int64_t gx = (cols + 31) / 32;
+    const int64_t c0 = ((int64_t)blockIdx.x % gx) * 32, r0 = ((int64_t)blockIdx.x / gx) * 32;
+    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
+        int64_t r = r0 + k, c = c0 + threadIdx.x;
+        if (r < rows && c < cols) tile[k][threadIdx.x] = in[r * cols + c];
+    }
+    __syncthreads();
+    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
+        int64_t c = c0 + k, r = r0 + threadIdx.x;
+        if (r < rows && c < cols) out[c * rows + r] = tile[threadIdx.x][k];
+    }
+}
+
+// ws arrays (each [N][B], batch index fastest): un, w, cp, dp (= rhs, then solution), and for periodic
+// systems wp (second right-hand side of Sherman-Morrison).
+template <typename T>
+__global__ void __launch_bounds__(128)
+newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, T *__restrict__ dp,
+                     T *__restrict__ wp, const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int64_t N,
+                     double inv_dx, int64_t n_steps, int bc, T tol, int max_iter,
+                     long long *__restrict__ iters_out) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const double dtb = (double)dt[b];
+    const T h = (T)(0.5 * dtb * inv_dx);
+    const T r = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
+    const T b0 = T(1) + T(2) * r;
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    long long iters = 0;
+#define AT(arr, i) arr[(int64_t)(i) * B + b]
+    for (int64_t n = 0; n < n_steps; ++n) {
+        for (int64_t i = 0; i < N; ++i) AT(w, i) = AT(un, i);
+        for (int k = 0;; ++k) {
+            // residual; dp <- -F
+            bool big = false;
+            {
+                T wm = dirichlet ? T(0) : AT(w, N - 1), wi = AT(w, 0);
+                const T w0 = wi;
+                for (int64_t i = 0; i < N; ++i) {
+                    const T wpv = (i + 1 < N) ? AT(w, i + 1) : w0;
+                    T F = t_fma(h * wi, wpv - wm, t_fma(-r, (wpv - wi) - (wi - wm), wi - AT(un, i)));
+                    if (dirichlet && (i == 0 || i == N - 1)) F = T(0);
+                    AT(dp, i) = -F;
+                    big |= !(t_abs(F) < tol);
+                    wm = wi; wi = wpv;
+                }
+            }
+            if (!big || k >= max_iter) break;
+            // J delta = -F
+            if (dirichlet) {      // identity rows at both ends: delta_0 = delta_{N-1} = 0
+                T cprev = T(0), dprev = T(0);
+                AT(cp, 0) = T(0); AT(dp, 0) = T(0);
+                T wm = AT(w, 0), wi = AT(w, 1);
+                for (int64_t i = 1; i <= N - 2; ++i) {
+                    const T wpv = AT(w, i + 1);
+                    const T hw = h * wi;
+                    const T a = -hw - r, bb = t_fma(h, wpv - wm, b0), e = hw - r;
+                    const T inv = T(1) / (bb - a * cprev);
+                    cprev = e * inv;
+                    dprev = (AT(dp, i) - a * dprev) * inv;
+                    AT(cp, i) = cprev; AT(dp, i) = dprev;
+                    wm = wi; wi = wpv;
+                }
+                T x = T(0);      // delta_{N-1}
+                for (int64_t i = N - 2; i >= 1; --i) {
+                    x = AT(dp, i) - AT(cp, i) * x;
+                    AT(w, i) += x;
+                }
+            } else {              // cyclic: Sherman-Morrison (D6) with gamma = -diag_0
+                const T w0 = AT(w, 0), w1 = AT(w, 1), wN1 = AT(w, N - 1), wN2 = AT(w, N - 2);
+                const T a0 = -h * w0 - r, d0 = t_fma(h, w1 - wN1, b0), e0 = h * w0 - r;
+                const T eN = h * wN1 - r;
+                const T gamma = -d0, alpha = a0, beta = eN;
+                const T ag = alpha / gamma;
+                T inv = T(1) / (d0 - gamma);
+                T cprev = e0 * inv, dprev = AT(dp, 0) * inv, wprev = gamma * inv;
+                AT(cp, 0) = cprev; AT(dp, 0) = dprev; AT(wp, 0) = wprev;
+                T wm = w0, wi = w1;
+                for (int64_t i = 1; i < N; ++i) {
+                    const T wpv = (i + 1 < N) ? AT(w, i + 1) : w0;
+                    const T hw = h * wi;
+                    const T a = -hw - r, e = hw - r;
+                    T bb = t_fma(h, wpv - wm, b0);
+                    T ws2 = T(0);
+                    if (i == N - 1) { bb = bb - alpha * beta / gamma; ws2 = beta; }
+                    inv = T(1) / (bb - a * cprev);
+                    cprev = e * inv;
+                    dprev = (AT(dp, i) - a * dprev) * inv;
+                    wprev = (ws2 - a * wprev) * inv;
+                    AT(cp, i) = cprev; AT(dp, i) = dprev; AT(wp, i) = wprev;
+                    wm = wi; wi = wpv;
+                }
+                (void)wN2;
+                T y = dprev, qq = wprev;
+                const T yN = y, qN = qq;
+                for (int64_t i = N - 2; i >= 0; --i) {
+                    const T c = AT(cp, i);
+                    y = AT(dp, i) - c * y;
+                    qq = AT(wp, i) - c * qq;
+                    AT(dp, i) = y; AT(wp, i) = qq;
+                }
+                const T fact = (y + ag * yN) / (T(1) + qq + ag * qN);
+                for (int64_t i = 0; i < N; ++i) AT(w, i) += AT(dp, i) - fact * AT(wp, i);
+            }
+            ++iters;
+        }
+        for (int64_t i = 0; i < N; ++i) AT(un, i) = AT(w, i);
+    }
+#undef AT
+    if (iters_out) iters_out[b] = iters;
+}
+
+}  // namespace
+
+bool newton_hybrid_fits(int is_f64, int64_t N) {
+    int P, Tn;
+    return newton_geometry(is_f64, N, &P, &Tn);
+}
+size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc) {
+    return (size_t)B * (size_t)N * (bc == BURGERS_BC_PERIODIC ? 5 : 4);
+}
+
+template <typename T>
+int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                  double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s) {
+    if (n_steps == 0) {
+        if (iters_out && cudaMemsetAsync(iters_out, 0, (size_t)B * sizeof(long long), s) != cudaSuccess)
+            return BURGERS_ERR_CUDA;
+        return BURGERS_OK;
+    }
+    if (plan == BURGERS_PLAN_HYBRID) {
+        int P, Tn;
+        if (!newton_geometry(sizeof(T) == 8, N, &P, &Tn)) return BURGERS_ERR_PLAN;
+        if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+        switch (P) {
+            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
+            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
+            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
+        }
+        return BURGERS_ERR_PLAN;
+    }
+    // THOMAS
+    const size_t BN = (size_t)B * (size_t)N;
+    T *un = ws, *w = ws + BN, *cp = ws + 2 * BN, *dp = ws + 3 * BN;
+    T *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 4 * BN : nullptr;
+    const int64_t nblk = ((N + 31) / 32) * ((B + 31) / 32);
+    if (nblk > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+    dim3 tb(32, 8);
+    newton_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(u, un, B, N);
+    int st = last_launch_status();
+    if (st != BURGERS_OK) return st;
+    const int threads = (B <= 148 * 32 * 4) ? 32 : 128;
+    newton_thomas_kernel<T><<<(unsigned)((B + threads - 1) / threads), threads, 0, s>>>(
+        un, w, cp, dp, wp, nu, dt, B, N, 1.0 / dx, n_steps, bc, (T)tol, max_iter, iters_out);
+    st = last_launch_status();
+    if (st != BURGERS_OK) return st;
+    newton_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(un, u, N, B);
+    return last_launch_status();
+}
+
+template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, int, long long *, int, float *, cudaStream_t);
+template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, int, long long *, int, double *, cudaStream_t);
+
+}  // namespace burgers

@@ -1,0 +1,127 @@
+"""GPU parity of the Newton-Raphson fully implicit BTCS (D11;
+PAPER.md:137-159 Eq.10-15): the CUDA path through the C ABI against the CPU oracle on the same seeded
+inputs, both plans (one CTA per system / one thread per system), both boundary types, fp64 and fp32.
+
+The stopping rule is a floating-point decision (max|F| < tol), so parity cases use a tolerance far
+below the parity bar: a disagreement about the LAST iteration then changes the result by less than
+tol-level, which Newton's quadratic convergence puts at rounding level."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from parity import rel_err, to_dev
+from refs import colehopf_sin, read_golden
+from paper_2601_12204_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_12204_b200 import binding
+    return binding
+
+
+def run(B, u0, L, nu, dt, n, bc, tol, max_iter=50, plan=0):
+    import torch
+    u = to_dev(np.ascontiguousarray(u0).copy())
+    it = torch.zeros(u.shape[0] if u.dim() == 2 else 1, dtype=torch.int64, device="cuda")
+    B.burgers_newton(u, L, to_dev(nu), to_dev(dt), n, bc, tol=tol, max_iter=max_iter, iters_out=it, plan=plan)
+    return u.cpu().numpy(), it.cpu().numpy()
+
+
+def test_worked_example_iterates_on_gpu(B):
+    G = read_golden("newton_4node.txt")
+    u4 = np.array([[1.0, 2.0, -1.0, 0.0]])
+    nu = np.array([0.1]); dt = np.array([0.1])
+    for k in (1, 2, 3):
+        got, it = run(B, u4, 4.0, nu, dt, 1, B.BC_PERIODIC, tol=0.0, max_iter=k)
+        np.testing.assert_allclose(got[0], G[f"newton{k}_periodic"], atol=1e-14)
+        assert it[0] == k
+        got, _ = run(B, u4, 3.0, nu, dt, 1, B.BC_DIRICHLET, tol=0.0, max_iter=k)
+        np.testing.assert_allclose(got[0], G[f"newton{k}_dirichlet"], atol=1e-14)
+
+
+def test_c1_sine_vs_oracle_and_colehopf(B):
+    w = W.c1_sine()
+    dtc = oracle.dt_from_cfl(w.u0, w.L, w.nu, 4.0, w.bc)[0]
+    n, dt = W.steps_for_final_time(dtc, 1.0)
+    assert n == 42
+    dta = np.array([dt])
+    ref, it_ref = oracle.newton_btcs(w.u0, w.L, w.nu, dta, n, w.bc, tol=1e-12, return_iters=True)
+    for plan in (B.PLAN_HYBRID, B.PLAN_THOMAS):
+        got, it = run(B, w.u0, w.L, w.nu, dta, n, w.bc, tol=1e-12, plan=plan)
+        assert rel_err(got, ref, w.u0) <= 1e-10, plan
+        assert abs(int(it[0]) - int(it_ref[0])) <= n      # at most one iteration per step apart
+    x = np.arange(w.N) * (w.L / w.N)
+    rms = math.sqrt(np.mean((got[0] - colehopf_sin(x, 1.0, 0.05)) ** 2))
+    assert 3.5e-3 < rms < 5e-3        # second-order scheme: 4.2e-3 (the lagged upwind BTCS: 1.8e-2)
+
+
+def test_c3_reduced_both_plans(B):
+    w = W.c3_periodic_btcs(B=24, N=2048, n_steps=30)
+    assert B.plan_query(B.OP_NEWTON, True, w.B, w.N, w.bc) == B.PLAN_HYBRID
+    dt = oracle.dt_from_cfl(w.u0, w.L, w.nu, w.cfl, w.bc)
+    ref, it_ref = oracle.newton_btcs(w.u0, w.L, w.nu, dt, 30, w.bc, tol=1e-12, return_iters=True)
+    for plan in (B.PLAN_AUTO, B.PLAN_THOMAS):
+        got, it = run(B, w.u0, w.L, w.nu, dt, 30, w.bc, tol=1e-12, plan=plan)
+        assert rel_err(got, ref, w.u0) <= 1e-10, plan
+        assert np.all(np.abs(it - it_ref) <= 30)
+    # the paper's criterion: fewer iterations, same answer to about tol
+    got6, it6 = run(B, w.u0, w.L, w.nu, dt, 30, w.bc, tol=1e-6)
+    assert rel_err(got6, ref, w.u0) <= 1e-5
+    assert np.all(it6 <= it) and np.all(it6 >= 30)
+
+
+@pytest.mark.parametrize("dtype,tol,bar", [(np.float64, 1e-12, 1e-10), (np.float32, 2e-6, 1e-4)])
+def test_dirichlet_and_fp32(B, dtype, tol, bar):
+    w = W.c2_dirichlet_batch(B=7, N=1024, dtype=dtype)
+    u0 = w.u0.copy(); u0[:, 0] = dtype(0.25); u0[:, -1] = dtype(-0.5)
+    dt = oracle.dt_from_cfl(u0.astype(np.float64), w.L, w.nu.astype(np.float64), 10.0, w.bc).astype(dtype)
+    ref = oracle.newton_btcs(u0.astype(np.float64), w.L, w.nu.astype(np.float64), dt.astype(np.float64), 25, w.bc,
+                             tol=1e-12)
+    for plan in (B.PLAN_HYBRID, B.PLAN_THOMAS):
+        got, _ = run(B, u0, w.L, w.nu, dt, 25, w.bc, tol=tol, plan=plan)
+        assert rel_err(got, ref, u0) <= bar, plan
+        np.testing.assert_array_equal(got[:, 0], u0[:, 0])
+        np.testing.assert_array_equal(got[:, -1], u0[:, -1])
+
+
+def test_sizes_plans_and_semantics(B):
+    rng = np.random.default_rng(21)
+    for N in (3, 5, 8, 33, 64, 201, 512, 1000, 4096):
+        for bc, L in ((B.BC_PERIODIC, 2.0), (B.BC_DIRICHLET, 1.0)):
+            x = np.arange(N) / N
+            u0 = np.stack([a * np.sin(2 * math.pi * k * x + p) + m for a, k, p, m in
+                           zip(rng.uniform(0.5, 1.5, 3), (1, 2, 3), rng.uniform(0, 6, 3), (-0.3, 0.0, 0.8))])
+            dx = L / N if bc == B.BC_PERIODIC else L / (N - 1)
+            # keep the cell Peclet number |u| dx / nu below 2 (D11: no pivoting, J diagonally dominant)
+            nu = np.maximum(rng.uniform(0.05, 0.2, 3), 0.75 * np.abs(u0).max(axis=1) * dx)
+            dt = oracle.dt_from_cfl(u0, L, nu, 2.0, bc)
+            ref = oracle.newton_btcs(u0, L, nu, dt, 6, bc, tol=1e-13)
+            got, _ = run(B, u0, L, nu, dt, 6, bc, tol=1e-13)
+            assert rel_err(got, ref, u0) <= 1e-10, (N, bc)
+            if B.plan_query(B.OP_NEWTON, True, 3, N, bc) == B.PLAN_HYBRID:
+                got, _ = run(B, u0, L, nu, dt, 6, bc, tol=1e-13, plan=B.PLAN_THOMAS)
+                assert rel_err(got, ref, u0) <= 1e-10, (N, bc, "thomas")
+    # max_iter = 0 and n_steps = 0 leave u alone; a constant state needs no iteration
+    u0 = rng.uniform(-1, 1, (2, 64)); nu = np.array([0.1, 0.1]); dt = np.array([0.01, 0.01])
+    got, it = run(B, u0, 1.0, nu, dt, 3, B.BC_PERIODIC, tol=1e-12, max_iter=0)
+    np.testing.assert_array_equal(got, u0); assert np.all(it == 0)
+    got, it = run(B, u0, 1.0, nu, dt, 0, B.BC_PERIODIC, tol=1e-12)
+    np.testing.assert_array_equal(got, u0)
+    c = np.full((2, 64), 0.6)
+    got, it = run(B, c, 1.0, nu, dt, 4, B.BC_PERIODIC, tol=1e-12)
+    np.testing.assert_array_equal(got, c); assert np.all(it == 0)
+    # argument errors
+    import torch
+    u = to_dev(u0.copy())
+    with pytest.raises(B.BurgersError):
+        B.burgers_newton(u, 1.0, to_dev(nu), to_dev(dt), 1, B.BC_PERIODIC, tol=-1.0)
+    with pytest.raises(B.BurgersError):
+        B.burgers_newton(u, 1.0, to_dev(nu), to_dev(dt), 1, B.BC_PERIODIC, max_iter=-1)
+    with pytest.raises(B.BurgersError):
+        B.burgers_newton(to_dev(rng.uniform(-1, 1, (2, 201))), 1.0, to_dev(nu), to_dev(dt), 1, B.BC_PERIODIC,
+                         plan=B.PLAN_HYBRID)
