@@ -68,6 +68,10 @@ def make_workload(name, rank=0, world=1, reduced=False):
         Bg = 4096 * world
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
         return w, dict(op="btcs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES)
+    if name == "c3_newton":      # SURVEY 8(f) NEXT-1 on C3's inputs: Newton-BTCS, central convection, tol 1e-6
+        Bg = 4096 * world
+        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
+        return w, dict(op="newton", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES, tol=1e-6, max_iter=50)
     if name == "c4a":
         w = W.c4a_long_explicit(n_steps=200 if reduced else 2000)
         return w, dict(op="explicit", scheme=0, instr=I_EULER_F32, lanes=FP32_LANES)
@@ -155,6 +159,9 @@ def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
         t0 = time.perf_counter()
         if spec["op"] == "btcs":
             oracle.btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+        elif spec["op"] == "newton":
+            oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
+                               max_iter=spec["max_iter"], threads=threads)
         elif w.B == 1:
             oracle.explicit_long(u0[0], w.L, nu[0], dt[0], n, w.bc, threads=threads)
         else:
@@ -193,6 +200,11 @@ class GpuRunner:
             self.plan = B.plan_query(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             need = B.workspace_bytes(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
+        elif spec["op"] == "newton":
+            self.plan = B.plan_query(B.OP_NEWTON, is64, w.B, w.N, w.bc)
+            need = B.workspace_bytes(B.OP_NEWTON, is64, w.B, w.N, w.bc)
+            self.launches = B.launch_count(B.OP_NEWTON, is64, w.B, w.N, w.bc, n_steps=w.n_steps)
+            self.iters = torch.zeros(w.B, dtype=torch.int64, device=device)
         else:
             self.plan = B.plan_query(B.OP_BTCS, is64, w.B, w.N, w.bc)
             need = B.workspace_bytes(B.OP_BTCS, is64, w.B, w.N, w.bc)
@@ -212,6 +224,9 @@ class GpuRunner:
         w, B = self.w, self.B
         if self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
+        elif self.spec["op"] == "newton":
+            B.burgers_newton(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
+                             max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws)
         else:
             B.burgers_btcs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
 
@@ -246,7 +261,11 @@ class GpuRunner:
             if self.spec["op"] == "explicit":
                 B.burgers_explicit_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc, self.spec["scheme"])
             else:
-                B.burgers_btcs_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc)
+                if self.spec["op"] == "newton":
+                    B.burgers_newton_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc, tol=self.spec["tol"],
+                                          max_iter=self.spec["max_iter"])
+                else:
+                    B.burgers_btcs_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc)
             t1 = time.perf_counter()
             if i >= warmup:
                 ms.append((t1 - t0) * 1e3)
@@ -320,7 +339,8 @@ def run_ours(args):
     value = total_updates / (ms * 1e-3)
     out = {
         "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
-        else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else "grid-point updates/s (B*N*steps/s), BTCS"),
+        else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else
+              ("grid-point updates/s (B*N*steps/s), Newton BTCS" if spec["op"] == "newton" else "grid-point updates/s (B*N*steps/s), BTCS")),
         "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
@@ -342,7 +362,7 @@ def run_ours(args):
                       "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
-        for name in ("c2_f64", "c3", "c4a", "c4b", "c5"):
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton"):
             if name == args.workload:
                 continue
             try:
@@ -357,6 +377,9 @@ def run_ours(args):
                                 "ms_per_step": statistics.mean(s_ms), "alu_frac": rf["frac"],
                                 "hbm_accounting_frac": rf["hbm_accounting_frac"],
                                 "dtype": "f32" if w2.dtype == np.float32 else "f64"}
+                if spec2["op"] == "newton":
+                    extras[name]["newton_iterations_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
+                    extras[name]["tol"] = spec2["tol"]
                 del r2
                 torch.cuda.empty_cache()
             except Exception as ex:  # a missing plan must not hide the headline number
@@ -410,7 +433,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")

@@ -170,6 +170,11 @@ int burgers_btcs_host_f32(float *u, int64_t B, int64_t N, double L, const float 
                           const float *dt, int64_t n_steps, int bc);
 int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
                           const double *dt, int64_t n_steps, int bc);
+int burgers_newton_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out);
+int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                            const double *dt, int64_t n_steps, int bc, double tol, int max_iter,
+                            int64_t *iters_out);
 int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu,
                          double C, int bc, float *dt_out);
 int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L,

@@ -31,7 +31,7 @@ EXPORTS = [
     "burgers_explicit_plan_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
     "burgers_btcs_plan_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
-    "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
+    "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
     "burgers_launch_count", "burgers_strerror", "burgers_version",
 ]
 
@@ -51,6 +51,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_newton_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p]
+    getattr(_lib, f"burgers_newton_host_{_sfx}").restype = _int
     getattr(_lib, f"burgers_explicit_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int]
     getattr(_lib, f"burgers_btcs_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int]
     getattr(_lib, f"dt_from_cfl_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p]
@@ -266,6 +268,17 @@ def burgers_btcs_host(u, L, nu, dt, n_steps, bc):
                                                    dt.ctypes.data, int(n_steps), int(bc))
     _check(st, f"burgers_btcs_host_{sfx}")
     return u
+
+
+def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return_iters=False):
+    _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    iters = np.zeros(B, dtype=np.int64)
+    st = getattr(_lib, f"burgers_newton_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, dt.ctypes.data,
+                                                     int(n_steps), int(bc), float(tol), int(max_iter),
+                                                     iters.ctypes.data)
+    _check(st, f"burgers_newton_host_{sfx}")
+    return (u, iters) if return_iters else u
 
 
 def dt_from_cfl_host(u, L, nu, C, bc):

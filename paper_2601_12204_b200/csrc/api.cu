@@ -158,6 +158,23 @@ int btcs_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
 }
 
 template <typename T>
+int newton_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
+                double tol, int max_iter, int64_t *iters_out) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
+    const size_t wsb = burgers_workspace_bytes(BURGERS_OP_NEWTON, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
+    DevBuf dit;
+    if (iters_out && !dit.alloc((size_t)B * sizeof(int64_t))) return BURGERS_ERR_CUDA;
+    st = host_step<T>(u, B, N, nu, dt, wsb, [&](T *du, const T *dnu, const T *ddt, void *ws) {
+        return newton_call<T>(du, B, N, L, dnu, ddt, n_steps, bc, tol, max_iter, (int64_t *)dit.p, BURGERS_PLAN_AUTO,
+                              ws, wsb, nullptr);
+    });
+    if (st != BURGERS_OK || !iters_out) return st;
+    return cuda_status(cudaMemcpy(iters_out, dit.p, (size_t)B * sizeof(int64_t), cudaMemcpyDeviceToHost));
+}
+
+template <typename T>
 int cfl_host(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out) {
     if (!u || !nu || !dt_out) return BURGERS_ERR_NULL;
     if (B < 1 || N < 3) return BURGERS_ERR_SHAPE;
@@ -248,6 +265,14 @@ int burgers_btcs_host_f32(float *u, int64_t B, int64_t N, double L, const float 
 int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
                           int64_t n_steps, int bc) {
     return btcs_host<double>(u, B, N, L, nu, dt, n_steps, bc);
+}
+int burgers_newton_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out) {
+    return newton_host<float>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out);
+}
+int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out) {
+    return newton_host<double>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out);
 }
 int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C,
                          int bc, float *dt_out) {

@@ -125,3 +125,13 @@ def test_sizes_plans_and_semantics(B):
     with pytest.raises(B.BurgersError):
         B.burgers_newton(to_dev(rng.uniform(-1, 1, (2, 201))), 1.0, to_dev(nu), to_dev(dt), 1, B.BC_PERIODIC,
                          plan=B.PLAN_HYBRID)
+
+
+def test_host_entry_point_matches_device_path(B):
+    w = W.c3_periodic_btcs(B=5, N=256, n_steps=8)
+    dt = B.dt_from_cfl_host(w.u0, w.L, w.nu, 10.0, w.bc)
+    uh = w.u0.copy()
+    _, ih = B.burgers_newton_host(uh, w.L, w.nu, dt, 8, w.bc, tol=1e-9, return_iters=True)
+    ud, idv = run(B, w.u0, w.L, w.nu, dt, 8, w.bc, tol=1e-9)
+    np.testing.assert_array_equal(uh, ud)
+    np.testing.assert_array_equal(ih, idv)
