@@ -353,8 +353,16 @@ def run_ours(args):
         "gpu_launches": int(r.launches * args.steps),
         "clocks": clocks,
     }
+    def cfl_leg(w_, s_ms, o_ms):
+        """a1 (dt_from_cfl): HBM-bound, sizeof(T) bytes per point once; event time = step - op."""
+        ms_ = max(1e-6, statistics.mean(s_ms) - statistics.mean(o_ms))
+        gbs = w_.B * w_.N * w_.u0.dtype.itemsize / (ms_ * 1e-3) / 1e9
+        return {"ms": ms_, "achieved_gbs": gbs, "hbm_frac": gbs / pk["hbm_gbs"],
+                "note": "CUDA-event time of the dt_from_cfl call (includes ~2 us of event/launch overhead)"}
+
     if rank == 0:
         out["roofline"] = roofline(spec, w, op_ms, pk, args.workload, int(r.launches))
+        out["cfl"] = cfl_leg(w, step_ms, op_ms)
         e_ms, h2d, d2h = r.e2e(max(1, min(args.steps, 3)), 1)
         out["e2e"] = {"value": w.updates * world / (statistics.mean(e_ms) * 1e-3), "unit": "updates/s",
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
@@ -376,7 +384,8 @@ def run_ours(args):
                                 "updates_per_s": w2.updates / (statistics.mean(s_ms) * 1e-3),
                                 "ms_per_step": statistics.mean(s_ms), "alu_frac": rf["frac"],
                                 "hbm_accounting_frac": rf["hbm_accounting_frac"],
-                                "dtype": "f32" if w2.dtype == np.float32 else "f64"}
+                                "dtype": "f32" if w2.dtype == np.float32 else "f64",
+                                "cfl_hbm_frac": cfl_leg(w2, s_ms, o_ms)["hbm_frac"]}
                 if spec2["op"] == "newton":
                     extras[name]["newton_iterations_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
                     extras[name]["tol"] = spec2["tol"]

@@ -63,11 +63,11 @@ def _load():
     lib.oracle_btcs.restype = ci
     lib.oracle_dt_from_cfl.argtypes = [p, i64, i64, f64, p, f64, ci, p]
     lib.oracle_dt_from_cfl.restype = ci
-    lib.oracle_newton_residual.argtypes = [p, p, i64, f64, f64, f64, ci, ci, f64, p]
+    lib.oracle_newton_residual.argtypes = [p, p, i64, f64, f64, f64, f64, ci, ci, f64, p]
     lib.oracle_newton_residual.restype = None
-    lib.oracle_newton_jacobian.argtypes = [p, i64, f64, f64, f64, ci, ci, f64, p, p, p]
+    lib.oracle_newton_jacobian.argtypes = [p, i64, f64, f64, f64, f64, ci, ci, f64, p, p, p]
     lib.oracle_newton_jacobian.restype = None
-    lib.oracle_newton_btcs.argtypes = [p, i64, i64, f64, p, p, i64, ci, f64, ci, ci, f64, p, ci]
+    lib.oracle_newton_btcs.argtypes = [p, i64, i64, f64, p, p, f64, i64, ci, f64, ci, ci, f64, p, ci]
     lib.oracle_newton_btcs.restype = ci
     lib.oracle_max_threads.argtypes = []
     lib.oracle_max_threads.restype = ci
@@ -193,35 +193,36 @@ def dt_from_cfl(u, L, nu, C, bc) -> np.ndarray:
     return out
 
 
-def newton_residual(w, un, L, nu, dt, bc, adv=None) -> np.ndarray:
-    """Residual F(w) of Eq.11 for one trajectory (D11)."""
+def newton_residual(w, un, L, nu, dt, bc, adv=None, theta=1.0) -> np.ndarray:
+    """Residual F(w) of Eq.11 (theta-weighted, D11) for one trajectory."""
     w, un = _f64(w).reshape(-1), _f64(un).reshape(-1)
     F = np.empty_like(w)
-    _load().oracle_newton_residual(_ptr(w), _ptr(un), w.size, float(L), float(nu), float(dt), int(bc),
+    _load().oracle_newton_residual(_ptr(w), _ptr(un), w.size, float(L), float(nu), float(dt), float(theta), int(bc),
                                    int(adv is not None), float(adv or 0.0), _ptr(F))
     return F
 
 
-def newton_jacobian(w, L, nu, dt, bc, adv=None):
+def newton_jacobian(w, L, nu, dt, bc, adv=None, theta=1.0):
     """(sub, diag, sup) of the tridiagonal Jacobian of Eq.11 at w (D11)."""
     w = _f64(w).reshape(-1)
     out = [np.empty_like(w) for _ in range(3)]
-    _load().oracle_newton_jacobian(_ptr(w), w.size, float(L), float(nu), float(dt), int(bc),
+    _load().oracle_newton_jacobian(_ptr(w), w.size, float(L), float(nu), float(dt), float(theta), int(bc),
                                    int(adv is not None), float(adv or 0.0), *[_ptr(o) for o in out])
     return tuple(out)
 
 
 def newton_btcs(u0, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, adv=None, threads=None,
-                return_iters=False):
-    """Fully implicit central-convection BTCS by Newton-Raphson (D11); returns a new array
-    (and the per-trajectory iteration totals when return_iters)."""
+                return_iters=False, theta=1.0):
+    """Implicit central-convection theta-scheme by Newton-Raphson (D11; theta = 1: the paper's BTCS
+    Eq.11, theta = 1/2: Crank-Nicolson); returns a new array (and the per-trajectory iteration
+    totals when return_iters)."""
     u = _f64(u0).copy()
     shape = u.shape
     u = u.reshape(-1, shape[-1])
     B, N = u.shape
     nu_a, dt_a = _per_traj(nu, B), _per_traj(dt, B)
     iters = np.zeros(B, dtype=np.int64)
-    rc = _load().oracle_newton_btcs(_ptr(u), B, N, float(L), _ptr(nu_a), _ptr(dt_a), int(n_steps),
+    rc = _load().oracle_newton_btcs(_ptr(u), B, N, float(L), _ptr(nu_a), _ptr(dt_a), float(theta), int(n_steps),
                                     int(bc), float(tol), int(max_iter), int(adv is not None),
                                     float(adv or 0.0), ctypes.c_void_p(iters.ctypes.data),
                                     int(threads or default_threads()))

@@ -366,24 +366,38 @@ int oracle_dt_from_cfl(const double *u, int64_t B, int64_t N, double L,
  * Newton (Eq.12-13): w^0 = u^n; while max_i |F_i(w^k)| >= tol and k < max_iter:
  *   solve J(w^k) delta = -F(w^k), w^{k+1} = w^k + delta.   (criterion: PAPER.md:245)
  * Dirichlet: end nodes fixed (F = 0, delta = 0 there); periodic: cyclic system.
+ * theta-scheme ("Crank-Nicolson"): with
+ *   G_i(v) = h v_i (v_{i+1} - v_{i-1}) - r (v_{i+1} - 2 v_i + v_{i-1})     (dt times the central operator)
+ * the residual is  F_i(w) = w_i - u_i^n + theta G_i(w) + (1 - theta) G_i(u^n)  and the Jacobian
+ * I + theta dG/dw;  theta = 1 is Eq.11 (BTCS), theta = 1/2 Crank-Nicolson (second order in time),
+ * theta = 0 forward Euler with central convection (residual zero after one trivial iteration).
  * Test hook use_adv: the multiplying w_i is replaced by the constant adv (linear
  * advection-diffusion: J does not depend on w, one iteration is exact).
  * No pivoting: J is diagonally dominant when the cell Peclet number
  * |w| dx / nu <= 2 and h (w_{i+1} - w_{i-1}) > -1 (D11).
  */
+static double newton_G(const double *v, int64_t i, int64_t N, double h, double r,
+                       int use_adv, double adv)
+{
+    int64_t im = (i == 0) ? N - 1 : i - 1;
+    int64_t ip = (i == N - 1) ? 0 : i + 1;
+    double a = use_adv ? adv : v[i];
+    return h * a * (v[ip] - v[im]) - r * (v[ip] - 2.0 * v[i] + v[im]);
+}
+
 static void newton_residual(const double *w, const double *un, int64_t N, double h,
-                            double r, int bc, int use_adv, double adv, double *F)
+                            double r, double theta, int bc, int use_adv, double adv, double *F)
 {
     for (int64_t i = 0; i < N; ++i) {
         if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) { F[i] = 0.0; continue; }
-        int64_t im = (i == 0) ? N - 1 : i - 1;
-        int64_t ip = (i == N - 1) ? 0 : i + 1;
-        double a = use_adv ? adv : w[i];
-        F[i] = w[i] - un[i] + h * a * (w[ip] - w[im]) - r * (w[ip] - 2.0 * w[i] + w[im]);
+        double Gw = newton_G(w, i, N, h, r, use_adv, adv);
+        if (theta == 1.0) { F[i] = w[i] - un[i] + Gw; continue; }     /* Eq.11 as printed */
+        double Gu = newton_G(un, i, N, h, r, use_adv, adv);
+        F[i] = w[i] - un[i] + theta * Gw + (1.0 - theta) * Gu;
     }
 }
 
-static void newton_jacobian(const double *w, int64_t N, double h, double r, int bc,
+static void newton_jacobian(const double *w, int64_t N, double h, double r, double theta, int bc,
                             int use_adv, double adv, double *sub, double *diag, double *sup)
 {
     for (int64_t i = 0; i < N; ++i) {
@@ -391,30 +405,31 @@ static void newton_jacobian(const double *w, int64_t N, double h, double r, int 
         int64_t im = (i == 0) ? N - 1 : i - 1;
         int64_t ip = (i == N - 1) ? 0 : i + 1;
         double a = use_adv ? adv : w[i];
-        sub[i] = -h * a - r;
-        diag[i] = 1.0 + (use_adv ? 0.0 : h * (w[ip] - w[im])) + 2.0 * r;
-        sup[i] = h * a - r;
+        sub[i] = theta * (-h * a - r);
+        diag[i] = 1.0 + theta * ((use_adv ? 0.0 : h * (w[ip] - w[im])) + 2.0 * r);
+        sup[i] = theta * (h * a - r);
     }
 }
 
 /* Exposed for the pins (worked example, finite-difference Jacobian check). */
 void oracle_newton_residual(const double *w, const double *un, int64_t N, double L, double nu,
-                            double dt, int bc, int use_adv, double adv, double *F)
+                            double dt, double theta, int bc, int use_adv, double adv, double *F)
 {
     double dx = grid_dx(N, L, bc);
-    newton_residual(w, un, N, dt / (2.0 * dx), nu * dt / (dx * dx), bc, use_adv, adv, F);
+    newton_residual(w, un, N, dt / (2.0 * dx), nu * dt / (dx * dx), theta, bc, use_adv, adv, F);
 }
-void oracle_newton_jacobian(const double *w, int64_t N, double L, double nu, double dt, int bc,
-                            int use_adv, double adv, double *sub, double *diag, double *sup)
+void oracle_newton_jacobian(const double *w, int64_t N, double L, double nu, double dt, double theta,
+                            int bc, int use_adv, double adv, double *sub, double *diag, double *sup)
 {
     double dx = grid_dx(N, L, bc);
-    newton_jacobian(w, N, dt / (2.0 * dx), nu * dt / (dx * dx), bc, use_adv, adv, sub, diag, sup);
+    newton_jacobian(w, N, dt / (2.0 * dx), nu * dt / (dx * dx), theta, bc, use_adv, adv, sub, diag, sup);
 }
 
 /* One trajectory; returns the total number of Newton iterations (linear solves).
  * wk: 13N doubles. */
-static int64_t newton_one(double *u, int64_t N, double dx, double nu, double dt, int64_t n_steps,
-                          int bc, double tol, int max_iter, int use_adv, double adv, double *wk)
+static int64_t newton_one(double *u, int64_t N, double dx, double nu, double dt, double theta,
+                          int64_t n_steps, int bc, double tol, int max_iter, int use_adv, double adv,
+                          double *wk)
 {
     double *w = wk, *F = wk + N, *sub = wk + 2 * N, *diag = wk + 3 * N, *sup = wk + 4 * N,
            *rhs = wk + 5 * N, *x = wk + 6 * N, *wk2 = wk + 7 * N; /* 6N */
@@ -423,11 +438,11 @@ static int64_t newton_one(double *u, int64_t N, double dx, double nu, double dt,
     for (int64_t n = 0; n < n_steps; ++n) {
         for (int64_t i = 0; i < N; ++i) w[i] = u[i];
         for (int k = 0;; ++k) {
-            newton_residual(w, u, N, h, r, bc, use_adv, adv, F);
+            newton_residual(w, u, N, h, r, theta, bc, use_adv, adv, F);
             double m = 0.0;
             for (int64_t i = 0; i < N; ++i) { double a = fabs(F[i]); if (!(a <= m)) m = a; }
             if (m < tol || k >= max_iter) break;
-            newton_jacobian(w, N, h, r, bc, use_adv, adv, sub, diag, sup);
+            newton_jacobian(w, N, h, r, theta, bc, use_adv, adv, sub, diag, sup);
             for (int64_t i = 0; i < N; ++i) rhs[i] = -F[i];
             if (bc == BC_PERIODIC) cyclic_sm(N, sub, diag, sup, rhs, x, wk2);
             else thomas(N, sub, diag, sup, rhs, x, wk2, wk2 + N);   /* identity rows at the ends */
@@ -441,10 +456,11 @@ static int64_t newton_one(double *u, int64_t N, double dx, double nu, double dt,
 
 /* B trajectories, in place; iters_out[b] (may be NULL) = Newton iterations summed over the steps. */
 int oracle_newton_btcs(double *u, int64_t B, int64_t N, double L, const double *nu,
-                       const double *dt, int64_t n_steps, int bc, double tol, int max_iter,
-                       int use_adv, double adv, int64_t *iters_out, int nthreads)
+                       const double *dt, double theta, int64_t n_steps, int bc, double tol,
+                       int max_iter, int use_adv, double adv, int64_t *iters_out, int nthreads)
 {
     if (!u || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0) || max_iter < 0) return -1;
+    if (!(theta >= 0.0 && theta <= 1.0)) return -1;
     if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
     double dx = grid_dx(N, L, bc);
     int fail = 0;
@@ -459,7 +475,7 @@ int oracle_newton_btcs(double *u, int64_t B, int64_t N, double L, const double *
         } else {
 #pragma omp for schedule(dynamic, 1)
             for (int64_t b = 0; b < B; ++b) {
-                int64_t it = newton_one(u + b * N, N, dx, nu[b], dt[b], n_steps, bc, tol, max_iter,
+                int64_t it = newton_one(u + b * N, N, dx, nu[b], dt[b], theta, n_steps, bc, tol, max_iter,
                                         use_adv, adv, wk);
                 if (iters_out) iters_out[b] = it;
             }

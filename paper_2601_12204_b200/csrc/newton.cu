@@ -127,7 +127,7 @@ bool pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
 
 bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out) {
     const int bytes = is_f64 ? 8 : 4;
-    const int cand[3] = {8, 16, 4};           // 8 first: five arrays of P values live in registers
+    const int cand[3] = {16, 8, 4};
     int bestP = 0;
     for (int i = 0; i < 3; ++i) {
         const int P = cand[i];
@@ -224,7 +224,7 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                     AT(w, i) += x;
                 }
             } else {              // cyclic: Sherman-Morrison (D6) with gamma = -diag_0
-                const T w0 = AT(w, 0), w1 = AT(w, 1), wN1 = AT(w, N - 1), wN2 = AT(w, N - 2);
+                const T w0 = AT(w, 0), w1 = AT(w, 1), wN1 = AT(w, N - 1);
                 const T a0 = -h * w0 - r, d0 = t_fma(h, w1 - wN1, b0), e0 = h * w0 - r;
                 const T eN = h * wN1 - r;
                 const T gamma = -d0, alpha = a0, beta = eN;
@@ -247,7 +247,6 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                     AT(cp, i) = cprev; AT(dp, i) = dprev; AT(wp, i) = wprev;
                     wm = wi; wi = wpv;
                 }
-                (void)wN2;
                 T y = dprev, qq = wprev;
                 const T yN = y, qN = qq;
                 for (int64_t i = N - 2; i >= 0; --i) {

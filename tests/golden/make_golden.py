@@ -92,23 +92,28 @@ def btcs_exact(u, dx, nu, dt, bc):
     return rows, [u[0]] + x + [u[N - 1]]
 
 
-def newton_exact(u, dx, nu, dt, bc, iters):
+def newton_exact(u, dx, nu, dt, bc, iters, theta=Fr(1)):
     """`iters` Newton iterations on the residual of PAPER.md Eq.11 (central convection, all terms at
-    n+1) from w0 = u^n, with the Jacobian obtained by differentiating Eq.11 (Q5/D11)."""
+    n+1) from w0 = u^n, with the Jacobian obtained by differentiating Eq.11 (Q5/D11).
+    theta != 1: theta-scheme F = w - u + theta G(w) + (1-theta) G(u), G = dt * central operator."""
     N = len(u)
     h, r = dt / (2 * dx), nu * dt / dx ** 2
     idx = list(range(N)) if bc == "periodic" else list(range(1, N - 1))
     w = list(u)
     out = []
+
+    def G(v, i):
+        return h * v[i] * (v[(i + 1) % N] - v[(i - 1) % N]) - r * (v[(i + 1) % N] - 2 * v[i] + v[(i - 1) % N])
+
     for _ in range(iters):
         F = {}
         M = [[Fr(0)] * N for _ in range(N)]
         for i in idx:
             wm, wp, wi = w[(i - 1) % N], w[(i + 1) % N], w[i]
-            F[i] = wi - u[i] + h * wi * (wp - wm) - r * (wp - 2 * wi + wm)      # Eq.11
-            M[i][(i - 1) % N] += -h * wi - r
-            M[i][i] += 1 + h * (wp - wm) + 2 * r
-            M[i][(i + 1) % N] += h * wi - r
+            F[i] = wi - u[i] + theta * G(w, i) + (1 - theta) * G(u, i)          # Eq.11 at theta = 1
+            M[i][(i - 1) % N] += theta * (-h * wi - r)
+            M[i][i] += 1 + theta * (h * (wp - wm) + 2 * r)
+            M[i][(i + 1) % N] += theta * (h * wi - r)
         Mi = [[M[i][j] for j in idx] for i in idx]          # frozen end nodes: delta = 0
         d = solve_exact(Mi, [-F[i] for i in idx])           # Eq.12
         for i, di in zip(idx, d):
@@ -138,6 +143,11 @@ def write_newton_example():
     lines.append("# Dirichlet: same u, L=3 (dx=1), end nodes frozen at 1 and 0")
     for k, w in enumerate(newton_exact(u, dx, nu, dt, "dirichlet", 3), 1):
         lines.append(f"newton{k}_dirichlet " + fmt(w))
+    lines.append("# theta = 1/2 (Crank-Nicolson on the central operator), same data")
+    for k, w in enumerate(newton_exact(u, dx, nu, dt, "periodic", 3, Fr(1, 2)), 1):
+        lines.append(f"cn{k}_periodic " + fmt(w))
+    for k, w in enumerate(newton_exact(u, dx, nu, dt, "dirichlet", 3, Fr(1, 2)), 1):
+        lines.append(f"cn{k}_dirichlet " + fmt(w))
     with open(os.path.join(HERE, "newton_4node.txt"), "w") as f:
         f.write("\n".join(lines) + "\n")
 

@@ -129,3 +129,59 @@ def test_invariants_and_threads():
     a = oracle.newton_btcs(ub, L, 0.1, 0.01, 4, P, threads=1)
     b = oracle.newton_btcs(ub, L, 0.1, 0.01, 4, P, threads=4)
     np.testing.assert_array_equal(a, b)
+
+
+# ---------------------------------------------------------------- theta-scheme
+def test_theta_half_worked_example():
+    G = read_golden("newton_4node.txt")
+    for k in (1, 2, 3):
+        w = oracle.newton_btcs(U4, 4.0, 0.1, 0.1, 1, P, tol=0.0, max_iter=k, theta=0.5)
+        np.testing.assert_allclose(w, G[f"cn{k}_periodic"], atol=2e-15)
+        w = oracle.newton_btcs(U4, 3.0, 0.1, 0.1, 1, D, tol=0.0, max_iter=k, theta=0.5)
+        np.testing.assert_allclose(w, G[f"cn{k}_dirichlet"], atol=2e-15)
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.25, 1.0])
+def test_theta_scheme_amplification_factor(theta):
+    # linearised: G = (1 - (1-theta) zeta) / (1 + theta zeta), zeta = i c sin(th) + 4 r sin^2(th/2)
+    N, L, nu, k, n, adv = 32, 2 * math.pi, 0.03, 5, 9, 1.3
+    dx = L / N
+    dt = 0.7 * dx
+    th = 2 * math.pi * k / N
+    zeta = 1j * (adv * dt / dx) * math.sin(th) + 4 * (nu * dt / dx ** 2) * math.sin(th / 2) ** 2
+    Gf = (1 - (1 - theta) * zeta) / (1 + theta * zeta)
+    i = np.arange(N)
+    u0 = np.cos(th * i - 0.3)
+    got = oracle.newton_btcs(u0, L, nu, dt, n, P, tol=1e-13, adv=adv, theta=theta)
+    np.testing.assert_allclose(got, np.real(Gf ** n * np.exp(1j * (th * i - 0.3))), atol=1e-13)
+
+
+def test_theta_zero_is_forward_euler_with_central_convection():
+    rng = np.random.default_rng(2)
+    N, L, nu, dt = 24, 3.0, 0.1, 0.004
+    u0 = rng.uniform(-1, 1, N)
+    dx = L / N
+    want = u0 - dt * (u0 * (np.roll(u0, -1) - np.roll(u0, 1)) / (2 * dx)
+                      - nu * (np.roll(u0, -1) - 2 * u0 + np.roll(u0, 1)) / dx ** 2)
+    got, it = oracle.newton_btcs(u0, L, nu, dt, 1, P, tol=1e-14, theta=0.0, return_iters=True)
+    np.testing.assert_allclose(got, want, atol=1e-15)
+    assert it[0] == 1        # J = I: one (trivial) iteration
+
+
+def test_crank_nicolson_is_second_order_with_dt_proportional_to_dx():
+    # dt = dx/4 (NOT dx^2): Crank-Nicolson O(dt^2 + dx^2) keeps order 2, BTCS (theta = 1) drops to order 1
+    L, nu = 2 * math.pi, 0.05
+
+    def err(N, theta):
+        x = np.arange(N) * (L / N)
+        n = int(round(1.0 / (0.25 * L / N)))
+        u = oracle.newton_btcs(np.sin(x), L, nu, 1.0 / n, n, P, tol=1e-13, theta=theta)
+        return math.sqrt(np.mean((u - colehopf_sin(x, 1.0, nu)) ** 2))
+
+    e_cn = [err(N, 0.5) for N in (128, 256, 512)]
+    e_be = [err(N, 1.0) for N in (128, 256, 512)]
+    o_cn = [math.log2(e_cn[i] / e_cn[i + 1]) for i in range(2)]
+    o_be = [math.log2(e_be[i] / e_be[i + 1]) for i in range(2)]
+    assert all(1.9 < o < 2.1 for o in o_cn), (e_cn, o_cn)
+    assert all(0.85 < o < 1.35 for o in o_be), (e_be, o_be)
+    assert e_cn[2] < 0.2 * e_be[2]
