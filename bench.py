@@ -68,10 +68,11 @@ def make_workload(name, rank=0, world=1, reduced=False):
         Bg = 4096 * world
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
         return w, dict(op="btcs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES)
-    if name == "c3_newton":      # SURVEY 8(f) NEXT-1 on C3's inputs: Newton-BTCS, central convection, tol 1e-6
-        Bg = 4096 * world
+    if name in ("c3_newton", "c3_cn"):   # SURVEY 8(f) NEXT-1 / NEXT-2 on C3's inputs: Newton solve of the fully implicit
+        Bg = 4096 * world                #   (theta = 1) / Crank-Nicolson (theta = 1/2) central scheme, tol 1e-6
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
-        return w, dict(op="newton", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES, tol=1e-6, max_iter=50)
+        return w, dict(op="newton", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES, tol=1e-6, max_iter=50,
+                       theta=1.0 if name == "c3_newton" else 0.5)
     if name == "c4a":
         w = W.c4a_long_explicit(n_steps=200 if reduced else 2000)
         return w, dict(op="explicit", scheme=0, instr=I_EULER_F32, lanes=FP32_LANES)
@@ -161,7 +162,7 @@ def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
             oracle.btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
         elif spec["op"] == "newton":
             oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
-                               max_iter=spec["max_iter"], threads=threads)
+                               max_iter=spec["max_iter"], threads=threads, theta=spec["theta"])
         elif w.B == 1:
             oracle.explicit_long(u0[0], w.L, nu[0], dt[0], n, w.bc, threads=threads)
         else:
@@ -226,7 +227,7 @@ class GpuRunner:
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
         elif self.spec["op"] == "newton":
             B.burgers_newton(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
-                             max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws)
+                             max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws, theta=self.spec["theta"])
         else:
             B.burgers_btcs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
 
@@ -263,7 +264,7 @@ class GpuRunner:
             else:
                 if self.spec["op"] == "newton":
                     B.burgers_newton_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc, tol=self.spec["tol"],
-                                          max_iter=self.spec["max_iter"])
+                                          max_iter=self.spec["max_iter"], theta=self.spec["theta"])
                 else:
                     B.burgers_btcs_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc)
             t1 = time.perf_counter()
@@ -370,7 +371,7 @@ def run_ours(args):
                       "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
-        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton"):
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn"):
             if name == args.workload:
                 continue
             try:
@@ -389,6 +390,7 @@ def run_ours(args):
                 if spec2["op"] == "newton":
                     extras[name]["newton_iterations_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
                     extras[name]["tol"] = spec2["tol"]
+                    extras[name]["theta"] = spec2["theta"]
                 del r2
                 torch.cuda.empty_cache()
             except Exception as ex:  # a missing plan must not hide the headline number
@@ -442,7 +444,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")

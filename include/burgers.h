@@ -34,7 +34,7 @@
  *    (Eq.16-17).
  *  - Errors: NULL pointer -> BURGERS_ERR_NULL; B<1, N<3, n_steps<0 ->
  *    BURGERS_ERR_SHAPE; unknown bc/scheme/plan/op -> BURGERS_ERR_ENUM; L<=0, C<=0
- *    or non-finite, tol < 0 or NaN, max_iter < 0 -> BURGERS_ERR_VALUE; workspace too small (or NULL when a
+ *    or non-finite, tol < 0 or NaN, max_iter < 0, theta outside [0,1] -> BURGERS_ERR_VALUE; workspace too small (or NULL when a
  *    non-zero size is required) -> BURGERS_ERR_WORKSPACE; a CUDA launch/runtime
  *    failure -> BURGERS_ERR_CUDA; a plan that cannot run this shape ->
  *    BURGERS_ERR_PLAN.  Device-side values (nu<0, dt<=0, NaN in u) are not
@@ -138,17 +138,20 @@ int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const doubl
  * Jacobian J_{i,i-1} = -dt w_i/(2dx) - r, J_{i,i} = 1 + dt (w_{i+1} - w_{i-1})/(2dx) + 2r,
  * J_{i,i+1} = dt w_i/(2dx) - r, r = nu dt/dx^2 (Eq.14; Eq.15 of the paper is garbled, Q5),
  * until max_i |F_i| < tol or max_iter iterations were done (PAPER.md:245 uses tol = 1e-6).
+ * theta in [0,1] ("Crank-Nicolson"): with G(v) = dt times the
+ * bracket of Eq.11, F(w) = w - u^n + theta G(w) + (1-theta) G(u^n); theta = 1 is Eq.11 itself,
+ * theta = 1/2 Crank-Nicolson (second order in time), theta = 0 forward Euler with central convection.
  * Dirichlet end nodes stay fixed; periodic systems are cyclic.  No pivoting: J is diagonally
  * dominant when |w| dx / nu <= 2 and dt (w_{i+1} - w_{i-1})/(2dx) > -1.
  * iters_out: DEVICE pointer to B int64 (Newton iterations summed over the steps), or NULL.
  * plan: BURGERS_PLAN_AUTO, BURGERS_PLAN_HYBRID (one CTA per system, N = P 2^k that fits one CTA, no
  * workspace) or BURGERS_PLAN_THOMAS (one thread per system, any N, needs workspace). */
 int burgers_newton_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
-                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out,
-                       int plan, void *ws, size_t ws_bytes, void *stream);
+                       int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                       int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream);
 int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
-                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out,
-                       int plan, void *ws, size_t ws_bytes, void *stream);
+                       int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                       int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream);
 
 /* ---- CFL time step (PAPER.md:116-118 Eq.7-8, :287 Eq.24) -----------------------
  * dt_out[b] = C * min(dx / max_i |u[b][i]|, dx^2 / (2 nu[b])), with x/0 = +inf
@@ -171,10 +174,11 @@ int burgers_btcs_host_f32(float *u, int64_t B, int64_t N, double L, const float 
 int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
                           const double *dt, int64_t n_steps, int bc);
 int burgers_newton_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
-                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out);
-int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
-                            const double *dt, int64_t n_steps, int bc, double tol, int max_iter,
+                            int64_t n_steps, int bc, double theta, double tol, int max_iter,
                             int64_t *iters_out);
+int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                            const double *dt, int64_t n_steps, int bc, double theta, double tol,
+                            int max_iter, int64_t *iters_out);
 int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu,
                          double C, int bc, float *dt_out);
 int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L,

@@ -49,9 +49,9 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_btcs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_btcs_plan_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _p, _sz, _p]
     getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
-    getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _int, _p, _sz, _p]
+    getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").restype = _int
-    getattr(_lib, f"burgers_newton_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p]
+    getattr(_lib, f"burgers_newton_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p]
     getattr(_lib, f"burgers_newton_host_{_sfx}").restype = _int
     getattr(_lib, f"burgers_explicit_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int]
     getattr(_lib, f"burgers_btcs_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int]
@@ -193,9 +193,11 @@ def burgers_btcs(u, L, nu, dt, n_steps, bc, ws=None, plan=PLAN_AUTO):
     return u
 
 
-def burgers_newton(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, iters_out=None, ws=None, plan=PLAN_AUTO):
-    """In-place fully implicit central-convection BTCS by Newton-Raphson (include/burgers.h:
-    burgers_newton_*).  iters_out: optional int64 CUDA tensor [B] receiving the iteration totals."""
+def burgers_newton(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, iters_out=None, ws=None, plan=PLAN_AUTO,
+                   theta=1.0):
+    """In-place implicit central-convection theta-scheme by Newton-Raphson (include/burgers.h:
+    burgers_newton_*; theta = 1: the paper's BTCS Eq.11, 1/2: Crank-Nicolson).  iters_out: optional
+    int64 CUDA tensor [B] receiving the iteration totals."""
     import torch
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
@@ -211,8 +213,8 @@ def burgers_newton(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, iters_out=N
     need = workspace_bytes(OP_NEWTON, u.dtype == torch.float64, B, N, bc, 0, plan)
     wsp, wsb, ws = _ws(ws, need, u.device)
     st = getattr(_lib, f"burgers_newton_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(),
-                                                int(n_steps), int(bc), float(tol), int(max_iter), ip, int(plan),
-                                                wsp, wsb, _stream())
+                                                int(n_steps), int(bc), float(theta), float(tol), int(max_iter), ip,
+                                                int(plan), wsp, wsb, _stream())
     _check(st, f"burgers_newton_{sfx}")
     return u
 
@@ -270,12 +272,12 @@ def burgers_btcs_host(u, L, nu, dt, n_steps, bc):
     return u
 
 
-def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return_iters=False):
+def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return_iters=False, theta=1.0):
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
     B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
     iters = np.zeros(B, dtype=np.int64)
     st = getattr(_lib, f"burgers_newton_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, dt.ctypes.data,
-                                                     int(n_steps), int(bc), float(tol), int(max_iter),
+                                                     int(n_steps), int(bc), float(theta), float(tol), int(max_iter),
                                                      iters.ctypes.data)
     _check(st, f"burgers_newton_host_{sfx}")
     return (u, iters) if return_iters else u

@@ -81,10 +81,11 @@ int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
 
 template <typename T>
 int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
-                double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream) {
+                double theta, double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes,
+                void *stream) {
     int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
-    if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
+    if (!(tol >= 0.0) || max_iter < 0 || !(theta >= 0.0 && theta <= 1.0)) return BURGERS_ERR_VALUE;
     const int is_f64 = sizeof(T) == 8;
     if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
     if (plan != BURGERS_PLAN_HYBRID && plan != BURGERS_PLAN_THOMAS) return BURGERS_ERR_ENUM;
@@ -94,7 +95,7 @@ int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, 
         if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
     }
     static_assert(sizeof(long long) == sizeof(int64_t), "iters_out is int64");
-    return launch_newton<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, tol, max_iter,
+    return launch_newton<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, theta, tol, max_iter,
                             reinterpret_cast<long long *>(iters_out), plan, (T *)ws, (cudaStream_t)stream);
 }
 
@@ -159,15 +160,15 @@ int btcs_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
 
 template <typename T>
 int newton_host(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
-                double tol, int max_iter, int64_t *iters_out) {
+                double theta, double tol, int max_iter, int64_t *iters_out) {
     int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
-    if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
+    if (!(tol >= 0.0) || max_iter < 0 || !(theta >= 0.0 && theta <= 1.0)) return BURGERS_ERR_VALUE;
     const size_t wsb = burgers_workspace_bytes(BURGERS_OP_NEWTON, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
     DevBuf dit;
     if (iters_out && !dit.alloc((size_t)B * sizeof(int64_t))) return BURGERS_ERR_CUDA;
     st = host_step<T>(u, B, N, nu, dt, wsb, [&](T *du, const T *dnu, const T *ddt, void *ws) {
-        return newton_call<T>(du, B, N, L, dnu, ddt, n_steps, bc, tol, max_iter, (int64_t *)dit.p, BURGERS_PLAN_AUTO,
+        return newton_call<T>(du, B, N, L, dnu, ddt, n_steps, bc, theta, tol, max_iter, (int64_t *)dit.p, BURGERS_PLAN_AUTO,
                               ws, wsb, nullptr);
     });
     if (st != BURGERS_OK || !iters_out) return st;
@@ -231,14 +232,14 @@ int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const doubl
 }
 
 int burgers_newton_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
-                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, int plan,
-                       void *ws, size_t ws_bytes, void *stream) {
-    return newton_call<float>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
+                       int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out,
+                       int plan, void *ws, size_t ws_bytes, void *stream) {
+    return newton_call<float>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
 }
 int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
-                       int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, int plan,
-                       void *ws, size_t ws_bytes, void *stream) {
-    return newton_call<double>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
+                       int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out,
+                       int plan, void *ws, size_t ws_bytes, void *stream) {
+    return newton_call<double>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
 }
 
 int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C, int bc,
@@ -267,12 +268,12 @@ int burgers_btcs_host_f64(double *u, int64_t B, int64_t N, double L, const doubl
     return btcs_host<double>(u, B, N, L, nu, dt, n_steps, bc);
 }
 int burgers_newton_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
-                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out) {
-    return newton_host<float>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out);
+                            int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out) {
+    return newton_host<float>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out);
 }
 int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
-                            int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out) {
-    return newton_host<double>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out);
+                            int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out) {
+    return newton_host<double>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out);
 }
 int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C,
                          int bc, float *dt_out) {
@@ -353,7 +354,7 @@ const char *burgers_strerror(int status) {
         case BURGERS_ERR_NULL: return "null pointer argument";
         case BURGERS_ERR_SHAPE: return "bad shape (need B>=1, N>=3, n_steps>=0, grid within limits)";
         case BURGERS_ERR_ENUM: return "unknown bc / scheme / plan / op";
-        case BURGERS_ERR_VALUE: return "bad value (need finite L>0, C>0, tol>=0, max_iter>=0)";
+        case BURGERS_ERR_VALUE: return "bad value (need finite L>0, C>0, tol>=0, max_iter>=0, 0<=theta<=1)";
         case BURGERS_ERR_WORKSPACE: return "workspace missing or too small (see burgers_workspace_bytes)";
         case BURGERS_ERR_CUDA: return "CUDA runtime / launch failure";
         case BURGERS_ERR_PLAN: return "requested plan cannot run this shape";

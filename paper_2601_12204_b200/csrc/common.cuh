@@ -73,7 +73,7 @@ bool btcs_long_fits(int64_t N, int bc);
 // ---------------------------------------------------------------- Newton BTCS (newton.cu)
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                  double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s);
+                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s);
 bool newton_hybrid_fits(int is_f64, int64_t N);
 size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc);
 

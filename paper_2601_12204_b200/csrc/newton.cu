@@ -10,6 +10,9 @@
 // (stopping rule: "maximum residual falling below 1e-6"; tol is an argument).
 // Dirichlet end nodes are identity rows with zero right-hand side; periodic systems are cyclic.
 // Residual and Jacobian are fused into the solver: nothing but u touches HBM.
+// theta-scheme ("Crank-Nicolson"): with G(v) = dt times the central
+// operator, F(w) = w - u^n + theta G(w) + (1-theta) G(u^n) and J = I + theta dG/dw; theta = 1 is Eq.11.
+// The kernels keep k_i = (1-theta) G_i(u^n) - u_i^n per step, so F_i = (w_i + k_i) + theta G_i(w).
 //
 // Two plans:
 //   HYBRID  one CTA per system, w and u^n resident in registers for all n_steps; per Newton iteration
@@ -36,7 +39,7 @@ constexpr int newton_max_threads(int bytes, int P) {
 template <typename T, int P>
 __global__ void __launch_bounds__(newton_max_threads(sizeof(T), P))
 newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
-                     double inv_dx, int64_t n_steps, int bc, T tol, int max_iter,
+                     double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
                      long long *__restrict__ iters_out) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -51,11 +54,12 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     const double dtb = (double)dt[blockIdx.x];
     const T h = (T)(0.5 * dtb * inv_dx);
     const T r = (T)((double)nu[blockIdx.x] * dtb * inv_dx * inv_dx);
-    const T b0 = T(1) + T(2) * r;
+    const T th = theta * h, tr = theta * r, omt = T(1) - theta;     // Jacobian: I + theta dG/dw
+    const T b0 = T(1) + T(2) * tr;
     const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
     const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
 
-    T w[P], un[P];
+    T w[P], un[P];       // un holds k_i = (1-theta) G_i(u^n) - u_i^n once the first residual of a step is done
 #pragma unroll
     for (int c = 0; c < P / V; ++c) {
         int4 q4 = *reinterpret_cast<const int4 *>(row + c * V);
@@ -80,7 +84,9 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
                 const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
                 const T dc = wp - wm;
                 const T lap = (wp - w[j]) - (w[j] - wm);
-                T F = t_fma(h * w[j], dc, t_fma(-r, lap, w[j] - un[j]));
+                const T g = t_fma(h * w[j], dc, -r * lap);              // G_i(w)
+                if (k == 0) un[j] = t_fma(omt, g, -un[j]);              // w = u^n here
+                T F = t_fma(theta, g, w[j] + un[j]);
                 if ((j == 0 && fixL) || (j == P - 1 && fixR)) F = T(0);
                 q[j] = -F;
                 big |= !(t_abs(F) < tol);          // NaN counts as not converged
@@ -94,10 +100,10 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
                 [&](int j, T &a, T &b, T &e) {
                     if ((j == 0 && fixL) || (j == P - 1 && fixR)) { a = T(0); b = T(1); e = T(0); return; }
                     const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
-                    const T hw = h * w[j];
-                    a = -hw - r;
-                    b = t_fma(h, wp - wm, b0);
-                    e = hw - r;
+                    const T hw = th * w[j];
+                    a = -hw - tr;
+                    b = t_fma(th, wp - wm, b0);
+                    e = hw - tr;
                 },
                 q, f, c, first, last);
             T x0, xL;
@@ -144,10 +150,10 @@ bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out) {
 
 template <typename T, int P>
 int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                    double tol, int max_iter, long long *iters_out, int Tn, cudaStream_t s) {
+                    double theta, double tol, int max_iter, long long *iters_out, int Tn, cudaStream_t s) {
     const size_t smem = (size_t)11 * Tn * sizeof(T);
-    newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)tol,
-                                                            max_iter, iters_out);
+    newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
+                                                            (T)tol, max_iter, iters_out);
     return last_launch_status();
 }
 
@@ -168,20 +174,22 @@ __global__ void newton_transpose_kernel(const T *__restrict__ in, T *__restrict_
     }
 }
 
-// ws arrays (each [N][B], batch index fastest): un, w, cp, dp (= rhs, then solution), and for periodic
-// systems wp (second right-hand side of Sherman-Morrison).
+// ws arrays (each [N][B], batch index fastest): un, w, cp, dp (= rhs, then solution), kn (the per-step
+// constant k_i = (1-theta) G_i(u^n) - u_i^n), and for periodic systems wp (second right-hand side of
+// Sherman-Morrison).
 template <typename T>
 __global__ void __launch_bounds__(128)
 newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, T *__restrict__ dp,
-                     T *__restrict__ wp, const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int64_t N,
-                     double inv_dx, int64_t n_steps, int bc, T tol, int max_iter,
+                     T *__restrict__ kn, T *__restrict__ wp, const T *__restrict__ nu, const T *__restrict__ dt,
+                     int64_t B, int64_t N, double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
                      long long *__restrict__ iters_out) {
     const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= B) return;
     const double dtb = (double)dt[b];
     const T h = (T)(0.5 * dtb * inv_dx);
     const T r = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
-    const T b0 = T(1) + T(2) * r;
+    const T th = theta * h, tr = theta * r, omt = T(1) - theta;
+    const T b0 = T(1) + T(2) * tr;
     const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
     long long iters = 0;
 #define AT(arr, i) arr[(int64_t)(i) * B + b]
@@ -195,7 +203,9 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                 const T w0 = wi;
                 for (int64_t i = 0; i < N; ++i) {
                     const T wpv = (i + 1 < N) ? AT(w, i + 1) : w0;
-                    T F = t_fma(h * wi, wpv - wm, t_fma(-r, (wpv - wi) - (wi - wm), wi - AT(un, i)));
+                    const T g = t_fma(h * wi, wpv - wm, -r * ((wpv - wi) - (wi - wm)));     // G_i(w)
+                    if (k == 0) AT(kn, i) = t_fma(omt, g, -AT(un, i));                      // w = u^n here
+                    T F = t_fma(theta, g, wi + AT(kn, i));
                     if (dirichlet && (i == 0 || i == N - 1)) F = T(0);
                     AT(dp, i) = -F;
                     big |= !(t_abs(F) < tol);
@@ -210,8 +220,8 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                 T wm = AT(w, 0), wi = AT(w, 1);
                 for (int64_t i = 1; i <= N - 2; ++i) {
                     const T wpv = AT(w, i + 1);
-                    const T hw = h * wi;
-                    const T a = -hw - r, bb = t_fma(h, wpv - wm, b0), e = hw - r;
+                    const T hw = th * wi;
+                    const T a = -hw - tr, bb = t_fma(th, wpv - wm, b0), e = hw - tr;
                     const T inv = T(1) / (bb - a * cprev);
                     cprev = e * inv;
                     dprev = (AT(dp, i) - a * dprev) * inv;
@@ -225,8 +235,8 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                 }
             } else {              // cyclic: Sherman-Morrison (D6) with gamma = -diag_0
                 const T w0 = AT(w, 0), w1 = AT(w, 1), wN1 = AT(w, N - 1);
-                const T a0 = -h * w0 - r, d0 = t_fma(h, w1 - wN1, b0), e0 = h * w0 - r;
-                const T eN = h * wN1 - r;
+                const T a0 = -th * w0 - tr, d0 = t_fma(th, w1 - wN1, b0), e0 = th * w0 - tr;
+                const T eN = th * wN1 - tr;
                 const T gamma = -d0, alpha = a0, beta = eN;
                 const T ag = alpha / gamma;
                 T inv = T(1) / (d0 - gamma);
@@ -235,9 +245,9 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
                 T wm = w0, wi = w1;
                 for (int64_t i = 1; i < N; ++i) {
                     const T wpv = (i + 1 < N) ? AT(w, i + 1) : w0;
-                    const T hw = h * wi;
-                    const T a = -hw - r, e = hw - r;
-                    T bb = t_fma(h, wpv - wm, b0);
+                    const T hw = th * wi;
+                    const T a = -hw - tr, e = hw - tr;
+                    T bb = t_fma(th, wpv - wm, b0);
                     T ws2 = T(0);
                     if (i == N - 1) { bb = bb - alpha * beta / gamma; ws2 = beta; }
                     inv = T(1) / (bb - a * cprev);
@@ -273,12 +283,12 @@ bool newton_hybrid_fits(int is_f64, int64_t N) {
     return newton_geometry(is_f64, N, &P, &Tn);
 }
 size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc) {
-    return (size_t)B * (size_t)N * (bc == BURGERS_BC_PERIODIC ? 5 : 4);
+    return (size_t)B * (size_t)N * (bc == BURGERS_BC_PERIODIC ? 6 : 5);
 }
 
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                  double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s) {
+                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s) {
     if (n_steps == 0) {
         if (iters_out && cudaMemsetAsync(iters_out, 0, (size_t)B * sizeof(long long), s) != cudaSuccess)
             return BURGERS_ERR_CUDA;
@@ -289,16 +299,16 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
         if (!newton_geometry(sizeof(T) == 8, N, &P, &Tn)) return BURGERS_ERR_PLAN;
         if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
         switch (P) {
-            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
-            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
-            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, tol, max_iter, iters_out, Tn, s);
+            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
+            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
+            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
         }
         return BURGERS_ERR_PLAN;
     }
     // THOMAS
     const size_t BN = (size_t)B * (size_t)N;
-    T *un = ws, *w = ws + BN, *cp = ws + 2 * BN, *dp = ws + 3 * BN;
-    T *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 4 * BN : nullptr;
+    T *un = ws, *w = ws + BN, *cp = ws + 2 * BN, *dp = ws + 3 * BN, *kn = ws + 4 * BN;
+    T *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 5 * BN : nullptr;
     const int64_t nblk = ((N + 31) / 32) * ((B + 31) / 32);
     if (nblk > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
     dim3 tb(32, 8);
@@ -307,14 +317,14 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
     if (st != BURGERS_OK) return st;
     const int threads = (B <= 148 * 32 * 4) ? 32 : 128;
     newton_thomas_kernel<T><<<(unsigned)((B + threads - 1) / threads), threads, 0, s>>>(
-        un, w, cp, dp, wp, nu, dt, B, N, 1.0 / dx, n_steps, bc, (T)tol, max_iter, iters_out);
+        un, w, cp, dp, kn, wp, nu, dt, B, N, 1.0 / dx, n_steps, bc, (T)theta, (T)tol, max_iter, iters_out);
     st = last_launch_status();
     if (st != BURGERS_OK) return st;
     newton_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(un, u, N, B);
     return last_launch_status();
 }
 
-template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, int, long long *, int, float *, cudaStream_t);
-template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, int, long long *, int, double *, cudaStream_t);
+template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t);
+template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, double, int, long long *, int, double *, cudaStream_t);
 
 }  // namespace burgers

@@ -78,14 +78,17 @@ def test_argument_errors_are_synchronous(B):
     assert c(one, 1, 8, 1.0, one, 0.4, 3, one, None) == B.ERR_ENUM
     assert c(one, 1, 1, 1.0, one, 0.4, 0, one, None) == B.ERR_SHAPE
     nw = lib.burgers_newton_f64
-    assert nw(None, 1, 8, 1.0, one, one, 1, 0, 1e-6, 10, None, 0, None, 0, None) == B.ERR_NULL
-    assert nw(one, 1, 8, 1.0, one, one, 1, 0, -1.0, 10, None, 0, None, 0, None) == B.ERR_VALUE
-    assert nw(one, 1, 8, 1.0, one, one, 1, 0, float("nan"), 10, None, 0, None, 0, None) == B.ERR_VALUE
-    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1e-6, -1, None, 0, None, 0, None) == B.ERR_VALUE
-    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1e-6, 10, None, B.PLAN_LONG, None, 0, None) == B.ERR_ENUM
-    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 1e-6, 10, None, B.PLAN_HYBRID, None, 0, None) == B.ERR_PLAN
-    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 1e-6, 10, None, B.PLAN_AUTO, None, 0, None) == B.ERR_WORKSPACE
-    assert lib.burgers_newton_host_f32(one, 1, 8, 1.0, one, one, 1, 0, -2.0, 10, None) == B.ERR_VALUE
+    assert nw(None, 1, 8, 1.0, one, one, 1, 0, 1.0, 1e-6, 10, None, 0, None, 0, None) == B.ERR_NULL
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1.0, -1.0, 10, None, 0, None, 0, None) == B.ERR_VALUE
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1.0, float("nan"), 10, None, 0, None, 0, None) == B.ERR_VALUE
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1.0, 1e-6, -1, None, 0, None, 0, None) == B.ERR_VALUE
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1.5, 1e-6, 10, None, 0, None, 0, None) == B.ERR_VALUE
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, float("nan"), 1e-6, 10, None, 0, None, 0, None) == B.ERR_VALUE
+    assert nw(one, 1, 8, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_LONG, None, 0, None) == B.ERR_ENUM
+    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_HYBRID, None, 0, None) == B.ERR_PLAN
+    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_AUTO, None, 0, None) == B.ERR_WORKSPACE
+    assert lib.burgers_newton_host_f32(one, 1, 8, 1.0, one, one, 1, 0, 1.0, -2.0, 10, None) == B.ERR_VALUE
+    assert lib.burgers_newton_host_f64(one, 1, 8, 1.0, one, one, 1, 0, -0.1, 1e-6, 10, None) == B.ERR_VALUE
     # host variants validate the same way
     assert lib.burgers_explicit_host_f32(None, 1, 8, 1.0, one, one, 1, 0, 0) == B.ERR_NULL
     assert lib.burgers_btcs_host_f64(one, 1, 8, 1.0, one, one, -2, 0) == B.ERR_SHAPE
@@ -120,7 +123,7 @@ def test_plan_queries(B):
     assert B.plan_query(B.OP_NEWTON, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
     assert B.plan_query(B.OP_NEWTON, True, 1, 201, B.BC_DIRICHLET) == B.PLAN_THOMAS
     assert B.workspace_bytes(B.OP_NEWTON, True, 4096, 2048, B.BC_PERIODIC) == 0
-    assert B.workspace_bytes(B.OP_NEWTON, True, 2, 201, B.BC_PERIODIC) >= 5 * 2 * 201 * 8
+    assert B.workspace_bytes(B.OP_NEWTON, True, 2, 201, B.BC_PERIODIC) >= 6 * 2 * 201 * 8
     assert B.launch_count(B.OP_NEWTON, True, 4096, 2048, 0, n_steps=1000) == 1
     assert B.launch_count(B.OP_CFL, False, 1024, 4096, 1) == 1
     assert B.launch_count(B.OP_CFL, False, 1, 1 << 24, 0) == 2

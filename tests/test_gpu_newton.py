@@ -24,11 +24,12 @@ def B():
     return binding
 
 
-def run(B, u0, L, nu, dt, n, bc, tol, max_iter=50, plan=0):
+def run(B, u0, L, nu, dt, n, bc, tol, max_iter=50, plan=0, theta=1.0):
     import torch
     u = to_dev(np.ascontiguousarray(u0).copy())
     it = torch.zeros(u.shape[0] if u.dim() == 2 else 1, dtype=torch.int64, device="cuda")
-    B.burgers_newton(u, L, to_dev(nu), to_dev(dt), n, bc, tol=tol, max_iter=max_iter, iters_out=it, plan=plan)
+    B.burgers_newton(u, L, to_dev(nu), to_dev(dt), n, bc, tol=tol, max_iter=max_iter, iters_out=it, plan=plan,
+                     theta=theta)
     return u.cpu().numpy(), it.cpu().numpy()
 
 
@@ -135,3 +136,45 @@ def test_host_entry_point_matches_device_path(B):
     ud, idv = run(B, w.u0, w.L, w.nu, dt, 8, w.bc, tol=1e-9)
     np.testing.assert_array_equal(uh, ud)
     np.testing.assert_array_equal(ih, idv)
+
+
+# ---------------------------------------------------------------- theta-scheme
+def test_theta_half_worked_example_on_gpu(B):
+    G = read_golden("newton_4node.txt")
+    u4 = np.array([[1.0, 2.0, -1.0, 0.0]])
+    nu = np.array([0.1]); dt = np.array([0.1])
+    for k in (1, 2, 3):
+        got, _ = run(B, u4, 4.0, nu, dt, 1, B.BC_PERIODIC, tol=0.0, max_iter=k, theta=0.5)
+        np.testing.assert_allclose(got[0], G[f"cn{k}_periodic"], atol=1e-14)
+        got, _ = run(B, u4, 3.0, nu, dt, 1, B.BC_DIRICHLET, tol=0.0, max_iter=k, theta=0.5)
+        np.testing.assert_allclose(got[0], G[f"cn{k}_dirichlet"], atol=1e-14)
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.3, 0.0])
+def test_theta_scheme_parity_both_plans(B, theta):
+    w = W.c3_periodic_btcs(B=12, N=1024, n_steps=20)
+    C = 10.0 if theta >= 0.5 else 0.2        # theta < 1/2 is only conditionally stable
+    dt = oracle.dt_from_cfl(w.u0, w.L, w.nu, C, w.bc)
+    ref = oracle.newton_btcs(w.u0, w.L, w.nu, dt, 20, w.bc, tol=1e-12, theta=theta)
+    for plan in (B.PLAN_HYBRID, B.PLAN_THOMAS):
+        got, _ = run(B, w.u0, w.L, w.nu, dt, 20, w.bc, tol=1e-12, plan=plan, theta=theta)
+        assert rel_err(got, ref, w.u0) <= 1e-10, (theta, plan)
+    wd = W.c2_dirichlet_batch(B=5, N=512, dtype=np.float64)
+    dtd = oracle.dt_from_cfl(wd.u0, wd.L, wd.nu, C, wd.bc)
+    ref = oracle.newton_btcs(wd.u0, wd.L, wd.nu, dtd, 15, wd.bc, tol=1e-12, theta=theta)
+    for plan in (B.PLAN_HYBRID, B.PLAN_THOMAS):
+        got, _ = run(B, wd.u0, wd.L, wd.nu, dtd, 15, wd.bc, tol=1e-12, plan=plan, theta=theta)
+        assert rel_err(got, ref, wd.u0) <= 1e-10, (theta, plan, "dirichlet")
+
+
+def test_crank_nicolson_second_order_on_gpu(B):
+    # dt = dx/4: Crank-Nicolson stays second order (oracle pin: 1.9 < order < 2.1); checked here on the GPU
+    L, nu = 2 * math.pi, 0.05
+    errs = []
+    for N in (256, 512, 1024):
+        x = np.arange(N) * (L / N)
+        n = int(round(1.0 / (0.25 * L / N)))
+        got, _ = run(B, np.sin(x)[None, :], L, np.array([nu]), np.array([1.0 / n]), n, B.BC_PERIODIC, tol=1e-13,
+                     theta=0.5)
+        errs.append(math.sqrt(np.mean((got[0] - colehopf_sin(x, 1.0, nu)) ** 2)))
+    assert 1.9 < math.log2(errs[0] / errs[1]) < 2.1 and 1.9 < math.log2(errs[1] / errs[2]) < 2.1, errs
