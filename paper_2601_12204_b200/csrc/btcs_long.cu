@@ -89,6 +89,8 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
     constexpr int WB = 32 * RB;               // bytes per warp region of a stage
     __shared__ __align__(128) T stage[2][Tn * P];
     __shared__ T sA[2][Tn], sC[2][Tn], sD[2][Tn];
+    __shared__ T sFA[Tn], sFC[Tn], sFD[Tn];   // first interface rows (own arrays: the PCR buffers of the
+                                              // previous tile may still be read when these are written)
     const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
     // Programmatic dependent launch: let the next step's grid be scheduled while this one runs
     // (its CTAs become resident as ours retire), and wait here for the previous step's grid to
@@ -173,12 +175,12 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         if (t == Tn - 1) last.C = T(0);
 
         // ---- cyclic-reduction step: one row per thread in x_L
-        sA[1][t] = first.A; sC[1][t] = first.C; sD[1][t] = first.D;
+        sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
         __syncthreads();
         Row<T> row;
         {
             const int tn = (t + 1 < Tn) ? t + 1 : t;       // t = Tn-1: last.C == 0, values unused
-            const T nA = sA[1][tn], nC = sC[1][tn], nD = sD[1][tn];
+            const T nA = sFA[tn], nC = sFC[tn], nD = sFD[tn];
             const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
             row.A = -last.A * first.A * m;
             row.C = -last.C * nC * m;
