@@ -68,6 +68,11 @@ def make_workload(name, rank=0, world=1, reduced=False):
         Bg = 4096 * world
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
         return w, dict(op="btcs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES)
+    if name == "c2_traj":        # SURVEY 8(f) NEXT-4b: C2 fp32 with a snapshot of all trajectories every 50 steps
+        Bg = 1024 * world
+        w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
+                                 n_steps=1000 if reduced else 10000)
+        return w, dict(op="explicit", scheme=0, instr=I_EULER_F32, lanes=FP32_LANES, snap_every=50)
     if name in ("c3_newton", "c3_cn"):   # SURVEY 8(f) NEXT-1 / NEXT-2 on C3's inputs: Newton solve of the fully implicit
         Bg = 4096 * world                #   (theta = 1) / Crank-Nicolson (theta = 1/2) central scheme, tol 1e-6
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
@@ -212,6 +217,9 @@ class GpuRunner:
             self.launches = B.launch_count(B.OP_BTCS, is64, w.B, w.N, w.bc, n_steps=w.n_steps)
         self.launches += B.launch_count(B.OP_CFL, is64, w.B, w.N, w.bc)
         self.ws = torch.empty(need, dtype=torch.uint8, device=device) if need else None
+        self.snaps = None
+        if spec.get("snap_every"):
+            self.snaps = torch.empty((w.n_steps // spec["snap_every"], w.B, w.N), dtype=self.u0.dtype, device=device)
         self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
 
     def reset(self):
@@ -223,7 +231,10 @@ class GpuRunner:
 
     def op(self):
         w, B = self.w, self.B
-        if self.spec["op"] == "explicit":
+        if self.spec["op"] == "explicit" and self.snaps is not None:
+            B.burgers_explicit_traj(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"],
+                                    self.spec["snap_every"], snaps=self.snaps, ws=self.ws)
+        elif self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
         elif self.spec["op"] == "newton":
             B.burgers_newton(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
@@ -371,7 +382,7 @@ def run_ours(args):
                       "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
-        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn"):
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj"):
             if name == args.workload:
                 continue
             try:
@@ -387,6 +398,9 @@ def run_ours(args):
                                 "hbm_accounting_frac": rf["hbm_accounting_frac"],
                                 "dtype": "f32" if w2.dtype == np.float32 else "f64",
                                 "cfl_hbm_frac": cfl_leg(w2, s_ms, o_ms)["hbm_frac"]}
+                if r2.snaps is not None:
+                    extras[name]["snapshots"] = int(r2.snaps.shape[0])
+                    extras[name]["snapshot_bytes"] = int(r2.snaps.numel() * r2.snaps.element_size())
                 if spec2["op"] == "newton":
                     extras[name]["newton_iterations_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
                     extras[name]["tol"] = spec2["tol"]
@@ -444,7 +458,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")

@@ -111,6 +111,20 @@ int burgers_explicit_plan_f64(double *u, int64_t B, int64_t N, double L,
                               int bc, int scheme, int plan, int tblock, int ppt,
                               void *ws, size_t ws_bytes, void *stream);
 
+/* Same time stepping with TRAJECTORY output (SURVEY.md 8(f) NEXT-4b; the paper's stated purpose is data
+ * generation): after every snap_every-th step (steps snap_every, 2 snap_every, ...)
+ * the state is also written to snaps[k][B][N], k = 0 .. n_steps/snap_every - 1 (DEVICE pointer, room
+ * for floor(n_steps/snap_every) * B * N elements); u holds the final state as usual.  The RESIDENT
+ * plan writes the snapshots from the resident state inside the one kernel; the TILED plan runs one
+ * launch sequence per snapshot interval.  snap_every < 1 -> BURGERS_ERR_SHAPE. */
+int burgers_explicit_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                              int64_t n_steps, int bc, int scheme, int64_t snap_every, float *snaps,
+                              void *ws, size_t ws_bytes, void *stream);
+int burgers_explicit_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu,
+                              const double *dt, int64_t n_steps, int bc, int scheme,
+                              int64_t snap_every, double *snaps, void *ws, size_t ws_bytes,
+                              void *stream);
+
 /* ---- BTCS (Eq.23; D4-D7) ----------------------
  * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:
  *   sub_i = -r - max(c_i,0),  diag_i = 1 + 2r + |c_i|,  sup_i = -r + min(c_i,0).

@@ -229,3 +229,19 @@ def newton_btcs(u0, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, adv=None, thr
     if rc != 0:
         raise ValueError("oracle_newton_btcs: bad arguments")
     return (u.reshape(shape), iters) if return_iters else u.reshape(shape)
+
+
+def explicit_trajectory(u0, L, nu, dt, n_steps, bc, scheme, snap_every, threads=None):
+    """Snapshots of explicit time stepping after every snap_every-th step: [n_steps // snap_every][B][N]
+    plus the final state.  Plain composition of `explicit` calls (p then q steps == p+q steps, bitwise:
+    pinned by tests/test_oracle_pins.py::test_steps_compose_bitwise)."""
+    u = _f64(u0).copy()
+    snaps = []
+    done = 0
+    while done + snap_every <= n_steps:
+        u = explicit(u, L, nu, dt, snap_every, bc, scheme, threads=threads)
+        snaps.append(u.copy())
+        done += snap_every
+    if done < n_steps:
+        u = explicit(u, L, nu, dt, n_steps - done, bc, scheme, threads=threads)
+    return u, (np.stack(snaps) if snaps else np.empty((0,) + u.shape))

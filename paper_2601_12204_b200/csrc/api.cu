@@ -32,7 +32,7 @@ int btcs_auto_plan(int is_f64, int64_t B, int64_t N, int bc) {
 template <typename T>
 int explicit_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
                   int bc, int scheme, int plan, int tblock, int ppt, void *ws, size_t ws_bytes,
-                  void *stream) {
+                  void *stream, T *snaps = nullptr, int64_t snap_every = 0) {
     int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
     if (!scheme_ok(scheme)) return BURGERS_ERR_ENUM;
@@ -45,8 +45,8 @@ int explicit_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt
         const size_t need = (size_t)B * (size_t)N * sizeof(T);
         if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
     }
-    return launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, scheme, g, (T *)ws,
-                              (cudaStream_t)stream);
+    return launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, scheme, g, (T *)ws, snaps,
+                              snap_every, (cudaStream_t)stream);
 }
 
 template <typename T>
@@ -212,6 +212,23 @@ int burgers_explicit_plan_f64(double *u, int64_t B, int64_t N, double L, const d
                               const double *dt, int64_t n_steps, int bc, int scheme, int plan,
                               int tblock, int ppt, void *ws, size_t ws_bytes, void *stream) {
     return explicit_call<double>(u, B, N, L, nu, dt, n_steps, bc, scheme, plan, tblock, ppt, ws, ws_bytes, stream);
+}
+
+int burgers_explicit_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                              int64_t n_steps, int bc, int scheme, int64_t snap_every, float *snaps,
+                              void *ws, size_t ws_bytes, void *stream) {
+    if (!snaps) return BURGERS_ERR_NULL;
+    if (snap_every < 1) return BURGERS_ERR_SHAPE;
+    return explicit_call<float>(u, B, N, L, nu, dt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes, stream,
+                                snaps, snap_every);
+}
+int burgers_explicit_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                              int64_t n_steps, int bc, int scheme, int64_t snap_every, double *snaps,
+                              void *ws, size_t ws_bytes, void *stream) {
+    if (!snaps) return BURGERS_ERR_NULL;
+    if (snap_every < 1) return BURGERS_ERR_SHAPE;
+    return explicit_call<double>(u, B, N, L, nu, dt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes, stream,
+                                 snaps, snap_every);
 }
 
 int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

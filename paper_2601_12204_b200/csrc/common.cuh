@@ -44,7 +44,7 @@ int explicit_geometry(int is_f64, int64_t B, int64_t N, int bc, int scheme, int 
 template <typename T>
 int launch_explicit(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                     int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                    cudaStream_t s);
+                    T *snaps, int64_t snap_every, cudaStream_t s);
 // max threads per CTA the explicit kernel <T,P,scheme> may be launched with (register limit)
 int explicit_max_threads(int is_f64, int P, int scheme);
 

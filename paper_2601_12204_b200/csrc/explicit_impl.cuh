@@ -58,6 +58,11 @@ struct Params {
     // ping-pong buffers hold w, so only the first launch scales and only the last one unscales.
     // Frozen Dirichlet end nodes are ALWAYS stored unscaled (their original bits).
     int in_scaled, out_scaled;
+    // Trajectory output (SURVEY 8(f) NEXT-4b; RESIDENT plan, kernel template SNAP): after every
+    // snap_every-th step the state is also written to snaps[k][B][N], k = 0, 1, ...
+    T *snaps;
+    int64_t snap_every;
+    int64_t snap_stride;   // B*N
 };
 
 template <typename T> __device__ __forceinline__ T t_abs(T x);
@@ -133,9 +138,10 @@ constexpr int max_threads_for(int bytes, int P, int scheme) {
     return t;
 }
 
-template <typename T, int P, int SCHEME, bool TILED, bool WARP>
+template <typename T, int P, int SCHEME, bool TILED, bool WARP, bool SNAP = false>
 __global__ void __launch_bounds__(WARP ? 32 : max_threads_for(sizeof(T), P, SCHEME))
 explicit_kernel(const Params<T> p) {
+    static_assert(!(SNAP && TILED), "snapshots are fused into the RESIDENT plan only");
     constexpr bool SPLIT = (sizeof(T) == 4) && (SCHEME == BURGERS_SCHEME_EULER);
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -213,6 +219,43 @@ explicit_kernel(const Params<T> p) {
     const T keepL = v[0], keepR = v[P - 1];       // stored back bit-exactly when frozen
     int buf = 0;
     T left, right;
+    // trajectory output: val(j) is the (scaled) state of point j; unscaled with a reciprocal and one
+    // remainder correction (the final state uses the exact quotient)
+    int64_t snap_left = SNAP ? p.snap_every : 0;
+    T *snap_row = SNAP ? p.snaps + b * N : nullptr;
+    const T inv_scale = T(1) / scale;
+    auto snapshot = [&](auto val) {
+        if (!SNAP) return;
+        if (--snap_left != 0) return;
+        snap_left = p.snap_every;
+        auto out = [&](int j) {
+            T x = val(j);
+            if (SCALED) {
+                T qn = x * inv_scale;
+                qn = t_fma(t_fma(-qn, scale, x), inv_scale, qn);
+                x = qn;
+                if (j == 0 && fixL) x = keepL;
+                if (j == P - 1 && fixR) x = keepR;
+            }
+            return x;
+        };
+        if (active) {
+            if (vec_ok) {
+#pragma unroll
+                for (int c = 0; c < P / V; ++c) {
+                    int4 q;
+                    T *e = reinterpret_cast<T *>(&q);
+#pragma unroll
+                    for (int k = 0; k < V; ++k) e[k] = out(c * V + k);
+                    *reinterpret_cast<int4 *>(snap_row + g0 + c * V) = q;
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < P; ++j) snap_row[g0 + j] = out(j);
+            }
+        }
+        snap_row += p.snap_stride;
+    };
 
     if (SCHEME == BURGERS_SCHEME_EULER) {
         T base[SPLIT ? P : 1], s[SPLIT ? P : 1];
@@ -251,6 +294,7 @@ explicit_kernel(const Params<T> p) {
                     base[j] = nb;
                 }
             }
+            snapshot([&](int j) { return v[j]; });
         }
         if (SPLIT && !p.out_scaled) {       // u = (base + s)/scale, rounded once
 #pragma unroll
@@ -289,6 +333,7 @@ explicit_kernel(const Params<T> p) {
                     dm = dp;
                 }
             }
+            snapshot([&](int j) { return v[j]; });
         }
         if (SCALED && !p.out_scaled) {
 #pragma unroll
@@ -343,6 +388,9 @@ int launch_P(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStream_t 
     const size_t smem = (size_t)4 * g.block * sizeof(T);
     if (tiled) {
         explicit_kernel<T, P, SCHEME, true, false><<<(unsigned)grid, g.block, smem, s>>>(p);
+    } else if (p.snaps) {
+        if (g.block == 32) explicit_kernel<T, P, SCHEME, false, true, true><<<(unsigned)grid, 32, 0, s>>>(p);
+        else explicit_kernel<T, P, SCHEME, false, false, true><<<(unsigned)grid, g.block, smem, s>>>(p);
     } else if (g.block == 32) {
         explicit_kernel<T, P, SCHEME, false, true><<<(unsigned)grid, 32, 0, s>>>(p);
     } else {
@@ -367,34 +415,54 @@ int launch_scheme(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStre
 template <typename T>
 int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                          int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                         cudaStream_t s) {
+                         T *snaps, int64_t snap_every, cudaStream_t s) {
     if (n_steps == 0) return BURGERS_OK;
     Params<T> p;
     p.nu = nu; p.dt = dt; p.N = N; p.inv_dx = 1.0 / dx; p.nth = g.nth; p.bc = bc;
     p.halo = g.halo; p.W = g.W; p.tiles = g.tiles;
     p.in_scaled = 0; p.out_scaled = 0;
-    if (g.plan == BURGERS_PLAN_RESIDENT) {
-        p.src = u; p.dst = u; p.steps = n_steps;
+    p.snaps = nullptr; p.snap_every = 0; p.snap_stride = B * N;
+    auto launch = [&]() {
         return scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
                                               : launch_scheme<T, BURGERS_SCHEME_RK4>(p, g, B, s);
+    };
+    if (g.plan == BURGERS_PLAN_RESIDENT) {   // snapshots are written by the kernel itself
+        p.src = u; p.dst = u; p.steps = n_steps;
+        if (snaps && snap_every > 0 && n_steps >= snap_every) { p.snaps = snaps; p.snap_every = snap_every; }
+        return launch();
     }
-    // TILED: ping-pong between u and ws, tblock steps per launch; arrange the parity so that the
-    // last launch writes u when possible, else copy back once.
-    T *cur = u, *nxt = ws;
-    int64_t done = 0;
+    // TILED: ping-pong between u and ws, tblock steps per launch; copy back when the last launch
+    // wrote ws.  With snapshots: one such sequence per snap_every steps, then a device copy.
+    auto run = [&](int64_t steps) {
+        T *cur = u, *nxt = ws;
+        int64_t done = 0;
+        while (done < steps) {
+            const int64_t k = (steps - done < g.tblock) ? steps - done : g.tblock;
+            p.src = cur; p.dst = nxt; p.steps = k;
+            p.in_scaled = (done > 0); p.out_scaled = (done + k < steps);
+            int st = launch();
+            if (st != BURGERS_OK) return st;
+            T *tmp = cur; cur = nxt; nxt = tmp;
+            done += k;
+        }
+        if (cur != u &&
+            cudaMemcpyAsync(u, cur, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+            return (int)BURGERS_ERR_CUDA;
+        return (int)BURGERS_OK;
+    };
+    if (!(snaps && snap_every > 0)) return run(n_steps);
+    int64_t done = 0, k = 0;
     while (done < n_steps) {
-        const int64_t k = (n_steps - done < g.tblock) ? n_steps - done : g.tblock;
-        p.src = cur; p.dst = nxt; p.steps = k;
-        p.in_scaled = (done > 0); p.out_scaled = (done + k < n_steps);
-        int st = scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
-                                                : launch_scheme<T, BURGERS_SCHEME_RK4>(p, g, B, s);
+        const int64_t chunk = (n_steps - done < snap_every) ? n_steps - done : snap_every;
+        int st = run(chunk);
         if (st != BURGERS_OK) return st;
-        T *tmp = cur; cur = nxt; nxt = tmp;
-        done += k;
-    }
-    if (cur != u) {
-        if (cudaMemcpyAsync(u, cur, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
-            return BURGERS_ERR_CUDA;
+        done += chunk;
+        if (chunk == snap_every) {
+            if (cudaMemcpyAsync(snaps + k * B * N, u, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, s) !=
+                cudaSuccess)
+                return BURGERS_ERR_CUDA;
+            ++k;
+        }
     }
     return BURGERS_OK;
 }

@@ -1,0 +1,65 @@
+"""Trajectory output of the explicit schemes (SURVEY 8(f) NEXT-4b: snapshots for data generation,
+PAPER.md:22, :409): burgers_explicit_traj_* against the oracle stepped snapshot by snapshot."""
+import numpy as np
+import pytest
+
+import oracle
+from parity import TOL, oracle_dt, rel_err, to_dev
+from paper_2601_12204_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2601_12204_b200 import binding
+    return binding
+
+
+def check(B, w, n, scheme, every, cfl=None):
+    dt = oracle_dt(w.u0, w.L, w.nu, cfl or w.cfl, w.bc, w.dtype)
+    ref_u, ref_s = oracle.explicit_trajectory(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64),
+                                              dt.astype(np.float64), n, w.bc, scheme, every)
+    u = to_dev(w.u0.copy())
+    _, snaps = B.burgers_explicit_traj(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, scheme, every)
+    got_u, got_s = u.cpu().numpy(), snaps.cpu().numpy()
+    assert got_s.shape == ref_s.shape == (n // every,) + w.u0.shape
+    assert rel_err(got_u, ref_u, w.u0) <= TOL[w.dtype]
+    for k in range(n // every):
+        assert rel_err(got_s[k], ref_s[k], w.u0) <= TOL[w.dtype], k
+    return got_u, got_s, dt
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_resident_euler_and_rk4(B, dtype):
+    w = W.c2_dirichlet_batch(B=6, N=2048, dtype=dtype)
+    got_u, got_s, dt = check(B, w, 230, B.SCHEME_EULER, 50)        # ragged tail of 30 steps
+    np.testing.assert_array_equal(got_s[:, :, 0], np.broadcast_to(w.u0[:, 0], got_s[:, :, 0].shape))
+    check(B, w, 40, B.SCHEME_RK4, 8, cfl=0.8)
+    check(B, w, 12, B.SCHEME_EULER, 1)                              # every step
+    w5 = W.c5_rk4_ensemble(rows=np.arange(0, 65536, 8192), dtype=dtype)
+    check(B, w5, 90, B.SCHEME_RK4, 30)
+    if dtype == np.float64:     # fp64 steps compose bitwise: a snapshot equals a separate call of that length
+        u = to_dev(w.u0.copy())
+        B.burgers_explicit(u, w.L, to_dev(w.nu), to_dev(dt), 100, w.bc, B.SCHEME_EULER)
+        np.testing.assert_array_equal(u.cpu().numpy(), got_s[1])
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_tiled_plan_chunks(B, dtype):
+    w = W.c4a_long_explicit(N=(1 << 15) + 24, n_steps=0, dtype=dtype)
+    assert B.plan_query(B.OP_EXPLICIT, dtype == np.float64, 1, w.N, w.bc, 0) == B.PLAN_TILED
+    check(B, w, 150, B.SCHEME_EULER, 70)
+    check(B, w, 30, B.SCHEME_RK4, 10, cfl=0.5)     # at this N the two limits coincide: c + 2r = 2C must stay < 1.39 (D9)
+
+
+def test_semantics(B):
+    w = W.c2_dirichlet_batch(B=2, N=256, dtype=np.float64)
+    dt = oracle_dt(w.u0, w.L, w.nu, 0.4, w.bc, w.dtype)
+    u = to_dev(w.u0.copy())
+    _, snaps = B.burgers_explicit_traj(u, w.L, to_dev(w.nu), to_dev(dt), 5, w.bc, 0, 10)   # no snapshot due
+    assert snaps.shape[0] == 0
+    ref = oracle.explicit(w.u0, w.L, w.nu, dt, 5, w.bc, 0)
+    assert rel_err(u.cpu().numpy(), ref, w.u0) <= 1e-12
+    with pytest.raises(B.BurgersError):
+        B.burgers_explicit_traj(u, w.L, to_dev(w.nu), to_dev(dt), 5, w.bc, 0, 0)
