@@ -145,6 +145,15 @@ int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const doubl
                           const double *dt, int64_t n_steps, int bc, int plan, void *ws,
                           size_t ws_bytes, void *stream);
 
+/* BTCS with trajectory output, semantics as burgers_explicit_traj_*: one run of the AUTO plan per
+ * snapshot interval followed by a device copy (workspace as for burgers_btcs_*). */
+int burgers_btcs_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                          int64_t n_steps, int bc, int64_t snap_every, float *snaps, void *ws,
+                          size_t ws_bytes, void *stream);
+int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                          int64_t n_steps, int bc, int64_t snap_every, double *snaps, void *ws,
+                          size_t ws_bytes, void *stream);
+
 /* ---- fully implicit BTCS with central convection, Newton-Raphson (Eq.10-15) ----
  * (D11.)  Per step solve F(w) = 0 for w = u^{n+1},
  *   F_i = w_i - u_i^n + dt [ w_i (w_{i+1} - w_{i-1})/(2 dx) - nu (w_{i+1} - 2 w_i + w_{i-1})/dx^2 ]   (Eq.11)

@@ -29,7 +29,7 @@ PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG, PLAN_
 EXPORTS = [
     "burgers_explicit_f32", "burgers_explicit_f64", "burgers_explicit_plan_f32",
     "burgers_explicit_plan_f64", "burgers_explicit_traj_f32", "burgers_explicit_traj_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
-    "burgers_btcs_plan_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
+    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
     "burgers_launch_count", "burgers_strerror", "burgers_version",
@@ -49,6 +49,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_btcs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_explicit_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_explicit_traj_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_btcs_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_plan_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _p, _sz, _p]
     getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p, _int, _p, _sz, _p]
@@ -199,6 +201,27 @@ def burgers_explicit_traj(u, L, nu, dt, n_steps, bc, scheme, snap_every, snaps=N
                                                        int(n_steps), int(bc), int(scheme), int(snap_every),
                                                        snaps.data_ptr(), wsp, wsb, _stream())
     _check(st, f"burgers_explicit_traj_{sfx}")
+    return u, snaps[:ns]
+
+
+def burgers_btcs_traj(u, L, nu, dt, n_steps, bc, snap_every, snaps=None, ws=None):
+    """BTCS time stepping with trajectory output (include/burgers.h: burgers_btcs_traj_*)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    ns = int(n_steps) // int(snap_every) if snap_every >= 1 else 0
+    if snaps is None:
+        snaps = torch.empty((max(ns, 1), B, N), dtype=u.dtype, device=u.device)
+    _dev(snaps, "snaps", u.dtype)
+    if snaps.numel() < ns * B * N:
+        raise ValueError("snaps is too small")
+    need = workspace_bytes(OP_BTCS, u.dtype == torch.float64, B, N, bc, 0)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    st = getattr(_lib, f"burgers_btcs_traj_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(),
+                                                   int(n_steps), int(bc), int(snap_every), snaps.data_ptr(),
+                                                   wsp, wsb, _stream())
+    _check(st, f"burgers_btcs_traj_{sfx}")
     return u, snaps[:ns]
 
 

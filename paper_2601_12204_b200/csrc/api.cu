@@ -79,6 +79,31 @@ int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
     return BURGERS_ERR_ENUM;
 }
 
+// BTCS with trajectory output: one call of the plan per snapshot interval (the state is stored once
+// per interval anyway), then a device copy of u into snaps[k].
+template <typename T>
+int btcs_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
+                   int64_t snap_every, T *snaps, void *ws, size_t ws_bytes, void *stream) {
+    if (!snaps) return BURGERS_ERR_NULL;
+    if (snap_every < 1) return BURGERS_ERR_SHAPE;
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    int64_t done = 0, k = 0;
+    while (done < n_steps) {
+        const int64_t chunk = (n_steps - done < snap_every) ? n_steps - done : snap_every;
+        st = btcs_call<T>(u, B, N, L, nu, dt, chunk, bc, BURGERS_PLAN_AUTO, ws, ws_bytes, stream);
+        if (st != BURGERS_OK) return st;
+        done += chunk;
+        if (chunk == snap_every) {
+            if (cudaMemcpyAsync(snaps + k * B * N, u, (size_t)B * (size_t)N * sizeof(T), cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)stream) != cudaSuccess)
+                return BURGERS_ERR_CUDA;
+            ++k;
+        }
+    }
+    return BURGERS_OK;
+}
+
 template <typename T>
 int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
                 double theta, double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes,
@@ -246,6 +271,17 @@ int burgers_btcs_plan_f32(float *u, int64_t B, int64_t N, double L, const float 
 int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
                           int64_t n_steps, int bc, int plan, void *ws, size_t ws_bytes, void *stream) {
     return btcs_call<double>(u, B, N, L, nu, dt, n_steps, bc, plan, ws, ws_bytes, stream);
+}
+
+int burgers_btcs_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                          int64_t n_steps, int bc, int64_t snap_every, float *snaps, void *ws, size_t ws_bytes,
+                          void *stream) {
+    return btcs_traj_call<float>(u, B, N, L, nu, dt, n_steps, bc, snap_every, snaps, ws, ws_bytes, stream);
+}
+int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                          int64_t n_steps, int bc, int64_t snap_every, double *snaps, void *ws, size_t ws_bytes,
+                          void *stream) {
+    return btcs_traj_call<double>(u, B, N, L, nu, dt, n_steps, bc, snap_every, snaps, ws, ws_bytes, stream);
 }
 
 int burgers_newton_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

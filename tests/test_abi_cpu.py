@@ -27,7 +27,7 @@ def _declared():
 
 def test_header_symbols_exported(B):
     names = _declared()
-    assert len(names) >= 27
+    assert len(names) >= 29
     lib = ctypes.CDLL(B.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in burgers.h but not exported"
@@ -66,6 +66,9 @@ def test_argument_errors_are_synchronous(B):
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 2, None, None, 0, None) == B.ERR_NULL
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 0, one, None, 0, None) == B.ERR_SHAPE
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 7, 2, one, None, 0, None) == B.ERR_ENUM
+    bt = lib.burgers_btcs_traj_f64
+    assert bt(one, 1, 8, 1.0, one, one, 4, 0, 2, None, None, 0, None) == B.ERR_NULL
+    assert bt(one, 1, 8, 1.0, one, one, 4, 0, 0, one, None, 0, None) == B.ERR_SHAPE
     h = lib.burgers_btcs_f64
     assert h(None, 1, 8, 1.0, one, one, 1, 0, None, 0, None) == B.ERR_NULL
     assert h(one, 1, 8, 1.0, one, one, 1, 7, None, 0, None) == B.ERR_ENUM

@@ -63,3 +63,19 @@ def test_semantics(B):
     assert rel_err(u.cpu().numpy(), ref, w.u0) <= 1e-12
     with pytest.raises(B.BurgersError):
         B.burgers_explicit_traj(u, w.L, to_dev(w.nu), to_dev(dt), 5, w.bc, 0, 0)
+
+
+def test_btcs_trajectory(B):
+    for w, n, every in ((W.c3_periodic_btcs(B=6, N=512, n_steps=0), 23, 5),
+                        (W.c2_dirichlet_batch(B=3, N=1000, dtype=np.float64), 12, 4),       # THOMAS plan
+                        (W.c4b_long_btcs(N=1 << 14, n_steps=0), 9, 3)):                     # LONG plan
+        dt = oracle_dt(w.u0, w.L, w.nu, 10.0, w.bc, w.dtype)
+        u = to_dev(w.u0.copy())
+        _, snaps = B.burgers_btcs_traj(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, every)
+        assert snaps.shape[0] == n // every
+        ref = w.u0.astype(np.float64)
+        for k in range(n // every):
+            ref = oracle.btcs(ref, w.L, w.nu, dt, every, w.bc)
+            assert rel_err(snaps[k].cpu().numpy(), ref, w.u0) <= 1e-10, (w.name, k)
+        ref = oracle.btcs(ref, w.L, w.nu, dt, n - (n // every) * every, w.bc)
+        assert rel_err(u.cpu().numpy(), ref, w.u0) <= 1e-10
