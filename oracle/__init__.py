@@ -69,6 +69,8 @@ def _load():
     lib.oracle_newton_jacobian.restype = None
     lib.oracle_newton_btcs.argtypes = [p, i64, i64, f64, p, p, f64, i64, ci, f64, ci, ci, f64, p, ci]
     lib.oracle_newton_btcs.restype = ci
+    lib.oracle_btcs_gs.argtypes = [p, i64, i64, f64, p, p, i64, ci, f64, ci, ci, f64, p, ci]
+    lib.oracle_btcs_gs.restype = ci
     lib.oracle_max_threads.argtypes = []
     lib.oracle_max_threads.restype = ci
     _lib = lib
@@ -245,3 +247,20 @@ def explicit_trajectory(u0, L, nu, dt, n_steps, bc, scheme, snap_every, threads=
     if done < n_steps:
         u = explicit(u, L, nu, dt, n_steps - done, bc, scheme, threads=threads)
     return u, (np.stack(snaps) if snaps else np.empty((0,) + u.shape))
+
+
+def btcs_gs(u0, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=1000, adv=None, threads=None, return_iters=False):
+    """BTCS (D4) with the linear system solved by lexicographic Gauss-Seidel sweeps to max residual
+    < tol (D12); returns a new array (and the per-trajectory sweep totals)."""
+    u = _f64(u0).copy()
+    shape = u.shape
+    u = u.reshape(-1, shape[-1])
+    B, N = u.shape
+    nu_a, dt_a = _per_traj(nu, B), _per_traj(dt, B)
+    iters = np.zeros(B, dtype=np.int64)
+    rc = _load().oracle_btcs_gs(_ptr(u), B, N, float(L), _ptr(nu_a), _ptr(dt_a), int(n_steps), int(bc),
+                                float(tol), int(max_iter), int(adv is not None), float(adv or 0.0),
+                                ctypes.c_void_p(iters.ctypes.data), int(threads or default_threads()))
+    if rc != 0:
+        raise ValueError("oracle_btcs_gs: bad arguments")
+    return (u.reshape(shape), iters) if return_iters else u.reshape(shape)

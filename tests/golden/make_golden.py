@@ -148,8 +148,32 @@ def write_newton_example():
         lines.append(f"cn{k}_periodic " + fmt(w))
     for k, w in enumerate(newton_exact(u, dx, nu, dt, "dirichlet", 3, Fr(1, 2)), 1):
         lines.append(f"cn{k}_dirichlet " + fmt(w))
+    lines.append("# Gauss-Seidel sweeps on the lagged upwind BTCS system (D4/D12), same data, x0 = u^n")
+    for k, x in enumerate(gs_exact(u, dx, nu, dt, "periodic", 3), 1):
+        lines.append(f"gs{k}_periodic " + fmt(x))
+    for k, x in enumerate(gs_exact(u, dx, nu, dt, "dirichlet", 3), 1):
+        lines.append(f"gs{k}_dirichlet " + fmt(x))
     with open(os.path.join(HERE, "newton_4node.txt"), "w") as f:
         f.write("\n".join(lines) + "\n")
+
+
+def gs_exact(u, dx, nu, dt, bc, sweeps):
+    """`sweeps` lexicographic Gauss-Seidel sweeps on the BTCS system of D4 from x0 = u^n."""
+    N = len(u)
+    r = nu * dt / dx ** 2
+    rows = []
+    for i in range(N):
+        c = u[i] * dt / dx
+        rows.append((-r - max(c, 0), 1 + 2 * r + abs(c), -r + min(c, 0)))
+    idx = list(range(N)) if bc == "periodic" else list(range(1, N - 1))
+    x = list(u)
+    out = []
+    for _ in range(sweeps):
+        for i in idx:
+            sub, diag, sup = rows[i]
+            x[i] = (u[i] - sub * x[(i - 1) % N] - sup * x[(i + 1) % N]) / diag
+        out.append(list(x))
+    return out
 
 
 def fmt(vals):
