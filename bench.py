@@ -68,6 +68,11 @@ def make_workload(name, rank=0, world=1, reduced=False):
         Bg = 4096 * world
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
         return w, dict(op="btcs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES)
+    if name == "c3_gs":          # C3's trajectories, CFL-sized dt (C = 0.4, the regime of the paper's
+        Bg = 4096 * world        #   "5-7 iterations"), BTCS with Gauss-Seidel sweeps to max residual < 1e-6, 100 steps
+        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=10 if reduced else 100)
+        w.cfl = 0.4
+        return w, dict(op="gs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES, tol=1e-6, max_iter=1000)
     if name == "c2_traj":        # SURVEY 8(f) NEXT-4b: C2 fp32 with a snapshot of all trajectories every 50 steps
         Bg = 1024 * world
         w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
@@ -165,6 +170,9 @@ def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
         t0 = time.perf_counter()
         if spec["op"] == "btcs":
             oracle.btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+        elif spec["op"] == "gs":
+            oracle.btcs_gs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"], max_iter=spec["max_iter"],
+                           threads=threads)
         elif spec["op"] == "newton":
             oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
                                max_iter=spec["max_iter"], threads=threads, theta=spec["theta"])
@@ -206,6 +214,11 @@ class GpuRunner:
             self.plan = B.plan_query(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             need = B.workspace_bytes(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
+        elif spec["op"] == "gs":
+            self.plan = B.plan_query(B.OP_GS, is64, w.B, w.N, w.bc)
+            need = B.workspace_bytes(B.OP_GS, is64, w.B, w.N, w.bc)
+            self.launches = B.launch_count(B.OP_GS, is64, w.B, w.N, w.bc, n_steps=w.n_steps)
+            self.iters = torch.zeros(w.B, dtype=torch.int64, device=device)
         elif spec["op"] == "newton":
             self.plan = B.plan_query(B.OP_NEWTON, is64, w.B, w.N, w.bc)
             need = B.workspace_bytes(B.OP_NEWTON, is64, w.B, w.N, w.bc)
@@ -236,6 +249,9 @@ class GpuRunner:
                                     self.spec["snap_every"], snaps=self.snaps, ws=self.ws)
         elif self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
+        elif self.spec["op"] == "gs":
+            B.burgers_btcs_gs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
+                              max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws)
         elif self.spec["op"] == "newton":
             B.burgers_newton(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
                              max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws, theta=self.spec["theta"])
@@ -269,6 +285,16 @@ class GpuRunner:
             hu.copy_(hu0)
             self.flush.zero_(); torch.cuda.synchronize()
             t0 = time.perf_counter()
+            if self.spec["op"] == "gs":       # no _host entry point: pinned host -> device, device calls, device -> pinned host
+                du, dnu = hu.to(self.dev, non_blocking=True), hnu.to(self.dev, non_blocking=True)
+                ddt = B.dt_from_cfl(du, w.L, dnu, w.cfl, w.bc)
+                B.burgers_btcs_gs(du, w.L, dnu, ddt, w.n_steps, w.bc, tol=self.spec["tol"], max_iter=self.spec["max_iter"],
+                                  ws=self.ws)
+                hu.copy_(du); torch.cuda.synchronize()
+                t1 = time.perf_counter()
+                if i >= warmup:
+                    ms.append((t1 - t0) * 1e3)
+                continue
             dt = B.dt_from_cfl_host(u_np, w.L, nu_np, w.cfl, w.bc)
             if self.spec["op"] == "explicit":
                 B.burgers_explicit_host(u_np, w.L, nu_np, dt, w.n_steps, w.bc, self.spec["scheme"])
@@ -352,7 +378,8 @@ def run_ours(args):
     out = {
         "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
         else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else
-              ("grid-point updates/s (B*N*steps/s), Newton BTCS" if spec["op"] == "newton" else "grid-point updates/s (B*N*steps/s), BTCS")),
+              ("grid-point updates/s (B*N*steps/s), Newton BTCS" if spec["op"] == "newton" else
+               ("grid-point updates/s (B*N*steps/s), Gauss-Seidel BTCS" if spec["op"] == "gs" else "grid-point updates/s (B*N*steps/s), BTCS"))),
         "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
@@ -382,7 +409,7 @@ def run_ours(args):
                       "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
-        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj"):
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs"):
             if name == args.workload:
                 continue
             try:
@@ -401,6 +428,9 @@ def run_ours(args):
                 if r2.snaps is not None:
                     extras[name]["snapshots"] = int(r2.snaps.shape[0])
                     extras[name]["snapshot_bytes"] = int(r2.snaps.numel() * r2.snaps.element_size())
+                if spec2["op"] == "gs":
+                    extras[name]["gs_sweeps_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
+                    extras[name]["tol"] = spec2["tol"]
                 if spec2["op"] == "newton":
                     extras[name]["newton_iterations_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
                     extras[name]["tol"] = spec2["tol"]
@@ -458,7 +488,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")

@@ -66,7 +66,8 @@ enum {
 };
 enum { BURGERS_BC_PERIODIC = 0, BURGERS_BC_DIRICHLET = 1 };
 enum { BURGERS_SCHEME_EULER = 0, BURGERS_SCHEME_RK4 = 1 };
-enum { BURGERS_OP_EXPLICIT = 0, BURGERS_OP_BTCS = 1, BURGERS_OP_CFL = 2, BURGERS_OP_NEWTON = 3 };
+enum { BURGERS_OP_EXPLICIT = 0, BURGERS_OP_BTCS = 1, BURGERS_OP_CFL = 2, BURGERS_OP_NEWTON = 3,
+       BURGERS_OP_GS = 4 };
 
 /* Kernel plans.  AUTO picks by shape; the others force one
  * plan (tests use this for cross-plan agreement, G10) and return
@@ -153,6 +154,19 @@ int burgers_btcs_traj_f32(float *u, int64_t B, int64_t N, double L, const float 
 int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
                           int64_t n_steps, int bc, int64_t snap_every, double *snaps, void *ws,
                           size_t ws_bytes, void *stream);
+
+/* ---- BTCS with a Gauss-Seidel inner solver -----------
+ * The system of burgers_btcs_* solved per step by lexicographic Gauss-Seidel sweeps from x = u^n until
+ * max_i |rhs_i - (A x)_i| < tol or max_iter sweeps were done (D12) -- the paper's iterative
+ * variant, kept for its iteration counts and for comparison; the direct solvers are exact and cheaper.
+ * One thread per system; needs workspace (burgers_workspace_bytes(BURGERS_OP_GS, ...)).
+ * iters_out: DEVICE pointer to B int64 (sweeps summed over the steps), or NULL. */
+int burgers_btcs_gs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                        int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out,
+                        void *ws, size_t ws_bytes, void *stream);
+int burgers_btcs_gs_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                        int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out,
+                        void *ws, size_t ws_bytes, void *stream);
 
 /* ---- fully implicit BTCS with central convection, Newton-Raphson (Eq.10-15) ----
  * (D11.)  Per step solve F(w) = 0 for w = u^{n+1},

@@ -23,13 +23,13 @@ OK = 0
 ERR_NULL, ERR_SHAPE, ERR_ENUM, ERR_VALUE, ERR_WORKSPACE, ERR_CUDA, ERR_PLAN = -1, -2, -3, -4, -5, -6, -7
 BC_PERIODIC, BC_DIRICHLET = 0, 1
 SCHEME_EULER, SCHEME_RK4 = 0, 1
-OP_EXPLICIT, OP_BTCS, OP_CFL, OP_NEWTON = 0, 1, 2, 3
+OP_EXPLICIT, OP_BTCS, OP_CFL, OP_NEWTON, OP_GS = 0, 1, 2, 3, 4
 PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG, PLAN_LONG_GENERAL = 0, 1, 2, 3, 4, 5, 6
 
 EXPORTS = [
     "burgers_explicit_f32", "burgers_explicit_f64", "burgers_explicit_plan_f32",
     "burgers_explicit_plan_f64", "burgers_explicit_traj_f32", "burgers_explicit_traj_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
-    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
+    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
     "burgers_launch_count", "burgers_strerror", "burgers_version",
@@ -51,6 +51,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_explicit_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_btcs_gs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_gs_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_plan_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _p, _sz, _p]
     getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p, _int, _p, _sz, _p]
@@ -239,6 +241,27 @@ def burgers_btcs(u, L, nu, dt, n_steps, bc, ws=None, plan=PLAN_AUTO):
     st = fn(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(), int(n_steps), int(bc),
             int(plan), wsp, wsb, _stream())
     _check(st, f"burgers_btcs_{sfx}")
+    return u
+
+
+def burgers_btcs_gs(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=1000, iters_out=None, ws=None):
+    """In-place BTCS with a Gauss-Seidel inner solver (include/burgers.h: burgers_btcs_gs_*)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    if nu.numel() != B or dt.numel() != B:
+        raise ValueError("nu and dt must have length B")
+    ip = None
+    if iters_out is not None:
+        _dev(iters_out, "iters_out", torch.int64)
+        ip = ctypes.c_void_p(iters_out.data_ptr())
+    need = workspace_bytes(OP_GS, u.dtype == torch.float64, B, N, bc)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    st = getattr(_lib, f"burgers_btcs_gs_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(),
+                                                 int(n_steps), int(bc), float(tol), int(max_iter), ip, wsp, wsb,
+                                                 _stream())
+    _check(st, f"burgers_btcs_gs_{sfx}")
     return u
 
 

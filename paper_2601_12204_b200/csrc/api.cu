@@ -105,6 +105,18 @@ int btcs_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *d
 }
 
 template <typename T>
+int gs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc, double tol,
+            int max_iter, int64_t *iters_out, void *ws, size_t ws_bytes, void *stream) {
+    int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
+    const size_t need = btcs_gs_ws_elems(B, N) * sizeof(T);
+    if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
+    return launch_btcs_gs<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, tol, max_iter,
+                             reinterpret_cast<long long *>(iters_out), (T *)ws, (cudaStream_t)stream);
+}
+
+template <typename T>
 int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
                 double theta, double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes,
                 void *stream) {
@@ -284,6 +296,17 @@ int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const doubl
     return btcs_traj_call<double>(u, B, N, L, nu, dt, n_steps, bc, snap_every, snaps, ws, ws_bytes, stream);
 }
 
+int burgers_btcs_gs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                        int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, void *ws,
+                        size_t ws_bytes, void *stream) {
+    return gs_call<float>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, ws, ws_bytes, stream);
+}
+int burgers_btcs_gs_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                        int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out, void *ws,
+                        size_t ws_bytes, void *stream) {
+    return gs_call<double>(u, B, N, L, nu, dt, n_steps, bc, tol, max_iter, iters_out, ws, ws_bytes, stream);
+}
+
 int burgers_newton_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                        int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out,
                        int plan, void *ws, size_t ws_bytes, void *stream) {
@@ -354,6 +377,7 @@ size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, i
         if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
         return plan == BURGERS_PLAN_THOMAS ? align_up(newton_thomas_ws_elems(B, N, bc) * esz, 256) : 0;
     }
+    if (op == BURGERS_OP_GS) return align_up(btcs_gs_ws_elems(B, N) * esz, 256);
     if (op == BURGERS_OP_BTCS) {
         if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
         if (plan == BURGERS_PLAN_THOMAS) return align_up(btcs_thomas_ws_elems(B, N, bc) * esz, 256);
@@ -373,6 +397,7 @@ int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, i
     }
     if (op == BURGERS_OP_BTCS) return btcs_auto_plan(dtype_is_f64, B, N, bc);
     if (op == BURGERS_OP_NEWTON) return newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
+    if (op == BURGERS_OP_GS) return BURGERS_PLAN_THOMAS;
     if (op == BURGERS_OP_CFL) return BURGERS_PLAN_AUTO;
     return BURGERS_ERR_ENUM;
 }
@@ -391,6 +416,7 @@ int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int
         if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;
         return plan == BURGERS_PLAN_HYBRID ? 1 : 3;
     }
+    if (op == BURGERS_OP_GS) return 3;
     if (op == BURGERS_OP_BTCS) {
         if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
         if (plan == BURGERS_PLAN_THOMAS) return btcs_thomas_launch_count(n_steps);

@@ -70,6 +70,12 @@ size_t btcs_long_ws_bytes(int esz, int64_t B, int64_t N);
 int64_t btcs_long_launch_count(int64_t n_steps, int general_only);
 bool btcs_long_fits(int64_t N, int bc);
 
+// ---------------------------------------------------------------- Gauss-Seidel BTCS (btcs_gs.cu)
+template <typename T>
+int launch_btcs_gs(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                   double tol, int max_iter, long long *iters_out, T *ws, cudaStream_t s);
+size_t btcs_gs_ws_elems(int64_t B, int64_t N);
+
 // ---------------------------------------------------------------- Newton BTCS (newton.cu)
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
