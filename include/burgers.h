@@ -126,6 +126,20 @@ int burgers_explicit_traj_f64(double *u, int64_t B, int64_t N, double L, const d
                               int64_t snap_every, double *snaps, void *ws, size_t ws_bytes,
                               void *stream);
 
+/* Explicit stepping with an ADAPTIVE time step (SURVEY.md 8(f) NEXT-4a; "timesteps chosen to
+ * satisfy the CFL criteria"): n_outer times { dt_b = C min(dx/max|u_b|, dx^2/(2 nu_b)) from the current
+ * state (dt_from_cfl_*); m_steps steps of the scheme with it }.  Everything is enqueued on the stream;
+ * nothing synchronises with the host.  dt_scratch: DEVICE [B] (holds the last dt on return);
+ * t_out: DEVICE double [B] receiving the simulated time sum m_steps*dt_b, or NULL. */
+int burgers_explicit_adaptive_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C,
+                                  int64_t n_outer, int64_t m_steps, int bc, int scheme,
+                                  float *dt_scratch, double *t_out, void *ws, size_t ws_bytes,
+                                  void *stream);
+int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, const double *nu, double C,
+                                  int64_t n_outer, int64_t m_steps, int bc, int scheme,
+                                  double *dt_scratch, double *t_out, void *ws, size_t ws_bytes,
+                                  void *stream);
+
 /* ---- BTCS (Eq.23; D4-D7) ----------------------
  * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:
  *   sub_i = -r - max(c_i,0),  diag_i = 1 + 2r + |c_i|,  sup_i = -r + min(c_i,0).

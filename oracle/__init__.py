@@ -264,3 +264,17 @@ def btcs_gs(u0, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=1000, adv=None, threa
     if rc != 0:
         raise ValueError("oracle_btcs_gs: bad arguments")
     return (u.reshape(shape), iters) if return_iters else u.reshape(shape)
+
+
+def explicit_adaptive(u0, L, nu, C, n_outer, m_steps, bc, scheme, dtype=np.float64, threads=None):
+    """n_outer times { dt = dt_from_cfl(u) rounded to `dtype`; m_steps explicit steps with it }: plain
+    composition of the pinned `dt_from_cfl` and `explicit`.  Returns (u, t) with t = sum m_steps*dt."""
+    u = _f64(u0).copy()
+    u2 = u.reshape(-1, u.shape[-1])
+    t = np.zeros(u2.shape[0])
+    for _ in range(n_outer):
+        dt = dt_from_cfl(u2.astype(dtype).astype(np.float64) if dtype != np.float64 else u2, L, nu, C, bc)
+        dt = dt.astype(dtype).astype(np.float64)
+        u2 = explicit(u2, L, nu, dt, m_steps, bc, scheme, threads=threads)
+        t += m_steps * dt
+    return u2.reshape(u.shape), t

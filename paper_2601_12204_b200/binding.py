@@ -28,7 +28,7 @@ PLAN_AUTO, PLAN_RESIDENT, PLAN_TILED, PLAN_THOMAS, PLAN_HYBRID, PLAN_LONG, PLAN_
 
 EXPORTS = [
     "burgers_explicit_f32", "burgers_explicit_f64", "burgers_explicit_plan_f32",
-    "burgers_explicit_plan_f64", "burgers_explicit_traj_f32", "burgers_explicit_traj_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
+    "burgers_explicit_plan_f64", "burgers_explicit_traj_f32", "burgers_explicit_traj_f64", "burgers_explicit_adaptive_f32", "burgers_explicit_adaptive_f64", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
     "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
@@ -49,6 +49,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_btcs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_explicit_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_explicit_traj_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_explicit_adaptive_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _i64, _i64, _int, _int, _p, _p, _p, _sz, _p]
+    getattr(_lib, f"burgers_explicit_adaptive_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_gs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _p, _sz, _p]
@@ -204,6 +206,24 @@ def burgers_explicit_traj(u, L, nu, dt, n_steps, bc, scheme, snap_every, snaps=N
                                                        snaps.data_ptr(), wsp, wsb, _stream())
     _check(st, f"burgers_explicit_traj_{sfx}")
     return u, snaps[:ns]
+
+
+def burgers_explicit_adaptive(u, L, nu, C, n_outer, m_steps, bc, scheme, ws=None):
+    """Explicit stepping with the CFL time step recomputed every m_steps steps (include/burgers.h:
+    burgers_explicit_adaptive_*).  Returns (u, t, dt_last): t = simulated time per trajectory (float64)."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype)
+    B, N = _shape(u)
+    dt = torch.empty(B, dtype=u.dtype, device=u.device)
+    t = torch.zeros(B, dtype=torch.float64, device=u.device)
+    need = workspace_bytes(OP_EXPLICIT, u.dtype == torch.float64, B, N, bc, scheme)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    st = getattr(_lib, f"burgers_explicit_adaptive_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), float(C),
+                                                           int(n_outer), int(m_steps), int(bc), int(scheme),
+                                                           dt.data_ptr(), t.data_ptr(), wsp, wsb, _stream())
+    _check(st, f"burgers_explicit_adaptive_{sfx}")
+    return u, t, dt
 
 
 def burgers_btcs_traj(u, L, nu, dt, n_steps, bc, snap_every, snaps=None, ws=None):

@@ -79,6 +79,43 @@ int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
     return BURGERS_ERR_ENUM;
 }
 
+template <typename T>
+int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out, void *stream);
+
+// Adaptive time step (SURVEY 8(f) NEXT-4a): n_outer times { dt = dt_from_cfl(u); m explicit steps with it;
+// t += m dt }, all enqueued on the stream, no host synchronisation.
+template <typename T>
+__global__ void accumulate_time_kernel(double *__restrict__ t, const T *__restrict__ dt, int64_t B, double m) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b < B) t[b] += m * (double)dt[b];
+}
+
+template <typename T>
+int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, int64_t n_outer, int64_t m_steps,
+                  int bc, int scheme, T *dt_scratch, double *t_out, void *ws, size_t ws_bytes, void *stream) {
+    if (!dt_scratch) return BURGERS_ERR_NULL;
+    if (n_outer < 0 || m_steps < 1) return BURGERS_ERR_SHAPE;
+    int st = check_common(u, nu, dt_scratch, B, N, L, 0, bc);
+    if (st != BURGERS_OK) return st;
+    if (!scheme_ok(scheme)) return BURGERS_ERR_ENUM;
+    if (!(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (t_out && cudaMemsetAsync(t_out, 0, (size_t)B * sizeof(double), s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    for (int64_t k = 0; k < n_outer; ++k) {
+        st = cfl_call<T>(u, B, N, L, nu, C, bc, dt_scratch, stream);
+        if (st != BURGERS_OK) return st;
+        st = explicit_call<T>(u, B, N, L, nu, dt_scratch, m_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes,
+                              stream);
+        if (st != BURGERS_OK) return st;
+        if (t_out) {
+            accumulate_time_kernel<T><<<(unsigned)((B + 255) / 256), 256, 0, s>>>(t_out, dt_scratch, B, (double)m_steps);
+            st = last_launch_status();
+            if (st != BURGERS_OK) return st;
+        }
+    }
+    return BURGERS_OK;
+}
+
 // BTCS with trajectory output: one call of the plan per snapshot interval (the state is stored once
 // per interval anyway), then a device copy of u into snaps[k].
 template <typename T>
@@ -266,6 +303,17 @@ int burgers_explicit_traj_f64(double *u, int64_t B, int64_t N, double L, const d
     if (snap_every < 1) return BURGERS_ERR_SHAPE;
     return explicit_call<double>(u, B, N, L, nu, dt, n_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes, stream,
                                  snaps, snap_every);
+}
+
+int burgers_explicit_adaptive_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C,
+                                  int64_t n_outer, int64_t m_steps, int bc, int scheme, float *dt_scratch,
+                                  double *t_out, void *ws, size_t ws_bytes, void *stream) {
+    return adaptive_call<float>(u, B, N, L, nu, C, n_outer, m_steps, bc, scheme, dt_scratch, t_out, ws, ws_bytes, stream);
+}
+int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, const double *nu, double C,
+                                  int64_t n_outer, int64_t m_steps, int bc, int scheme, double *dt_scratch,
+                                  double *t_out, void *ws, size_t ws_bytes, void *stream) {
+    return adaptive_call<double>(u, B, N, L, nu, C, n_outer, m_steps, bc, scheme, dt_scratch, t_out, ws, ws_bytes, stream);
 }
 
 int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

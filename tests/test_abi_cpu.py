@@ -27,7 +27,7 @@ def _declared():
 
 def test_header_symbols_exported(B):
     names = _declared()
-    assert len(names) >= 31
+    assert len(names) >= 33
     lib = ctypes.CDLL(B.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in burgers.h but not exported"
@@ -66,6 +66,11 @@ def test_argument_errors_are_synchronous(B):
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 2, None, None, 0, None) == B.ERR_NULL
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 0, one, None, 0, None) == B.ERR_SHAPE
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 7, 2, one, None, 0, None) == B.ERR_ENUM
+    ad = lib.burgers_explicit_adaptive_f64
+    assert ad(one, 1, 8, 1.0, one, 0.4, 3, 5, 0, 0, None, None, None, 0, None) == B.ERR_NULL
+    assert ad(one, 1, 8, 1.0, one, 0.4, 3, 0, 0, 0, one, None, None, 0, None) == B.ERR_SHAPE
+    assert ad(one, 1, 8, 1.0, one, -0.4, 3, 5, 0, 0, one, None, None, 0, None) == B.ERR_VALUE
+    assert ad(one, 1, 8, 1.0, one, 0.4, 3, 5, 0, 9, one, None, None, 0, None) == B.ERR_ENUM
     gs = lib.burgers_btcs_gs_f64
     assert gs(one, 1, 8, 1.0, one, None, 1, 0, 1e-6, 10, None, one, 1 << 20, None) == B.ERR_NULL
     assert gs(one, 1, 8, 1.0, one, one, 1, 0, -1e-6, 10, None, one, 1 << 20, None) == B.ERR_VALUE
