@@ -555,6 +555,80 @@ int oracle_btcs_gs(double *u, int64_t B, int64_t N, double L, const double *nu, 
     return fail ? -1 : 0;
 }
 
+/* ---------------------------------------------------------------------------
+ * D13 (SURVEY 8(f) NEXT-4c): DISCRETE ADJOINT of the forward-Euler scheme (D3), the
+ * reverse-mode derivative the paper obtains from JAX.
+ * One step is u^{n+1} = Phi(u^n), Phi_i = u_i + dt F_i(u) (D2).  With cx = dt/dx,
+ * rr = nu dt/dx^2 and the upwind switch held fixed (it is locally constant):
+ *   u_i > 0 :  dPhi_i/du_{i-1} = cx u_i + rr,  dPhi_i/du_i = 1 - cx (2u_i - u_{i-1}) - 2rr,  dPhi_i/du_{i+1} = rr
+ *   u_i <= 0:  dPhi_i/du_{i-1} = rr,  dPhi_i/du_i = 1 - cx (u_{i+1} - 2u_i) - 2rr,  dPhi_i/du_{i+1} = rr - cx u_i
+ * Dirichlet end nodes: Phi_i = u_i (row of the identity).  Given lam^N = dJ/du^N, the adjoint
+ * recursion is lam^n = (dPhi/du (u^n))^T lam^{n+1}, n = N-1..0, and lam^0 = dJ/du^0 (dt, nu fixed).
+ * The forward states are recomputed and stored (N * n_steps doubles per trajectory).
+ * Test hook use_adv as in D2 (the map is then linear and the adjoint its exact transpose).
+ */
+static void adjoint_step(const double *u, const double *lam, double *out, int64_t N, double cx,
+                         double rr, int bc, int use_adv, double adv)
+{
+    /* out_j = sum_i dPhi_i/du_j lam_i: scatter row i of the Jacobian into columns */
+    for (int64_t j = 0; j < N; ++j) out[j] = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) { out[i] += lam[i]; continue; }
+        int64_t im = (i == 0) ? N - 1 : i - 1;
+        int64_t ip = (i == N - 1) ? 0 : i + 1;
+        double a = use_adv ? adv : u[i];
+        double dm, d0, dp;
+        if (a > 0.0) {
+            dm = cx * a + rr;
+            d0 = 1.0 - cx * a - (use_adv ? 0.0 : cx * (u[i] - u[im])) - 2.0 * rr;
+            dp = rr;
+        } else {
+            dm = rr;
+            d0 = 1.0 + cx * a - (use_adv ? 0.0 : cx * (u[ip] - u[i])) - 2.0 * rr;
+            dp = rr - cx * a;
+        }
+        out[im] += dm * lam[i];
+        out[i] += d0 * lam[i];
+        out[ip] += dp * lam[i];
+    }
+}
+
+int oracle_explicit_adjoint(const double *u0, double *lam, int64_t B, int64_t N, double L,
+                            const double *nu, const double *dt, int64_t n_steps, int bc, int use_adv,
+                            double adv, int nthreads)
+{
+    if (!u0 || !lam || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 1)
+    for (int64_t b = 0; b < B; ++b) {
+        double *st = (double *)malloc((size_t)(n_steps + 7) * (size_t)N * sizeof(double));
+        if (!st) {
+#pragma omp atomic write
+            fail = 1;
+            continue;
+        }
+        double *wk = st + (size_t)(n_steps + 1) * N; /* 5N + N */
+        for (int64_t i = 0; i < N; ++i) st[i] = u0[b * N + i];
+        for (int64_t n = 0; n < n_steps; ++n) {      /* forward, storing u^0..u^{n_steps} */
+            double *cur = st + (size_t)(n + 1) * N;
+            for (int64_t i = 0; i < N; ++i) cur[i] = st[(size_t)n * N + i];
+            explicit_one(cur, N, dx, nu[b], dt[b], 1, bc, SCHEME_EULER, use_adv, adv, wk);
+        }
+        double cx = dt[b] / dx, rr = nu[b] * dt[b] / (dx * dx);
+        double *tmp = wk + 5 * N;
+        for (int64_t n = n_steps - 1; n >= 0; --n) {
+            adjoint_step(st + (size_t)n * N, lam + b * N, tmp, N, cx, rr, bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) lam[b * N + i] = tmp[i];
+        }
+        free(st);
+    }
+    return fail ? -1 : 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP
