@@ -140,6 +140,19 @@ int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, con
                                   double *dt_scratch, double *t_out, void *ws, size_t ws_bytes,
                                   void *stream);
 
+/* Discrete ADJOINT of n_steps forward-Euler steps (SURVEY.md 8(f) NEXT-4c; the reverse-mode derivative
+ * the paper takes from JAX; D13).  u0: the initial state (not
+ * modified); lam: in dJ/du^N, out dJ/du^0 = (du^N/du^0)^T lam, with dt and nu held fixed and the upwind
+ * switch locally constant.  The forward states are recomputed into the workspace
+ * (burgers_adjoint_workspace_bytes: about n_steps * B * N elements), B <= 65535. */
+int burgers_explicit_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L,
+                                 const float *nu, const float *dt, int64_t n_steps, int bc, void *ws,
+                                 size_t ws_bytes, void *stream);
+int burgers_explicit_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L,
+                                 const double *nu, const double *dt, int64_t n_steps, int bc, void *ws,
+                                 size_t ws_bytes, void *stream);
+size_t burgers_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+
 /* ---- BTCS (Eq.23; D4-D7) ----------------------
  * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:
  *   sub_i = -r - max(c_i,0),  diag_i = 1 + 2r + |c_i|,  sup_i = -r + min(c_i,0).

@@ -116,6 +116,44 @@ int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, i
     return BURGERS_OK;
 }
 
+// Discrete adjoint of n_steps forward-Euler steps: forward sweep with one snapshot per step (explicit
+// kernel, trajectory output), then one adjoint launch per step in reverse.
+// ws layout: [lam ping-pong B*N][u work B*N][states max(n_steps-1,0)*B*N][workspace of the explicit op].
+template <typename T>
+size_t adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps) {
+    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
+    const size_t st = align_up((size_t)(n_steps > 1 ? n_steps - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
+    return 2 * bn + st + burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc, BURGERS_SCHEME_EULER,
+                                                 BURGERS_PLAN_AUTO);
+}
+
+template <typename T>
+int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
+                 int bc, void *ws, size_t ws_bytes, void *stream) {
+    if (!lam) return BURGERS_ERR_NULL;
+    int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (n_steps == 0) return BURGERS_OK;
+    if (!ws || ws_bytes < adjoint_ws_bytes<T>(B, N, bc, n_steps)) return BURGERS_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
+    const size_t stb = align_up((size_t)(n_steps > 1 ? n_steps - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
+    unsigned char *base = static_cast<unsigned char *>(ws);
+    T *pong = reinterpret_cast<T *>(base);
+    T *work = reinterpret_cast<T *>(base + bn);
+    T *states = reinterpret_cast<T *>(base + 2 * bn);
+    void *ews = base + 2 * bn + stb;
+    const size_t ews_bytes = ws_bytes - (2 * bn + stb);
+    if (n_steps > 1) {      // forward: u^1 .. u^{n_steps-1}
+        if (cudaMemcpyAsync(work, u0, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+            return BURGERS_ERR_CUDA;
+        st = explicit_call<T>(work, B, N, L, nu, dt, n_steps - 1, bc, BURGERS_SCHEME_EULER, BURGERS_PLAN_AUTO, 0, 0, ews,
+                              ews_bytes, stream, states, 1);
+        if (st != BURGERS_OK) return st;
+    }
+    return launch_adjoint_steps<T>(u0, states, lam, pong, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, s);
+}
+
 // BTCS with trajectory output: one call of the plan per snapshot interval (the state is stored once
 // per interval anyway), then a device copy of u into snaps[k].
 template <typename T>
@@ -314,6 +352,19 @@ int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, con
                                   int64_t n_outer, int64_t m_steps, int bc, int scheme, double *dt_scratch,
                                   double *t_out, void *ws, size_t ws_bytes, void *stream) {
     return adaptive_call<double>(u, B, N, L, nu, C, n_outer, m_steps, bc, scheme, dt_scratch, t_out, ws, ws_bytes, stream);
+}
+
+int burgers_explicit_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                 const float *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
+    return adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+}
+int burgers_explicit_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                 const double *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
+    return adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+}
+size_t burgers_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
+    if (B < 1 || N < 3 || n_steps < 0) return 0;
+    return dtype_is_f64 ? adjoint_ws_bytes<double>(B, N, bc, n_steps) : adjoint_ws_bytes<float>(B, N, bc, n_steps);
 }
 
 int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

@@ -70,6 +70,11 @@ size_t btcs_long_ws_bytes(int esz, int64_t B, int64_t N);
 int64_t btcs_long_launch_count(int64_t n_steps, int general_only);
 bool btcs_long_fits(int64_t N, int bc);
 
+// ---------------------------------------------------------------- adjoint of explicit Euler (adjoint.cu)
+template <typename T>
+int launch_adjoint_steps(const T *u0, const T *states, T *lam, T *pong, int64_t B, int64_t N, double dx,
+                         const T *nu, const T *dt, int64_t n_steps, int bc, cudaStream_t s);
+
 // ---------------------------------------------------------------- Gauss-Seidel BTCS (btcs_gs.cu)
 template <typename T>
 int launch_btcs_gs(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,

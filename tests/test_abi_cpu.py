@@ -27,7 +27,7 @@ def _declared():
 
 def test_header_symbols_exported(B):
     names = _declared()
-    assert len(names) >= 33
+    assert len(names) >= 36
     lib = ctypes.CDLL(B.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in burgers.h but not exported"
@@ -66,6 +66,12 @@ def test_argument_errors_are_synchronous(B):
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 2, None, None, 0, None) == B.ERR_NULL
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 0, 0, one, None, 0, None) == B.ERR_SHAPE
     assert tj(one, 1, 8, 1.0, one, one, 4, 0, 7, 2, one, None, 0, None) == B.ERR_ENUM
+    aj = lib.burgers_explicit_adjoint_f64
+    assert aj(one, None, 1, 8, 1.0, one, one, 3, 0, None, 0, None) == B.ERR_NULL
+    assert aj(one, one, 1, 8, 1.0, one, one, 3, 0, None, 0, None) == B.ERR_WORKSPACE
+    assert aj(one, one, 1, 8, 1.0, one, one, -3, 0, None, 0, None) == B.ERR_SHAPE
+    lib.burgers_adjoint_workspace_bytes.restype = ctypes.c_size_t
+    assert lib.burgers_adjoint_workspace_bytes(1, 4, 100, 0, 11) >= (2 + 10) * 4 * 100 * 8
     ad = lib.burgers_explicit_adaptive_f64
     assert ad(one, 1, 8, 1.0, one, 0.4, 3, 5, 0, 0, None, None, None, 0, None) == B.ERR_NULL
     assert ad(one, 1, 8, 1.0, one, 0.4, 3, 0, 0, 0, one, None, None, 0, None) == B.ERR_SHAPE
