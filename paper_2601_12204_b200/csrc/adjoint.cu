@@ -9,8 +9,12 @@
 // and the identity row for Dirichlet end nodes.  One adjoint step gathers column j:
 //   lam^n_j = dPhi_{j-1}/du_j lam_{j-1} + dPhi_j/du_j lam_j + dPhi_{j+1}/du_j lam_{j+1}   at u^n.
 // The forward states u^0..u^{N-1} come from the trajectory output of the explicit kernel (one
-// snapshot per step, written by the RESIDENT kernel from its on-chip state); the backward sweep is one
-// streaming launch per step (HBM-bound: reads u^n and lam, writes lam).
+// snapshot per step, written by the RESIDENT kernel from its on-chip state).  Backward sweep, two plans:
+//   RESIDENT  one CTA per trajectory keeps lam in registers for all steps (P consecutive points per
+//             thread, edge values of u^n and lam exchanged through shared memory, one barrier per step)
+//             and STREAMS the stored states, prefetching u^{n-1} while step n is computed: HBM-bound at
+//             sizeof(T) bytes per point and step.  Needs N = P * threads with threads <= 512.
+//   STREAMING one launch per step over all points (any N): reads u^n and lam, writes lam.
 #include "common.cuh"
 
 namespace burgers {
@@ -52,11 +56,112 @@ adjoint_step_kernel(const T *__restrict__ u, const T *__restrict__ lam, T *__res
     out[b * N + j] = acc;
 }
 
+// ---- RESIDENT backward sweep
+template <typename T, int P>
+__global__ void __launch_bounds__(512)
+adjoint_resident_kernel(const T *__restrict__ u0, const T *__restrict__ states, T *__restrict__ lam,
+                        const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int64_t N, double inv_dx,
+                        int64_t n_steps, int bc) {
+    constexpr int V = 16 / sizeof(T);
+    static_assert(P % V == 0, "a thread row must be a whole number of 16-byte vectors");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T *edge = reinterpret_cast<T *>(smem_raw);          // [2][4][nth]
+    const int t = threadIdx.x, nth = blockDim.x;
+    const int64_t b = blockIdx.x;
+    const double dtb = (double)dt[b];
+    const T cx = (T)(dtb * inv_dx);
+    const T rr = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    const int64_t off = b * N + (int64_t)t * P, BN = B * N;
+    auto load = [&](const T *src, T (&dst)[P]) {
+#pragma unroll
+        for (int c = 0; c < P / V; ++c) {
+            const int4 q = *reinterpret_cast<const int4 *>(src + off + c * V);
+            const T *e = reinterpret_cast<const T *>(&q);
+#pragma unroll
+            for (int k = 0; k < V; ++k) dst[c * V + k] = e[k];
+        }
+    };
+    auto state = [&](int64_t n) { return (n == 0) ? u0 : states + (size_t)(n - 1) * (size_t)BN; };
+    T l[P], uc[P];
+    load(lam, l);
+    load(state(n_steps - 1), uc);
+    const int tl = (t == 0) ? nth - 1 : t - 1, tr = (t == nth - 1) ? 0 : t + 1;
+    const bool firstT = (t == 0), lastT = (t == nth - 1);
+    int buf = 0;
+    for (int64_t n = n_steps - 1; n >= 0; --n) {
+        T un[P];
+        if (n > 0) load(state(n - 1), un);              // prefetch the next (earlier) state
+        T *e = edge + buf * 4 * nth;
+        e[t] = uc[0]; e[nth + t] = uc[P - 1]; e[2 * nth + t] = l[0]; e[3 * nth + t] = l[P - 1];
+        __syncthreads();
+        const T uL = e[nth + tl], uR = e[tr], lL = e[3 * nth + tl], lR = e[2 * nth + tr];
+        buf ^= 1;
+        T ln[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            const T um = j ? uc[j - 1] : uL, uj = uc[j], up = (j < P - 1) ? uc[j + 1] : uR;
+            const T lm = j ? l[j - 1] : lL, lp = (j < P - 1) ? l[j + 1] : lR;
+            // global positions of j-1, j, j+1 relative to the Dirichlet end nodes 0 and N-1
+            const bool j_first = firstT && j == 0, j_last = lastT && j == P - 1;
+            const bool m_first = firstT && j == 1;                               // node j-1 is node 0
+            const bool p_last = (lastT && j == P - 2);                          // node j+1 is node N-1
+            T acc;
+            if (dirichlet && (j_first || j_last)) {
+                acc = l[j];
+            } else {
+                const T g = (uj > T(0)) ? (uj - um) : (up - uj);
+                const T d0 = T(1) - cx * ((uj > T(0)) ? uj : -uj) - cx * g - T(2) * rr;
+                acc = d0 * l[j];
+            }
+            if (!(dirichlet && (j_first || m_first))) acc += ((um > T(0)) ? rr : rr - cx * um) * lm;
+            if (!(dirichlet && (j_last || p_last))) acc += ((up > T(0)) ? cx * up + rr : rr) * lp;
+            ln[j] = acc;
+        }
+#pragma unroll
+        for (int j = 0; j < P; ++j) { l[j] = ln[j]; uc[j] = un[j]; }
+    }
+#pragma unroll
+    for (int c = 0; c < P / V; ++c) {
+        int4 q;
+        T *e = reinterpret_cast<T *>(&q);
+#pragma unroll
+        for (int k = 0; k < V; ++k) e[k] = l[c * V + k];
+        *reinterpret_cast<int4 *>(lam + off + c * V) = q;
+    }
+}
+
+// P consecutive points per thread, N/P threads (<= 512): the smallest P that fits
+int adjoint_resident_P(int64_t N, int esz) {
+    const int V = 16 / esz;
+    for (int P = (V > 4 ? V : 4); P * esz <= 128; P *= 2)      // four P-value arrays live in registers
+        if (N % P == 0 && N / P <= 512 && N >= 2 * P) return P;
+    return 0;
+}
+
+template <typename T, int P>
+int launch_resident(const T *u0, const T *states, T *lam, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                    int64_t n_steps, int bc, cudaStream_t s) {
+    const int nth = (int)(N / P);
+    adjoint_resident_kernel<T, P><<<(unsigned)B, nth, (size_t)8 * nth * sizeof(T), s>>>(u0, states, lam, nu, dt, B, N,
+                                                                                      1.0 / dx, n_steps, bc);
+    return last_launch_status();
+}
+
 }  // namespace
 
 template <typename T>
 int launch_adjoint_steps(const T *u0, const T *states, T *lam, T *pong, int64_t B, int64_t N, double dx,
                          const T *nu, const T *dt, int64_t n_steps, int bc, cudaStream_t s) {
+    switch (adjoint_resident_P(N, (int)sizeof(T))) {
+        case 4: return launch_resident<T, 4>(u0, states, lam, B, N, dx, nu, dt, n_steps, bc, s);
+        case 8: return launch_resident<T, 8>(u0, states, lam, B, N, dx, nu, dt, n_steps, bc, s);
+        case 16: return launch_resident<T, 16>(u0, states, lam, B, N, dx, nu, dt, n_steps, bc, s);
+        case 32:
+            if (sizeof(T) == 4) return launch_resident<float, 32>((const float *)u0, (const float *)states, (float *)lam, B,
+                                                                  N, dx, (const float *)nu, (const float *)dt, n_steps, bc, s);
+            break;
+    }
     if (B > 65535) return BURGERS_ERR_SHAPE;
     dim3 grid((unsigned)((N + 255) / 256), (unsigned)B);
     T *cur = lam, *nxt = pong;
