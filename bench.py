@@ -73,6 +73,11 @@ def make_workload(name, rank=0, world=1, reduced=False):
         w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=10 if reduced else 100)
         w.cfl = 0.4
         return w, dict(op="gs", scheme=None, instr=I_BTCS_HYBRID, lanes=FP64_LANES, tol=1e-6, max_iter=1000)
+    if name == "c2_adjoint":     # SURVEY 8(f) NEXT-4c: reverse-mode derivative of 1000 Euler steps of 256 C2 trajectories
+        Bg = 256 * world
+        w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
+                                 n_steps=100 if reduced else 1000)
+        return w, dict(op="adjoint", scheme=0, instr=I_EULER_F32, lanes=FP32_LANES)
     if name == "c2_traj":        # SURVEY 8(f) NEXT-4b: C2 fp32 with a snapshot of all trajectories every 50 steps
         Bg = 1024 * world
         w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
@@ -214,6 +219,12 @@ class GpuRunner:
             self.plan = B.plan_query(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             need = B.workspace_bytes(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"])
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
+        elif spec["op"] == "adjoint":
+            self.plan = 0
+            need = int(B.raw().burgers_adjoint_workspace_bytes(int(is64), w.B, w.N, w.bc, w.n_steps))
+            self.launches = 2          # forward trajectory kernel + resident backward kernel
+            self.lam0 = torch.randn(self.u0.shape, dtype=self.u0.dtype, device=device,
+                                    generator=torch.Generator(device=device).manual_seed(1220404))
         elif spec["op"] == "gs":
             self.plan = B.plan_query(B.OP_GS, is64, w.B, w.N, w.bc)
             need = B.workspace_bytes(B.OP_GS, is64, w.B, w.N, w.bc)
@@ -236,11 +247,12 @@ class GpuRunner:
         self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
 
     def reset(self):
-        self.u.copy_(self.u0)
+        self.u.copy_(self.lam0 if self.spec["op"] == "adjoint" else self.u0)     # adjoint: u holds lambda
         self.flush.zero_()          # L2 flush between timed iterations (outside the event pairs)
 
     def cfl(self):
-        self.B.dt_from_cfl(self.u, self.w.L, self.nu, self.w.cfl, self.w.bc, out=self.dt)
+        src = self.u0 if self.spec["op"] == "adjoint" else self.u
+        self.B.dt_from_cfl(src, self.w.L, self.nu, self.w.cfl, self.w.bc, out=self.dt)
 
     def op(self):
         w, B = self.w, self.B
@@ -249,6 +261,8 @@ class GpuRunner:
                                     self.spec["snap_every"], snaps=self.snaps, ws=self.ws)
         elif self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
+        elif self.spec["op"] == "adjoint":
+            B.burgers_explicit_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
         elif self.spec["op"] == "gs":
             B.burgers_btcs_gs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
                               max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws)
@@ -409,7 +423,7 @@ def run_ours(args):
                       "note": "host-buffer C-ABI calls (dt_from_cfl_host + burgers_*_host), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
-        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs"):
+        for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs", "c2_adjoint"):
             if name == args.workload:
                 continue
             try:
@@ -428,6 +442,11 @@ def run_ours(args):
                 if r2.snaps is not None:
                     extras[name]["snapshots"] = int(r2.snaps.shape[0])
                     extras[name]["snapshot_bytes"] = int(r2.snaps.numel() * r2.snaps.element_size())
+                if spec2["op"] == "adjoint":
+                    esz2 = w2.u0.dtype.itemsize
+                    extras[name]["state_bytes_written_and_read"] = int(2 * (w2.n_steps - 1) * w2.B * w2.N * esz2)
+                    extras[name]["hbm_frac_of_state_traffic"] = (2 * (w2.n_steps - 1) * w2.B * w2.N * esz2 /
+                                                                 (statistics.mean(o_ms) * 1e-3) / (pk["hbm_gbs"] * 1e9))
                 if spec2["op"] == "gs":
                     extras[name]["gs_sweeps_per_step"] = float(r2.iters.double().mean().item()) / w2.n_steps
                     extras[name]["tol"] = spec2["tol"]
@@ -488,7 +507,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs"])
+    ap.add_argument("--workload", default="c2_f32", choices=["c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs", "c2_adjoint"])
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")
