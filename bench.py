@@ -299,11 +299,16 @@ class GpuRunner:
             hu.copy_(hu0)
             self.flush.zero_(); torch.cuda.synchronize()
             t0 = time.perf_counter()
-            if self.spec["op"] == "gs":       # no _host entry point: pinned host -> device, device calls, device -> pinned host
+            if self.spec["op"] in ("gs", "adjoint"):   # no _host entry point: pinned host -> device, device calls, device -> pinned host
                 du, dnu = hu.to(self.dev, non_blocking=True), hnu.to(self.dev, non_blocking=True)
                 ddt = B.dt_from_cfl(du, w.L, dnu, w.cfl, w.bc)
-                B.burgers_btcs_gs(du, w.L, dnu, ddt, w.n_steps, w.bc, tol=self.spec["tol"], max_iter=self.spec["max_iter"],
-                                  ws=self.ws)
+                if self.spec["op"] == "gs":
+                    B.burgers_btcs_gs(du, w.L, dnu, ddt, w.n_steps, w.bc, tol=self.spec["tol"],
+                                      max_iter=self.spec["max_iter"], ws=self.ws)
+                else:                                  # (the seed lambda is already on the device)
+                    dl = self.lam0.clone()
+                    B.burgers_explicit_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws)
+                    du = dl
                 hu.copy_(du); torch.cuda.synchronize()
                 t1 = time.perf_counter()
                 if i >= warmup:
