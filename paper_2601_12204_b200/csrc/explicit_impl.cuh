@@ -222,7 +222,7 @@ explicit_kernel(const Params<T> p) {
     // trajectory output: val(j) is the (scaled) state of point j; unscaled with a reciprocal and one
     // remainder correction (the final state uses the exact quotient)
     int64_t snap_left = SNAP ? p.snap_every : 0;
-    T *snap_row = SNAP ? p.snaps + b * N : nullptr;
+    T *snap_row = SNAP ? p.snaps + b * N + g0 : nullptr;     // this thread's row in the next snapshot
     const T inv_scale = T(1) / scale;
     auto snapshot = [&](auto val) {
         if (!SNAP) return;
@@ -239,7 +239,35 @@ explicit_kernel(const Params<T> p) {
             }
             return x;
         };
-        if (active) {
+        constexpr int CRs = (P % V == 0) ? P / V : 0;          // 16-byte chunks per thread row
+        if (CRs >= 1 && CRs <= 8 && vec_ok) {
+            // Stage the warp's rows in shared memory (XOR-swizzled 16-byte chunks: conflict-free both
+            // ways) so that the global stores are 512 contiguous bytes per request instead of one
+            // 16-byte piece of 32 different rows.  Whole warps take part; rows past N are not stored.
+            constexpr int CRd = (CRs >= 1 && CRs <= 8) ? CRs : 1;     // (keeps the dead branch well-formed)
+            constexpr int RB = CRd * 16, SW = 8 / CRd;
+            unsigned char *stg = smem_raw + (size_t)4 * blockDim.x * sizeof(T) + (size_t)(t >> 5) * 32 * RB;
+            const int lane = t & 31;
+#pragma unroll
+            for (int c = 0; c < CRd; ++c) {
+                int4 q;
+                T *e = reinterpret_cast<T *>(&q);
+#pragma unroll
+                for (int k = 0; k < V; ++k) e[k] = out(c * V + k);
+                *reinterpret_cast<int4 *>(stg + lane * RB + ((c ^ ((lane / SW) % CRd)) * 16)) = q;
+            }
+            __syncwarp();
+            const int64_t wbase = (int64_t)(t >> 5) * 32 * P;      // first point of the warp's rows
+#pragma unroll
+            for (int k = 0; k < CRd; ++k) {
+                const int qi = k * 32 + lane, r = qi / CRd, c = qi % CRd;
+                const int64_t g = wbase + (int64_t)qi * V;
+                if (g < N)
+                    *reinterpret_cast<int4 *>(snap_row - g0 + g) =
+                        *reinterpret_cast<const int4 *>(stg + r * RB + ((c ^ ((r / SW) % CRd)) * 16));
+            }
+            __syncwarp();
+        } else if (active) {
             if (vec_ok) {
 #pragma unroll
                 for (int c = 0; c < P / V; ++c) {
@@ -247,11 +275,11 @@ explicit_kernel(const Params<T> p) {
                     T *e = reinterpret_cast<T *>(&q);
 #pragma unroll
                     for (int k = 0; k < V; ++k) e[k] = out(c * V + k);
-                    *reinterpret_cast<int4 *>(snap_row + g0 + c * V) = q;
+                    *reinterpret_cast<int4 *>(snap_row + c * V) = q;
                 }
             } else {
 #pragma unroll
-                for (int j = 0; j < P; ++j) snap_row[g0 + j] = out(j);
+                for (int j = 0; j < P; ++j) snap_row[j] = out(j);
             }
         }
         snap_row += p.snap_stride;
@@ -388,9 +416,16 @@ int launch_P(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStream_t 
     const size_t smem = (size_t)4 * g.block * sizeof(T);
     if (tiled) {
         explicit_kernel<T, P, SCHEME, true, false><<<(unsigned)grid, g.block, smem, s>>>(p);
-    } else if (p.snaps) {
-        if (g.block == 32) explicit_kernel<T, P, SCHEME, false, true, true><<<(unsigned)grid, 32, 0, s>>>(p);
-        else explicit_kernel<T, P, SCHEME, false, false, true><<<(unsigned)grid, g.block, smem, s>>>(p);
+    } else if (p.snaps) {          // + one staged row per thread for the coalesced snapshot stores
+        const size_t ssm = smem + (size_t)g.block * P * sizeof(T);
+        if (ssm > 48 * 1024) {
+            cudaFuncSetAttribute(explicit_kernel<T, P, SCHEME, false, true, true>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm);
+            cudaFuncSetAttribute(explicit_kernel<T, P, SCHEME, false, false, true>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssm);
+        }
+        if (g.block == 32) explicit_kernel<T, P, SCHEME, false, true, true><<<(unsigned)grid, 32, ssm, s>>>(p);
+        else explicit_kernel<T, P, SCHEME, false, false, true><<<(unsigned)grid, g.block, ssm, s>>>(p);
     } else if (g.block == 32) {
         explicit_kernel<T, P, SCHEME, false, true><<<(unsigned)grid, 32, 0, s>>>(p);
     } else {
