@@ -144,7 +144,7 @@ int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, con
  * the paper takes from JAX; D13).  u0: the initial state (not
  * modified); lam: in dJ/du^N, out dJ/du^0 = (du^N/du^0)^T lam, with dt and nu held fixed and the upwind
  * switch locally constant.  The forward states are recomputed into the workspace
- * (burgers_adjoint_workspace_bytes: about n_steps * B * N elements), B <= 65535. */
+ * (burgers_adjoint_workspace_bytes; checkpointed when they would not fit, see below). */
 int burgers_explicit_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L,
                                  const float *nu, const float *dt, int64_t n_steps, int bc, void *ws,
                                  size_t ws_bytes, void *stream);
@@ -152,6 +152,19 @@ int burgers_explicit_adjoint_f64(const double *u0, double *lam, int64_t B, int64
                                  const double *nu, const double *dt, int64_t n_steps, int bc, void *ws,
                                  size_t ws_bytes, void *stream);
 size_t burgers_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+/* Same with an explicit checkpoint segment: the steps are cut into segments of `segment` steps, the
+ * state at every segment start is stored by a first forward sweep, and each segment is recomputed (one
+ * snapshot per step) just before it is swept backwards: memory (n_steps/segment + segment) states, one
+ * extra forward sweep.  segment = 0: automatic (one segment while all states fit 8 GiB, else
+ * ceil(sqrt(n_steps))) -- this is what burgers_explicit_adjoint_* use.  segment < 0 -> BURGERS_ERR_SHAPE. */
+int burgers_explicit_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L,
+                                      const float *nu, const float *dt, int64_t n_steps, int bc,
+                                      int64_t segment, void *ws, size_t ws_bytes, void *stream);
+int burgers_explicit_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L,
+                                      const double *nu, const double *dt, int64_t n_steps, int bc,
+                                      int64_t segment, void *ws, size_t ws_bytes, void *stream);
+size_t burgers_adjoint_ckpt_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc,
+                                            int64_t n_steps, int64_t segment);
 
 /* ---- BTCS (Eq.23; D4-D7) ----------------------
  * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:

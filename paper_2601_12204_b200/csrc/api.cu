@@ -116,42 +116,78 @@ int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, i
     return BURGERS_OK;
 }
 
-// Discrete adjoint of n_steps forward-Euler steps: forward sweep with one snapshot per step (explicit
-// kernel, trajectory output), then one adjoint launch per step in reverse.
-// ws layout: [lam ping-pong B*N][u work B*N][states max(n_steps-1,0)*B*N][workspace of the explicit op].
+// Discrete adjoint of n_steps forward-Euler steps with CHECKPOINTING: the forward states are needed in
+// reverse order.  The steps are cut into segments of m steps; a first forward sweep stores the state at
+// every segment start (trajectory output with snap_every = m), then, last segment first, the segment
+// is recomputed from its checkpoint with one snapshot per step and swept backwards.  m = n_steps (one
+// segment, nothing recomputed) while all states fit kAdjointFullBytes, else ceil(sqrt(n_steps)), which
+// minimises the memory (n_steps/m + m states) at the cost of a second forward sweep.
+// ws layout: [lam ping-pong B*N][u work B*N][checkpoints (K-1)*B*N][segment states (m-1)*B*N][explicit ws].
+constexpr size_t kAdjointFullBytes = (size_t)8 << 30;
+
+inline int64_t adjoint_segment(size_t esz, int64_t B, int64_t N, int64_t n_steps, int64_t segment) {
+    if (segment > 0) return segment < n_steps ? segment : (n_steps > 0 ? n_steps : 1);
+    if (n_steps <= 1 || (size_t)n_steps * (size_t)B * (size_t)N * esz <= kAdjointFullBytes) return n_steps > 0 ? n_steps : 1;
+    int64_t m = (int64_t)std::ceil(std::sqrt((double)n_steps));
+    return m < 1 ? 1 : m;
+}
+
 template <typename T>
-size_t adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps) {
+size_t adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps, int64_t segment) {
+    const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
+    const int64_t K = (n_steps + m - 1) / m;
     const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t st = align_up((size_t)(n_steps > 1 ? n_steps - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
-    return 2 * bn + st + burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc, BURGERS_SCHEME_EULER,
-                                                 BURGERS_PLAN_AUTO);
+    const size_t ck = align_up((size_t)(K > 1 ? K - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
+    const size_t st = align_up((size_t)(m > 1 ? m - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
+    return 2 * bn + ck + st + burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc,
+                                                      BURGERS_SCHEME_EULER, BURGERS_PLAN_AUTO);
 }
 
 template <typename T>
 int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
-                 int bc, void *ws, size_t ws_bytes, void *stream) {
+                 int bc, int64_t segment, void *ws, size_t ws_bytes, void *stream) {
     if (!lam) return BURGERS_ERR_NULL;
     int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
+    if (segment < 0) return BURGERS_ERR_SHAPE;
     if (n_steps == 0) return BURGERS_OK;
-    if (!ws || ws_bytes < adjoint_ws_bytes<T>(B, N, bc, n_steps)) return BURGERS_ERR_WORKSPACE;
+    if (!ws || ws_bytes < adjoint_ws_bytes<T>(B, N, bc, n_steps, segment)) return BURGERS_ERR_WORKSPACE;
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t stb = align_up((size_t)(n_steps > 1 ? n_steps - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
+    const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
+    const int64_t K = (n_steps + m - 1) / m;
+    const size_t BN = (size_t)B * (size_t)N;
+    const size_t bn = align_up(BN * sizeof(T), 256);
+    const size_t ckb = align_up((size_t)(K > 1 ? K - 1 : 0) * BN * sizeof(T), 256);
+    const size_t stb = align_up((size_t)(m > 1 ? m - 1 : 0) * BN * sizeof(T), 256);
     unsigned char *base = static_cast<unsigned char *>(ws);
     T *pong = reinterpret_cast<T *>(base);
     T *work = reinterpret_cast<T *>(base + bn);
-    T *states = reinterpret_cast<T *>(base + 2 * bn);
-    void *ews = base + 2 * bn + stb;
-    const size_t ews_bytes = ws_bytes - (2 * bn + stb);
-    if (n_steps > 1) {      // forward: u^1 .. u^{n_steps-1}
-        if (cudaMemcpyAsync(work, u0, (size_t)B * N * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
-            return BURGERS_ERR_CUDA;
-        st = explicit_call<T>(work, B, N, L, nu, dt, n_steps - 1, bc, BURGERS_SCHEME_EULER, BURGERS_PLAN_AUTO, 0, 0, ews,
-                              ews_bytes, stream, states, 1);
+    T *ckpt = reinterpret_cast<T *>(base + 2 * bn);
+    T *seg = reinterpret_cast<T *>(base + 2 * bn + ckb);
+    void *ews = base + 2 * bn + ckb + stb;
+    const size_t ews_bytes = ws_bytes - (2 * bn + ckb + stb);
+    const double dx = grid_dx(N, L, bc);
+    auto forward = [&](const T *from, int64_t steps, T *snaps, int64_t every) {
+        if (cudaMemcpyAsync(work, from, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+            return (int)BURGERS_ERR_CUDA;
+        return explicit_call<T>(work, B, N, L, nu, dt, steps, bc, BURGERS_SCHEME_EULER, BURGERS_PLAN_AUTO, 0, 0, ews,
+                                ews_bytes, stream, snaps, every);
+    };
+    if (K > 1) {            // checkpoints u^{m}, u^{2m}, ..., u^{(K-1)m}
+        st = forward(u0, (K - 1) * m, ckpt, m);
         if (st != BURGERS_OK) return st;
     }
-    return launch_adjoint_steps<T>(u0, states, lam, pong, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, s);
+    for (int64_t k = K - 1; k >= 0; --k) {
+        const T *start = (k == 0) ? u0 : ckpt + (size_t)(k - 1) * BN;
+        const int64_t len = (k == K - 1) ? n_steps - k * m : m;
+        if (len > 1) {      // states u^{km+1} .. u^{km+len-1} of this segment
+            st = forward(start, len - 1, seg, 1);
+            if (st != BURGERS_OK) return st;
+        }
+        st = launch_adjoint_steps<T>(start, seg, lam, pong, B, N, dx, nu, dt, len, bc, s);
+        if (st != BURGERS_OK) return st;
+    }
+    return BURGERS_OK;
 }
 
 // BTCS with trajectory output: one call of the plan per snapshot interval (the state is stored once
@@ -356,15 +392,30 @@ int burgers_explicit_adaptive_f64(double *u, int64_t B, int64_t N, double L, con
 
 int burgers_explicit_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
                                  const float *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
-    return adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+    return adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, 0, ws, ws_bytes, stream);
 }
 int burgers_explicit_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
                                  const double *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
-    return adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+    return adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, 0, ws, ws_bytes, stream);
+}
+int burgers_explicit_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                      const float *dt, int64_t n_steps, int bc, int64_t segment, void *ws,
+                                      size_t ws_bytes, void *stream) {
+    return adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream);
+}
+int burgers_explicit_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                      const double *dt, int64_t n_steps, int bc, int64_t segment, void *ws,
+                                      size_t ws_bytes, void *stream) {
+    return adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream);
+}
+size_t burgers_adjoint_ckpt_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps,
+                                            int64_t segment) {
+    if (B < 1 || N < 3 || n_steps < 0 || segment < 0) return 0;
+    return dtype_is_f64 ? adjoint_ws_bytes<double>(B, N, bc, n_steps, segment)
+                        : adjoint_ws_bytes<float>(B, N, bc, n_steps, segment);
 }
 size_t burgers_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
-    if (B < 1 || N < 3 || n_steps < 0) return 0;
-    return dtype_is_f64 ? adjoint_ws_bytes<double>(B, N, bc, n_steps) : adjoint_ws_bytes<float>(B, N, bc, n_steps);
+    return burgers_adjoint_ckpt_workspace_bytes(dtype_is_f64, B, N, bc, n_steps, 0);
 }
 
 int burgers_btcs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

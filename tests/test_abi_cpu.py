@@ -27,7 +27,7 @@ def _declared():
 
 def test_header_symbols_exported(B):
     names = _declared()
-    assert len(names) >= 36
+    assert len(names) >= 39
     lib = ctypes.CDLL(B.LIB_PATH)
     for n in names:
         assert hasattr(lib, n), f"{n} declared in burgers.h but not exported"
@@ -70,6 +70,10 @@ def test_argument_errors_are_synchronous(B):
     assert aj(one, None, 1, 8, 1.0, one, one, 3, 0, None, 0, None) == B.ERR_NULL
     assert aj(one, one, 1, 8, 1.0, one, one, 3, 0, None, 0, None) == B.ERR_WORKSPACE
     assert aj(one, one, 1, 8, 1.0, one, one, -3, 0, None, 0, None) == B.ERR_SHAPE
+    assert lib.burgers_explicit_adjoint_ckpt_f32(one, one, 1, 8, 1.0, one, one, 3, 0, -1, one, 1 << 20, None) == B.ERR_SHAPE
+    full = B.raw().burgers_adjoint_ckpt_workspace_bytes(1, 4, 100, 0, 100, 0)
+    ck = B.raw().burgers_adjoint_ckpt_workspace_bytes(1, 4, 100, 0, 100, 10)
+    assert full >= (2 + 99) * 4 * 100 * 8 and (2 + 9 + 9) * 4 * 100 * 8 <= ck < full // 3
     lib.burgers_adjoint_workspace_bytes.restype = ctypes.c_size_t
     assert lib.burgers_adjoint_workspace_bytes(1, 4, 100, 0, 11) >= (2 + 10) * 4 * 100 * 8
     ad = lib.burgers_explicit_adaptive_f64

@@ -65,3 +65,27 @@ def test_zero_and_one_step(B):
     lam = to_dev(lam_T.copy()); B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 1, w.bc)
     ref = oracle.explicit_adjoint(w.u0, lam_T, w.L, w.nu, dt, 1, w.bc)
     np.testing.assert_allclose(lam.cpu().numpy(), ref, atol=1e-14)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-10), (np.float32, 1e-4)])
+def test_checkpointed_adjoint(B, dtype, tol):
+    """Segments of 1, 7, 16 and 100 steps (ragged last segment, single-step segments, one segment) give the
+    gradient of the un-checkpointed run: bitwise in fp64 (the recomputed states are the same numbers)."""
+    rng = np.random.default_rng(10)
+    w = W.c3_periodic_btcs(B=4, N=256, n_steps=0, dtype=dtype)
+    n = 45
+    dt = oracle_dt(w.u0, w.L, w.nu, 0.4, w.bc, dtype)
+    lam_T = rng.standard_normal(w.u0.shape).astype(dtype)
+    ref = oracle.explicit_adjoint(w.u0.astype(np.float64), lam_T.astype(np.float64), w.L, w.nu.astype(np.float64),
+                                  dt.astype(np.float64), n, w.bc)
+    scale = np.abs(ref).max(axis=1, keepdims=True)
+    full = None
+    for segment in (0, 1, 7, 16, 100):
+        lam = to_dev(lam_T.copy())
+        B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, segment=segment)
+        got = lam.cpu().numpy()
+        assert (np.abs(got.astype(np.float64) - ref) / scale).max() <= tol, segment
+        if full is None:
+            full = got
+        elif dtype == np.float64:
+            np.testing.assert_array_equal(got, full)

@@ -160,3 +160,27 @@ def test_c4b_full_windows_and_residual(B):
         err = np.abs(got[0, idx[cc]] - ref[cc]).max() / np.abs(w.u0).max()
         assert err <= 1e-10, (start, err)
     _max_principle(got, w.u0, 1e-12)
+
+
+def test_c2_full_adjoint_checkpointed(B):
+    """Reverse-mode derivative of the whole C2 fp32 run (1024 trajectories, 10 000 Euler steps): 168 GB of
+    forward states, so the call checkpoints (100 segments of 100 steps, 3.3 GB).  Sampled trajectories
+    against the oracle's adjoint, which stores every state."""
+    w = W.c2_dirichlet_batch(dtype=np.float32)
+    u0, nu = to_dev(w.u0), to_dev(w.nu)
+    dt = B.dt_from_cfl(u0, w.L, nu, w.cfl, w.bc)
+    rng = np.random.default_rng(77)
+    lam_T = rng.standard_normal(w.u0.shape).astype(np.float32)
+    lam = to_dev(lam_T.copy())
+    need = B.raw().burgers_adjoint_workspace_bytes(0, w.B, w.N, w.bc, w.n_steps)
+    assert need < 6 << 30                                   # checkpointed: far below the 168 GB of all states
+    B.burgers_explicit_adjoint(u0, lam, w.L, nu, dt, w.n_steps, w.bc)
+    got = lam.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(got))
+    np.testing.assert_array_equal(u0.cpu().numpy(), w.u0)
+    rows = np.array([0, 313, 700, w.B - 1])
+    dth = dt.cpu().numpy().astype(np.float64)
+    ref = oracle.explicit_adjoint(w.u0[rows].astype(np.float64), lam_T[rows].astype(np.float64), w.L,
+                                  w.nu[rows].astype(np.float64), dth[rows], w.n_steps, w.bc)
+    scale = np.abs(ref).max(axis=1, keepdims=True)
+    assert (np.abs(got[rows] - ref) / scale).max() <= 1e-4
