@@ -160,6 +160,14 @@ def cpu_info():
     return model
 
 
+def metric_name(spec):
+    base = "grid-point updates/s (B*N*steps/s), "
+    if spec["op"] == "explicit":
+        return base + ("forward Euler upwind/central" if spec["scheme"] == 0 else "RK4")
+    return base + {"btcs": "BTCS", "newton": "Newton BTCS (central convection, theta-scheme)",
+                   "gs": "Gauss-Seidel BTCS", "adjoint": "adjoint of forward Euler"}[spec["op"]]
+
+
 # ------------------------------------------------------------------------------- oracle leg
 def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
     """Times the CPU oracle (as it stands) on a bounded sample of workload `w`: whole trajectories
@@ -178,6 +186,9 @@ def oracle_sample_run(w, spec, target_s=12.0, budget_updates=None):
         elif spec["op"] == "gs":
             oracle.btcs_gs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"], max_iter=spec["max_iter"],
                            threads=threads)
+        elif spec["op"] == "adjoint":
+            lam = np.random.default_rng(1220404).standard_normal(u0[rows].shape)
+            oracle.explicit_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
         elif spec["op"] == "newton":
             oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
                                max_iter=spec["max_iter"], threads=threads, theta=spec["theta"])
@@ -395,10 +406,7 @@ def run_ours(args):
     total_updates = w.updates * world
     value = total_updates / (ms * 1e-3)
     out = {
-        "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
-        else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else
-              ("grid-point updates/s (B*N*steps/s), Newton BTCS" if spec["op"] == "newton" else
-               ("grid-point updates/s (B*N*steps/s), Gauss-Seidel BTCS" if spec["op"] == "gs" else "grid-point updates/s (B*N*steps/s), BTCS"))),
+        "metric": metric_name(spec),
         "value": value, "unit": "updates/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if w.dtype == np.float32 else "f64", "data": "synthetic",
@@ -490,8 +498,7 @@ def run_reference(args):
     upd = sum(v[0] for v in vals); sec = sum(v[1] for v in vals)
     value = upd / sec
     out = {"impl": "reference",
-           "metric": "grid-point updates/s (B*N*steps/s), forward Euler upwind/central" if spec["scheme"] == 0
-           else ("grid-point updates/s (B*N*steps/s), RK4" if spec["scheme"] == 1 else "grid-point updates/s (B*N*steps/s), BTCS"),
+           "metric": metric_name(spec),
            "value": value, "unit": "updates/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": sec / max(1, len(vals)) * 1e3, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
