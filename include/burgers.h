@@ -91,8 +91,10 @@ enum {
  * g_i = u_i - u_{i-1} if u_i > 0 else u_{i+1} - u_i.
  * dt[b] is held fixed over the call.  RK4: the upwind direction is re-decided from
  * each stage value; Dirichlet end nodes have k = 0 in every stage.
- * fp32: the state is carried as a two-term sum on chip (compensated
- * accumulation), rounded to fp32 once when written back. */
+ * fp32: on chip the state is carried scaled by dt/dx and (Euler) as a two-term sum
+ * (compensated accumulation); it is unscaled and rounded to fp32 once
+ * when written back, so p then q steps agree with p+q steps to rounding, not bitwise
+ * (fp64 is bitwise).  dt[b] = 0 leaves trajectory b untouched; dt[b] < 0 is not supported. */
 int burgers_explicit_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
                          const float *dt, int64_t n_steps, int bc, int scheme,
                          void *ws, size_t ws_bytes, void *stream);
