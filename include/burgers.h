@@ -201,7 +201,9 @@ int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const doubl
  * The system of burgers_btcs_* solved per step by lexicographic Gauss-Seidel sweeps from x = u^n until
  * max_i |rhs_i - (A x)_i| < tol or max_iter sweeps were done (D12) -- the paper's iterative
  * variant, kept for its iteration counts and for comparison; the direct solvers are exact and cheaper.
- * One thread per system; needs workspace (burgers_workspace_bytes(BURGERS_OP_GS, ...)).
+ * 64 <= N <= 4096: one CTA per system, the sweep evaluated as a scan of the affine maps x_i = p_i + q_i x_{i-1}
+ * (the sequential sweep up to rounding order), no workspace; other N: one thread per system, needs workspace.
+ * burgers_workspace_bytes(BURGERS_OP_GS, ...) says which (0 = none; ws may then be NULL).
  * iters_out: DEVICE pointer to B int64 (sweeps summed over the steps), or NULL. */
 int burgers_btcs_gs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                         int64_t n_steps, int bc, double tol, int max_iter, int64_t *iters_out,

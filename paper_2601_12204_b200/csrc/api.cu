@@ -222,7 +222,7 @@ int gs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int6
     if (st != BURGERS_OK) return st;
     if (!(tol >= 0.0) || max_iter < 0) return BURGERS_ERR_VALUE;
     const size_t need = btcs_gs_ws_elems(B, N) * sizeof(T);
-    if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
+    if (need && (!ws || ws_bytes < need)) return BURGERS_ERR_WORKSPACE;
     return launch_btcs_gs<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, tol, max_iter,
                              reinterpret_cast<long long *>(iters_out), (T *)ws, (cudaStream_t)stream);
 }

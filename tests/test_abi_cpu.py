@@ -85,7 +85,9 @@ def test_argument_errors_are_synchronous(B):
     assert gs(one, 1, 8, 1.0, one, None, 1, 0, 1e-6, 10, None, one, 1 << 20, None) == B.ERR_NULL
     assert gs(one, 1, 8, 1.0, one, one, 1, 0, -1e-6, 10, None, one, 1 << 20, None) == B.ERR_VALUE
     assert gs(one, 1, 8, 1.0, one, one, 1, 0, 1e-6, 10, None, None, 0, None) == B.ERR_WORKSPACE
-    assert B.workspace_bytes(B.OP_GS, True, 4, 100, 0) >= 2 * 4 * 100 * 8
+    assert B.workspace_bytes(B.OP_GS, True, 4, 100, 0) == 0                       # CTA per system: no scratch
+    assert B.workspace_bytes(B.OP_GS, True, 4, 40, 0) >= 2 * 4 * 40 * 8           # thread per system
+    assert B.workspace_bytes(B.OP_GS, True, 4, 5000, 0) >= 2 * 4 * 5000 * 8
     bt = lib.burgers_btcs_traj_f64
     assert bt(one, 1, 8, 1.0, one, one, 4, 0, 2, None, None, 0, None) == B.ERR_NULL
     assert bt(one, 1, 8, 1.0, one, one, 4, 0, 0, one, None, 0, None) == B.ERR_SHAPE

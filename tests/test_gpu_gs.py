@@ -61,3 +61,26 @@ def test_paper_setting_sweeps_per_step(B):
     dt = oracle.dt_from_cfl(u0, L, np.array([nu]), 0.4, 0)
     _, it = run(B, u0, L, np.array([nu]), dt, 100, 0, tol=1e-6)
     assert 5.5 <= it[0] / 100 <= 7.5          # "5-7 iterations per step"
+
+
+@pytest.mark.parametrize("N,bc_name", [(64, "p"), (1000, "p"), (1024, "d"), (1025, "p"), (2048, "p"), (2047, "d"),
+                                       (2049, "d"), (4096, "p"), (4095, "d"), (63, "p"), (4097, "p")])
+def test_cta_plan_shapes(B, N, bc_name):
+    """Every branch of the plan choice (CTA per system with 4 or 8 rows per thread and 1..16 warps, ragged
+    last threads, and the thread-per-system plan on both sides of its range) against the oracle."""
+    if bc_name == "p":
+        w = W.c3_periodic_btcs(B=3, N=N, n_steps=0)
+    else:
+        w = W.c2_dirichlet_batch(B=3, N=N, dtype=np.float64)
+    n = 6
+    dt = oracle.dt_from_cfl(w.u0, w.L, w.nu, 0.4, w.bc)
+    ref, it_ref = oracle.btcs_gs(w.u0, w.L, w.nu, dt, n, w.bc, tol=1e-9, return_iters=True)
+    got, it = run(B, w.u0, w.L, w.nu, dt, n, w.bc, tol=1e-9)
+    assert rel_err(got, ref, w.u0) <= 1e-10, (N, bc_name)
+    assert np.all(np.abs(it - it_ref) <= n), (it, it_ref)
+    assert it.min() >= n                                   # at least one sweep per step at this tolerance
+    # max_iter caps the sweeps of every step
+    got2, it2 = run(B, w.u0, w.L, w.nu, dt, n, w.bc, tol=0.0, max_iter=3)
+    ref2 = oracle.btcs_gs(w.u0, w.L, w.nu, dt, n, w.bc, tol=0.0, max_iter=3)
+    assert np.all(it2 == 3 * n)
+    assert rel_err(got2, ref2, w.u0) <= 1e-10
