@@ -264,6 +264,16 @@ int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const f
                          double C, int bc, float *dt_out);
 int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L,
                          const double *nu, double C, int bc, double *dt_out);
+/* The whole hot path of SURVEY.md 8(a) on HOST buffers in one call: u and nu are uploaded once,
+ * dt = dt_from_cfl(u0, C) is computed on the device and used for all n_steps
+ * of op = BURGERS_OP_EXPLICIT (`scheme` = BURGERS_SCHEME_*) or BURGERS_OP_BTCS (`scheme` ignored), AUTO
+ * plan; u is overwritten with the result; dt_out (B values, may be NULL) receives the step used.
+ * Same kernels, hence bitwise the same result, as dt_from_cfl_host_* followed by burgers_*_host_*, with
+ * one upload of the state instead of two.  Errors as for the separate calls. */
+int burgers_solve_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C,
+                           int64_t n_steps, int bc, int op, int scheme, float *dt_out);
+int burgers_solve_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, double C,
+                           int64_t n_steps, int bc, int op, int scheme, double *dt_out);
 
 /* ---- queries (pure functions of the shape; no device work) -------------------- */
 /* Scratch bytes needed by op (BURGERS_OP_*) with `plan` (BURGERS_PLAN_AUTO allowed).

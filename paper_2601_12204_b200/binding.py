@@ -33,7 +33,8 @@ EXPORTS = [
     "burgers_adjoint_ckpt_workspace_bytes", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
     "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
-    "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
+    "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64",
+    "burgers_solve_host_f32", "burgers_solve_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
     "burgers_launch_count", "burgers_strerror", "burgers_version",
 ]
 
@@ -70,6 +71,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_explicit_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int]
     getattr(_lib, f"burgers_btcs_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int]
     getattr(_lib, f"dt_from_cfl_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p]
+    getattr(_lib, f"burgers_solve_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _i64, _int, _int, _int, _p]
+    getattr(_lib, f"burgers_solve_host_{_sfx}").restype = _int
     for _n in ("burgers_explicit_", "burgers_explicit_plan_", "burgers_btcs_", "burgers_btcs_plan_",
                "dt_from_cfl_", "burgers_explicit_host_", "burgers_btcs_host_", "dt_from_cfl_host_"):
         getattr(_lib, _n + _sfx).restype = _int
@@ -391,6 +394,19 @@ def burgers_btcs_host(u, L, nu, dt, n_steps, bc):
                                                    dt.ctypes.data, int(n_steps), int(bc))
     _check(st, f"burgers_btcs_host_{sfx}")
     return u
+
+
+def burgers_solve_host(u, L, nu, C, n_steps, bc, op=OP_EXPLICIT, scheme=0, return_dt=False):
+    """The whole hot path on host buffers in one call (include/burgers.h: burgers_solve_host_*): dt from the
+    CFL number C on the device, then n_steps of the explicit scheme or of BTCS; u is updated in place."""
+    _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype)
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    dt = np.empty(B, dtype=u.dtype) if return_dt else None
+    st = getattr(_lib, f"burgers_solve_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, float(C),
+                                                    int(n_steps), int(bc), int(op), int(scheme),
+                                                    dt.ctypes.data if return_dt else None)
+    _check(st, f"burgers_solve_host_{sfx}")
+    return (u, dt) if return_dt else u
 
 
 def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return_iters=False, theta=1.0):

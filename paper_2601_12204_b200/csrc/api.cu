@@ -339,6 +339,36 @@ int cfl_host(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, 
     return cuda_status(cudaStreamSynchronize(s));
 }
 
+// The whole hot path on host buffers with ONE upload of the state: dt_from_cfl on the device, the
+// time-stepping call with that dt, one download (8(a): CFL step + time stepping).
+template <typename T>
+int solve_host(T *u, int64_t B, int64_t N, double L, const T *nu, double C, int64_t n_steps, int bc, int op,
+               int scheme, T *dt_out) {
+    int st = check_common(u, nu, u, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (op != BURGERS_OP_EXPLICIT && op != BURGERS_OP_BTCS) return BURGERS_ERR_ENUM;
+    if (op == BURGERS_OP_EXPLICIT && !scheme_ok(scheme)) return BURGERS_ERR_ENUM;
+    if (!(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
+    const size_t wsb = burgers_workspace_bytes(op, sizeof(T) == 8, B, N, bc, scheme, BURGERS_PLAN_AUTO);
+    const size_t ub = (size_t)B * (size_t)N * sizeof(T), vb = (size_t)B * sizeof(T);
+    DevBuf du, dnu, ddt, dws;
+    if (!du.alloc(ub) || !dnu.alloc(vb) || !ddt.alloc(vb) || !dws.alloc(wsb)) return BURGERS_ERR_CUDA;
+    cudaStream_t s = nullptr;
+    if (cudaMemcpyAsync(du.p, u, ub, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    if (cudaMemcpyAsync(dnu.p, nu, vb, cudaMemcpyHostToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    st = cfl_call<T>((const T *)du.p, B, N, L, (const T *)dnu.p, C, bc, (T *)ddt.p, nullptr);
+    if (st == BURGERS_OK)
+        st = (op == BURGERS_OP_EXPLICIT)
+                 ? explicit_call<T>((T *)du.p, B, N, L, (const T *)dnu.p, (const T *)ddt.p, n_steps, bc, scheme,
+                                    BURGERS_PLAN_AUTO, 0, 0, dws.p, wsb, nullptr)
+                 : btcs_call<T>((T *)du.p, B, N, L, (const T *)dnu.p, (const T *)ddt.p, n_steps, bc,
+                                BURGERS_PLAN_AUTO, dws.p, wsb, nullptr);
+    if (st != BURGERS_OK) { cudaStreamSynchronize(s); return st; }
+    if (cudaMemcpyAsync(u, du.p, ub, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    if (dt_out && cudaMemcpyAsync(dt_out, ddt.p, vb, cudaMemcpyDeviceToHost, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    return cuda_status(cudaStreamSynchronize(s));
+}
+
 }  // namespace
 
 extern "C" {
@@ -500,6 +530,14 @@ int burgers_newton_host_f32(float *u, int64_t B, int64_t N, double L, const floa
 int burgers_newton_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
                             int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out) {
     return newton_host<double>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out);
+}
+int burgers_solve_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C, int64_t n_steps,
+                           int bc, int op, int scheme, float *dt_out) {
+    return solve_host<float>(u, B, N, L, nu, C, n_steps, bc, op, scheme, dt_out);
+}
+int burgers_solve_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, double C, int64_t n_steps,
+                           int bc, int op, int scheme, double *dt_out) {
+    return solve_host<double>(u, B, N, L, nu, C, n_steps, bc, op, scheme, dt_out);
 }
 int dt_from_cfl_host_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C,
                          int bc, float *dt_out) {

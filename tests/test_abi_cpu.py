@@ -81,6 +81,12 @@ def test_argument_errors_are_synchronous(B):
     assert ad(one, 1, 8, 1.0, one, 0.4, 3, 0, 0, 0, one, None, None, 0, None) == B.ERR_SHAPE
     assert ad(one, 1, 8, 1.0, one, -0.4, 3, 5, 0, 0, one, None, None, 0, None) == B.ERR_VALUE
     assert ad(one, 1, 8, 1.0, one, 0.4, 3, 5, 0, 9, one, None, None, 0, None) == B.ERR_ENUM
+    sh = lib.burgers_solve_host_f64
+    assert sh(one, 1, 8, 1.0, None, 0.4, 1, 0, B.OP_EXPLICIT, 0, None) == B.ERR_NULL
+    assert sh(one, 1, 8, 1.0, one, 0.4, 1, 0, B.OP_NEWTON, 0, None) == B.ERR_ENUM
+    assert sh(one, 1, 8, 1.0, one, 0.4, 1, 0, B.OP_EXPLICIT, 5, None) == B.ERR_ENUM
+    assert sh(one, 1, 8, 1.0, one, -0.4, 1, 0, B.OP_BTCS, 0, None) == B.ERR_VALUE
+    assert sh(one, 1, 2, 1.0, one, 0.4, 1, 0, B.OP_BTCS, 0, None) == B.ERR_SHAPE
     gs = lib.burgers_btcs_gs_f64
     assert gs(one, 1, 8, 1.0, one, None, 1, 0, 1e-6, 10, None, one, 1 << 20, None) == B.ERR_NULL
     assert gs(one, 1, 8, 1.0, one, one, 1, 0, -1e-6, 10, None, one, 1 << 20, None) == B.ERR_VALUE

@@ -321,6 +321,32 @@ def test_host_entry_points_match_device_path(B):
     np.testing.assert_array_equal(uh, run_btcs(B, w3.u0, w3.L, w3.nu, dt3, 10, w3.bc))
 
 
+def test_solve_host_is_the_two_calls_in_one(B):
+    """burgers_solve_host_*: one upload, CFL + time stepping on the device.  Bitwise the two-call host path
+    (same kernels), and within the parity bar of the oracle run on the oracle's own dt."""
+    w = W.c2_dirichlet_batch(B=6, N=2048, dtype=np.float32)
+    for scheme, osch, cfl in ((B.SCHEME_EULER, oracle.EULER, 0.4), (B.SCHEME_RK4, oracle.RK4, 0.5)):
+        u1, dt1 = B.burgers_solve_host(w.u0.copy(), w.L, w.nu, cfl, 150, w.bc, op=B.OP_EXPLICIT, scheme=scheme,
+                                       return_dt=True)
+        dt_h = B.dt_from_cfl_host(w.u0, w.L, w.nu, cfl, w.bc)
+        np.testing.assert_array_equal(dt1, dt_h)
+        u2 = B.burgers_explicit_host(w.u0.copy(), w.L, w.nu, dt_h, 150, w.bc, scheme)
+        np.testing.assert_array_equal(u1, u2)
+        ref = oracle.explicit(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64), dt1.astype(np.float64), 150,
+                              w.bc, osch)
+        assert rel_err(u1, ref, w.u0) <= TOL[np.dtype(np.float32)]
+    w3 = W.c3_periodic_btcs(B=5, N=256, n_steps=10)
+    u1, dt1 = B.burgers_solve_host(w3.u0.copy(), w3.L, w3.nu, 10.0, 10, w3.bc, op=B.OP_BTCS, return_dt=True)
+    ref_dt = oracle.dt_from_cfl(w3.u0, w3.L, w3.nu, 10.0, w3.bc)
+    assert np.all(np.abs(dt1 - ref_dt) <= 2 * np.spacing(ref_dt))
+    assert rel_err(u1, oracle.btcs(w3.u0, w3.L, w3.nu, dt1, 10, w3.bc), w3.u0) <= 1e-10
+    u2 = B.burgers_btcs_host(w3.u0.copy(), w3.L, w3.nu, dt1, 10, w3.bc)
+    np.testing.assert_array_equal(u1, u2)
+    assert B.burgers_solve_host(w3.u0.copy(), w3.L, w3.nu, 10.0, 0, w3.bc, op=B.OP_BTCS).tolist() == w3.u0.tolist()
+    with pytest.raises(Exception):
+        B.burgers_solve_host(w3.u0.copy(), w3.L, w3.nu, 10.0, 1, w3.bc, op=B.OP_NEWTON)
+
+
 def test_library_is_loaded_in_this_process(B):
     maps = open("/proc/self/maps").read()
     assert "libburgers.so" in maps
