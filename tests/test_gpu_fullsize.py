@@ -12,6 +12,8 @@ by one, exactly:
     per step (Green's function of the diffusion part; convection only strengthens the diagonal):
     at r = 5, lam = 0.642, i.e. < 1e-12 beyond 63 cells per step, so a margin of 64*n_steps cells
     makes the window's centre exact to far below the 1e-10 tolerance;
+the rows of SURVEY 8(f) that bench.py times (Newton / Crank-Nicolson and Gauss-Seidel on C3's inputs, C2 with
+trajectory output, the checkpointed adjoint of the whole C2 run) are checked the same way at the end of the file;
 plus properties that hold at any size, checked on ALL outputs: finiteness, the discrete maximum
 principle (D4 / D9), frozen Dirichlet ends, and for BTCS the defining residual
 A(u^n) u^{n+1} = u^n of the last step evaluated in fp64 numpy over the whole grid.
@@ -184,3 +186,71 @@ def test_c2_full_adjoint_checkpointed(B):
                                   w.nu[rows].astype(np.float64), dth[rows], w.n_steps, w.bc)
     scale = np.abs(ref).max(axis=1, keepdims=True)
     assert (np.abs(got[rows] - ref) / scale).max() <= 1e-4
+
+
+# ---- the §8(f) rows at the sizes and settings bench.py times (`schemes`: c3_newton, c3_cn, c3_gs, c2_traj) ----
+
+def _c3_inputs(B, cfl):
+    import torch
+    w = W.c3_periodic_btcs()                                       # B=4096, N=2048
+    u, nu = to_dev(w.u0.copy()), to_dev(w.nu)
+    dt = B.dt_from_cfl(u, w.L, nu, cfl, w.bc)
+    it = torch.zeros(w.B, dtype=torch.int64, device="cuda")
+    rows = np.sort(np.random.default_rng(5).choice(w.B, 12, replace=False))
+    rows[0], rows[-1] = 0, w.B - 1
+    return w, u, nu, dt, it, rows
+
+
+@pytest.mark.parametrize("theta", [1.0, 0.5])
+def test_c3_full_newton_and_crank_nicolson(B, theta):
+    """bench.py's c3_newton / c3_cn: 1 000 steps, tol 1e-6.  Newton converges quadratically, so an iterate
+    accepted at residual < 1e-6 is the converged one to ~1e-12 and a stopping decision taken differently at a
+    tie cannot move the result above the bar; the iteration totals may differ by such ties only."""
+    w, u, nu, dt, it, rows = _c3_inputs(B, W.c3_periodic_btcs().cfl)
+    B.burgers_newton(u, w.L, nu, dt, w.n_steps, w.bc, tol=1e-6, max_iter=50, iters_out=it, theta=theta)
+    got, dth, itg = u.cpu().numpy(), dt.cpu().numpy(), it.cpu().numpy()
+    ref, it_ref = oracle.newton_btcs(w.u0[rows], w.L, w.nu[rows], dth[rows], w.n_steps, w.bc, tol=1e-6, max_iter=50,
+                                     return_iters=True, theta=theta)
+    assert rel_err(got[rows], ref, w.u0[rows]) <= 1e-9
+    assert np.all(np.abs(itg[rows] - it_ref) <= 0.01 * it_ref)
+    assert np.all(np.isfinite(got)) and itg.min() >= w.n_steps and itg.max() <= 4 * w.n_steps
+
+
+def test_c3_full_gauss_seidel(B):
+    """bench.py's c3_gs: C = 0.4, 100 steps, tol 1e-6 (the CTA-per-system plan at N = 2048)."""
+    w, u, nu, dt, it, rows = _c3_inputs(B, 0.4)
+    n = 100
+    B.burgers_btcs_gs(u, w.L, nu, dt, n, w.bc, tol=1e-6, max_iter=1000, iters_out=it)
+    got, dth, itg = u.cpu().numpy(), dt.cpu().numpy(), it.cpu().numpy()
+    ref, it_ref = oracle.btcs_gs(w.u0[rows], w.L, w.nu[rows], dth[rows], n, w.bc, tol=1e-6, max_iter=1000,
+                                 return_iters=True)
+    np.testing.assert_array_equal(itg[rows], it_ref)              # same sweeps: iterates agree to rounding
+    assert rel_err(got[rows], ref, w.u0[rows]) <= 1e-10
+    direct = oracle.btcs(w.u0[rows], w.L, w.nu[rows], dth[rows], n, w.bc)
+    assert rel_err(got[rows], direct, w.u0[rows]) <= 10 * n * 1e-6
+    _max_principle(got, w.u0, 1e-12)                               # every sweep is a convex combination (M-matrix)
+    assert 3.0 <= itg.mean() / n <= 8.0
+
+
+def test_c2_full_trajectory_snapshots(B):
+    """bench.py's c2_traj: C2 fp32, a snapshot of all 1024 trajectories every 50 steps (200 snapshots, 3.4 GB)."""
+    import torch
+    w = W.c2_dirichlet_batch(dtype=np.float32)
+    u, nu = to_dev(w.u0.copy()), to_dev(w.nu)
+    dt = B.dt_from_cfl(u, w.L, nu, w.cfl, w.bc)
+    _, snaps = B.burgers_explicit_traj(u, w.L, nu, dt, w.n_steps, w.bc, B.SCHEME_EULER, 50)
+    assert tuple(snaps.shape) == (200, w.B, w.N)
+    rows = np.array([0, 411, w.B - 1])
+    dth = dt.cpu().numpy().astype(np.float64)
+    ref_u, ref_snaps = oracle.explicit_trajectory(w.u0[rows].astype(np.float64), w.L, w.nu[rows].astype(np.float64),
+                                                  dth[rows], w.n_steps, w.bc, oracle.EULER, 50)
+    got = snaps[:, torch.as_tensor(rows, device="cuda"), :].cpu().numpy()
+    assert got.shape == ref_snaps.shape
+    scale = np.abs(w.u0[rows]).max()
+    assert np.abs(got - ref_snaps).max() / scale <= 1e-4
+    assert rel_err(u.cpu().numpy()[rows], ref_u, w.u0[rows]) <= 1e-4
+    # the last snapshot is the final state up to the rounding of the unscaling (snapshots: reciprocal + one
+    # correction, final state: exact quotient; burgers.h); the frozen Dirichlet ends are in every snapshot, bit-exact
+    assert (snaps[-1] - u).abs().max().item() <= 2.4e-7 * float(scale)
+    assert torch.equal(snaps[:, :, 0], to_dev(w.u0[:, 0]).expand(200, -1))
+    assert torch.equal(snaps[:, :, -1], to_dev(w.u0[:, -1]).expand(200, -1))
