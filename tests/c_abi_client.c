@@ -1,0 +1,23 @@
+/* A plain C99 consumer of include/burgers.h (compiled and run by tests/test_abi_cpu.py): the header must be
+ * valid C, the library must link without any C++ or torch symbol on the caller's side, and argument errors
+ * must come back as status codes before any device work (so this runs on a box without a GPU). */
+#include <stdio.h>
+#include <string.h>
+
+#include "burgers.h"
+
+int main(void) {
+    double u[8] = {0}, nu[1] = {0.1}, dt[1] = {0.1};
+    float uf[8] = {0}, nuf[1] = {0.1f};
+    int bad = 0;
+    bad += burgers_explicit_f64(u, 1, 8, -1.0, nu, dt, 1, BURGERS_BC_PERIODIC, BURGERS_SCHEME_EULER, NULL, 0, NULL) != BURGERS_ERR_VALUE;
+    bad += burgers_btcs_f64(NULL, 1, 8, 1.0, nu, dt, 1, BURGERS_BC_PERIODIC, NULL, 0, NULL) != BURGERS_ERR_NULL;
+    bad += burgers_btcs_f64(u, 1, 2, 1.0, nu, dt, 1, BURGERS_BC_PERIODIC, NULL, 0, NULL) != BURGERS_ERR_SHAPE;
+    bad += dt_from_cfl_f32(uf, 1, 8, 1.0, nuf, 0.4, 7, nuf, NULL) != BURGERS_ERR_ENUM;
+    bad += burgers_solve_host_f32(uf, 1, 8, 1.0, nuf, 0.4, 1, BURGERS_BC_DIRICHLET, BURGERS_OP_CFL, 0, NULL) != BURGERS_ERR_ENUM;
+    bad += burgers_workspace_bytes(BURGERS_OP_BTCS, 1, 1, (int64_t)1 << 22, BURGERS_BC_PERIODIC, 0, BURGERS_PLAN_AUTO) == 0;
+    bad += burgers_plan_query(BURGERS_OP_BTCS, 1, 4096, 2048, BURGERS_BC_PERIODIC, 0) != BURGERS_PLAN_HYBRID;
+    bad += strlen(burgers_strerror(BURGERS_ERR_WORKSPACE)) == 0;
+    printf("version %d bad %d\n", burgers_version(), bad);
+    return bad;
+}

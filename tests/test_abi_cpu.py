@@ -184,3 +184,18 @@ def test_product_does_not_import_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", txt, flags=re.M), f
                 assert "burgers_oracle" not in txt and "liboracle" not in txt, f
+
+
+def test_plain_c_client_compiles_links_and_runs(tmp_path):
+    """include/burgers.h is valid C99 (-pedantic -Werror) and a C program needs nothing but the header and
+    libburgers.so; argument errors are status codes, returned before any device work."""
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    libdir = os.path.join(root, "paper_2601_12204_b200")
+    exe = str(tmp_path / "c_abi_client")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(root, "include"),
+                    os.path.join(root, "tests", "c_abi_client.c"), "-o", exe, "-L", libdir, "-lburgers",
+                    "-Wl,-rpath," + libdir], check=True)
+    r = subprocess.run([exe], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.startswith("version ") and r.stdout.strip().endswith("bad 0")
