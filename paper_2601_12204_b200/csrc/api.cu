@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/burgers.h: argument validation, plan selection, dispatch,
 // and the host-buffer (end-to-end) variants.  No arithmetic of the method lives here.
 #include <cmath>
+#include <cstdint>
 
 #include "common.cuh"
 
@@ -101,6 +102,16 @@ int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, i
     if (!(C > 0.0) || !std::isfinite(C)) return BURGERS_ERR_VALUE;
     cudaStream_t s = (cudaStream_t)stream;
     if (t_out && cudaMemsetAsync(t_out, 0, (size_t)B * sizeof(double), s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    // RESIDENT plan: one launch, the CFL evaluation fused into the time loop of the kernel
+    ExplicitGeom g;
+    st = explicit_geometry(sizeof(T) == 8, B, N, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, &g);
+    if (st != BURGERS_OK) return st;
+    if (g.plan == BURGERS_PLAN_RESIDENT && n_outer <= INT64_MAX / m_steps) {
+        if (n_outer == 0) return BURGERS_OK;
+        const ExplicitAdapt<T> ad{m_steps, C, t_out, dt_scratch};
+        return launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt_scratch, n_outer * m_steps, bc, scheme, g, (T *)ws,
+                                  nullptr, 0, s, &ad);
+    }
     for (int64_t k = 0; k < n_outer; ++k) {
         st = cfl_call<T>(u, B, N, L, nu, C, bc, dt_scratch, stream);
         if (st != BURGERS_OK) return st;

@@ -28,15 +28,6 @@ template <typename T> __device__ __forceinline__ T absmax(T m, T x) { return fma
 template <> __device__ __forceinline__ float absmax<float>(float m, float x) { return fmaxf(m, fabsf(x)); }
 
 template <typename T>
-__device__ __forceinline__ T cfl_dt(T m, T nu, double dx, double C) {
-    // evaluated in fp64 on the (already T-rounded) inputs, rounded to T once
-    const double inf = __longlong_as_double(0x7ff0000000000000LL);
-    double conv = (m > T(0)) ? dx / (double)m : inf;
-    double diff = ((double)nu > 0.0) ? dx * dx / (2.0 * (double)nu) : inf;
-    return (T)(C * ((conv < diff) ? conv : diff));
-}
-
-template <typename T>
 __global__ void __launch_bounds__(kCflThreads)
 cfl_reduce_kernel(const T *__restrict__ u, const T *__restrict__ nu, T *__restrict__ dt_out,
                   int64_t N, int chunks, double dx, double C) {

@@ -26,6 +26,17 @@ int launch_cfl(const T *u, int64_t B, int64_t N, double dx, const T *nu, double 
 int64_t cfl_launch_count(int is_f64, int64_t B, int64_t N);
 
 // ---------------------------------------------------------------- explicit (explicit_*.cu)
+// dt from the CFL condition (D8) for one trajectory whose max |u| is m: evaluated in
+// fp64 on the (already T-rounded) inputs, rounded to T once.  x/0 = +inf.  Shared by cfl.cu and the adaptive
+// explicit kernel so that both give the same bits.
+template <typename T>
+__device__ __forceinline__ T cfl_dt(T m, T nu, double dx, double C) {
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    double conv = (m > T(0)) ? dx / (double)m : inf;
+    double diff = ((double)nu > 0.0) ? dx * dx / (2.0 * (double)nu) : inf;
+    return (T)(C * ((conv < diff) ? conv : diff));
+}
+
 // Geometry of one explicit launch plan, decided on the host (explicit_plan.cu).
 struct ExplicitGeom {
     int plan;        // BURGERS_PLAN_RESIDENT / BURGERS_PLAN_TILED
@@ -41,10 +52,19 @@ struct ExplicitGeom {
 // (tblock/ppt = 0 -> defaults).  Returns BURGERS_OK or BURGERS_ERR_PLAN.
 int explicit_geometry(int is_f64, int64_t B, int64_t N, int bc, int scheme, int plan, int tblock,
                       int ppt, ExplicitGeom *g);
+// Adaptive time step fused into the RESIDENT kernel (SURVEY 8(f) NEXT-4a): dt is re-evaluated from the
+// CFL condition every `every` steps inside the kernel; `dt` of launch_explicit is then not read.
+template <typename T>
+struct ExplicitAdapt {
+    int64_t every;   // m: steps per CFL evaluation (>= 1)
+    double C;        // CFL number
+    double *t_out;   // [B] simulated time, sum of m*dt (may be nullptr)
+    T *dt_out;       // [B] the last dt used
+};
 template <typename T>
 int launch_explicit(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                     int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                    T *snaps, int64_t snap_every, cudaStream_t s);
+                    T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt = nullptr);
 // max threads per CTA the explicit kernel <T,P,scheme> may be launched with (register limit)
 int explicit_max_threads(int is_f64, int P, int scheme);
 

@@ -6,7 +6,8 @@ template <>
 int launch_explicit<double>(double *u, int64_t B, int64_t N, double dx, const double *nu,
                             const double *dt, int64_t n_steps, int bc, int scheme,
                             const ExplicitGeom &g, double *ws, double *snaps,
-                            int64_t snap_every, cudaStream_t s) {
-    return expl::launch_explicit_impl<double>(u, B, N, dx, nu, dt, n_steps, bc, scheme, g, ws, snaps, snap_every, s);
+                            int64_t snap_every, cudaStream_t s,
+                           const ExplicitAdapt<double> *adapt) {
+    return expl::launch_explicit_impl<double>(u, B, N, dx, nu, dt, n_steps, bc, scheme, g, ws, snaps, snap_every, s, adapt);
 }
 }  // namespace burgers

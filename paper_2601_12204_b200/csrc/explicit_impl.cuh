@@ -63,7 +63,29 @@ struct Params {
     T *snaps;
     int64_t snap_every;
     int64_t snap_stride;   // B*N
+    // Adaptive time step (SURVEY 8(f) NEXT-4a; RESIDENT plan, kernel template ADAPT): every
+    // adapt_every steps dt = dt_from_cfl(current state, adapt_C) is re-evaluated inside the kernel
+    // (CTA-wide max |u|, the formula of cfl.cu); `dt` is then not read.  0 = fixed dt.
+    int64_t adapt_every;
+    double adapt_C, dx;
+    double *t_out;         // [B] sum of adapt_every*dt over the evaluations, or nullptr
+    T *dt_out;             // [B] the last dt
 };
+
+// max over the CTA of a non-negative value (NaN operands are ignored, as in cfl.cu)
+template <typename T, bool WARP>
+__device__ __forceinline__ T cta_max(T m, T *red) {
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, off));
+    if (WARP) return m;
+    const int nw = (blockDim.x + 31) >> 5;
+    __syncthreads();                       // `red` may still be read from the previous use
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    T r = red[0];
+    for (int w = 1; w < nw; ++w) r = fmax(r, red[w]);
+    return r;
+}
 
 template <typename T> __device__ __forceinline__ T t_abs(T x);
 template <> __device__ __forceinline__ float t_abs<float>(float x) { return fabsf(x); }
@@ -138,10 +160,22 @@ constexpr int max_threads_for(int bytes, int P, int scheme) {
     return t;
 }
 
-template <typename T, int P, int SCHEME, bool TILED, bool WARP, bool SNAP = false>
-__global__ void __launch_bounds__(WARP ? 32 : max_threads_for(sizeof(T), P, SCHEME))
+// ADAPT: the rarely executed CFL evaluation must not cost the time loop its occupancy: cap the kernel
+// at the 128 registers of the fixed-dt kernels (2 CTAs of 256 threads, 4 of 128, ...).
+constexpr int adapt_min_ctas(int bytes, int P, int scheme) {
+    int arrays = (scheme == BURGERS_SCHEME_RK4) ? 3 : (bytes == 4 ? 3 : 1);
+    int est = P * (bytes / 4) * arrays + 40;                 // as max_threads_for
+    int mt = max_threads_for(bytes, P, scheme);
+    int n = (est <= 136) ? 512 / mt : 1;                     // kernels that need more keep the full budget
+    return n > 0 ? n : 1;
+}
+
+template <typename T, int P, int SCHEME, bool TILED, bool WARP, bool SNAP = false, bool ADAPT = false>
+__global__ void __launch_bounds__(WARP ? 32 : max_threads_for(sizeof(T), P, SCHEME),
+                                  (ADAPT && !WARP) ? adapt_min_ctas(sizeof(T), P, SCHEME) : 0)   // (0 = unspecified)
 explicit_kernel(const Params<T> p) {
     static_assert(!(SNAP && TILED), "snapshots are fused into the RESIDENT plan only");
+    static_assert(!(ADAPT && TILED), "the CFL evaluation is fused into the RESIDENT plan only");
     constexpr bool SPLIT = (sizeof(T) == 4) && (SCHEME == BURGERS_SCHEME_EULER);
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -159,16 +193,23 @@ explicit_kernel(const Params<T> p) {
     const T *srow = p.src + b * N;
     T *drow = p.dst + b * N;
 
-    // per-trajectory constants, evaluated in fp64 and rounded once
+    // per-trajectory constants, evaluated in fp64 and rounded once (ADAPT: set again below, once the
+    // state is loaded)
     constexpr bool SCALED = (sizeof(T) == 4);
-    const double dtb = (double)p.dt[b];
-    const T cx = (T)(dtb * p.inv_dx);
-    const T rr = (T)((double)p.nu[b] * dtb * p.inv_dx * p.inv_dx);
+    const T nu_b = p.nu[b];
+    T dt_cur = ADAPT ? T(0) : p.dt[b];
+    T cx, rr;
+    auto set_dt = [&](T dt_new) {
+        const double dtb = (double)dt_new;
+        cx = (T)(dtb * p.inv_dx);
+        rr = (T)((double)nu_b * dtb * p.inv_dx * p.inv_dx);
+    };
+    set_dt(dt_cur);
     // fp32: the state is carried as w = scale*u with scale = cx.  dt == 0 (cx == 0) leaves u
     // unchanged: no steps, scale 1.
-    const bool degenerate = SCALED && (cx == T(0));
-    const T scale = (SCALED && !degenerate) ? cx : T(1);
-    const int64_t steps = degenerate ? 0 : p.steps;
+    bool degenerate = SCALED && (cx == T(0));
+    T scale = (SCALED && !degenerate) ? cx : T(1);
+    int64_t steps = degenerate ? 0 : p.steps;
 
     // ---------------- load
     T v[P];
@@ -206,6 +247,20 @@ explicit_kernel(const Params<T> p) {
         }
     }
 
+    // ADAPT: the first dt comes from the loaded state (the same max and the same formula as dt_from_cfl_*)
+    __shared__ T red[ADAPT ? 32 : 1];
+    if (ADAPT) {
+        T m = T(0);
+#pragma unroll
+        for (int j = 0; j < P; ++j) m = fmax(m, t_abs(v[j]));
+        dt_cur = cfl_dt<T>(cta_max<T, WARP>(m, red), nu_b, p.dx, p.adapt_C);
+        set_dt(dt_cur);
+        degenerate = SCALED && (cx == T(0));
+        scale = (SCALED && !degenerate) ? cx : T(1);
+        steps = degenerate ? 0 : p.steps;
+    }
+    double t_acc = (ADAPT && steps > 0) ? (double)p.adapt_every * (double)dt_cur : 0.0;
+
     // neighbours for the halo exchange; open edges (TILED) read their own value: garbage that
     // never reaches the stored centre.
     const int last_t = nth - 1;
@@ -223,7 +278,7 @@ explicit_kernel(const Params<T> p) {
     // remainder correction (the final state uses the exact quotient)
     int64_t snap_left = SNAP ? p.snap_every : 0;
     T *snap_row = SNAP ? p.snaps + b * N + g0 : nullptr;     // this thread's row in the next snapshot
-    const T inv_scale = T(1) / scale;
+    T inv_scale = T(1) / scale;
     auto snapshot = [&](auto val) {
         if (!SNAP) return;
         if (--snap_left != 0) return;
@@ -285,6 +340,31 @@ explicit_kernel(const Params<T> p) {
         snap_row += p.snap_stride;
     };
 
+    // Adaptive: a new dt from the current state held (scaled) in v[].  Returns false when the new dt
+    // gives cx = 0 in fp32 (nothing to scale the state by: dt = 0 from here on, the state stays).  For the
+    // scaled state, rho_hi + rho_lo = new scale / old scale as a two-term value, so that rescaling does
+    // not add a rounding error per evaluation.  All threads of the CTA call this together.
+    T rho_hi = T(1), rho_lo = T(0);
+    auto next_dt = [&]() -> bool {
+        T m = T(0);
+#pragma unroll
+        for (int j = 0; j < P; ++j) m = fmax(m, t_abs(v[j]));
+        const T umax = cta_max<T, WARP>(m, red) / scale;
+        const T dt_new = cfl_dt<T>(umax, nu_b, p.dx, p.adapt_C);
+        const T scale_old = scale;
+        dt_cur = dt_new;
+        set_dt(dt_new);
+        if (SCALED) {
+            if (cx == T(0)) return false;
+            rho_hi = cx / scale_old;
+            rho_lo = t_fma(-rho_hi, scale_old, cx) / scale_old;
+            scale = cx;
+            inv_scale = T(1) / scale;
+        }
+        t_acc += (double)p.adapt_every * (double)dt_new;
+        return true;
+    };
+
     if (SCHEME == BURGERS_SCHEME_EULER) {
         T base[SPLIT ? P : 1], s[SPLIT ? P : 1];
         if (SPLIT) {       // w = scale*u as an exact two-term sum (or w itself from the last launch)
@@ -296,13 +376,17 @@ explicit_kernel(const Params<T> p) {
                 v[j] = base[j];
             }
         }
-        for (int64_t n = 0; n < steps; ++n) {
+        // One time step.  Fixed dt: the plain loop over it.  ADAPT: segments of adapt_every steps with a
+        // CFL evaluation between them (the first dt was set above).
+        auto step = [&](int64_t n) {
             exchange<T, WARP>(v[0], v[P - 1], left, right, tl, tr, edge, buf);
-            T dm = v[0] - left;
+            // (points in DESCENDING order: same arithmetic, same bits, but the instruction schedule ptxas
+            // finds for it is 3 % faster in fp32 -- measured, C2: 10.59 -> 10.28 ms; fp64 unchanged)
+            T dp = right - v[P - 1];
 #pragma unroll
-            for (int j = 0; j < P; ++j) {
+            for (int j = P - 1; j >= 0; --j) {
                 const T c = v[j];
-                const T dp = ((j + 1 < P) ? v[j + 1] : right) - c;
+                const T dm = c - ((j > 0) ? v[j - 1] : left);
                 const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
                 if (SPLIT) {
                     const T sn = add_dtF<T, SCALED>(s[j], c, dm, dp, rr, cx);
@@ -312,7 +396,7 @@ explicit_kernel(const Params<T> p) {
                     const T vn = SCALED ? add_dtF<T, true>(c, c, dm, dp, rr, cx) : euler_unscaled<T>(c, dm, dp, rr, cx);
                     v[j] = frozen ? c : vn;
                 }
-                dm = dp;
+                dp = dm;
             }
             if (SPLIT && (n & 63) == 63) {  // renormalise: base <- fl(base+s), s <- exact remainder
 #pragma unroll
@@ -323,6 +407,35 @@ explicit_kernel(const Params<T> p) {
                 }
             }
             snapshot([&](int j) { return v[j]; });
+        };
+        if (!ADAPT) {
+            // (fp64: two steps per loop iteration give ptxas the schedule that is 6 % faster -- measured,
+            // C2 fp64: 17.49 -> 16.45 ms; fp32 is fastest with the plain loop)
+#pragma unroll(sizeof(T) == 8 ? 2 : 1)
+            for (int64_t n = 0; n < steps; ++n) step(n);
+        }
+        int64_t n = 0;
+        for (int64_t seg_end = (steps < p.adapt_every ? steps : p.adapt_every); ADAPT;) {
+            for (; n < seg_end; ++n) step(n);
+            if (n >= steps) break;
+            if (!next_dt()) break;
+            if (SPLIT) {
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    if ((j == 0 && fixL) || (j == P - 1 && fixR)) {
+                        const T keep = (j == 0) ? keepL : keepR;
+                        base[j] = keep * scale;
+                        s[j] = t_fma(keep, scale, -base[j]);
+                    } else {
+                        const T nb = base[j] * rho_hi;
+                        const T e = t_fma(base[j], rho_hi, -nb);
+                        s[j] = t_fma(s[j], rho_hi, t_fma(base[j], rho_lo, e));
+                        base[j] = nb;
+                    }
+                    v[j] = base[j] + s[j];
+                }
+            }
+            seg_end = (steps - n < p.adapt_every) ? steps : n + p.adapt_every;
         }
         if (SPLIT && !p.out_scaled) {       // u = (base + s)/scale, rounded once
 #pragma unroll
@@ -341,7 +454,7 @@ explicit_kernel(const Params<T> p) {
                 v[j] = raw ? v[j] * scale : v[j];
             }
         }
-        for (int64_t n = 0; n < steps; ++n) {
+        auto step = [&](int64_t) {
 #pragma unroll
             for (int stage = 0; stage < 4; ++stage) {
                 if (stage == 0) exchange<T, WARP>(v[0], v[P - 1], left, right, tl, tr, edge, buf);
@@ -362,6 +475,23 @@ explicit_kernel(const Params<T> p) {
                 }
             }
             snapshot([&](int j) { return v[j]; });
+        };
+        if (!ADAPT) {
+            for (int64_t n = 0; n < steps; ++n) step(n);
+        }
+        int64_t n = 0;
+        for (int64_t seg_end = (steps < p.adapt_every ? steps : p.adapt_every); ADAPT;) {
+            for (; n < seg_end; ++n) step(n);
+            if (n >= steps) break;
+            if (!next_dt()) break;
+            if (SCALED) {
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    if ((j == 0 && fixL) || (j == P - 1 && fixR)) v[j] = ((j == 0) ? keepL : keepR) * scale;
+                    else v[j] = t_fma(v[j], rho_hi, v[j] * rho_lo);
+                }
+            }
+            seg_end = (steps - n < p.adapt_every) ? steps : n + p.adapt_every;
         }
         if (SCALED && !p.out_scaled) {
 #pragma unroll
@@ -371,6 +501,11 @@ explicit_kernel(const Params<T> p) {
     if (SCALED) {          // frozen Dirichlet nodes: the loaded bits, not a scale/unscale round trip
         if (fixL) v[0] = keepL;
         if (fixR) v[P - 1] = keepR;
+    }
+
+    if (ADAPT && t == 0) {
+        if (p.t_out) p.t_out[b] = t_acc;
+        p.dt_out[b] = dt_cur;
     }
 
     // ---------------- store
@@ -416,6 +551,9 @@ int launch_P(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStream_t 
     const size_t smem = (size_t)4 * g.block * sizeof(T);
     if (tiled) {
         explicit_kernel<T, P, SCHEME, true, false><<<(unsigned)grid, g.block, smem, s>>>(p);
+    } else if (p.adapt_every > 0) {
+        if (g.block == 32) explicit_kernel<T, P, SCHEME, false, true, false, true><<<(unsigned)grid, 32, 0, s>>>(p);
+        else explicit_kernel<T, P, SCHEME, false, false, false, true><<<(unsigned)grid, g.block, smem, s>>>(p);
     } else if (p.snaps) {          // + one staged row per thread for the coalesced snapshot stores
         const size_t ssm = smem + (size_t)g.block * P * sizeof(T);
         if (ssm > 48 * 1024) {
@@ -450,13 +588,16 @@ int launch_scheme(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStre
 template <typename T>
 int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                          int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                         T *snaps, int64_t snap_every, cudaStream_t s) {
+                         T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt) {
     if (n_steps == 0) return BURGERS_OK;
+    if (adapt && g.plan != BURGERS_PLAN_RESIDENT) return BURGERS_ERR_PLAN;   // (the caller falls back)
     Params<T> p;
     p.nu = nu; p.dt = dt; p.N = N; p.inv_dx = 1.0 / dx; p.nth = g.nth; p.bc = bc;
     p.halo = g.halo; p.W = g.W; p.tiles = g.tiles;
     p.in_scaled = 0; p.out_scaled = 0;
     p.snaps = nullptr; p.snap_every = 0; p.snap_stride = B * N;
+    p.adapt_every = adapt ? adapt->every : 0; p.adapt_C = adapt ? adapt->C : 0.0; p.dx = dx;
+    p.t_out = adapt ? adapt->t_out : nullptr; p.dt_out = adapt ? adapt->dt_out : nullptr;
     auto launch = [&]() {
         return scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
                                               : launch_scheme<T, BURGERS_SCHEME_RK4>(p, g, B, s);
