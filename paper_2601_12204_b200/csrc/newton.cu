@@ -36,8 +36,11 @@ constexpr int newton_max_threads(int bytes, int P) {
     return t;
 }
 
-template <typename T, int P>
-__global__ void __launch_bounds__(newton_max_threads(sizeof(T), P))
+// SMALL: the instance for CTAs of at most 128 threads of the fp64, P = 16 kernel (C3's shape).  Asking for
+// 3 CTAs per SM makes ptxas fit it into 168 registers (116 bytes spilled) instead of 216: 12 instead of 8
+// warps per SM, measured 11 % faster.  Everything else keeps the budget newton_max_threads() assumes.
+template <typename T, int P, bool SMALL = false>
+__global__ void __launch_bounds__(SMALL ? 128 : newton_max_threads(sizeof(T), P), SMALL ? 3 : 1)
 newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                      double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
                      long long *__restrict__ iters_out) {
@@ -152,8 +155,12 @@ template <typename T, int P>
 int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
                     double theta, double tol, int max_iter, long long *iters_out, int Tn, cudaStream_t s) {
     const size_t smem = (size_t)11 * Tn * sizeof(T);
-    newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
-                                                            (T)tol, max_iter, iters_out);
+    if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+        newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                      (T)theta, (T)tol, max_iter, iters_out);
+    else
+        newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
+                                                                (T)tol, max_iter, iters_out);
     return last_launch_status();
 }
 
