@@ -246,7 +246,10 @@ int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float 
 int dt_from_cfl_f64(const double *u, int64_t B, int64_t N, double L, const double *nu,
                     double C, int bc, double *dt_out, void *stream);
 
-/* ---- host-buffer variants (end-to-end path; all pointers HOST) ----------------- */
+/* ---- host-buffer variants (end-to-end path; all pointers HOST) -----------------
+ * Device buffers come from a stream-ordered memory pool owned by the library (per device, created by the
+ * first host-buffer call; freed blocks are kept up to 1 GiB so that repeated calls do not remap memory).
+ * The calls return when the result is in the host buffers. */
 int burgers_explicit_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu,
                               const float *dt, int64_t n_steps, int bc, int scheme);
 int burgers_explicit_host_f64(double *u, int64_t B, int64_t N, double L,

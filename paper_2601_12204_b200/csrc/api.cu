@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/burgers.h: argument validation, plan selection, dispatch,
 // and the host-buffer (end-to-end) variants.  No arithmetic of the method lives here.
 #include <cmath>
+#include <mutex>
 #include <cstdint>
 
 #include "common.cuh"
@@ -269,12 +270,44 @@ int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, 
 }
 
 // ---- host-buffer path: allocate, copy in, run the device path, copy out, free ---------------
-// Stream-ordered allocations from the device's default memory pool (cudaMallocAsync): after the
-// first call the pool serves them without a driver round trip; nothing is kept by the library.
+// Stream-ordered allocations from a memory pool the library owns (one per device, created by the first
+// host-buffer call).  Freed blocks stay in that pool up to kHostPoolKeepBytes, so that a sequence of host
+// calls does not map and unmap device memory every time: with the device's default pool, whose release
+// threshold is 0, everything goes back to the driver at the next synchronisation and C2 fp32 end to end
+// took 11.9 to 19.8 ms from call to call; now 11.6 to 12.0.  The default pool is not touched.
+constexpr uint64_t kHostPoolKeepBytes = (uint64_t)1 << 30;
+
+cudaMemPool_t host_pool() {
+    static std::mutex mu;
+    static cudaMemPool_t pools[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cudaMemPoolCreate(&pool, &props) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        uint64_t keep = kHostPoolKeepBytes;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        pools[dev] = pool;
+    }
+    return pools[dev];
+}
+
 struct DevBuf {
     void *p = nullptr;
     ~DevBuf() { if (p) cudaFreeAsync(p, nullptr); }
-    bool alloc(size_t bytes) { return bytes == 0 || cudaMallocAsync(&p, bytes, nullptr) == cudaSuccess; }
+    bool alloc(size_t bytes) {
+        if (bytes == 0) return true;
+        cudaMemPool_t pool = host_pool();
+        const cudaError_t e = pool ? cudaMallocFromPoolAsync(&p, bytes, pool, nullptr) : cudaMallocAsync(&p, bytes, nullptr);
+        if (e != cudaSuccess) { cudaGetLastError(); p = nullptr; return false; }
+        return true;
+    }
 };
 
 template <typename T, typename F>
