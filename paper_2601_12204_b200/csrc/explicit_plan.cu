@@ -41,7 +41,10 @@ static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock
                            ExplicitGeom *g) {
     const int V = is_f64 ? 2 : 4;
     const int radius = (scheme == BURGERS_SCHEME_RK4) ? 4 : 1;
-    int P = ppt ? ppt : 16;
+    // defaults measured on C4a (fp32 Euler, N = 2^24, 2 000 steps): P = 16, tblock = 64: 9.43 ms; P = 32 with
+    // tblock = 128 / 256 / 400: 9.10 / 8.87 / 9.39 ms.  Other dtype / scheme: P = 16, tblock = 64 (RK4: 16).
+    const bool f32_euler = !is_f64 && scheme == BURGERS_SCHEME_EULER;
+    int P = ppt ? ppt : (f32_euler ? 32 : 16);
     // Dirichlet: the frozen end nodes must be the first / last point of a thread
     if (bc == BURGERS_BC_DIRICHLET) {
         if (ppt && N % P) return false;
@@ -50,7 +53,7 @@ static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock
     int nth = 256;
     const int maxt = explicit_max_threads(is_f64, P, scheme);
     if (nth > maxt) nth = maxt;
-    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 16 : 64;   // measured on C4a: 16 -> 11.9 ms, 64 -> 9.4 ms
+    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 16 : ((f32_euler && P == 32) ? 256 : 64);
     const int64_t Wt = (int64_t)nth * P;
     const int q = P > V ? P : V;
     int halo = 0;
