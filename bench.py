@@ -41,7 +41,7 @@ FP32_LANES, FP64_LANES = 128, 64
 I_EULER_F32, I_EULER_F64, I_RK4_F32, I_BTCS_HYBRID, I_BTCS_LONG = 7, 5, 32, 22, 22
 # dram__bytes_read.sum + dram__bytes_write.sum of the time-stepping kernel, per launch, from the
 # `ncu --set full` captures summarised in profiles/ (r01_ncu_full_<workload>.txt)
-NCU_TRAFFIC_BYTES = {"c2_f32": 16.8e6, "c2_f64": 33.6e6, "c3": 81.9e6, "c4a": 86.8e6, "c4b": 33.7e6, "c5": 509.8e6}
+NCU_TRAFFIC_BYTES = {"c2_f32": 16.8e6, "c2_f64": 33.6e6, "c3": 81.9e6, "c4a": 85.4e6, "c4b": 33.7e6, "c5": 572.4e6}
 
 
 def peaks():

@@ -29,9 +29,22 @@ static bool resident_fit(int is_f64, int64_t N, int scheme, int P, ExplicitGeom 
 
 static bool resident_geometry(int is_f64, int64_t N, int scheme, int ppt, ExplicitGeom *g) {
     if (ppt) return resident_fit(is_f64, N, scheme, ppt, g);
-    // prefer many points per thread (few halo exchanges per update) while keeping >= 2 warps
-    for (int P = 32; P >= 1; P /= 2)
-        if (N / P >= 64 && resident_fit(is_f64, N, scheme, P, g)) return true;
+    // Prefer many points per thread (few halo exchanges per update) while a CTA still has a full warp.
+    // Measured on B200 (ms, 8192-16384 trajectories; P = 8 / 16 / 32):
+    //   fp32 Euler  N=512: 1.34 / 1.07 / 2.48   N=1024: 5.14 / 4.38 / 4.93   N=2048: 10.3 / 8.67 / 8.21
+    //   fp32 RK4    N=512: 1.42 / 1.29 / 2.53   N=1024: 5.50 / 5.19 / 5.00   N=4096: 11.2 / 10.6 / 9.93
+    //   fp64 Euler  N=512: 1.85 / 1.66 / 3.31   N=2048: 14.3 / 12.8 / 13.1   N=4096: 14.8 / 13.0 / 13.1
+    //   fp64 RK4    N=512: 2.63 / 2.53 / 4.84   N=2048: 20.6 / 18.6 / 19.5   N=4096: 22.3 / 18.8 / 19.5
+    // hence: P = 32 needs two warps for Euler, one for fp32 RK4, and comes after P = 16 for fp64 RK4 (254
+    // registers); the smaller P need one full warp.
+    const bool rk4 = (scheme == BURGERS_SCHEME_RK4);
+    const int order_default[6] = {32, 16, 8, 4, 2, 1}, order_f64_rk4[6] = {16, 32, 8, 4, 2, 1};
+    const int *order = (rk4 && is_f64) ? order_f64_rk4 : order_default;
+    for (int i = 0; i < 6; ++i) {
+        const int P = order[i];
+        const int min_threads = (P == 32 && !rk4) ? 64 : 32;
+        if (N / P >= min_threads && resident_fit(is_f64, N, scheme, P, g)) return true;
+    }
     for (int P = 1; P <= 32; P *= 2)
         if (resident_fit(is_f64, N, scheme, P, g)) return true;
     return false;
