@@ -439,7 +439,7 @@ def run_ours(args):
         out["e2e"] = {"value": w.updates * world / (statistics.mean(e_ms) * 1e-3), "unit": "updates/s",
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": statistics.mean(e_ms),
-                      "note": "host-buffer C-ABI call burgers_solve_host_* (one upload, dt_from_cfl + time stepping on the device, one download), rank 0"}
+                      "note": "host-buffer C-ABI call burgers_solve_host_* (one upload, dt_from_cfl + time stepping on the device, one download; copies of one half of the batch overlap the kernels of the other), rank 0"}
     if world == 1 and not args.no_extras:
         extras = {}
         for name in ("c2_f64", "c3", "c4a", "c4b", "c5", "c3_newton", "c3_cn", "c2_traj", "c3_gs", "c2_adjoint"):

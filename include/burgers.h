@@ -274,7 +274,8 @@ int dt_from_cfl_host_f64(const double *u, int64_t B, int64_t N, double L,
  * of op = BURGERS_OP_EXPLICIT (`scheme` = BURGERS_SCHEME_*) or BURGERS_OP_BTCS (`scheme` ignored), AUTO
  * plan; u is overwritten with the result; dt_out (B values, may be NULL) receives the step used.
  * Same kernels, hence bitwise the same result, as dt_from_cfl_host_* followed by burgers_*_host_*, with
- * one upload of the state instead of two.  Errors as for the separate calls. */
+ * one upload of the state instead of two (large batches go through as two halves on two streams so that
+ * copies overlap kernels).  Errors as for the separate calls. */
 int burgers_solve_host_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C,
                            int64_t n_steps, int bc, int op, int scheme, float *dt_out);
 int burgers_solve_host_f64(double *u, int64_t B, int64_t N, double L, const double *nu, double C,

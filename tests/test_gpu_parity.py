@@ -347,6 +347,25 @@ def test_solve_host_is_the_two_calls_in_one(B):
         B.burgers_solve_host(w3.u0.copy(), w3.L, w3.nu, 10.0, 1, w3.bc, op=B.OP_NEWTON)
 
 
+def test_solve_host_in_two_halves_is_bitwise_the_single_pass(B):
+    """Batches of >= 8 MB whose plan needs no workspace go through burgers_solve_host_* as two halves on two
+    streams (copies overlap kernels).  Same plan, independent trajectories: the bits of the device path."""
+    w = W.c5_rk4_ensemble(B=2051, N=1024, n_steps=0, dtype=np.float32)          # 8.4 MB, odd B: uneven halves
+    for scheme, cfl, n in ((B.SCHEME_EULER, 0.4, 60), (B.SCHEME_RK4, 0.8, 25)):
+        assert B.plan_query(B.OP_EXPLICIT, False, w.B, w.N, w.bc, scheme) == B.PLAN_RESIDENT
+        u1, dt1 = B.burgers_solve_host(w.u0.copy(), w.L, w.nu, cfl, n, w.bc, op=B.OP_EXPLICIT, scheme=scheme,
+                                       return_dt=True)
+        dt_d = B.dt_from_cfl(to_dev(w.u0), w.L, to_dev(w.nu), cfl, w.bc)
+        np.testing.assert_array_equal(dt1, dt_d.cpu().numpy())
+        np.testing.assert_array_equal(u1, run_explicit(B, w.u0, w.L, w.nu, dt1, n, w.bc, scheme))
+    w3 = W.c3_periodic_btcs(B=1030, N=1024, n_steps=0)                           # fp64, 8.4 MB, HYBRID
+    assert B.plan_query(B.OP_BTCS, True, w3.B, w3.N, w3.bc) == B.PLAN_HYBRID
+    u1, dt1 = B.burgers_solve_host(w3.u0.copy(), w3.L, w3.nu, 10.0, 6, w3.bc, op=B.OP_BTCS, return_dt=True)
+    np.testing.assert_array_equal(u1, run_btcs(B, w3.u0, w3.L, w3.nu, dt1, 6, w3.bc))
+    rows = np.array([0, 514, 515, 1029])
+    assert rel_err(u1[rows], oracle.btcs(w3.u0[rows], w3.L, w3.nu[rows], dt1[rows], 6, w3.bc), w3.u0[rows]) <= 1e-10
+
+
 def test_library_is_loaded_in_this_process(B):
     maps = open("/proc/self/maps").read()
     assert "libburgers.so" in maps
