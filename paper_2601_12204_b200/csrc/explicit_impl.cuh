@@ -179,6 +179,7 @@ explicit_kernel(const Params<T> p) {
     static_assert(!(ADAPT && TILED), "the CFL evaluation is fused into the RESIDENT plan only");
     constexpr bool SPLIT = (sizeof(T) == 4) && (SCHEME == BURGERS_SCHEME_EULER);
     constexpr bool RK4_DESC = WARP && (sizeof(T) == 4);
+    constexpr bool EULER_DESC = !SNAP;
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     T *edge = reinterpret_cast<T *>(smem_raw);
@@ -383,12 +384,15 @@ explicit_kernel(const Params<T> p) {
         auto step = [&](int64_t n) {
             exchange<T, WARP>(v[0], v[P - 1], left, right, tl, tr, edge, buf);
             // (points in DESCENDING order: same arithmetic, same bits, but the instruction schedule ptxas
-            // finds for it is 3 % faster in fp32 -- measured, C2: 10.59 -> 10.28 ms; fp64 unchanged)
-            T dp = right - v[P - 1];
+            // finds for it is 3 % faster in fp32 -- measured, C2: 10.59 -> 10.28 ms; fp64 unchanged; the
+            // snapshot-writing instance is faster ascending: 10.73 -> 10.53 ms with 200 snapshots)
+            T carry = EULER_DESC ? right - v[P - 1] : v[0] - left;
 #pragma unroll
-            for (int j = P - 1; j >= 0; --j) {
+            for (int jj = 0; jj < P; ++jj) {
+                const int j = EULER_DESC ? P - 1 - jj : jj;
                 const T c = v[j];
-                const T dm = c - ((j > 0) ? v[j - 1] : left);
+                const T other = EULER_DESC ? c - ((j > 0) ? v[j - 1] : left) : ((j + 1 < P) ? v[j + 1] : right) - c;
+                const T dm = EULER_DESC ? other : carry, dp = EULER_DESC ? carry : other;
                 const bool frozen = (j == 0 && fixL) || (j == P - 1 && fixR);
                 if (SPLIT) {
                     const T sn = add_dtF<T, SCALED>(s[j], c, dm, dp, rr, cx);
@@ -398,7 +402,7 @@ explicit_kernel(const Params<T> p) {
                     const T vn = SCALED ? add_dtF<T, true>(c, c, dm, dp, rr, cx) : euler_unscaled<T>(c, dm, dp, rr, cx);
                     v[j] = frozen ? c : vn;
                 }
-                dp = dm;
+                carry = other;
             }
             if (SPLIT && (n & 63) == 63) {  // renormalise: base <- fl(base+s), s <- exact remainder
 #pragma unroll
