@@ -384,18 +384,28 @@ int cfl_host(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, 
     return cuda_status(cudaStreamSynchronize(s));
 }
 
-// Streams of the pipelined host path, created once per process.  Blocking streams: they are ordered
-// against the legacy default stream, on which the stream-ordered allocations above are made and freed.
+// Streams of the pipelined host path: one pair per device, created by the first call that uses them.
+// Blocking streams: they are ordered against the legacy default stream, on which the stream-ordered
+// allocations above are made and freed.
 struct HostPipe {
     static constexpr int K = 2;
     cudaStream_t s[K] = {};
-    bool ok = true;
-    HostPipe() {
-        for (int i = 0; i < K; ++i) ok = ok && (cudaStreamCreate(&s[i]) == cudaSuccess);
-    }
+    bool ok = false;
 };
 HostPipe &host_pipe() {
-    static HostPipe p;
+    static std::mutex mu;
+    static HostPipe pipes[64];
+    static HostPipe none;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return none;
+    std::lock_guard<std::mutex> lk(mu);
+    HostPipe &p = pipes[dev];
+    if (!p.ok) {
+        bool ok = true;
+        for (int i = 0; i < HostPipe::K; ++i) ok = ok && (cudaStreamCreate(&p.s[i]) == cudaSuccess);
+        if (!ok) { cudaGetLastError(); return none; }
+        p.ok = true;
+    }
     return p;
 }
 
