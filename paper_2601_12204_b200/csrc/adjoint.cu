@@ -83,15 +83,17 @@ adjoint_resident_kernel(const T *__restrict__ u0, const T *__restrict__ states, 
         }
     };
     auto state = [&](int64_t n) { return (n == 0) ? u0 : states + (size_t)(n - 1) * (size_t)BN; };
-    T l[P], uc[P];
+    // the states are streamed TWO steps ahead (un1: step n-1, un2: step n-2): with one step in flight the
+    // kernel kept only ~32 KB per SM outstanding and reached 0.61 of the HBM bandwidth
+    T l[P], uc[P], un1[P], un2[P];
     load(lam, l);
     load(state(n_steps - 1), uc);
+    if (n_steps >= 2) load(state(n_steps - 2), un1);
     const int tl = (t == 0) ? nth - 1 : t - 1, tr = (t == nth - 1) ? 0 : t + 1;
     const bool firstT = (t == 0), lastT = (t == nth - 1);
     int buf = 0;
     for (int64_t n = n_steps - 1; n >= 0; --n) {
-        T un[P];
-        if (n > 0) load(state(n - 1), un);              // prefetch the next (earlier) state
+        if (n > 1) load(state(n - 2), un2);             // prefetch the state of the step after next
         T *e = edge + buf * 4 * nth;
         e[t] = uc[0]; e[nth + t] = uc[P - 1]; e[2 * nth + t] = l[0]; e[3 * nth + t] = l[P - 1];
         __syncthreads();
@@ -119,7 +121,7 @@ adjoint_resident_kernel(const T *__restrict__ u0, const T *__restrict__ states, 
             ln[j] = acc;
         }
 #pragma unroll
-        for (int j = 0; j < P; ++j) { l[j] = ln[j]; uc[j] = un[j]; }
+        for (int j = 0; j < P; ++j) { l[j] = ln[j]; uc[j] = un1[j]; un1[j] = un2[j]; }
     }
 #pragma unroll
     for (int c = 0; c < P / V; ++c) {
