@@ -12,8 +12,10 @@
 // snapshot per step, written by the RESIDENT kernel from its on-chip state).  Backward sweep, two plans:
 //   RESIDENT  one CTA per trajectory keeps lam in registers for all steps (P consecutive points per
 //             thread, edge values of u^n and lam exchanged through shared memory, one barrier per step)
-//             and STREAMS the stored states, prefetching u^{n-1} while step n is computed: HBM-bound at
-//             sizeof(T) bytes per point and step.  Needs N = P * threads with threads <= 512.
+//             and STREAMS the stored states two steps ahead; the column is evaluated in the scaled
+//             variable w = cx u with every upwind coefficient formed once and applied as lam_j + increment
+//             (see the kernel).  sizeof(T) bytes of HBM traffic per point and step.  Needs N = P * threads
+//             with threads <= 512.
 //   STREAMING one launch per step over all points (any N): reads u^n and lam, writes lam.
 #include "common.cuh"
 
