@@ -99,10 +99,11 @@ btcs_gs_kernel(T *__restrict__ un, T *__restrict__ x, const T *__restrict__ nu, 
 template <typename T> __device__ __forceinline__ T shfl_up_t(T v, int off) { return __shfl_up_sync(0xffffffffu, v, off); }
 
 // Six P-element arrays live across an iteration (x, rhs/b, e/b, q, tol/b, p): P = 16 in fp64 needs the
-// full 255 registers, so 2 CTAs of 128 threads per SM; measured on C3's shape (N = 2048, fp64), P = 16
+// full register budget (241 when ptxas is left alone, which is 5 % faster than asking for 2 CTAs per SM), so 2 CTAs of
+// 128 threads per SM; measured on C3's shape (N = 2048, fp64), P = 16
 // x 128 threads beats 8 x 256 (6.1 against 7.7 ms per 100 steps) and 4 x 512 (13.3): the scan over the
 // threads, not the row arithmetic, is the expensive part, so few threads with many rows each.
-constexpr int gs_min_ctas(int P, int NT) { return NT > 128 ? 1 : (P >= 16 ? 2 : P >= 8 ? 3 : 4); }
+constexpr int gs_min_ctas(int P, int NT) { return NT > 128 ? 1 : (P >= 16 ? 0 : P >= 8 ? 3 : 4); }   // 0 = unspecified
 
 // CTA per system.  Thread t owns rows t*P .. t*P+P-1; rows >= N and the Dirichlet end nodes are
 // identity rows (q = 0, e/b = 0, rhs/b = x, b = 1).  blockDim.x = ceil(N / P) rounded up to a warp.
