@@ -54,10 +54,13 @@ static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock
                            ExplicitGeom *g) {
     const int V = is_f64 ? 2 : 4;
     const int radius = (scheme == BURGERS_SCHEME_RK4) ? 4 : 1;
-    // defaults measured on C4a (fp32 Euler, N = 2^24, 2 000 steps): P = 16, tblock = 64: 9.43 ms; P = 32 with
-    // tblock = 128 / 256 / 400: 9.10 / 8.87 / 9.39 ms.  Other dtype / scheme: P = 16, tblock = 64 (RK4: 16).
-    const bool f32_euler = !is_f64 && scheme == BURGERS_SCHEME_EULER;
-    int P = ppt ? ppt : (f32_euler ? 32 : 16);
+    // Defaults measured on C4a's grid (N = 2^24; ms, P = 16 -> P = 32 at the tblock below):
+    //   fp32 Euler (2 000 steps) tblock  64 / 128 / 256 / 400:  9.43 -> 9.56 / 9.10 / 8.87 / 9.39
+    //   fp64 Euler (1 000 steps) tblock  64 / 128 / 256:        7.85 -> 7.55 / 7.35 / 7.25
+    //   fp32 RK4   (  400 steps) tblock  16 /  32 /  64:        8.00 -> 7.89 / 7.58 / 7.46
+    //   fp64 RK4   (  200 steps) tblock  16 /  32 /  64:        7.59 -> 8.19 / 7.68 / 7.37
+    // hence 32 points per thread, 256 (Euler) / 64 (RK4) steps per launch.
+    int P = ppt ? ppt : 32;
     // Dirichlet: the frozen end nodes must be the first / last point of a thread
     if (bc == BURGERS_BC_DIRICHLET) {
         if (ppt && N % P) return false;
@@ -66,7 +69,7 @@ static bool tiled_geometry(int is_f64, int64_t N, int bc, int scheme, int tblock
     int nth = 256;
     const int maxt = explicit_max_threads(is_f64, P, scheme);
     if (nth > maxt) nth = maxt;
-    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? 16 : ((f32_euler && P == 32) ? 256 : 64);
+    if (tblock <= 0) tblock = (scheme == BURGERS_SCHEME_RK4) ? (P == 32 ? 64 : 16) : (P == 32 ? 256 : 64);
     const int64_t Wt = (int64_t)nth * P;
     const int q = P > V ? P : V;
     int halo = 0;
