@@ -17,12 +17,18 @@
  *  - Device entry points (no `_host` suffix): `u`, `nu`, `dt`, `dt_out`, `ws` are
  *    CUDA DEVICE pointers owned by the caller; `stream` is a cudaStream_t passed
  *    as void* (NULL = default stream).  Calls only enqueue work on `stream` and
- *    return; no device synchronisation inside.  The library allocates nothing
- *    persistent and keeps no global mutable state (re-entrant; concurrent calls
- *    on different streams with disjoint buffers are legal).
+ *    return; no device synchronisation inside.  The DEVICE entry points allocate
+ *    nothing and keep no global mutable state (re-entrant; concurrent calls on
+ *    different streams with disjoint buffers are legal, from one or several host
+ *    threads).
  *  - `_host` entry points: every pointer is a HOST pointer (pinned or pageable);
- *    the call allocates device buffers, copies in, runs the same device path,
- *    copies out, frees, and returns after the result is in host memory.
+ *    the call takes device buffers from a memory pool the LIBRARY owns (one per
+ *    device, created by the first `_host` call, freed blocks kept up to 1 GiB, never
+ *    destroyed) and, for large batches, two library-owned streams per device; it
+ *    copies in, runs the same device path, copies out, and returns after the result
+ *    is in host memory.  This per-device pool and stream pair is the only state
+ *    the library keeps.  `_host` calls work on the legacy default stream: calls from
+ *    several host threads are legal but serialise on the device.
  *  - Layout: `u` is [B][N] row-major (trajectory-contiguous), base 16-byte
  *    aligned; `nu`, `dt`, `dt_out` have length B (one value per trajectory).
  *    `u` is updated IN PLACE: after the call (stream-ordered) it holds the state
@@ -294,6 +300,23 @@ int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
 /* Number of kernel launches (memset/memcpy nodes excluded) the op enqueues. */
 int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
                              int scheme, int plan, int tblock, int64_t n_steps);
+/* ---- measurement aid (bench.py) -------------------------------------------------------
+ * One launch of a register-only micro-benchmark of the FP pipe the "alu" rooflines are quoted against:
+ * every SM at full occupancy, every thread `iters` rounds of 64 independent instructions of one kind:
+ *   BURGERS_PEAK_FFMA_CHAIN  a = fma(a, x, y), shared constant operands (operand-reuse cache): issue rate
+ *   BURGERS_PEAK_FFMA_3REG   a = fma(a, b, c), three distinct registers: register-operand bandwidth
+ *   BURGERS_PEAK_FADD_2REG   a = a + b
+ *   BURGERS_PEAK_DFMA_CHAIN / _DFMA_3REG / _DADD_2REG: the same in fp64.
+ * The caller times the launch (CUDA events on `stream`); *lane_instr_out (HOST pointer, may be NULL)
+ * receives the lane-instructions executed = threads x 64 x iters.  sink: DEVICE pointer to 8 writable
+ * bytes (never written in practice).  Computes nothing of the method. */
+enum {
+    BURGERS_PEAK_FFMA_CHAIN = 0, BURGERS_PEAK_FFMA_3REG = 1, BURGERS_PEAK_FADD_2REG = 2,
+    BURGERS_PEAK_DFMA_CHAIN = 3, BURGERS_PEAK_DFMA_3REG = 4, BURGERS_PEAK_DADD_2REG = 5,
+    BURGERS_PEAK_KINDS = 6
+};
+int burgers_pipe_peak(int kind, int64_t iters, void *sink, void *stream, double *lane_instr_out);
+
 const char *burgers_strerror(int status); /* static strings */
 int burgers_version(void);
 

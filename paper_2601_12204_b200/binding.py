@@ -35,7 +35,7 @@ EXPORTS = [
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64",
     "burgers_solve_host_f32", "burgers_solve_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
-    "burgers_launch_count", "burgers_strerror", "burgers_version",
+    "burgers_launch_count", "burgers_pipe_peak", "burgers_strerror", "burgers_version",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -86,6 +86,8 @@ _lib.burgers_plan_query.argtypes = [_int, _int, _i64, _i64, _int, _int]
 _lib.burgers_plan_query.restype = _int
 _lib.burgers_launch_count.argtypes = [_int, _int, _i64, _i64, _int, _int, _int, _int, _i64]
 _lib.burgers_launch_count.restype = _i64
+_lib.burgers_pipe_peak.argtypes = [_int, _i64, _p, _p, ctypes.POINTER(ctypes.c_double)]
+_lib.burgers_pipe_peak.restype = _int
 _lib.burgers_strerror.argtypes = [_int]
 _lib.burgers_strerror.restype = ctypes.c_char_p
 _lib.burgers_version.argtypes = []
@@ -162,6 +164,14 @@ def _shape(u):
     return u.shape[0], u.shape[1]
 
 
+def _check_vecs(B, **vecs):
+    """Every per-trajectory array (nu, dt, iters_out, ...) must hold exactly B elements: a short one would be
+    read or written out of bounds on the device."""
+    for name, t in vecs.items():
+        if t is not None and t.numel() != B:
+            raise ValueError(f"{name} must have length B = {B}, got {t.numel()}")
+
+
 def _ws(ws, need, device):
     import torch
     if need == 0:
@@ -186,8 +196,7 @@ def burgers_explicit(u, L, nu, dt, n_steps, bc, scheme, ws=None, plan=PLAN_AUTO,
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B or dt.numel() != B:
-        raise ValueError("nu and dt must have length B")
+    _check_vecs(B, nu=nu, dt=dt)
     need = workspace_bytes(OP_EXPLICIT, u.dtype == torch.float64, B, N, bc, scheme, plan)
     wsp, wsb, ws = _ws(ws, need, u.device)
     fn = getattr(_lib, f"burgers_explicit_plan_{sfx}")
@@ -204,8 +213,7 @@ def burgers_explicit_traj(u, L, nu, dt, n_steps, bc, scheme, snap_every, snaps=N
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B or dt.numel() != B:
-        raise ValueError("nu and dt must have length B")
+    _check_vecs(B, nu=nu, dt=dt)
     ns = int(n_steps) // int(snap_every) if snap_every >= 1 else 0
     if snaps is None:
         snaps = torch.empty((max(ns, 1), B, N), dtype=u.dtype, device=u.device)
@@ -228,6 +236,7 @@ def burgers_explicit_adaptive(u, L, nu, C, n_outer, m_steps, bc, scheme, ws=None
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype)
     B, N = _shape(u)
+    _check_vecs(B, nu=nu)
     dt = torch.empty(B, dtype=u.dtype, device=u.device)
     t = torch.zeros(B, dtype=torch.float64, device=u.device)
     need = workspace_bytes(OP_EXPLICIT, u.dtype == torch.float64, B, N, bc, scheme)
@@ -246,6 +255,7 @@ def burgers_explicit_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None, segment=0
     _dev(u0, "u0"); sfx = _sfx(u0)
     _dev(lam, "lam", u0.dtype); _dev(nu, "nu", u0.dtype); _dev(dt, "dt", u0.dtype)
     B, N = _shape(u0)
+    _check_vecs(B, nu=nu, dt=dt)
     if lam.numel() != u0.numel():
         raise ValueError("lam must have the shape of u0")
     need = int(_lib.burgers_adjoint_ckpt_workspace_bytes(int(u0.dtype == torch.float64), B, N, int(bc), int(n_steps),
@@ -264,6 +274,7 @@ def burgers_btcs_traj(u, L, nu, dt, n_steps, bc, snap_every, snaps=None, ws=None
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
+    _check_vecs(B, nu=nu, dt=dt)
     ns = int(n_steps) // int(snap_every) if snap_every >= 1 else 0
     if snaps is None:
         snaps = torch.empty((max(ns, 1), B, N), dtype=u.dtype, device=u.device)
@@ -285,8 +296,7 @@ def burgers_btcs(u, L, nu, dt, n_steps, bc, ws=None, plan=PLAN_AUTO):
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B or dt.numel() != B:
-        raise ValueError("nu and dt must have length B")
+    _check_vecs(B, nu=nu, dt=dt)
     need = workspace_bytes(OP_BTCS, u.dtype == torch.float64, B, N, bc, 0, plan)
     wsp, wsb, ws = _ws(ws, need, u.device)
     fn = getattr(_lib, f"burgers_btcs_plan_{sfx}")
@@ -302,11 +312,11 @@ def burgers_btcs_gs(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=1000, iters_ou
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B or dt.numel() != B:
-        raise ValueError("nu and dt must have length B")
+    _check_vecs(B, nu=nu, dt=dt)
     ip = None
     if iters_out is not None:
         _dev(iters_out, "iters_out", torch.int64)
+        _check_vecs(B, iters_out=iters_out)
         ip = ctypes.c_void_p(iters_out.data_ptr())
     need = workspace_bytes(OP_GS, u.dtype == torch.float64, B, N, bc)
     wsp, wsb, ws = _ws(ws, need, u.device)
@@ -326,13 +336,11 @@ def burgers_newton(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, iters_out=N
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B or dt.numel() != B:
-        raise ValueError("nu and dt must have length B")
+    _check_vecs(B, nu=nu, dt=dt)
     ip = None
     if iters_out is not None:
         _dev(iters_out, "iters_out", torch.int64)
-        if iters_out.numel() != B:
-            raise ValueError("iters_out must have length B")
+        _check_vecs(B, iters_out=iters_out)
         ip = ctypes.c_void_p(iters_out.data_ptr())
     need = workspace_bytes(OP_NEWTON, u.dtype == torch.float64, B, N, bc, 0, plan)
     wsp, wsb, ws = _ws(ws, need, u.device)
@@ -349,8 +357,7 @@ def dt_from_cfl(u, L, nu, C, bc, out=None):
     _dev(u, "u"); sfx = _sfx(u)
     _dev(nu, "nu", u.dtype)
     B, N = _shape(u)
-    if nu.numel() != B:
-        raise ValueError("nu must have length B")
+    _check_vecs(B, nu=nu)
     if out is None:
         out = torch.empty(B, dtype=u.dtype, device=u.device)
     _dev(out, "out", u.dtype)
@@ -360,6 +367,19 @@ def dt_from_cfl(u, L, nu, C, bc, out=None):
     return out
 
 
+PEAK_KINDS = ("ffma_chain", "ffma_3reg", "fadd_2reg", "dfma_chain", "dfma_3reg", "dadd_2reg")
+
+
+def pipe_peak(kind, iters, sink):
+    """One launch of the FP-pipe micro-benchmark `kind` (index into PEAK_KINDS) on the current stream
+    (include/burgers.h: burgers_pipe_peak); returns the lane-instructions it executes.  The caller times it."""
+    _dev(sink, "sink")
+    n = ctypes.c_double(0.0)
+    _check(_lib.burgers_pipe_peak(int(kind), int(iters), sink.data_ptr(), _stream(), ctypes.byref(n)),
+           "burgers_pipe_peak")
+    return n.value
+
+
 # ------------------------------------------------------------------ host (numpy) entry points
 def _host(a, name, dtype=None):
     if not isinstance(a, np.ndarray) or not a.flags.c_contiguous:
@@ -367,6 +387,14 @@ def _host(a, name, dtype=None):
     if dtype is not None and a.dtype != dtype:
         raise TypeError(f"{name} must have dtype {dtype}")
     return a
+
+
+def _hshape(u, **vecs):
+    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    for name, a in vecs.items():
+        if a.size != B:
+            raise ValueError(f"{name} must have length B = {B}, got {a.size}")
+    return B, N
 
 
 def _hsfx(a):
@@ -380,7 +408,7 @@ def _hsfx(a):
 def burgers_explicit_host(u, L, nu, dt, n_steps, bc, scheme):
     """Host-buffer explicit stepping: u (numpy, [B][N]) is updated in place."""
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
-    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    B, N = _hshape(u, nu=nu, dt=dt)
     st = getattr(_lib, f"burgers_explicit_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data,
                                                        dt.ctypes.data, int(n_steps), int(bc), int(scheme))
     _check(st, f"burgers_explicit_host_{sfx}")
@@ -389,7 +417,7 @@ def burgers_explicit_host(u, L, nu, dt, n_steps, bc, scheme):
 
 def burgers_btcs_host(u, L, nu, dt, n_steps, bc):
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
-    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    B, N = _hshape(u, nu=nu, dt=dt)
     st = getattr(_lib, f"burgers_btcs_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data,
                                                    dt.ctypes.data, int(n_steps), int(bc))
     _check(st, f"burgers_btcs_host_{sfx}")
@@ -400,7 +428,7 @@ def burgers_solve_host(u, L, nu, C, n_steps, bc, op=OP_EXPLICIT, scheme=0, retur
     """The whole hot path on host buffers in one call (include/burgers.h: burgers_solve_host_*): dt from the
     CFL number C on the device, then n_steps of the explicit scheme or of BTCS; u is updated in place."""
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype)
-    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    B, N = _hshape(u, nu=nu)
     dt = np.empty(B, dtype=u.dtype) if return_dt else None
     st = getattr(_lib, f"burgers_solve_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, float(C),
                                                     int(n_steps), int(bc), int(op), int(scheme),
@@ -411,7 +439,7 @@ def burgers_solve_host(u, L, nu, C, n_steps, bc, op=OP_EXPLICIT, scheme=0, retur
 
 def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return_iters=False, theta=1.0):
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype); _host(dt, "dt", u.dtype)
-    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    B, N = _hshape(u, nu=nu, dt=dt)
     iters = np.zeros(B, dtype=np.int64)
     st = getattr(_lib, f"burgers_newton_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, dt.ctypes.data,
                                                      int(n_steps), int(bc), float(theta), float(tol), int(max_iter),
@@ -422,7 +450,7 @@ def burgers_newton_host(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, return
 
 def dt_from_cfl_host(u, L, nu, C, bc):
     _host(u, "u"); sfx = _hsfx(u); _host(nu, "nu", u.dtype)
-    B, N = (1, u.shape[0]) if u.ndim == 1 else u.shape
+    B, N = _hshape(u, nu=nu)
     out = np.empty(B, dtype=u.dtype)
     st = getattr(_lib, f"dt_from_cfl_host_{sfx}")(u.ctypes.data, B, N, float(L), nu.ctypes.data, float(C),
                                                   int(bc), out.ctypes.data)

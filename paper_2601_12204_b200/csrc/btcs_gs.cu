@@ -27,22 +27,6 @@ namespace {
 using namespace btcs;
 
 template <typename T>
-__global__ void gs_transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int64_t rows, int64_t cols) {
-    __shared__ T tile[32][33];
-    const int64_t gx = (cols + 31) / 32;
-    const int64_t c0 = ((int64_t)blockIdx.x % gx) * 32, r0 = ((int64_t)blockIdx.x / gx) * 32;
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t r = r0 + k, c = c0 + threadIdx.x;
-        if (r < rows && c < cols) tile[k][threadIdx.x] = in[r * cols + c];
-    }
-    __syncthreads();
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t c = c0 + k, r = r0 + threadIdx.x;
-        if (r < rows && c < cols) out[c * rows + r] = tile[threadIdx.x][k];
-    }
-}
-
-template <typename T>
 __global__ void __launch_bounds__(128)
 btcs_gs_kernel(T *__restrict__ un, T *__restrict__ x, const T *__restrict__ nu, const T *__restrict__ dt,
                int64_t B, int64_t N, double inv_dx, int64_t n_steps, int bc, T tol, int max_iter,
@@ -255,19 +239,14 @@ int launch_btcs_gs(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *
     }
     const size_t BN = (size_t)B * (size_t)N;
     T *un = ws, *x = ws + BN;
-    const int64_t nblk = ((N + 31) / 32) * ((B + 31) / 32);
-    if (nblk > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
-    dim3 tb(32, 8);
-    gs_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(u, un, B, N);
-    int st = last_launch_status();
+    int st = launch_transpose<T>(u, un, B, N, s);
     if (st != BURGERS_OK) return st;
-    const int threads = (B <= 148 * 32 * 4) ? 32 : 128;
+    const int threads = thread_per_system_block(B);
     btcs_gs_kernel<T><<<(unsigned)((B + threads - 1) / threads), threads, 0, s>>>(
         un, x, nu, dt, B, N, 1.0 / dx, n_steps, bc, (T)tol, max_iter, iters_out);
     st = last_launch_status();
     if (st != BURGERS_OK) return st;
-    gs_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(un, u, N, B);
-    return last_launch_status();
+    return launch_transpose<T>(un, u, N, B, s);
 }
 
 template int launch_btcs_gs<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, int, long long *, float *, cudaStream_t);

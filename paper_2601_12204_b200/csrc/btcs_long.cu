@@ -460,7 +460,7 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
         }
         int st = last_launch_status();
         if (st != BURGERS_OK) return st;
-        btcs_long_fixup_kernel<T><<<148 * 4, 256, 0, s>>>(u, pong, B * N, n_steps, status);
+        btcs_long_fixup_kernel<T><<<(unsigned)(sms0 * 4), 256, 0, s>>>(u, pong, B * N, n_steps, status);
         st = last_launch_status();
         if (st != BURGERS_OK) return st;
     }

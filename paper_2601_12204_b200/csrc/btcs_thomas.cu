@@ -21,24 +21,6 @@ namespace burgers {
 namespace {
 
 template <typename T>
-__global__ void transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int64_t rows,
-                                 int64_t cols) {
-    // in[rows][cols] -> out[cols][rows]
-    __shared__ T tile[32][33];
-    const int64_t gx = (cols + 31) / 32;
-    const int64_t c0 = ((int64_t)blockIdx.x % gx) * 32, r0 = ((int64_t)blockIdx.x / gx) * 32;
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t r = r0 + k, c = c0 + threadIdx.x;
-        if (r < rows && c < cols) tile[k][threadIdx.x] = in[r * cols + c];
-    }
-    __syncthreads();
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t c = c0 + k, r = r0 + threadIdx.x;
-        if (r < rows && c < cols) out[c * rows + r] = tile[threadIdx.x][k];
-    }
-}
-
-template <typename T>
 struct Rows {
     T r, cx;
     __device__ __forceinline__ void at(T u, T &a, T &b, T &e) const {
@@ -144,19 +126,14 @@ int launch_btcs_thomas(T *u, int64_t B, int64_t N, double dx, const T *nu, const
     if (n_steps == 0) return BURGERS_OK;
     const size_t BN = (size_t)B * (size_t)N;
     T *ut = ws, *cp = ws + BN, *dp = ws + 2 * BN, *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 3 * BN : nullptr;
-    const int64_t nblk = ((N + 31) / 32) * ((B + 31) / 32);
-    if (nblk > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
-    dim3 tb(32, 8);
-    transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(u, ut, B, N);
-    int st = last_launch_status();
+    int st = launch_transpose<T>(u, ut, B, N, s);
     if (st != BURGERS_OK) return st;
-    const int threads = (B <= 148 * 32 * 4) ? 32 : 128;
+    const int threads = thread_per_system_block(B);
     btcs_thomas_kernel<T><<<(unsigned)((B + threads - 1) / threads), threads, 0, s>>>(
         ut, cp, dp, wp, nu, dt, B, N, 1.0 / dx, n_steps, bc);
     st = last_launch_status();
     if (st != BURGERS_OK) return st;
-    transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(ut, u, N, B);
-    return last_launch_status();
+    return launch_transpose<T>(ut, u, N, B, s);
 }
 
 template int launch_btcs_thomas<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, float *, cudaStream_t);

@@ -19,6 +19,13 @@ inline double grid_dx(int64_t N, double L, int bc) {
 inline int cuda_status(cudaError_t e) { return e == cudaSuccess ? BURGERS_OK : BURGERS_ERR_CUDA; }
 inline int last_launch_status() { return cuda_status(cudaGetLastError()); }
 
+// ---------------------------------------------------------------- re-layout (layout.cu)
+// in[rows][cols] -> out[cols][rows]; the thread-per-system plans work on the batch-minor layout [N][B].
+template <typename T>
+int launch_transpose(const T *in, T *out, int64_t rows, int64_t cols, cudaStream_t s);
+// CTA size of the thread-per-system kernels: one warp per CTA until every SM has four of them
+inline int thread_per_system_block(int64_t B) { return (B <= 148 * 32 * 4) ? 32 : 128; }
+
 // ---------------------------------------------------------------- CFL (cfl.cu)
 template <typename T>
 int launch_cfl(const T *u, int64_t B, int64_t N, double dx, const T *nu, double C, T *dt_out,
@@ -65,8 +72,20 @@ template <typename T>
 int launch_explicit(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                     int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
                     T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt = nullptr);
-// max threads per CTA the explicit kernel <T,P,scheme> may be launched with (register limit)
-int explicit_max_threads(int is_f64, int P, int scheme);
+// Register budget -> launch bound of explicit_kernel<T, P, scheme> (the one definition: the kernel's
+// __launch_bounds__ and the host-side geometry both use it).  State registers per thread: P points x
+// words x arrays (fp32 Euler: base, s, v; other Euler: v; RK4: v, y, acc) plus ~40 for addressing and
+// temporaries; 64 K registers per SM.
+constexpr int explicit_max_threads_for(int bytes, int P, int scheme) {
+    int arrays = (scheme == BURGERS_SCHEME_RK4) ? 3 : (bytes == 4 ? 3 : 1);
+    int regs = P * (bytes / 4) * arrays + 40;
+    int t = 1024;
+    while (t > 32 && t * regs > 65536) t /= 2;
+    return t;
+}
+inline int explicit_max_threads(int is_f64, int P, int scheme) {
+    return explicit_max_threads_for(is_f64 ? 8 : 4, P, scheme);
+}
 
 // ---------------------------------------------------------------- BTCS (btcs_*.cu)
 template <typename T>

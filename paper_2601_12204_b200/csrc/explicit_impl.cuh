@@ -150,15 +150,7 @@ __device__ __forceinline__ void exchange(T first, T last, T &left, T &right, int
     }
 }
 
-// Register budget -> launch bound.  State registers per thread: P points x words x arrays
-// (fp32 Euler: base, s, v; other Euler: v; RK4: v, y, acc) plus ~40 for addressing/temporaries.
-constexpr int max_threads_for(int bytes, int P, int scheme) {
-    int arrays = (scheme == BURGERS_SCHEME_RK4) ? 3 : (bytes == 4 ? 3 : 1);
-    int regs = P * (bytes / 4) * arrays + 40;
-    int t = 1024;
-    while (t > 32 && t * regs > 65536) t /= 2;
-    return t;
-}
+constexpr int max_threads_for(int bytes, int P, int scheme) { return explicit_max_threads_for(bytes, P, scheme); }
 
 // ADAPT: the rarely executed CFL evaluation must not cost the time loop its occupancy: cap the kernel
 // at the 128 registers of the fixed-dt kernels (2 CTAs of 256 threads, 4 of 128, ...).

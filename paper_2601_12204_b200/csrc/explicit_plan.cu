@@ -3,16 +3,6 @@
 
 namespace burgers {
 
-// must mirror expl::max_threads_for (explicit_impl.cuh)
-int explicit_max_threads(int is_f64, int P, int scheme) {
-    const int bytes = is_f64 ? 8 : 4;
-    const int arrays = (scheme == BURGERS_SCHEME_RK4) ? 3 : (bytes == 4 ? 3 : 1);
-    const int regs = P * (bytes / 4) * arrays + 40;
-    int t = 1024;
-    while (t > 32 && t * regs > 65536) t /= 2;
-    return t;
-}
-
 static bool valid_ppt(int p) { return p == 1 || p == 2 || p == 4 || p == 8 || p == 16 || p == 32; }
 
 static bool resident_fit(int is_f64, int64_t N, int scheme, int P, ExplicitGeom *g) {

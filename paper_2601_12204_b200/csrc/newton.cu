@@ -165,22 +165,6 @@ int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T 
 }
 
 // ------------------------------------------------------------------ thread-per-system plan
-template <typename T>
-__global__ void newton_transpose_kernel(const T *__restrict__ in, T *__restrict__ out, int64_t rows, int64_t cols) {
-    __shared__ T tile[32][33];
-    const int64_t gx = (cols + 31) / 32;
-    const int64_t c0 = ((int64_t)blockIdx.x % gx) * 32, r0 = ((int64_t)blockIdx.x / gx) * 32;
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t r = r0 + k, c = c0 + threadIdx.x;
-        if (r < rows && c < cols) tile[k][threadIdx.x] = in[r * cols + c];
-    }
-    __syncthreads();
-    for (int k = threadIdx.y; k < 32; k += blockDim.y) {
-        int64_t c = c0 + k, r = r0 + threadIdx.x;
-        if (r < rows && c < cols) out[c * rows + r] = tile[threadIdx.x][k];
-    }
-}
-
 // ws arrays (each [N][B], batch index fastest): un, w, cp, dp (= rhs, then solution), kn (the per-step
 // constant k_i = (1-theta) G_i(u^n) - u_i^n), and for periodic systems wp (second right-hand side of
 // Sherman-Morrison).
@@ -316,19 +300,14 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
     const size_t BN = (size_t)B * (size_t)N;
     T *un = ws, *w = ws + BN, *cp = ws + 2 * BN, *dp = ws + 3 * BN, *kn = ws + 4 * BN;
     T *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 5 * BN : nullptr;
-    const int64_t nblk = ((N + 31) / 32) * ((B + 31) / 32);
-    if (nblk > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
-    dim3 tb(32, 8);
-    newton_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(u, un, B, N);
-    int st = last_launch_status();
+    int st = launch_transpose<T>(u, un, B, N, s);
     if (st != BURGERS_OK) return st;
-    const int threads = (B <= 148 * 32 * 4) ? 32 : 128;
+    const int threads = thread_per_system_block(B);
     newton_thomas_kernel<T><<<(unsigned)((B + threads - 1) / threads), threads, 0, s>>>(
         un, w, cp, dp, kn, wp, nu, dt, B, N, 1.0 / dx, n_steps, bc, (T)theta, (T)tol, max_iter, iters_out);
     st = last_launch_status();
     if (st != BURGERS_OK) return st;
-    newton_transpose_kernel<T><<<(unsigned)nblk, tb, 0, s>>>(un, u, N, B);
-    return last_launch_status();
+    return launch_transpose<T>(un, u, N, B, s);
 }
 
 template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t);

@@ -82,6 +82,20 @@ def c1_sine(N: int = 256, nu: float = 0.05, scheme: int = EULER, cfl: float = 0.
                    final_time=1.0)
 
 
+def step_dirichlet(N: int = 201, nu: float = 0.01, cfl: float = 5.0, n_steps: int = 16, L: float = 1.0,
+                   dtype=np.float64) -> Workload:
+    """The paper's step initial condition (Eq.20): u0 = 1 for x < L/2, 0 otherwise, on the
+    paper's grid N = 201, nu = 0.01, Dirichlet ends (a = 1, b = 0 as found in u0).
+    ``cfl`` = 5 is the factor of "dt = 5 dx/u_max": a multiple of the CONVECTIVE bound alone
+    (at this N and nu the diffusive bound dx^2/(2 nu) is four times smaller, so dt_from_cfl would not give
+    it); callers form dt = meta["dt"] = cfl * dx / max|u0| themselves."""
+    dx = L / (N - 1)
+    x = np.arange(N, dtype=np.float64) * dx
+    u0 = np.where(x < 0.5 * L, 1.0, 0.0)[None, :]
+    return _finish(f"step-dirichlet-N{N}", u0, [nu], L, DIRICHLET, BTCS, cfl, n_steps, dtype,
+                   meta={"dt": cfl * dx / 1.0})
+
+
 def c2_dirichlet_batch(B: int = 1024, N: int = 4096, n_steps: int = 10000,
                        dtype=np.float32, seed: int = SEED_BASE + 2, rows=None) -> Workload:
     """Config 2: B Dirichlet trajectories on [0,1], 8 sine modes, nu log-uniform.

@@ -194,7 +194,7 @@ def test_plain_c_client_compiles_links_and_runs(tmp_path):
     libdir = os.path.join(root, "paper_2601_12204_b200")
     exe = str(tmp_path / "c_abi_client")
     subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(root, "include"),
-                    os.path.join(root, "tests", "c_abi_client.c"), "-o", exe, "-L", libdir, "-lburgers",
+                    os.path.join(root, "tests", "c_abi_client.c"), "-o", exe, "-L", libdir, "-lburgers", "-lm",
                     "-Wl,-rpath," + libdir], check=True)
     r = subprocess.run([exe], capture_output=True, text=True)
     assert r.returncode == 0, r.stdout + r.stderr

@@ -59,10 +59,16 @@ def test_many_tiny_and_largest_resident(B):
         assert rel_err(u.cpu().numpy()[sel], ref, u0[sel]) <= 1e-12
     u = to_dev(u0.copy()); B.burgers_btcs(u, 1.0, to_dev(nu), to_dev(dt * 10), 4, 0)
     assert rel_err(u.cpu().numpy()[sel], oracle.btcs(u0[sel], 1.0, nu[sel], dt[sel] * 10, 4, 0), u0[sel]) <= 1e-12
-    # the largest sizes the resident plans take
-    for dtype, N in ((np.float32, 32768), (np.float64, 16384)):
-        if B.plan_query(B.OP_EXPLICIT, dtype == np.float64, 2, N, 0, 0) != B.PLAN_RESIDENT:
-            continue
+    # the largest sizes the resident plans take (fp32 Euler: 32 points x 256 threads; fp64: 32 x 512), found
+    # through burgers_plan_query so that the test cannot silently run nothing
+    for dtype, expect in ((np.float32, 8192), (np.float64, 16384)):
+        is64 = dtype == np.float64
+        N = 64
+        while B.plan_query(B.OP_EXPLICIT, is64, 2, 2 * N, 0, 0) == B.PLAN_RESIDENT:
+            N *= 2
+        assert N == expect, (dtype, N)
+        assert B.plan_query(B.OP_EXPLICIT, is64, 2, N, 0, 0) == B.PLAN_RESIDENT
+        assert B.plan_query(B.OP_EXPLICIT, is64, 2, 2 * N, 0, 0) == B.PLAN_TILED
         x = np.arange(N) / N
         v0 = np.stack([np.sin(2 * math.pi * x), 0.3 + np.cos(6 * math.pi * x)]).astype(dtype)
         nv = np.array([0.01, 0.02], dtype=dtype)
@@ -83,3 +89,26 @@ def test_zero_time_step_changes_nothing(B, dtype):
             np.testing.assert_array_equal(u.cpu().numpy(), w.u0)
     u = to_dev(w.u0.copy()); B.burgers_btcs(u, w.L, to_dev(w.nu), to_dev(dt), 3, w.bc)
     np.testing.assert_array_equal(u.cpu().numpy(), w.u0)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_step_function_at_five_times_the_convective_limit(B, dtype):
+    """PAPER.md:193 (Eq.20) with Dirichlet ends on the paper's grid N = 201 at dt = 5 dx/u_max:
+    parity with the oracle, max principle, monotone front, frozen ends -- batched (every plan that takes
+    N = 201) and one trajectory."""
+    w = W.step_dirichlet(dtype=dtype)
+    tol = 1e-4 if dtype == np.float32 else 1e-10
+    for Bn in (1, 300):
+        u0 = np.repeat(w.u0, Bn, axis=0)
+        nu = np.repeat(w.nu, Bn)
+        dt = np.full(Bn, w.meta["dt"], dtype=dtype)
+        ref = oracle.btcs(u0.astype(np.float64), w.L, nu.astype(np.float64), dt.astype(np.float64), w.n_steps, w.bc)
+        for plan in (B.PLAN_AUTO, B.PLAN_THOMAS):
+            u = to_dev(u0.copy())
+            B.burgers_btcs(u, w.L, to_dev(nu), to_dev(dt), w.n_steps, w.bc, plan=plan)
+            got = u.cpu().numpy()
+            assert rel_err(got, ref, u0) <= tol, (Bn, plan)
+            slack = 1e-5 if dtype == np.float32 else 1e-13
+            assert got.min() >= -slack and got.max() <= 1 + slack
+            assert np.all(np.diff(got.astype(np.float64), axis=1) <= slack)
+            np.testing.assert_array_equal(got[:, 0], u0[:, 0]); np.testing.assert_array_equal(got[:, -1], u0[:, -1])

@@ -369,3 +369,31 @@ def test_solve_host_in_two_halves_is_bitwise_the_single_pass(B):
 def test_library_is_loaded_in_this_process(B):
     maps = open("/proc/self/maps").read()
     assert "libburgers.so" in maps
+
+
+def test_plain_c_program_drives_the_kernels(B, tmp_path):
+    """tests/c_abi_client.c `run`: a C99 program with nothing but burgers.h and libburgers.so runs the hot path
+    (burgers_solve_host_f64: CFL step + Euler, CFL step + BTCS) on a 1 x 64 grid; compared with the oracle."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    libdir = os.path.join(root, "paper_2601_12204_b200")
+    exe = str(tmp_path / "c_abi_client")
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I", os.path.join(root, "include"),
+                    os.path.join(root, "tests", "c_abi_client.c"), "-o", exe, "-L", libdir, "-lburgers", "-lm",
+                    "-Wl,-rpath," + libdir], check=True)
+    r = subprocess.run([exe, "run"], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout + r.stderr
+    lines = r.stdout.strip().splitlines()
+    L = 6.283185307179586
+    u0 = (np.sin(L * np.arange(64) / 64.0) + 0.25)[None, :]
+    nu = np.array([0.05])
+    for k, (C, n, name) in enumerate(((0.4, 50, "euler"), (4.0, 7, "btcs"))):
+        dt = float(lines[2 * k].split()[1])
+        tag, *vals = lines[2 * k + 1].split()
+        assert tag == name and len(vals) == 64
+        dt_ref = oracle.dt_from_cfl(u0, L, nu, C, 0)
+        assert abs(dt - dt_ref[0]) <= 2 * np.spacing(dt_ref[0])
+        ref = (oracle.explicit(u0, L, nu, np.array([dt]), n, 0, 0) if name == "euler"
+               else oracle.btcs(u0, L, nu, np.array([dt]), n, 0))
+        assert rel_err(np.array([float(v) for v in vals])[None, :], ref, u0) <= 1e-10, name

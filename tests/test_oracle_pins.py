@@ -339,3 +339,35 @@ def test_travelling_viscous_shock_dirichlet(scheme):
              oracle.explicit(u0, L, nu, dt, n, DIRICHLET, RK4 if scheme == "rk4" else EULER))
         errs.append(math.sqrt(np.mean((u - exact(T)) ** 2)))
     assert errs[0] < 0.15 and 0.7 < math.log2(errs[0] / errs[1]) < 1.3, errs
+
+
+# ---------------------------------------------------------------- E5: the step of PAPER.md:193 (Eq.20)
+def test_step_function_btcs_is_stable_at_five_times_the_convective_limit():
+    """"the implicit solver remained stable even for dt = 5 dx/u_max" on the step initial
+    condition of Eq.20 (N = 201, nu = 0.01).  For the lagged upwind BTCS of D4 this is a
+    theorem, not an observation: the matrix is an M-matrix with unit row sums (max principle for any dt) and,
+    with u >= 0, the scheme has Harten's implicit TVD form (C_{i-1/2} = r + c_i >= 0, D_{i+1/2} = r >= 0), so a
+    monotone profile stays monotone and its total variation cannot grow.  The explicit scheme at the same dt
+    (|c| + 2r = 5 + 20 >> 1) must blow up."""
+    from paper_2601_12204_b200 import workloads as WL
+    w = WL.step_dirichlet()
+    dx = w.L / (w.N - 1)
+    dt = np.array([w.meta["dt"]])
+    assert dt[0] == 5.0 * dx / np.abs(w.u0).max()                           # "dt = 5 dx/u_max", r = nu dt/dx^2 = 10
+    x = np.arange(w.N) * dx
+    front = []
+    for n in (1, 4, 8, 16):
+        u = oracle.btcs(w.u0, w.L, w.nu, dt, n, w.bc)[0]
+        assert u[0] == 1.0 and u[-1] == 0.0                                 # frozen ends (Q8)
+        assert u.min() >= 0.0 and u.max() <= 1.0 + 1e-14                    # max principle at C = 5
+        assert np.all(np.diff(u) <= 1e-14)                                  # monotone: no oscillation at the front
+        assert np.abs(np.diff(u)).sum() <= 1.0 + 1e-13                      # total variation does not grow
+        i = int(np.argmax(u < 0.5))
+        front.append(x[i - 1] + (u[i - 1] - 0.5) / (u[i - 1] - u[i]) * dx)
+    # the front travels to the right (u > 0: backward differences), at a speed of the order of the
+    # Rankine-Hugoniot value (u_L + u_R)/2 = 1/2 (the non-conservative lagged form at C = 5 is slower)
+    assert np.all(np.diff(front) > 0)
+    speed = (front[-1] - front[1]) / (12 * dt[0])
+    assert 0.3 < speed < 0.6, speed
+    blown = oracle.explicit(w.u0, w.L, w.nu, dt, 8, w.bc, EULER)[0]
+    assert not (np.abs(blown).max() <= 10.0)

@@ -1,5 +1,6 @@
 """N>1 host logic on CPU: two `gloo` ranks (world_size 2) shard a batched workload the way
-`bench.py --gpus 2` does (contiguous trajectory slices, no data-path
+`bench.py --gpus 2` does (the last two tests run bench.py's own entry point: `--gpus 2` launched without
+torchrun starts two ranks itself, with the GPU stepper replaced by a stub and gloo as the backend) (contiguous trajectory slices, no data-path
 collective), and the pieces are checked against the unsharded batch:
   - every rank's shard is bit-identical to the same rows of the full workload,
   - the shards tile the batch exactly (no row lost or duplicated),
@@ -8,8 +9,11 @@ collective), and the pieces are checked against the unsharded batch:
     exchange,
   - the max-over-ranks reduction bench.py uses for its timing returns the slowest rank's value.
 """
+import json
 import os
 import socket
+import subprocess
+import sys
 
 import numpy as np
 import pytest
@@ -94,3 +98,59 @@ def test_shard_rows_properties():
             assert max(sizes) - min(sizes) <= 1
     with pytest.raises(ValueError):
         W.shard_rows(8, 2, 2)
+
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+_STUB = """
+import sys
+sys.path.insert(0, {root!r})
+import os
+import bench
+
+
+class StubRunner:                       # GpuRunner's interface, no device: rank r "takes" 10 + r ms per step
+    def __init__(self, w, spec, device):
+        self.w, self.plan, self.launches, self.op_launches = w, 1, 2, 1
+        assert w.B == 1024 and str(device) == "cpu"
+
+    def timed(self, steps, warmup):
+        r = int(os.environ["RANK"])
+        return [10.0 + r] * steps, [9.0 + r] * steps
+
+    def e2e(self, steps, warmup):
+        return [12.0] * steps, 7, 5
+
+
+bench.BACKEND = "gloo"
+bench.RUNNER = StubRunner
+bench.main()
+"""
+
+
+@pytest.mark.timeout(300)
+def test_bench_gpus_2_spawns_two_ranks_by_itself(tmp_path):
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment re-executes itself under
+    torch.distributed.run with two ranks; each builds its own shard, the timing is the max over ranks and the
+    value counts the updates of both."""
+    stub = tmp_path / "bench_stub.py"
+    stub.write_text(_STUB.format(root=ROOT))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    p = subprocess.run([sys.executable, str(stub), "--gpus", "2", "--steps", "2", "--warmup", "1", "--no-extras",
+                        "--no-cpu", "--reduced"], capture_output=True, text=True, env=env, timeout=280)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, p.stdout                       # rank 0 alone prints, once
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["scaling"] == "weak"
+    assert out["ms_per_step"] == 11.0                       # max over ranks of (10, 11)
+    assert out["config"]["B_per_gpu"] == 1024 and "x2" in out["config"]["parallelism"]
+    assert out["value"] == pytest.approx(2 * 1024 * 4096 * 1000 / 11.0e-3, rel=1e-6)
+    assert out["gpu_launches"] == 4 and out["e2e"]["h2d_bytes_per_step"] == 7
+
+
+def test_bench_refuses_a_world_size_that_contradicts_gpus():
+    env = dict(os.environ, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "3", "--no-extras", "--no-cpu"],
+                       capture_output=True, text=True, env=env, timeout=120)
+    assert p.returncode != 0 and "WORLD_SIZE=2" in (p.stderr + p.stdout)
