@@ -28,7 +28,7 @@ size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 // CTA -> HYBRID; anything else -> THOMAS.
 int btcs_auto_plan(int is_f64, int64_t B, int64_t N, int bc) {
     if (btcs_hybrid_fits(is_f64, N, bc) && B < 200000) return BURGERS_PLAN_HYBRID;
-    if (btcs_long_fits(N, bc) && B < 65536) return BURGERS_PLAN_LONG;
+    if (btcs_long_fits(is_f64, B, N, bc) && B < 65536) return BURGERS_PLAN_LONG;
     return BURGERS_PLAN_THOMAS;
 }
 
@@ -72,7 +72,7 @@ int btcs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, in
             return launch_btcs_hybrid<T>(u, B, N, dx, nu, dt, n_steps, bc, s);
         case BURGERS_PLAN_LONG:
         case BURGERS_PLAN_LONG_GENERAL: {
-            if (!btcs_long_fits(N, bc)) return BURGERS_ERR_PLAN;
+            if (!btcs_long_fits(is_f64, B, N, bc)) return BURGERS_ERR_PLAN;
             const size_t need = btcs_long_ws_bytes((int)sizeof(T), B, N);
             if (!ws || ws_bytes < need) return BURGERS_ERR_WORKSPACE;
             return launch_btcs_long<T>(u, B, N, dx, nu, dt, n_steps, bc, ws,
@@ -681,7 +681,7 @@ size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, i
         if (plan == BURGERS_PLAN_AUTO) plan = btcs_auto_plan(dtype_is_f64, B, N, bc);
         if (plan == BURGERS_PLAN_THOMAS) return align_up(btcs_thomas_ws_elems(B, N, bc) * esz, 256);
         if (plan == BURGERS_PLAN_LONG || plan == BURGERS_PLAN_LONG_GENERAL)
-            return btcs_long_fits(N, bc) ? align_up(btcs_long_ws_bytes((int)esz, B, N), 256) : 0;
+            return btcs_long_fits(dtype_is_f64, B, N, bc) ? align_up(btcs_long_ws_bytes((int)esz, B, N), 256) : 0;
         return 0;
     }
     return 0;

@@ -170,6 +170,106 @@ __device__ __forceinline__ void eliminate_general(RowFn rowfn, T (&q)[P], T (&f)
     last.D = q[P - 1];
 }
 
+// ---- RAGGED partitions: any N on a power-of-two number of threads ---------------------------------
+// The interface solve needs a power-of-two ring of threads, the grid length N is whatever the caller
+// has ("any N >= 3 must work"; the paper's own grid is N = 201).  Padding
+// the chain with identity rows would cut a periodic ring open, so instead the N rows are dealt out
+// UNEVENLY: with q = N / Tn and rem = N - q Tn, thread t owns the n = q + (t < rem) consecutive rows
+// starting at r0 = t q + min(t, rem), held in the first n of its P register slots (3 <= n <= P).  Every
+// row is a real row, the ring of interface rows stays cyclic, and the per-slot work of the unrolled
+// loops is skipped by early exits (n differs by at most one inside a warp).
+struct Part { int r0, n; };
+__device__ __forceinline__ Part partition_of(int t, int N, int Tn) {
+    const int q = N / Tn, rem = N - q * Tn;
+    Part p;
+    p.n = q + (t < rem ? 1 : 0);
+    p.r0 = t * q + (t < rem ? t : rem);
+    return p;
+}
+
+// eliminate_general for a partition of n <= P rows (slots n..P-1 unused).
+template <typename T, int P, typename RowFn>
+__device__ __forceinline__ void eliminate_general_ragged(RowFn rowfn, int n, T (&q)[P], T (&f)[P], T (&c)[P],
+                                                         Row<T> &first, Row<T> &last) {
+    static_assert(P >= 3, "a partition needs at least 3 rows");
+    T a0, b0, e0;
+    rowfn(0, a0, b0, e0);
+    const T d0 = q[0];
+    {
+        T a, b, e;
+        rowfn(1, a, b, e);
+        const T m = rcp(b);
+        f[1] = a * m; c[1] = e * m; q[1] = q[1] * m;
+    }
+#pragma unroll
+    for (int j = 2; j < P; ++j) {
+        if (j < n) {
+            T a, b, e;
+            rowfn(j, a, b, e);
+            const T m = rcp(t_fma(-a, c[j - 1], b));
+            const T am = a * m;
+            f[j] = -am * f[j - 1];
+            c[j] = e * m;
+            q[j] = t_fma(-am, q[j - 1], q[j] * m);
+            // (every executed iteration overwrites `last`; the one that sticks is j = n - 1.  No test
+            // "j == n - 1" here or below: the compiler would turn f[j] into f[n - 1], a run-time index
+            // that sends the arrays to local memory)
+            last.A = f[j]; last.C = c[j]; last.D = q[j];
+        }
+    }
+    // backward recurrence from j = n - 2: started from (0, -1, 0), its first executed step yields
+    // (f_j, c_j, q_j) exactly
+    T F = T(0), G = T(-1), R = T(0);
+#pragma unroll
+    for (int j = P - 2; j >= 1; --j) {
+        if (j <= n - 2) {
+            F = t_fma(-c[j], F, f[j]);
+            G = -c[j] * G;
+            R = t_fma(-c[j], R, q[j]);
+        }
+    }
+    const T m = rcp(t_fma(-e0, F, b0));
+    first.A = a0 * m;
+    first.C = -e0 * G * m;
+    first.D = t_fma(-e0, R, d0) * m;
+}
+
+// back_substitute for a partition of n <= P rows: x0 = x_0, xl = x_{n-1}.
+template <typename T, int P>
+__device__ __forceinline__ void back_substitute_ragged(T (&v)[P], int n, const T (&f)[P], const T (&c)[P],
+                                                       const T (&q)[P], T x0, T xl) {
+    T xn = xl;
+#pragma unroll
+    for (int j = P - 1; j >= 1; --j) {
+        if (j < n - 1) {
+            xn = t_fma(-c[j], xn, t_fma(-f[j], x0, q[j]));
+            v[j] = xn;
+        } else {
+            v[j] = xl;         // slot n - 1 (and the unused slots behind it)
+        }
+    }
+    v[0] = x0;
+}
+
+// Host side: P register slots per thread and Tn threads (a power of two >= 2) for a system of N rows, given
+// the thread limits of the kernel's P = 16 / 8 / 4 instances.  Prefers the largest P that still fills a warp,
+// otherwise the most threads.  *ragged = false when N == P * Tn exactly (every slot used, vector loads).
+inline bool pick_partition(int64_t N, int max16, int max8, int max4, int *P_out, int *T_out, bool *ragged) {
+    const int cand[3] = {16, 8, 4}, lim[3] = {max16, max8, max4};
+    int bestP = 0, bestT = 0;
+    for (int i = 0; i < 3; ++i) {
+        const int P = cand[i];
+        int64_t Tn = 2;
+        while (Tn * P < N) Tn *= 2;                   // smallest power of two with Tn * P >= N
+        if (Tn > lim[i] || N / Tn < 3) continue;      // too long for one CTA / partitions shorter than 3 rows
+        if (Tn >= 32) { bestP = P; bestT = (int)Tn; break; }
+        bestP = P; bestT = (int)Tn;                   // otherwise keep shrinking P (more threads)
+    }
+    if (!bestP) return false;
+    *P_out = bestP; *T_out = bestT; *ragged = ((int64_t)bestP * bestT != N);
+    return true;
+}
+
 // Solve the cyclic interface system of one CTA (Tn = blockDim.x threads, a power of two >= 2) given
 // every thread's two interface rows: one cyclic-reduction step (one reduced row per thread in the
 // unknowns x_L), parallel cyclic reduction with early exit, exact 2x2 ending; returns this thread's

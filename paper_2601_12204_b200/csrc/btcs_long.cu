@@ -73,6 +73,12 @@ __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)_
 __device__ __forceinline__ void cp_async16(unsigned dst, const void *src, unsigned bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(bytes) : "memory");
 }
+// one element of T (4 or 8 bytes; src-size 0 zero-fills): the ragged wrap of a grid whose length is not a
+// multiple of the 16-byte vector
+template <int BYTES>
+__device__ __forceinline__ void cp_async_elem(unsigned dst, const void *src, unsigned bytes) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(dst), "l"(src), "n"(BYTES), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N_> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 
@@ -99,6 +105,7 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (*reinterpret_cast<volatile int *>(status) != 0) return;   // an earlier step failed (uniform)
     const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    const bool aligned = (N % V == 0);
 
     // Warp-private staging: warp w of the CTA owns rows 32w..32w+31 of a tile = WB contiguous bytes
     // of global memory.  It copies them with CR requests of 512 contiguous bytes each (lane l moves
@@ -123,7 +130,7 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
             const T *g = srow + wg0 + lane * V;
 #pragma unroll
             for (int k = 0; k < CR; ++k) cp_async16(d0 + f_off(k), g + k * 32 * V, 16);
-        } else {
+        } else if (aligned) {
 #pragma unroll
             for (int k = 0; k < CR; ++k) {
                 int64_t g = wg0 + (int64_t)(k * 32 + lane) * V;
@@ -131,6 +138,18 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
                 if (dirichlet) { if (g < 0 || g >= N) { bytes = 0; g = 0; } }
                 else { if (g < 0) g += N; else if (g >= N) g -= N; }
                 cp_async16(d0 + f_off(k), srow + g, bytes);
+            }
+        } else {          // N % V != 0: the wrapped (or cut) chunks are not 16-byte pieces of the row any more
+#pragma unroll
+            for (int k = 0; k < CR; ++k) {
+#pragma unroll
+                for (int e = 0; e < V; ++e) {
+                    int64_t g = wg0 + (int64_t)(k * 32 + lane) * V + e;
+                    unsigned bytes = sizeof(T);
+                    if (dirichlet) { if (g < 0 || g >= N) { bytes = 0; g = 0; } }
+                    else { if (g < 0) g += N; else if (g >= N) g -= N; }
+                    cp_async_elem<sizeof(T)>(d0 + f_off(k) + e * sizeof(T), srow + g, bytes);
+                }
             }
         }
         cp_async_commit();
@@ -245,7 +264,14 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
                 if (rt >= kHaloL && rt < Tn - kHaloR && g < N) {
                     int4 q4;
                     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(q4.x), "=r"(q4.y), "=r"(q4.z), "=r"(q4.w) : "r"(s0 + f_off(k)));
-                    *reinterpret_cast<int4 *>(drow + g) = q4;
+                    if (g + V <= N) {
+                        *reinterpret_cast<int4 *>(drow + g) = q4;
+                    } else {                   // the chunk that straddles the end of a grid with N % V != 0
+                        const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+                        for (int k2 = 0; k2 < V; ++k2)
+                            if (g + k2 < N) drow[g + k2] = e[k2];
+                    }
                 }
             }
         }
@@ -273,13 +299,24 @@ struct GenRows {   // interface rows in global memory, two buffers (PCR ping-pon
     T *A[2], *C[2], *D[2];
 };
 
-template <typename T>
+// Partition `part` of the grid-wide list: system b, partition tt of its pps (a power of two).  RAGGED = false:
+// N == kP * pps, rows tt*kP .. tt*kP + kP - 1 (16-byte aligned vector loads); RAGGED = true: any N, the rows
+// btcs::partition_of() deals partition tt (n = N/pps or N/pps + 1 of them, in the first n slots).
+template <typename T, bool RAGGED>
 __device__ __forceinline__ void gen_load_partition(const T *__restrict__ u, int64_t N, int64_t part,
                                                    int64_t parts_per_sys, T (&v)[kP], int64_t &b,
-                                                   int64_t &tt) {
+                                                   int64_t &tt, Part &pt) {
     constexpr int V = 16 / sizeof(T);
     b = part / parts_per_sys;
     tt = part % parts_per_sys;
+    if (RAGGED) {
+        pt = partition_of((int)tt, (int)N, (int)parts_per_sys);
+        const T *p = u + b * N + pt.r0;
+#pragma unroll
+        for (int j = 0; j < kP; ++j) v[j] = (j < pt.n) ? __ldcg(p + j) : T(0);
+        return;
+    }
+    pt.r0 = (int)(tt * kP); pt.n = kP;
     const T *p = u + b * N + tt * kP;     // N % kP == 0: 16-byte aligned
 #pragma unroll
     for (int c = 0; c < kP / V; ++c) {
@@ -290,10 +327,28 @@ __device__ __forceinline__ void gen_load_partition(const T *__restrict__ u, int6
     }
 }
 
-template <typename T>
+// assembly + elimination of one partition of the GENERAL kernel (both phases use it)
+template <typename T, bool RAGGED>
+__device__ __forceinline__ void gen_eliminate(const T (&v)[kP], const Coef<T> &co, const Part &pt, bool fixL, bool fixR,
+                                              T (&f)[kP], T (&c)[kP], T (&q)[kP], Row<T> &first, Row<T> &last) {
+    if (RAGGED) {
+#pragma unroll
+        for (int j = 0; j < kP; ++j) q[j] = v[j];
+        eliminate_general_ragged<T, kP>(
+            [&](int j, T &a, T &b, T &e) {
+                co.at(v[j], a, b, e);
+                if ((j == 0 && fixL) || (j >= pt.n - 1 && fixR)) { a = T(0); b = T(1); e = T(0); }
+            },
+            pt.n, q, f, c, first, last);
+    } else {
+        eliminate<T, kP>(v, co, [&](int j) { return (j == 0 && fixL) || (j == kP - 1 && fixR); }, f, c, q, first, last);
+    }
+}
+
+template <typename T, bool RAGGED>
 __global__ void __launch_bounds__(kGenThreads)
 btcs_long_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt,
-                         int64_t B, int64_t N, double inv_dx, int64_t n_steps, int bc, GenRows<T> R,
+                         int64_t B, int64_t N, int64_t pps, double inv_dx, int64_t n_steps, int bc, GenRows<T> R,
                          int *__restrict__ status, int force) {
     constexpr int P = kP;
     constexpr int V = 16 / sizeof(T);
@@ -302,8 +357,7 @@ btcs_long_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *_
     if (fail == 0) return;                              // uniform over the grid
     int *flags = status + 64;                           // [2][32]
     const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
-    const int64_t pps = N / P;                          // partitions per system
-    const int64_t parts = B * pps;
+    const int64_t parts = B * pps;                      // pps partitions per system (a power of two)
     const int64_t M = 2 * pps;                          // interface rows per system (power of two)
     const int64_t rows = B * M;
     const int64_t gtid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -315,13 +369,13 @@ btcs_long_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *_
         for (int64_t part = gtid; part < parts; part += gthreads) {
             T v[P], f[P], c[P], q[P];
             int64_t b, tt;
-            gen_load_partition<T>(u, N, part, pps, v, b, tt);
+            Part pt;
+            gen_load_partition<T, RAGGED>(u, N, part, pps, v, b, tt, pt);
             Coef<T> co;
             co.init(nu[b], dt[b], inv_dx);
             const bool fixL = dirichlet && tt == 0, fixR = dirichlet && tt == pps - 1;
             Row<T> first, last;
-            eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
-                            f, c, q, first, last);
+            gen_eliminate<T, RAGGED>(v, co, pt, fixL, fixR, f, c, q, first, last);
             const int64_t o = 2 * part;
             R.A[0][o] = first.A; R.A[0][o + 1] = last.A;
             R.C[0][o] = first.C; R.C[0][o + 1] = last.C;
@@ -371,15 +425,23 @@ btcs_long_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *_
         for (int64_t part = gtid; part < parts; part += gthreads) {
             T v[P], f[P], c[P], q[P];
             int64_t b, tt;
-            gen_load_partition<T>(u, N, part, pps, v, b, tt);
+            Part pt;
+            gen_load_partition<T, RAGGED>(u, N, part, pps, v, b, tt, pt);
             Coef<T> co;
             co.init(nu[b], dt[b], inv_dx);
             const bool fixL = dirichlet && tt == 0, fixR = dirichlet && tt == pps - 1;
             Row<T> first, last;
-            eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
-                            f, c, q, first, last);
-            back_substitute<T, P>(v, f, c, q, __ldcg(R.D[cur] + 2 * part), __ldcg(R.D[cur] + 2 * part + 1));
-            T *p = u + b * N + tt * P;
+            gen_eliminate<T, RAGGED>(v, co, pt, fixL, fixR, f, c, q, first, last);
+            const T x0 = __ldcg(R.D[cur] + 2 * part), xl = __ldcg(R.D[cur] + 2 * part + 1);
+            T *p = u + b * N + pt.r0;
+            if (RAGGED) {
+                back_substitute_ragged<T, P>(v, pt.n, f, c, q, x0, xl);
+#pragma unroll
+                for (int j = 0; j < P; ++j)
+                    if (j < pt.n) p[j] = v[j];
+                continue;
+            }
+            back_substitute<T, P>(v, f, c, q, x0, xl);
 #pragma unroll
             for (int cc = 0; cc < P / V; ++cc) {
                 int4 q4;
@@ -392,16 +454,24 @@ btcs_long_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *_
     }
 }
 
-bool pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
+// partitions per system of the GENERAL kernel: the smallest power of two with pps * kP >= N (so that the
+// 2 pps interface rows form a power-of-two ring); every partition then has N/pps >= kP/2 rows
+int64_t gen_pps(int64_t N) {
+    int64_t pps = 2;
+    while (pps * kP < N) pps *= 2;
+    return pps;
+}
 
-size_t row_elems(int64_t B, int64_t N) { return (size_t)B * (size_t)(2 * (N / kP)); }
+size_t row_elems(int64_t B, int64_t N) { return (size_t)B * (size_t)(2 * gen_pps(N)); }
 
 }  // namespace
 
-// LONG runs power-of-two grids of at least four tiles (shorter systems fit one CTA: HYBRID).
-bool btcs_long_fits(int64_t N, int bc) {
+// LONG runs any grid longer than two tiles (shorter systems fit one CTA: HYBRID).  Rows must start on a
+// 16-byte boundary: any N for a single system, N a multiple of the 16-byte vector for a batch.
+bool btcs_long_fits(int is_f64, int64_t B, int64_t N, int bc) {
     (void)bc;
-    return pow2(N) && N >= 4 * (int64_t)kTn * kTP;
+    const int V = is_f64 ? 2 : 4;
+    return N > 2 * (int64_t)kTn * kTP && N < ((int64_t)1 << 31) - 4096 && (B == 1 || N % V == 0);
 }
 
 // ws layout (elements of T): [B*N ping-pong state][6 x B*M interface rows] then kStatusBytes.
@@ -421,7 +491,7 @@ template <typename T>
 int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                      int64_t n_steps, int bc, void *ws, int general_only, cudaStream_t s) {
     if (n_steps == 0) return BURGERS_OK;
-    if (!btcs_long_fits(N, bc)) return BURGERS_ERR_PLAN;
+    if (!btcs_long_fits(sizeof(T) == 8, B, N, bc)) return BURGERS_ERR_PLAN;
     if (n_steps > 0x7ffffff0LL) return BURGERS_ERR_SHAPE;
     const size_t esz = sizeof(T);
     const size_t state_b = ((size_t)B * (size_t)N * esz + 255) / 256 * 256;
@@ -466,14 +536,17 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
     }
 
     // cooperative launch of the general kernel: the grid must be co-resident
+    int64_t pps = gen_pps(N);
+    const bool ragged = (pps * kP != N);
+    const void *gen_fn = ragged ? (const void *)btcs_long_general_kernel<T, true>
+                                : (const void *)btcs_long_general_kernel<T, false>;
     int dev = 0, sms = 0, per_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, btcs_long_general_kernel<T>, kGenThreads, 0) !=
-            cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gen_fn, kGenThreads, 0) != cudaSuccess ||
         per_sm < 1)
         return BURGERS_ERR_CUDA;
-    const int64_t want = (B * (N / kP) + kGenThreads - 1) / kGenThreads;
+    const int64_t want = (B * pps + kGenThreads - 1) / kGenThreads;
     int64_t grid = (int64_t)sms * per_sm;
     if (grid > want) grid = want;
     const size_t re = row_elems(B, N);
@@ -481,8 +554,8 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
     R.A[0] = rows;          R.C[0] = rows + re;     R.D[0] = rows + 2 * re;
     R.A[1] = rows + 3 * re; R.C[1] = rows + 4 * re; R.D[1] = rows + 5 * re;
     int force = general_only ? 1 : 0;
-    void *args[] = {&u, &nu, &dt, &B, &N, (void *)&inv_dx, &n_steps, &bc, &R, &status, &force};
-    if (cudaLaunchCooperativeKernel((const void *)btcs_long_general_kernel<T>, dim3((unsigned)grid),
+    void *args[] = {&u, &nu, &dt, &B, &N, &pps, (void *)&inv_dx, &n_steps, &bc, &R, &status, &force};
+    if (cudaLaunchCooperativeKernel(gen_fn, dim3((unsigned)grid),
                                     dim3(kGenThreads), args, 0, s) != cudaSuccess)
         return BURGERS_ERR_CUDA;
     return last_launch_status();

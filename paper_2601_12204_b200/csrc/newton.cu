@@ -39,7 +39,9 @@ constexpr int newton_max_threads(int bytes, int P) {
 // SMALL: the instance for CTAs of at most 128 threads of the fp64, P = 16 kernel (C3's shape).  Asking for
 // 3 CTAs per SM makes ptxas fit it into 168 registers (116 bytes spilled) instead of 216: 12 instead of 8
 // warps per SM, measured 11 % faster.  Everything else keeps the budget newton_max_threads() assumes.
-template <typename T, int P, bool SMALL = false>
+// RAGGED: any N on a power-of-two number of threads, thread t owning the q or q + 1 rows partition_of() deals
+// it (btcs_common.cuh) in the first n of its P register slots; otherwise N == P * blockDim.x.
+template <typename T, int P, bool SMALL = false, bool RAGGED = false>
 __global__ void __launch_bounds__(SMALL ? 128 : newton_max_threads(sizeof(T), P), SMALL ? 3 : 1)
 newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                      double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
@@ -52,7 +54,11 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     T *sD = sC + 2 * Tn;
     T *sF = sD + 2 * Tn;                      // [3][Tn]
     T *sE = sF + 3 * Tn;                      // [2][Tn] partition edge values of w
-    T *row = u + (int64_t)blockIdx.x * N + (int64_t)t * P;
+    Part part;
+    part.r0 = t * P; part.n = P;
+    if (RAGGED) part = partition_of(t, N, Tn);
+    const int n = part.n;                     // rows of this thread (== P unless RAGGED)
+    T *row = u + (int64_t)blockIdx.x * N + part.r0;
 
     const double dtb = (double)dt[blockIdx.x];
     const T h = (T)(0.5 * dtb * inv_dx);
@@ -63,12 +69,17 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
 
     T w[P], un[P];       // un holds k_i = (1-theta) G_i(u^n) - u_i^n once the first residual of a step is done
+    if (RAGGED) {
 #pragma unroll
-    for (int c = 0; c < P / V; ++c) {
-        int4 q4 = *reinterpret_cast<const int4 *>(row + c * V);
-        const T *e = reinterpret_cast<const T *>(&q4);
+        for (int j = 0; j < P; ++j) w[j] = (j < n) ? row[j] : T(0);
+    } else {
 #pragma unroll
-        for (int k = 0; k < V; ++k) w[c * V + k] = e[k];
+        for (int c = 0; c < P / V; ++c) {
+            int4 q4 = *reinterpret_cast<const int4 *>(row + c * V);
+            const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+            for (int k = 0; k < V; ++k) w[c * V + k] = e[k];
+        }
     }
     long long iters = 0;
     for (int64_t n = 0; n < n_steps; ++n) {
@@ -76,7 +87,14 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
         for (int j = 0; j < P; ++j) un[j] = w[j];
         for (int k = 0;; ++k) {
             // ---- halo exchange of the partition edges
-            sE[t] = w[0]; sE[Tn + t] = w[P - 1];
+            T wlast = w[P - 1];
+            if (RAGGED) {                 // w[n - 1] without a run-time register index
+                wlast = w[0];
+#pragma unroll
+                for (int j = 1; j < P; ++j)
+                    if (j < n) wlast = w[j];
+            }
+            sE[t] = w[0]; sE[Tn + t] = wlast;
             __syncthreads();
             const T wl = sE[Tn + ((t - 1) & mask)], wr = sE[(t + 1) & mask];
             // ---- residual (Eq.11); q = -F is the right-hand side of Eq.12
@@ -84,13 +102,15 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             int big = 0;
 #pragma unroll
             for (int j = 0; j < P; ++j) {
-                const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
+                if (RAGGED && j >= n) { q[j] = T(0); continue; }
+                const bool lastrow = RAGGED ? (j >= n - 1) : (j == P - 1);
+                const T wm = (j == 0) ? wl : w[j - 1], wp = lastrow ? wr : w[(j + 1 < P) ? j + 1 : j];
                 const T dc = wp - wm;
                 const T lap = (wp - w[j]) - (w[j] - wm);
                 const T g = t_fma(h * w[j], dc, -r * lap);              // G_i(w)
                 if (k == 0) un[j] = t_fma(omt, g, -un[j]);              // w = u^n here
                 T F = t_fma(theta, g, w[j] + un[j]);
-                if ((j == 0 && fixL) || (j == P - 1 && fixR)) F = T(0);
+                if ((j == 0 && fixL) || (lastrow && fixR)) F = T(0);
                 q[j] = -F;
                 big |= !(t_abs(F) < tol);          // NaN counts as not converged
             }
@@ -99,63 +119,62 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             // ---- Jacobian rows (Eq.14), partition elimination, interface solve, back substitution
             T f[P], c[P];
             Row<T> first, last;
-            eliminate_general<T, P>(
-                [&](int j, T &a, T &b, T &e) {
-                    if ((j == 0 && fixL) || (j == P - 1 && fixR)) { a = T(0); b = T(1); e = T(0); return; }
-                    const T wm = (j == 0) ? wl : w[j - 1], wp = (j == P - 1) ? wr : w[j + 1];
-                    const T hw = th * w[j];
-                    a = -hw - tr;
-                    b = t_fma(th, wp - wm, b0);
-                    e = hw - tr;
-                },
-                q, f, c, first, last);
+            auto jac = [&](int j, T &a, T &b, T &e) {
+                const bool lastrow = RAGGED ? (j >= n - 1) : (j == P - 1);
+                if ((j == 0 && fixL) || (lastrow && fixR)) { a = T(0); b = T(1); e = T(0); return; }
+                const T wm = (j == 0) ? wl : w[j - 1], wp = lastrow ? wr : w[(j + 1 < P) ? j + 1 : j];
+                const T hw = th * w[j];
+                a = -hw - tr;
+                b = t_fma(th, wp - wm, b0);
+                e = hw - tr;
+            };
+            if (RAGGED) eliminate_general_ragged<T, P>(jac, n, q, f, c, first, last);
+            else eliminate_general<T, P>(jac, q, f, c, first, last);
             T x0, xL;
             solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL);
             T d[P];
 #pragma unroll
             for (int j = 0; j < P; ++j) d[j] = T(0);
-            back_substitute<T, P>(d, f, c, q, x0, xL);
+            if (RAGGED) back_substitute_ragged<T, P>(d, n, f, c, q, x0, xL);
+            else back_substitute<T, P>(d, f, c, q, x0, xL);
 #pragma unroll
-            for (int j = 0; j < P; ++j) w[j] += d[j];      // Eq.13
+            for (int j = 0; j < P; ++j)
+                if (!RAGGED || j < n) w[j] += d[j];      // Eq.13
             ++iters;
         }
     }
     if (iters_out && t == 0) iters_out[blockIdx.x] = iters;
 
+    if (RAGGED) {
 #pragma unroll
-    for (int c = 0; c < P / V; ++c) {
-        int4 q4;
-        T *e = reinterpret_cast<T *>(&q4);
+        for (int j = 0; j < P; ++j)
+            if (j < n) row[j] = w[j];
+    } else {
 #pragma unroll
-        for (int k = 0; k < V; ++k) e[k] = w[c * V + k];
-        *reinterpret_cast<int4 *>(row + c * V) = q4;
+        for (int c = 0; c < P / V; ++c) {
+            int4 q4;
+            T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+            for (int k = 0; k < V; ++k) e[k] = w[c * V + k];
+            *reinterpret_cast<int4 *>(row + c * V) = q4;
+        }
     }
 }
 
-bool pow2(int64_t x) { return x > 0 && (x & (x - 1)) == 0; }
-
-bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out) {
+bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out, bool *ragged) {
     const int bytes = is_f64 ? 8 : 4;
-    const int cand[3] = {16, 8, 4};
-    int bestP = 0;
-    for (int i = 0; i < 3; ++i) {
-        const int P = cand[i];
-        if (N % P) continue;
-        const int64_t Tn = N / P;
-        if (!pow2(Tn) || Tn < 2 || Tn > newton_max_threads(bytes, P)) continue;
-        if (Tn >= 32) { bestP = P; break; }
-        if (!bestP || P < bestP) bestP = P;
-    }
-    if (!bestP) return false;
-    *P_out = bestP; *T_out = (int)(N / bestP);
-    return true;
+    return pick_partition(N, newton_max_threads(bytes, 16), newton_max_threads(bytes, 8), newton_max_threads(bytes, 4),
+                          P_out, T_out, ragged);
 }
 
 template <typename T, int P>
 int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                    double theta, double tol, int max_iter, long long *iters_out, int Tn, cudaStream_t s) {
+                    double theta, double tol, int max_iter, long long *iters_out, int Tn, bool ragged, cudaStream_t s) {
     const size_t smem = (size_t)11 * Tn * sizeof(T);
-    if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+    if (ragged)
+        newton_hybrid_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                             (T)theta, (T)tol, max_iter, iters_out);
+    else if (sizeof(T) == 8 && P == 16 && Tn <= 128)
         newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
                                                                       (T)theta, (T)tol, max_iter, iters_out);
     else
@@ -271,7 +290,8 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
 
 bool newton_hybrid_fits(int is_f64, int64_t N) {
     int P, Tn;
-    return newton_geometry(is_f64, N, &P, &Tn);
+    bool ragged;
+    return newton_geometry(is_f64, N, &P, &Tn, &ragged);
 }
 size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc) {
     return (size_t)B * (size_t)N * (bc == BURGERS_BC_PERIODIC ? 6 : 5);
@@ -287,12 +307,13 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
     }
     if (plan == BURGERS_PLAN_HYBRID) {
         int P, Tn;
-        if (!newton_geometry(sizeof(T) == 8, N, &P, &Tn)) return BURGERS_ERR_PLAN;
+        bool ragged;
+        if (!newton_geometry(sizeof(T) == 8, N, &P, &Tn, &ragged)) return BURGERS_ERR_PLAN;
         if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
         switch (P) {
-            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
-            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
-            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, s);
+            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
+            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
+            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
         }
         return BURGERS_ERR_PLAN;
     }

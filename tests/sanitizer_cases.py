@@ -27,6 +27,17 @@ from paper_2601_12204_b200 import binding as B            # noqa: E402
 from paper_2601_12204_b200 import workloads as W          # noqa: E402
 
 
+FAILED = []
+
+
+def _ok(what, err, tol):
+    """Report instead of raising, so that one run of a tool covers every case."""
+    good = bool(err <= tol)
+    print(f"    {what}: err {err:.3g} (tol {tol:g}) {'ok' if good else 'FAILED'}", flush=True)
+    if not good:
+        FAILED.append(what)
+
+
 def _dt(w, C):
     return oracle.dt_from_cfl(w.u0.astype(np.float64), w.L, w.nu.astype(np.float64), C, w.bc).astype(w.dtype)
 
@@ -40,7 +51,7 @@ def _explicit(w, n, scheme, tol, **kw):
     u = to_dev(w.u0.copy())
     B.burgers_explicit(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, scheme, **kw)
     ref = oracle.explicit(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), n, w.bc, scheme)
-    assert rel_err(u.cpu().numpy(), ref, w.u0) <= tol
+    _ok(f"explicit {w.name} scheme {scheme} {kw}", rel_err(u.cpu().numpy(), ref, w.u0), tol)
 
 
 def case_cfl():
@@ -76,7 +87,7 @@ def case_snap():
             u = to_dev(w.u0.copy())
             _, snaps = B.burgers_explicit_traj(u, w.L, to_dev(w.nu), to_dev(dt), 24, w.bc, scheme, 4)   # staged stores
             _, ref = oracle.explicit_trajectory(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), 24, w.bc, scheme, 4)
-            assert np.abs(snaps.cpu().numpy() - ref).max() / np.abs(w.u0).max() <= tol
+            _ok(f"snap {w.name}", np.abs(snaps.cpu().numpy() - ref).max() / np.abs(w.u0).max(), tol)
 
 
 def case_adapt():
@@ -85,7 +96,7 @@ def case_adapt():
             u = to_dev(w.u0.copy())
             _, t, _ = B.burgers_explicit_adaptive(u, w.L, to_dev(w.nu), w.cfl, 5, 6, w.bc, scheme)       # CTA-wide max, 5 evaluations
             ref, t_ref = oracle.explicit_adaptive(_f64(w.u0), w.L, _f64(w.nu), w.cfl, 5, 6, w.bc, scheme, dtype=dtype)
-            assert rel_err(u.cpu().numpy(), ref, w.u0) <= tol
+            _ok(f"adapt {w.name}", rel_err(u.cpu().numpy(), ref, w.u0), tol)
             assert np.allclose(t.cpu().numpy(), t_ref, rtol=1e-6)
 
 
@@ -94,7 +105,7 @@ def _btcs(w, n, C, tol, **kw):
     u = to_dev(w.u0.copy())
     B.burgers_btcs(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, **kw)
     ref = oracle.btcs(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), n, w.bc)
-    assert rel_err(u.cpu().numpy(), ref, w.u0) <= tol
+    _ok(f"btcs {w.name} C={C} {kw}", rel_err(u.cpu().numpy(), ref, w.u0), tol)
 
 
 def case_thomas():
@@ -110,7 +121,8 @@ def case_hybrid():
         _btcs(w, 4, 10.0, tol)                                 # PCR exits early (block-wide vote)
         _btcs(w, 3, 1.0e5, tol)                                # weak dominance of the reduced rows: full depth, 2x2 ending
         _btcs(W.c2_dirichlet_batch(B=3, N=1024, dtype=dtype), 4, 10.0, tol)    # Dirichlet identity rows
-        _btcs(W.c3_periodic_btcs(B=3, N=201, dtype=dtype), 4, 10.0, tol)       # the paper's N (whatever plan takes it)
+        _btcs(W.c3_periodic_btcs(B=3, N=201, dtype=dtype), 4, 10.0, tol)       # the paper's N: ragged partitions (6 / 7 rows)
+        _btcs(W.c2_dirichlet_batch(B=3, N=3001, dtype=dtype), 3, 1.0e5, tol)   # ragged, 256 threads, full depth
 
 
 def case_long():
@@ -125,6 +137,9 @@ def case_long():
         ws = W.c4b_long_btcs(N=1 << 15, dtype=dtype)
         _btcs(ws, 3, 3000.0, tol, plan=B.PLAN_LONG)            # halo check fails at step 0: cooperative GENERAL fallback, full depth
         _btcs(ws, 2, 10.0, tol, plan=B.PLAN_LONG_GENERAL)      # GENERAL alone, early exit by the level flags
+        wr = W.c4b_long_btcs(N=40003, dtype=dtype)             # odd N: element-wise wrap at the seam, ragged last tile,
+        _btcs(wr, 3, 10.0, tol)                                # ragged partitions in the fallback
+        _btcs(wr, 2, 3000.0, tol)
 
 
 def case_newton():
@@ -136,7 +151,7 @@ def case_newton():
                 u = to_dev(w.u0.copy())
                 B.burgers_newton(u, w.L, to_dev(w.nu), to_dev(dt), 3, w.bc, tol=ntol, max_iter=20, theta=theta)
                 ref = oracle.newton_btcs(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), 3, w.bc, tol=1e-12, max_iter=20, theta=theta)
-                assert rel_err(u.cpu().numpy(), ref, w.u0) <= tol
+                _ok(f"newton {w.name} theta={theta}", rel_err(u.cpu().numpy(), ref, w.u0), tol)
 
 
 def case_gs():
@@ -150,7 +165,7 @@ def case_gs():
             gtol = 1e-4 if dtype == np.float32 else 1e-9
             B.burgers_btcs_gs(u, w.L, to_dev(w.nu), to_dev(dt), 3, w.bc, tol=gtol, max_iter=200, iters_out=it)
             direct = oracle.btcs(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), 3, w.bc)
-            assert rel_err(u.cpu().numpy(), direct, w.u0) <= 30 * gtol
+            _ok(f"gs {w.name}", rel_err(u.cpu().numpy(), direct, w.u0), 30 * gtol)
             assert it.min().item() >= 3
 
 
@@ -164,7 +179,7 @@ def case_adjoint():
             lam = to_dev(lam_T.copy())
             B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 12, w.bc, segment=seg)
             ref = oracle.explicit_adjoint(_f64(w.u0), _f64(lam_T), w.L, _f64(w.nu), _f64(dt), 12, w.bc)
-            assert np.abs(lam.cpu().numpy() - ref).max() / np.abs(ref).max() <= tol
+            _ok(f"adjoint {w.name}", np.abs(lam.cpu().numpy() - ref).max() / np.abs(ref).max(), tol)
 
 
 CASES = {k[5:]: v for k, v in sorted(globals().items()) if k.startswith("case_")}
@@ -175,9 +190,11 @@ def main(argv):
     assert torch.cuda.is_available(), "needs a CUDA device"
     names = argv or list(CASES)
     for n in names:
+        print(f"case {n}:", flush=True)
         CASES[n]()
         torch.cuda.synchronize()
-        print(f"case {n}: ok", flush=True)
+    if FAILED:
+        raise SystemExit(f"FAILED: {FAILED}")
     print(f"{len(names)} cases ok")
 
 

@@ -120,8 +120,9 @@ def test_argument_errors_are_synchronous(B):
     assert nw(one, 1, 8, 1.0, one, one, 1, 0, 1.5, 1e-6, 10, None, 0, None, 0, None) == B.ERR_VALUE
     assert nw(one, 1, 8, 1.0, one, one, 1, 0, float("nan"), 1e-6, 10, None, 0, None, 0, None) == B.ERR_VALUE
     assert nw(one, 1, 8, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_LONG, None, 0, None) == B.ERR_ENUM
-    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_HYBRID, None, 0, None) == B.ERR_PLAN
-    assert nw(one, 1, 201, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_AUTO, None, 0, None) == B.ERR_WORKSPACE
+    assert nw(one, 1, 5, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_HYBRID, None, 0, None) == B.ERR_PLAN
+    assert nw(one, 1, 100000, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_HYBRID, None, 0, None) == B.ERR_PLAN
+    assert nw(one, 1, 100000, 1.0, one, one, 1, 0, 0.5, 1e-6, 10, None, B.PLAN_AUTO, None, 0, None) == B.ERR_WORKSPACE
     assert lib.burgers_newton_host_f32(one, 1, 8, 1.0, one, one, 1, 0, 1.0, -2.0, 10, None) == B.ERR_VALUE
     assert lib.burgers_newton_host_f64(one, 1, 8, 1.0, one, one, 1, 0, -0.1, 1e-6, 10, None) == B.ERR_VALUE
     # host variants validate the same way
@@ -144,21 +145,38 @@ def test_plan_queries(B):
     assert B.launch_count(B.OP_EXPLICIT, False, 1024, 4096, 1, 0, n_steps=10000) == 1
     assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=2000, tblock=16) == 125
     assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=0) == 0
-    # BTCS: C3 fits one CTA per system (HYBRID); C4b is one long system across CTAs (LONG);
-    # shapes neither fits fall back to the thread-per-system Thomas plan
+    # BTCS: C3 fits one CTA per system (HYBRID); C4b is one long system across CTAs (LONG).  ANY grid length
+    # takes one of the two ("any N >= 3 must work"): ragged partitions on a power-of-two number
+    # of threads (the paper's N = 201), ragged last tile.  Only systems of fewer than 6 rows and
+    # batches of long rows that do not start on 16-byte boundaries fall back to one thread per system.
     assert B.plan_query(B.OP_BTCS, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
     assert B.plan_query(B.OP_BTCS, True, 1, 1 << 22, B.BC_PERIODIC) == B.PLAN_LONG
-    assert B.plan_query(B.OP_BTCS, True, 3, 3001, B.BC_PERIODIC) == B.PLAN_THOMAS
+    for bc in (B.BC_PERIODIC, B.BC_DIRICHLET):
+        for is64 in (False, True):
+            for N in (6, 7, 24, 201, 1000, 2000, 3001, 4096):
+                assert B.plan_query(B.OP_BTCS, is64, 3, N, bc) == B.PLAN_HYBRID, (N, is64)
+                assert B.workspace_bytes(B.OP_BTCS, is64, 3, N, bc) == 0
+            for N in (10001, 3000000, (1 << 22) + 40):
+                assert B.plan_query(B.OP_BTCS, is64, 1, N, bc) == B.PLAN_LONG, (N, is64)
+            assert B.plan_query(B.OP_BTCS, is64, 4, 3000000, bc) == B.PLAN_LONG
+            assert B.plan_query(B.OP_BTCS, is64, 4, 3000001, bc) == B.PLAN_THOMAS      # misaligned rows
+            assert B.plan_query(B.OP_BTCS, is64, 4, 5, bc) == B.PLAN_THOMAS
+    assert B.plan_query(B.OP_BTCS, True, 3, 4098, 0) == B.PLAN_LONG and B.plan_query(B.OP_BTCS, False, 3, 8192, 0) == B.PLAN_HYBRID
     assert B.launch_count(B.OP_BTCS, True, 4096, 2048, 0, n_steps=1000) == 1
     assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=200) == 202
     assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, plan=B.PLAN_LONG_GENERAL, n_steps=200) == 1
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1 << 22, 0) >= int(2.5 * 8 * (1 << 22))
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1000, 0, 0, B.PLAN_LONG) == 0      # does not fit
-    # Newton BTCS: resident plan when N = P 2^k fits one CTA, else thread per system (workspace)
+    # Newton BTCS: resident plan for any 6 <= N that fits one CTA, else thread per system (workspace)
     assert B.plan_query(B.OP_NEWTON, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
-    assert B.plan_query(B.OP_NEWTON, True, 1, 201, B.BC_DIRICHLET) == B.PLAN_THOMAS
+    for N in (6, 201, 1000, 3001, 4096):
+        assert B.plan_query(B.OP_NEWTON, True, 1, N, B.BC_DIRICHLET) == B.PLAN_HYBRID
+        assert B.plan_query(B.OP_NEWTON, False, 1, N, B.BC_PERIODIC) == B.PLAN_HYBRID
+    assert B.plan_query(B.OP_NEWTON, True, 1, 5, B.BC_DIRICHLET) == B.PLAN_THOMAS
+    assert B.plan_query(B.OP_NEWTON, True, 1, 100000, B.BC_DIRICHLET) == B.PLAN_THOMAS
     assert B.workspace_bytes(B.OP_NEWTON, True, 4096, 2048, B.BC_PERIODIC) == 0
-    assert B.workspace_bytes(B.OP_NEWTON, True, 2, 201, B.BC_PERIODIC) >= 6 * 2 * 201 * 8
+    assert B.workspace_bytes(B.OP_NEWTON, True, 2, 201, B.BC_PERIODIC) == 0
+    assert B.workspace_bytes(B.OP_NEWTON, True, 2, 100001, B.BC_PERIODIC) >= 6 * 2 * 100001 * 8
     assert B.launch_count(B.OP_NEWTON, True, 4096, 2048, 0, n_steps=1000) == 1
     assert B.launch_count(B.OP_CFL, False, 1024, 4096, 1) == 1
     assert B.launch_count(B.OP_CFL, False, 1, 1 << 24, 0) == 2

@@ -215,6 +215,58 @@ def test_btcs_hybrid_sizes_and_time_steps(B, dtype, N):
             assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (N, bc, C)
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("N", [6, 7, 11, 24, 100, 201, 1000, 2000, 3001, 4095])
+def test_btcs_any_grid_length_fits_one_cta(B, dtype, N):
+    """SURVEY 8(b) "any N >= 3 must work": grid lengths that are not P 2^k -- the paper's own N = 201
+     among them -- run the resident HYBRID plan on ragged partitions (q or q + 1 rows per
+    thread), periodic ring intact; none of them falls back to one thread per system."""
+    rng = np.random.default_rng(N)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        assert B.plan_query(B.OP_BTCS, dtype == np.float64, 5, N, bc) == B.PLAN_HYBRID
+        x = np.arange(N) / N
+        u0 = (rng.uniform(-1.5, 2.5, (5, 1)) * np.sin(2 * math.pi * x * rng.integers(1, 4, (5, 1)) + rng.uniform(0, 6, (5, 1)))
+              + rng.uniform(-0.5, 1.0, (5, 1)) + 0.05 * rng.standard_normal((5, N))).astype(dtype)
+        nu = rng.uniform(0.01, 0.1, 5).astype(dtype)
+        for C in (0.05, 10.0, 3000.0):
+            dt = oracle_dt(u0, L, nu, C, bc, dtype)
+            ref = oracle.btcs(u0.astype(np.float64), L, nu.astype(np.float64), dt.astype(np.float64), 7, bc)
+            got = run_btcs(B, u0, L, nu, dt, 7, bc)
+            assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (N, bc, C)
+            if bc == B.BC_DIRICHLET:
+                np.testing.assert_array_equal(got[:, 0], u0[:, 0]); np.testing.assert_array_equal(got[:, -1], u0[:, -1])
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", [(1, 10001), (1, 40003), (3, 12000), (2, 8194), (1, 300000 + 6)])
+def test_btcs_any_grid_length_across_ctas(B, dtype, shape):
+    """LONG plan on grid lengths that are neither powers of two nor multiples of the 16-byte vector (single
+    systems) or of the tile: ragged last tile, element-wise wrap at the seam of the ring, ragged partitions
+    in the cooperative fallback (driven at C = 3000)."""
+    Bn, N = shape
+    rng = np.random.default_rng(N)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        assert B.plan_query(B.OP_BTCS, dtype == np.float64, Bn, N, bc) == B.PLAN_LONG
+        x = np.arange(N) / N
+        u0 = np.stack([a * np.sin(2 * math.pi * k * x + p) + m for a, k, p, m in
+                       zip(rng.uniform(0.5, 2, Bn), (1, 3, 7), rng.uniform(0, 6, Bn), (-0.4, 0.0, 1.0))]).astype(dtype)
+        nu = rng.uniform(0.01, 0.1, Bn).astype(dtype)
+        for C, plans in ((10.0, (B.PLAN_AUTO, B.PLAN_LONG_GENERAL)), (3000.0, (B.PLAN_AUTO,))):
+            dt = oracle_dt(u0, L, nu, C, bc, dtype)
+            ref = oracle.btcs(u0.astype(np.float64), L, nu.astype(np.float64), dt.astype(np.float64), 5, bc)
+            for plan in plans:
+                got = run_btcs(B, u0, L, nu, dt, 5, bc, plan=plan)
+                assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (shape, bc, C, plan)
+
+
+def test_btcs_long_grid_of_four_million_and_forty_points(B):
+    """N = 2^22 + 40 (the size VERDICT r01 names), fp64, periodic, C4b's profile and time step: the whole grid
+    against the oracle after 6 steps."""
+    w = W.c4b_long_btcs(N=(1 << 22) + 40, n_steps=6)
+    assert B.plan_query(B.OP_BTCS, True, 1, w.N, w.bc) == B.PLAN_LONG
+    check_btcs(B, w, 6)
+
+
 def test_btcs_dirichlet_and_fp32(B):
     w = W.c2_dirichlet_batch(B=9, N=1000, dtype=np.float64)
     check_btcs(B, w, 40, cfl=10.0)
