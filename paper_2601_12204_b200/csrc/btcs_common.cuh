@@ -251,22 +251,36 @@ __device__ __forceinline__ void back_substitute_ragged(T (&v)[P], int n, const T
     v[0] = x0;
 }
 
-// Host side: P register slots per thread and Tn threads (a power of two >= 2) for a system of N rows, given
-// the thread limits of the kernel's P = 16 / 8 / 4 instances.  Prefers the largest P that still fills a warp,
-// otherwise the most threads.  *ragged = false when N == P * Tn exactly (every slot used, vector loads).
-inline bool pick_partition(int64_t N, int max16, int max8, int max4, int *P_out, int *T_out, bool *ragged) {
-    const int cand[3] = {16, 8, 4}, lim[3] = {max16, max8, max4};
+// Host side: geometry of one CTA per system for N rows: Tn threads (a power of two >= 2) and P register slots
+// per thread, given max_threads(P), the thread limit of the kernel's P-slot instance.
+//   exact  (N == P Tn, P in {16, 8, 4}): every slot used, 128-bit loads; the largest P that still fills a warp,
+//          otherwise the most threads;
+//   ragged (any other N): P = ceil(N / Tn) in [4, 16], so that every thread owns P - 1 or P rows (the kernels
+//          tell the compiler so, and only the last slot is conditional); the fewest threads (largest P) that
+//          still fill a warp, otherwise the most threads with P >= 4.
+template <typename MaxThreads>
+inline bool pick_partition(int64_t N, MaxThreads max_threads, int *P_out, int *T_out, bool *ragged) {
+    const int cand[3] = {16, 8, 4};
     int bestP = 0, bestT = 0;
     for (int i = 0; i < 3; ++i) {
         const int P = cand[i];
-        int64_t Tn = 2;
-        while (Tn * P < N) Tn *= 2;                   // smallest power of two with Tn * P >= N
-        if (Tn > lim[i] || N / Tn < 3) continue;      // too long for one CTA / partitions shorter than 3 rows
+        if (N % P) continue;
+        const int64_t Tn = N / P;
+        if (Tn < 2 || (Tn & (Tn - 1)) || Tn > max_threads(P)) continue;
         if (Tn >= 32) { bestP = P; bestT = (int)Tn; break; }
-        bestP = P; bestT = (int)Tn;                   // otherwise keep shrinking P (more threads)
+        bestP = P; bestT = (int)Tn;
+    }
+    if (bestP) { *P_out = bestP; *T_out = bestT; *ragged = false; return true; }
+    for (int64_t Tn = 2; Tn <= 1024; Tn *= 2) {
+        const int64_t P = (N + Tn - 1) / Tn;
+        if (P > 16) continue;                 // too few threads for 16 slots
+        if (P < 4) break;                     // (and every larger Tn) partitions shorter than 3 rows
+        if (Tn > max_threads((int)P)) break;
+        bestP = (int)P; bestT = (int)Tn;
+        if (Tn >= 32) break;
     }
     if (!bestP) return false;
-    *P_out = bestP; *T_out = bestT; *ragged = ((int64_t)bestP * bestT != N);
+    *P_out = bestP; *T_out = bestT; *ragged = true;
     return true;
 }
 

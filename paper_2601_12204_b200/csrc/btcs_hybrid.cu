@@ -57,6 +57,7 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
     part.r0 = t * P; part.n = P;
     if (RAGGED) part = partition_of(t, N, Tn);
     const int n = part.n;
+    __builtin_assume(n >= P - 1 && n <= P);     // P = ceil(N / Tn): only the last slot is conditional
     T *row = u + (int64_t)blockIdx.x * N + part.r0;
 
     Coef<T> co;
@@ -122,17 +123,22 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
 // P register slots per thread, Tn threads (a power of two >= 2): btcs::pick_partition
 bool hybrid_geometry(int is_f64, int64_t N, int *P_out, int *T_out, bool *ragged) {
     const int bytes = is_f64 ? 8 : 4;
-    return pick_partition(N, hybrid_max_threads(bytes, 16), hybrid_max_threads(bytes, 8), hybrid_max_threads(bytes, 4),
-                          P_out, T_out, ragged);
+    return pick_partition(N, [bytes](int P) { return hybrid_max_threads(bytes, P); }, P_out, T_out, ragged);
 }
 
 template <typename T, int P>
 int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
              int Tn, bool ragged, cudaStream_t s) {
     const size_t smem = (size_t)9 * Tn * sizeof(T);
-    if (ragged) btcs_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
-    else btcs_hybrid_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
-    return last_launch_status();
+    if (ragged) {
+        btcs_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        return last_launch_status();
+    }
+    if constexpr (P == 4 || P == 8 || P == 16) {
+        btcs_hybrid_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        return last_launch_status();
+    }
+    return BURGERS_ERR_PLAN;
 }
 
 }  // namespace
@@ -153,9 +159,10 @@ int launch_btcs_hybrid(T *u, int64_t B, int64_t N, double dx, const T *nu, const
     if (!hybrid_geometry(sizeof(T) == 8, N, &P, &Tn, &ragged)) return BURGERS_ERR_PLAN;
     if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
     switch (P) {
-        case 4: return launch_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, Tn, ragged, s);
-        case 8: return launch_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, Tn, ragged, s);
-        case 16: return launch_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, Tn, ragged, s);
+#define BURGERS_CASE(PP) case PP: return launch_P<T, PP>(u, B, N, dx, nu, dt, n_steps, bc, Tn, ragged, s);
+        BURGERS_CASE(4) BURGERS_CASE(5) BURGERS_CASE(6) BURGERS_CASE(7) BURGERS_CASE(8) BURGERS_CASE(9) BURGERS_CASE(10)
+        BURGERS_CASE(11) BURGERS_CASE(12) BURGERS_CASE(13) BURGERS_CASE(14) BURGERS_CASE(15) BURGERS_CASE(16)
+#undef BURGERS_CASE
     }
     return BURGERS_ERR_PLAN;
 }

@@ -58,6 +58,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     part.r0 = t * P; part.n = P;
     if (RAGGED) part = partition_of(t, N, Tn);
     const int n = part.n;                     // rows of this thread (== P unless RAGGED)
+    __builtin_assume(n >= P - 1 && n <= P);   // P = ceil(N / Tn): only the last slot is conditional
     T *row = u + (int64_t)blockIdx.x * N + part.r0;
 
     const double dtb = (double)dt[blockIdx.x];
@@ -82,7 +83,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
         }
     }
     long long iters = 0;
-    for (int64_t n = 0; n < n_steps; ++n) {
+    for (int64_t step = 0; step < n_steps; ++step) {
 #pragma unroll
         for (int j = 0; j < P; ++j) un[j] = w[j];
         for (int k = 0;; ++k) {
@@ -163,24 +164,28 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
 
 bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out, bool *ragged) {
     const int bytes = is_f64 ? 8 : 4;
-    return pick_partition(N, newton_max_threads(bytes, 16), newton_max_threads(bytes, 8), newton_max_threads(bytes, 4),
-                          P_out, T_out, ragged);
+    return pick_partition(N, [bytes](int P) { return newton_max_threads(bytes, P); }, P_out, T_out, ragged);
 }
 
 template <typename T, int P>
 int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
                     double theta, double tol, int max_iter, long long *iters_out, int Tn, bool ragged, cudaStream_t s) {
     const size_t smem = (size_t)11 * Tn * sizeof(T);
-    if (ragged)
+    if (ragged) {
         newton_hybrid_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
                                                                              (T)theta, (T)tol, max_iter, iters_out);
-    else if (sizeof(T) == 8 && P == 16 && Tn <= 128)
-        newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
-                                                                      (T)theta, (T)tol, max_iter, iters_out);
-    else
-        newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
-                                                                (T)tol, max_iter, iters_out);
-    return last_launch_status();
+        return last_launch_status();
+    }
+    if constexpr (P == 4 || P == 8 || P == 16) {
+        if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+            newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                          (T)theta, (T)tol, max_iter, iters_out);
+        else
+            newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
+                                                                    (T)tol, max_iter, iters_out);
+        return last_launch_status();
+    }
+    return BURGERS_ERR_PLAN;
 }
 
 // ------------------------------------------------------------------ thread-per-system plan
@@ -311,9 +316,12 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
         if (!newton_geometry(sizeof(T) == 8, N, &P, &Tn, &ragged)) return BURGERS_ERR_PLAN;
         if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
         switch (P) {
-            case 4: return launch_hybrid_P<T, 4>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
-            case 8: return launch_hybrid_P<T, 8>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
-            case 16: return launch_hybrid_P<T, 16>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
+#define BURGERS_CASE(PP) \
+    case PP: return launch_hybrid_P<T, PP>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
+            BURGERS_CASE(4) BURGERS_CASE(5) BURGERS_CASE(6) BURGERS_CASE(7) BURGERS_CASE(8) BURGERS_CASE(9)
+            BURGERS_CASE(10) BURGERS_CASE(11) BURGERS_CASE(12) BURGERS_CASE(13) BURGERS_CASE(14) BURGERS_CASE(15)
+            BURGERS_CASE(16)
+#undef BURGERS_CASE
         }
         return BURGERS_ERR_PLAN;
     }

@@ -139,7 +139,7 @@ def case_long():
         _btcs(ws, 2, 10.0, tol, plan=B.PLAN_LONG_GENERAL)      # GENERAL alone, early exit by the level flags
         wr = W.c4b_long_btcs(N=40003, dtype=dtype)             # odd N: element-wise wrap at the seam, ragged last tile,
         _btcs(wr, 3, 10.0, tol)                                # ragged partitions in the fallback
-        _btcs(wr, 2, 3000.0, tol)
+        _btcs(wr, 2, 3000.0 if dtype == np.float64 else 300.0, tol)   # (fp32: cond ~ 1 + 4r times eps stays under the bar)
 
 
 def case_newton():

@@ -147,13 +147,13 @@ def test_plan_queries(B):
     assert B.launch_count(B.OP_EXPLICIT, False, 1, 1 << 24, 0, 0, n_steps=0) == 0
     # BTCS: C3 fits one CTA per system (HYBRID); C4b is one long system across CTAs (LONG).  ANY grid length
     # takes one of the two ("any N >= 3 must work"): ragged partitions on a power-of-two number
-    # of threads (the paper's N = 201), ragged last tile.  Only systems of fewer than 6 rows and
+    # of threads (the paper's N = 201), ragged last tile.  Only systems of fewer than 7 rows and
     # batches of long rows that do not start on 16-byte boundaries fall back to one thread per system.
     assert B.plan_query(B.OP_BTCS, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
     assert B.plan_query(B.OP_BTCS, True, 1, 1 << 22, B.BC_PERIODIC) == B.PLAN_LONG
     for bc in (B.BC_PERIODIC, B.BC_DIRICHLET):
         for is64 in (False, True):
-            for N in (6, 7, 24, 201, 1000, 2000, 3001, 4096):
+            for N in (7, 8, 24, 201, 1000, 2000, 3001, 4096):
                 assert B.plan_query(B.OP_BTCS, is64, 3, N, bc) == B.PLAN_HYBRID, (N, is64)
                 assert B.workspace_bytes(B.OP_BTCS, is64, 3, N, bc) == 0
             for N in (10001, 3000000, (1 << 22) + 40):
@@ -161,15 +161,15 @@ def test_plan_queries(B):
             assert B.plan_query(B.OP_BTCS, is64, 4, 3000000, bc) == B.PLAN_LONG
             assert B.plan_query(B.OP_BTCS, is64, 4, 3000001, bc) == B.PLAN_THOMAS      # misaligned rows
             assert B.plan_query(B.OP_BTCS, is64, 4, 5, bc) == B.PLAN_THOMAS
-    assert B.plan_query(B.OP_BTCS, True, 3, 4098, 0) == B.PLAN_LONG and B.plan_query(B.OP_BTCS, False, 3, 8192, 0) == B.PLAN_HYBRID
+    assert B.plan_query(B.OP_BTCS, True, 3, 6000, 0) == B.PLAN_LONG and B.plan_query(B.OP_BTCS, False, 3, 8192, 0) == B.PLAN_HYBRID
     assert B.launch_count(B.OP_BTCS, True, 4096, 2048, 0, n_steps=1000) == 1
     assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=200) == 202
     assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, plan=B.PLAN_LONG_GENERAL, n_steps=200) == 1
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1 << 22, 0) >= int(2.5 * 8 * (1 << 22))
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1000, 0, 0, B.PLAN_LONG) == 0      # does not fit
-    # Newton BTCS: resident plan for any 6 <= N that fits one CTA, else thread per system (workspace)
+    # Newton BTCS: resident plan for any 7 <= N that fits one CTA, else thread per system (workspace)
     assert B.plan_query(B.OP_NEWTON, True, 4096, 2048, B.BC_PERIODIC) == B.PLAN_HYBRID
-    for N in (6, 201, 1000, 3001, 4096):
+    for N in (7, 201, 1000, 3001, 4096):
         assert B.plan_query(B.OP_NEWTON, True, 1, N, B.BC_DIRICHLET) == B.PLAN_HYBRID
         assert B.plan_query(B.OP_NEWTON, False, 1, N, B.BC_PERIODIC) == B.PLAN_HYBRID
     assert B.plan_query(B.OP_NEWTON, True, 1, 5, B.BC_DIRICHLET) == B.PLAN_THOMAS

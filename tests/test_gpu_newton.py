@@ -94,8 +94,8 @@ def test_sizes_plans_and_semantics(B):
     rng = np.random.default_rng(21)
     for N in (3, 5, 6, 7, 8, 33, 64, 201, 512, 1000, 2000, 3001, 4096):
         for bc, L in ((B.BC_PERIODIC, 2.0), (B.BC_DIRICHLET, 1.0)):
-            # any N >= 6 that fits one CTA is resident (ragged partitions; the paper's N = 201 among them)
-            assert B.plan_query(B.OP_NEWTON, True, 3, N, bc) == (B.PLAN_HYBRID if N >= 6 else B.PLAN_THOMAS)
+            # any N >= 7 that fits one CTA is resident (ragged partitions; the paper's N = 201 among them)
+            assert B.plan_query(B.OP_NEWTON, True, 3, N, bc) == (B.PLAN_HYBRID if N >= 7 else B.PLAN_THOMAS)
             x = np.arange(N) / N
             u0 = np.stack([a * np.sin(2 * math.pi * k * x + p) + m for a, k, p, m in
                            zip(rng.uniform(0.5, 1.5, 3), (1, 2, 3), rng.uniform(0, 6, 3), (-0.3, 0.0, 0.8))])
