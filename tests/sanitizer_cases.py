@@ -47,7 +47,7 @@ def _f64(a):
 
 
 def _explicit(w, n, scheme, tol, **kw):
-    dt = _dt(w, w.cfl)
+    dt = _dt(w, 0.4 if scheme == 0 else 0.8)
     u = to_dev(w.u0.copy())
     B.burgers_explicit(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, scheme, **kw)
     ref = oracle.explicit(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), n, w.bc, scheme)
@@ -144,8 +144,9 @@ def case_long():
 
 def case_newton():
     for dtype, tol, ntol in ((np.float32, 1e-4, 1e-5), (np.float64, 1e-10, 1e-12)):
-        for w in (W.c3_periodic_btcs(B=3, N=2048, dtype=dtype), W.c2_dirichlet_batch(B=3, N=1024, dtype=dtype),
-                  W.c3_periodic_btcs(B=40, N=201, dtype=dtype)):
+        w201 = W.c3_periodic_btcs(B=40, N=201, dtype=dtype)       # ragged partitions; nu raised so that the cell Peclet
+        w201.nu[:] = 0.1                                          # number |u| dx / nu stays below 2 (D11: no pivoting)
+        for w in (W.c3_periodic_btcs(B=3, N=2048, dtype=dtype), W.c2_dirichlet_batch(B=3, N=1024, dtype=dtype), w201):
             for theta in (1.0, 0.5):
                 dt = _dt(w, 2.0)
                 u = to_dev(w.u0.copy())
