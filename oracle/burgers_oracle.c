@@ -629,6 +629,110 @@ int oracle_explicit_adjoint(const double *u0, double *lam, int64_t B, int64_t N,
     return fail ? -1 : 0;
 }
 
+/* ---------------------------------------------------------------------------
+ * D14: DISCRETE ADJOINT of the classical RK4 scheme of D3
+ * (Eq.22; gradients of "the numerical solution").
+ * One step:  y1 = u, k_s = F(y_s), y2 = u + dt/2 k1, y3 = u + dt/2 k2, y4 = u + dt k3,
+ *            u' = u + dt/6 (k1 + 2 k2 + 2 k3 + k4).
+ * Reverse mode, given lam' = dJ/du' (J_s = dF/dy at y_s, the upwind switch held fixed):
+ *   kb4 = dt/6 lam', kb3 = dt/3 lam', kb2 = dt/3 lam', kb1 = dt/6 lam', ub = lam';
+ *   yb4 = J4^T kb4:  ub += yb4, kb3 += dt   yb4;
+ *   yb3 = J3^T kb3:  ub += yb3, kb2 += dt/2 yb3;
+ *   yb2 = J2^T kb2:  ub += yb2, kb1 += dt/2 yb2;
+ *   yb1 = J1^T kb1:  ub += yb1;                         lam = ub.
+ * Rows of J = dF/dy (D2: F_i = -y_i g_i/dx + nu (y_{i+1} - 2 y_i + y_{i-1})/dx^2):
+ *   y_i > 0 :  dF_i/dy_{i-1} =  y_i/dx + nu/dx^2,  dF_i/dy_i = -(2 y_i - y_{i-1})/dx - 2 nu/dx^2,  dF_i/dy_{i+1} = nu/dx^2
+ *   y_i <= 0:  dF_i/dy_{i-1} =  nu/dx^2,  dF_i/dy_i = -(y_{i+1} - 2 y_i)/dx - 2 nu/dx^2,  dF_i/dy_{i+1} = -y_i/dx + nu/dx^2
+ * Dirichlet end nodes: F = 0, zero rows (and u' = u there, which `ub = lam'` carries).
+ * Test hook use_adv as in D2 (constant speed a: the rows are (a/dx + nu/dx^2, -a/dx - 2 nu/dx^2,
+ * nu/dx^2) for a > 0, mirrored otherwise; the step is then linear and the adjoint its transpose).
+ */
+static void rhs_jacT(const double *y, const double *v, double *out, int64_t N, double dx, double nu,
+                     int bc, int use_adv, double adv)
+{
+    /* out_j = sum_i dF_i/dy_j v_i: scatter row i of J into columns */
+    double d2 = nu / (dx * dx);
+    for (int64_t j = 0; j < N; ++j) out[j] = 0.0;
+    for (int64_t i = 0; i < N; ++i) {
+        if (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) continue;
+        int64_t im = (i == 0) ? N - 1 : i - 1;
+        int64_t ip = (i == N - 1) ? 0 : i + 1;
+        double a = use_adv ? adv : y[i];
+        double jm, j0, jp;
+        if (a > 0.0) {
+            jm = a / dx + d2;
+            j0 = -a / dx - (use_adv ? 0.0 : (y[i] - y[im]) / dx) - 2.0 * d2;
+            jp = d2;
+        } else {
+            jm = d2;
+            j0 = a / dx - (use_adv ? 0.0 : (y[ip] - y[i]) / dx) - 2.0 * d2;
+            jp = -a / dx + d2;
+        }
+        out[im] += jm * v[i];
+        out[i] += j0 * v[i];
+        out[ip] += jp * v[i];
+    }
+}
+
+int oracle_rk4_adjoint(const double *u0, double *lam, int64_t B, int64_t N, double L,
+                       const double *nu, const double *dt, int64_t n_steps, int bc, int use_adv,
+                       double adv, int nthreads)
+{
+    if (!u0 || !lam || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 1)
+    for (int64_t b = 0; b < B; ++b) {
+        /* states u^0..u^{n_steps-1}, then 5N (explicit_one) + 3 stage values + 4 kb + ub + yb */
+        double *st = (double *)malloc((size_t)(n_steps + 15) * (size_t)N * sizeof(double));
+        if (!st) {
+#pragma omp atomic write
+            fail = 1;
+            continue;
+        }
+        double *wk = st + (size_t)(n_steps + 1) * N;
+        double *y2 = wk + 5 * N, *y3 = wk + 6 * N, *y4 = wk + 7 * N, *kk = wk + 8 * N;
+        double *kb1 = wk + 9 * N, *kb2 = wk + 10 * N, *kb3 = wk + 11 * N, *kb4 = wk + 12 * N, *yb = wk + 13 * N;
+        double h = dt[b];
+        for (int64_t i = 0; i < N; ++i) st[i] = u0[b * N + i];
+        for (int64_t n = 0; n + 1 < n_steps; ++n) {  /* forward, storing u^0..u^{n_steps-1} */
+            double *cur = st + (size_t)(n + 1) * N;
+            for (int64_t i = 0; i < N; ++i) cur[i] = st[(size_t)n * N + i];
+            explicit_one(cur, N, dx, nu[b], h, 1, bc, SCHEME_RK4, use_adv, adv, wk);
+        }
+        double *ub = lam + b * N;
+        for (int64_t n = n_steps - 1; n >= 0; --n) {
+            const double *u = st + (size_t)n * N;
+            /* the stage values of step n again, exactly as explicit_one forms them */
+            rhs_F(u, kk, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y2[i] = u[i] + 0.5 * h * kk[i];
+            rhs_F(y2, kk, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y3[i] = u[i] + 0.5 * h * kk[i];
+            rhs_F(y3, kk, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) y4[i] = u[i] + h * kk[i];
+            for (int64_t i = 0; i < N; ++i) {
+                kb4[i] = h / 6.0 * ub[i];
+                kb3[i] = h / 3.0 * ub[i];
+                kb2[i] = h / 3.0 * ub[i];
+                kb1[i] = h / 6.0 * ub[i];
+            }
+            rhs_jacT(y4, kb4, yb, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) { ub[i] += yb[i]; kb3[i] += h * yb[i]; }
+            rhs_jacT(y3, kb3, yb, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) { ub[i] += yb[i]; kb2[i] += 0.5 * h * yb[i]; }
+            rhs_jacT(y2, kb2, yb, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) { ub[i] += yb[i]; kb1[i] += 0.5 * h * yb[i]; }
+            rhs_jacT(u, kb1, yb, N, dx, nu[b], bc, use_adv, adv);
+            for (int64_t i = 0; i < N; ++i) ub[i] += yb[i];
+        }
+        free(st);
+    }
+    return fail ? -1 : 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

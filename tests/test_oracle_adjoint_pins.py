@@ -1,5 +1,5 @@
-"""Pins of the oracle's discrete adjoint of forward Euler (D13)
-against the (already pinned) forward oracle: the dot-product identity in the linear case, and central
+"""Pins of the oracle's discrete adjoints of forward Euler (D13) and of classical RK4 (D14)
+ against the (already pinned) forward oracle: the dot-product identity in the linear case, and central
 finite differences of the forward map in the nonlinear case."""
 import numpy as np
 import pytest
@@ -9,45 +9,67 @@ import oracle
 P, D = oracle.PERIODIC, oracle.DIRICHLET
 
 
+SCHEMES = [oracle.EULER, oracle.RK4]
+
+
+@pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("bc", [P, D])
 @pytest.mark.parametrize("adv", [0.9, -0.6])
-def test_linear_case_is_the_exact_transpose(bc, adv):
+def test_linear_case_is_the_exact_transpose(bc, adv, scheme):
     # constant advection speed: u^N = M u^0 with a fixed matrix M, and the adjoint must be M^T:
     # <lam, M v> == <M^T lam, v> for arbitrary v, lam
     rng = np.random.default_rng(1)
     N, L, nu, dt, n = 37, 1.0, 0.02, 0.004, 25
     v, lam = rng.standard_normal(N), rng.standard_normal(N)
-    Mv = oracle.explicit(v, L, nu, dt, n, bc, oracle.EULER, adv=adv)
-    Mt_lam = oracle.explicit_adjoint(v, lam, L, nu, dt, n, bc, adv=adv)
+    Mv = oracle.explicit(v, L, nu, dt, n, bc, scheme, adv=adv)
+    Mt_lam = oracle.explicit_adjoint(v, lam, L, nu, dt, n, bc, adv=adv, scheme=scheme)
     assert abs(lam @ Mv - Mt_lam @ v) <= 1e-13 * (np.abs(lam) @ np.abs(Mv) + 1)
 
 
+@pytest.mark.parametrize("scheme", SCHEMES)
 @pytest.mark.parametrize("bc", [P, D])
-def test_nonlinear_gradient_matches_finite_differences(bc):
+def test_nonlinear_gradient_matches_finite_differences(bc, scheme):
     rng = np.random.default_rng(7)
     N, L, nu, n = 24, 1.0, 0.03, 40
     x = np.arange(N) / N
     u0 = 0.8 + 0.5 * np.sin(2 * np.pi * x) - 1.6 * (x > 0.6)       # both signs, away from zero at the nodes
     assert np.abs(u0).min() > 0.05
-    dt = oracle.dt_from_cfl(u0, L, nu, 0.4, bc)[0]
+    dt = oracle.dt_from_cfl(u0, L, nu, 0.4 if scheme == oracle.EULER else 0.8, bc)[0]
     lam = rng.standard_normal(N)
-    grad = oracle.explicit_adjoint(u0, lam, L, nu, dt, n, bc)
+    grad = oracle.explicit_adjoint(u0, lam, L, nu, dt, n, bc, scheme=scheme)
     # (the map is continuous but has kinks where a node value crosses zero; a +-1e-6 perturbation
     # straddles one only if some node is within ~1e-6 of zero at some step)
     eps = 1e-6
     for j in range(N):
         e = np.zeros(N); e[j] = eps
-        Jp = lam @ oracle.explicit(u0 + e, L, nu, dt, n, bc, oracle.EULER)
-        Jm = lam @ oracle.explicit(u0 - e, L, nu, dt, n, bc, oracle.EULER)
+        Jp = lam @ oracle.explicit(u0 + e, L, nu, dt, n, bc, scheme)
+        Jm = lam @ oracle.explicit(u0 - e, L, nu, dt, n, bc, scheme)
         fd = (Jp - Jm) / (2 * eps)
         assert abs(fd - grad[j]) <= 2e-7 * (1 + np.abs(grad).max()), (j, fd, grad[j])
 
 
-def test_zero_steps_and_batches():
+@pytest.mark.parametrize("scheme", SCHEMES)
+def test_zero_steps_and_batches(scheme):
     rng = np.random.default_rng(2)
     u0 = rng.uniform(0.2, 1.0, (3, 16)); lam = rng.standard_normal((3, 16))
-    np.testing.assert_array_equal(oracle.explicit_adjoint(u0, lam, 1.0, 0.1, 0.001, 0, P), lam)
+    np.testing.assert_array_equal(oracle.explicit_adjoint(u0, lam, 1.0, 0.1, 0.001, 0, P, scheme=scheme), lam)
     nu = np.array([0.05, 0.1, 0.2]); dt = np.array([1e-3, 2e-3, 5e-4])
-    g = oracle.explicit_adjoint(u0, lam, 1.0, nu, dt, 9, P)
+    g = oracle.explicit_adjoint(u0, lam, 1.0, nu, dt, 9, P, scheme=scheme)
     for b in range(3):
-        np.testing.assert_array_equal(g[b], oracle.explicit_adjoint(u0[b], lam[b], 1.0, nu[b], dt[b], 9, P))
+        np.testing.assert_array_equal(g[b], oracle.explicit_adjoint(u0[b], lam[b], 1.0, nu[b], dt[b], 9, P, scheme=scheme))
+
+
+def test_rk4_adjoint_of_one_step_is_the_transposed_step_matrix():
+    """One RK4 step with a constant advection speed is u' = R(dt A) u with R(z) = 1 + z + z^2/2 + z^3/6 + z^4/24
+    and A the (circulant) matrix of the D2 operator: the adjoint of one step must equal R(dt A)^T lam, built here
+    from A assembled column by column with the pinned oracle.rhs -- no oracle adjoint code involved."""
+    rng = np.random.default_rng(11)
+    N, L, nu, dt, adv = 19, 1.0, 0.02, 0.004, 0.7
+    A = np.stack([oracle.rhs(np.eye(N)[j], L, nu, P, adv=adv) for j in range(N)], axis=1)      # A[:, j] = F(e_j)
+    Z = dt * A
+    R = np.eye(N) + Z + Z @ Z / 2 + Z @ Z @ Z / 6 + Z @ Z @ Z @ Z / 24
+    lam = rng.standard_normal(N)
+    got = oracle.explicit_adjoint(rng.standard_normal(N), lam, L, nu, dt, 1, P, adv=adv, scheme=oracle.RK4)
+    np.testing.assert_allclose(got, R.T @ lam, rtol=0, atol=1e-14)
+    got3 = oracle.explicit_adjoint(rng.standard_normal(N), lam, L, nu, dt, 3, P, adv=adv, scheme=oracle.RK4)
+    np.testing.assert_allclose(got3, np.linalg.matrix_power(R.T, 3) @ lam, rtol=0, atol=1e-14)
