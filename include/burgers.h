@@ -176,6 +176,20 @@ int burgers_explicit_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, 
 size_t burgers_adjoint_ckpt_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc,
                                             int64_t n_steps, int64_t segment);
 
+/* The same for either explicit scheme: scheme = BURGERS_SCHEME_EULER (D13) or BURGERS_SCHEME_RK4 -- the discrete
+ * adjoint of the classical RK4 step (D14; PAPER.md:224-229 Eq.22, :231): with G_s = dt dF/dy at the
+ * stage value y_s,  t4 = G4^T lam/6, t3 = G3^T (lam/3 + t4), t2 = G2^T (lam/3 + t3/2), t1 = G1^T (lam/6 + t2/2),
+ * lam <- lam + t4 + t3 + t2 + t1 per step, the stage values rebuilt from the stored (checkpointed) u^n.
+ * segment as above (0 = automatic). */
+int burgers_explicit_adjoint_scheme_f32(const float *u0, float *lam, int64_t B, int64_t N, double L,
+                                        const float *nu, const float *dt, int64_t n_steps, int bc,
+                                        int scheme, int64_t segment, void *ws, size_t ws_bytes, void *stream);
+int burgers_explicit_adjoint_scheme_f64(const double *u0, double *lam, int64_t B, int64_t N, double L,
+                                        const double *nu, const double *dt, int64_t n_steps, int bc,
+                                        int scheme, int64_t segment, void *ws, size_t ws_bytes, void *stream);
+size_t burgers_adjoint_scheme_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int scheme,
+                                              int64_t n_steps, int64_t segment);
+
 /* ---- BTCS (Eq.23; D4-D7) ----------------------
  * Per step solve  A(u^n) u^{n+1} = u^n  with, c_i = u_i^n dt/dx, r = nu dt/dx^2:
  *   sub_i = -r - max(c_i,0),  diag_i = 1 + 2r + |c_i|,  sup_i = -r + min(c_i,0).

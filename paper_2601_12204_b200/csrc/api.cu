@@ -145,26 +145,30 @@ inline int64_t adjoint_segment(size_t esz, int64_t B, int64_t N, int64_t n_steps
     return m < 1 ? 1 : m;
 }
 
+// (RK4: + the stage values and transposed-Jacobian products of the backward sweep, adjoint_rk4.cu)
 template <typename T>
-size_t adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps, int64_t segment) {
+size_t adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps, int64_t segment, int scheme) {
     const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
     const int64_t K = (n_steps + m - 1) / m;
     const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
     const size_t ck = align_up((size_t)(K > 1 ? K - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
     const size_t st = align_up((size_t)(m > 1 ? m - 1 : 0) * (size_t)B * (size_t)N * sizeof(T), 256);
-    return 2 * bn + ck + st + burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc,
-                                                      BURGERS_SCHEME_EULER, BURGERS_PLAN_AUTO);
+    const size_t rk = scheme == BURGERS_SCHEME_RK4 ? align_up(adjoint_rk4_ws_elems(B, N) * sizeof(T), 256) : 0;
+    return 2 * bn + ck + st + rk + burgers_workspace_bytes(BURGERS_OP_EXPLICIT, sizeof(T) == 8, B, N, bc, scheme,
+                                                           BURGERS_PLAN_AUTO);
 }
 
 template <typename T>
 int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
-                 int bc, int64_t segment, void *ws, size_t ws_bytes, void *stream) {
+                 int bc, int64_t segment, void *ws, size_t ws_bytes, void *stream, int scheme = BURGERS_SCHEME_EULER) {
     if (!lam) return BURGERS_ERR_NULL;
     int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
+    if (!scheme_ok(scheme)) return BURGERS_ERR_ENUM;
     if (segment < 0) return BURGERS_ERR_SHAPE;
     if (n_steps == 0) return BURGERS_OK;
-    if (!ws || ws_bytes < adjoint_ws_bytes<T>(B, N, bc, n_steps, segment)) return BURGERS_ERR_WORKSPACE;
+    if (!ws || ws_bytes < adjoint_ws_bytes<T>(B, N, bc, n_steps, segment, scheme)) return BURGERS_ERR_WORKSPACE;
+    const bool rk4 = (scheme == BURGERS_SCHEME_RK4);
     cudaStream_t s = (cudaStream_t)stream;
     const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
     const int64_t K = (n_steps + m - 1) / m;
@@ -177,8 +181,10 @@ int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *n
     T *work = reinterpret_cast<T *>(base + bn);
     T *ckpt = reinterpret_cast<T *>(base + 2 * bn);
     T *seg = reinterpret_cast<T *>(base + 2 * bn + ckb);
-    void *ews = base + 2 * bn + ckb + stb;
-    const size_t ews_bytes = ws_bytes - (2 * bn + ckb + stb);
+    const size_t rkb = rk4 ? align_up(adjoint_rk4_ws_elems(B, N) * sizeof(T), 256) : 0;
+    T *rkws = reinterpret_cast<T *>(base + 2 * bn + ckb + stb);
+    void *ews = base + 2 * bn + ckb + stb + rkb;
+    const size_t ews_bytes = ws_bytes - (2 * bn + ckb + stb + rkb);
     const double dx = grid_dx(N, L, bc);
     auto forward = [&](const T *from, int64_t steps, T *snaps, int64_t every) {
         if (cudaMemcpyAsync(work, from, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
@@ -188,13 +194,12 @@ int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *n
         // N = 4096, 1 000 steps: forward + backward 2.02 -> 1.85 ms.  Same arithmetic per point, same bits.
         int plan_x = BURGERS_PLAN_AUTO, ppt_x = 0;
         ExplicitGeom g8;
-        if (every == 1 && explicit_geometry(sizeof(T) == 8, B, N, bc, BURGERS_SCHEME_EULER, BURGERS_PLAN_RESIDENT, 0, 8,
-                                            &g8) == BURGERS_OK) {
+        if (every == 1 && explicit_geometry(sizeof(T) == 8, B, N, bc, scheme, BURGERS_PLAN_RESIDENT, 0, 8, &g8) == BURGERS_OK) {
             plan_x = BURGERS_PLAN_RESIDENT;
             ppt_x = 8;
         }
-        return explicit_call<T>(work, B, N, L, nu, dt, steps, bc, BURGERS_SCHEME_EULER, plan_x, 0, ppt_x, ews, ews_bytes,
-                                stream, snaps, every);
+        return explicit_call<T>(work, B, N, L, nu, dt, steps, bc, scheme, plan_x, 0, ppt_x, ews, ews_bytes, stream, snaps,
+                                every);
     };
     if (K > 1) {            // checkpoints u^{m}, u^{2m}, ..., u^{(K-1)m}
         st = forward(u0, (K - 1) * m, ckpt, m);
@@ -207,7 +212,8 @@ int adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *n
             st = forward(start, len - 1, seg, 1);
             if (st != BURGERS_OK) return st;
         }
-        st = launch_adjoint_steps<T>(start, seg, lam, pong, B, N, dx, nu, dt, len, bc, s);
+        st = rk4 ? launch_adjoint_rk4_steps<T>(start, seg, lam, rkws, B, N, dx, nu, dt, len, bc, s)
+                 : launch_adjoint_steps<T>(start, seg, lam, pong, B, N, dx, nu, dt, len, bc, s);
         if (st != BURGERS_OK) return st;
     }
     return BURGERS_OK;
@@ -551,9 +557,23 @@ int burgers_explicit_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, 
 }
 size_t burgers_adjoint_ckpt_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps,
                                             int64_t segment) {
-    if (B < 1 || N < 3 || n_steps < 0 || segment < 0) return 0;
-    return dtype_is_f64 ? adjoint_ws_bytes<double>(B, N, bc, n_steps, segment)
-                        : adjoint_ws_bytes<float>(B, N, bc, n_steps, segment);
+    return burgers_adjoint_scheme_workspace_bytes(dtype_is_f64, B, N, bc, BURGERS_SCHEME_EULER, n_steps, segment);
+}
+size_t burgers_adjoint_scheme_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int scheme, int64_t n_steps,
+                                              int64_t segment) {
+    if (B < 1 || N < 3 || n_steps < 0 || segment < 0 || !scheme_ok(scheme)) return 0;
+    return dtype_is_f64 ? adjoint_ws_bytes<double>(B, N, bc, n_steps, segment, scheme)
+                        : adjoint_ws_bytes<float>(B, N, bc, n_steps, segment, scheme);
+}
+int burgers_explicit_adjoint_scheme_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                        const float *dt, int64_t n_steps, int bc, int scheme, int64_t segment, void *ws,
+                                        size_t ws_bytes, void *stream) {
+    return adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream, scheme);
+}
+int burgers_explicit_adjoint_scheme_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                        const double *dt, int64_t n_steps, int bc, int scheme, int64_t segment, void *ws,
+                                        size_t ws_bytes, void *stream) {
+    return adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream, scheme);
 }
 size_t burgers_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
     return burgers_adjoint_ckpt_workspace_bytes(dtype_is_f64, B, N, bc, n_steps, 0);

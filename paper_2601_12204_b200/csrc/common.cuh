@@ -114,6 +114,12 @@ template <typename T>
 int launch_adjoint_steps(const T *u0, const T *states, T *lam, T *pong, int64_t B, int64_t N, double dx,
                          const T *nu, const T *dt, int64_t n_steps, int bc, cudaStream_t s);
 
+// ---------------------------------------------------------------- adjoint of RK4 (adjoint_rk4.cu)
+template <typename T>
+int launch_adjoint_rk4_steps(const T *start, const T *states, T *lam, T *ws, int64_t B, int64_t N, double dx, const T *nu,
+                             const T *dt, int64_t len, int bc, cudaStream_t s);
+size_t adjoint_rk4_ws_elems(int64_t B, int64_t N);
+
 // ---------------------------------------------------------------- Gauss-Seidel BTCS (btcs_gs.cu)
 template <typename T>
 int launch_btcs_gs(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,

@@ -89,3 +89,53 @@ def test_checkpointed_adjoint(B, dtype, tol):
             full = got
         elif dtype == np.float64:
             np.testing.assert_array_equal(got, full)
+
+
+# ---------------------------------------------------------------- adjoint of classical RK4 (D14)
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-10), (np.float32, 1e-4)])
+def test_rk4_adjoint_matches_oracle(B, dtype, tol):
+    """PAPER.md:224-229 (Eq.22), :231: reverse-mode derivative of RK4 steps, against the oracle's adjoint (pinned by the
+    dot-product identity, R(dt A)^T and finite differences).  Shapes: mixed signs periodic, Dirichlet with a ragged N,
+    a grid whose forward pass is TILED, a checkpointed run (segments of 7 steps), C5's pulses."""
+    rng = np.random.default_rng(16)
+    for w, n, seg in ((W.c3_periodic_btcs(B=5, N=512, n_steps=0, dtype=dtype), 40, 0),
+                      (W.c2_dirichlet_batch(B=4, N=1000, dtype=dtype), 25, 0),
+                      (W.c4a_long_explicit(N=(1 << 15) + 8, n_steps=0, dtype=dtype), 12, 0),
+                      (W.c3_periodic_btcs(B=3, N=256, n_steps=0, dtype=dtype), 30, 7),
+                      (W.c5_rk4_ensemble(B=6, N=1024, dtype=dtype), 30, 0)):
+        dt = oracle_dt(w.u0, w.L, w.nu, 0.8, w.bc, dtype)
+        lam_T = rng.standard_normal(w.u0.shape).astype(dtype)
+        ref = oracle.explicit_adjoint(w.u0.astype(np.float64), lam_T.astype(np.float64), w.L, w.nu.astype(np.float64),
+                                      dt.astype(np.float64), n, w.bc, scheme=oracle.RK4)
+        u0 = to_dev(w.u0.copy()); lam = to_dev(lam_T.copy())
+        B.burgers_explicit_adjoint(u0, lam, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, segment=seg, scheme=B.SCHEME_RK4)
+        got = lam.cpu().numpy().astype(np.float64)
+        scale = np.abs(ref).max(axis=1, keepdims=True)
+        assert (np.abs(got - ref) / scale).max() <= tol, (w.name, seg)
+        np.testing.assert_array_equal(u0.cpu().numpy(), w.u0)          # u0 untouched
+
+
+def test_rk4_adjoint_dot_product_identity_with_the_gpu_forward_path(B):
+    """J(u0) = <lam_T, u^N(u0)> with the GPU's own RK4 forward path: its directional derivative along v (central
+    differences) equals <adjoint(lam_T), v>; zero steps leave lam alone; bad scheme -> error."""
+    rng = np.random.default_rng(19)
+    w = W.c3_periodic_btcs(B=2, N=256, n_steps=0)
+    dt = oracle_dt(w.u0, w.L, w.nu, 0.8, w.bc, np.float64)
+    n = 30
+    lam_T = rng.standard_normal(w.u0.shape); v = rng.standard_normal(w.u0.shape)
+    lam = to_dev(lam_T.copy())
+    B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, scheme=B.SCHEME_RK4)
+    g = lam.cpu().numpy()
+    eps = 1e-6
+
+    def J(u0):
+        u = to_dev(u0.copy()); B.burgers_explicit(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc, B.SCHEME_RK4)
+        return (lam_T * u.cpu().numpy()).sum(axis=1)
+    fd = (J(w.u0 + eps * v) - J(w.u0 - eps * v)) / (2 * eps)
+    an = (g * v).sum(axis=1)
+    assert np.all(np.abs(fd - an) <= 1e-6 * (1 + np.abs(an)))
+    lam = to_dev(lam_T.copy())
+    B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 0, w.bc, scheme=B.SCHEME_RK4)
+    np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
+    with pytest.raises(B.BurgersError):
+        B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 3, w.bc, scheme=7)
