@@ -408,7 +408,7 @@ def measure_pipe_peaks(device, pk):
     return out
 
 
-def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None):
+def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None, verbose=True):
     """Dominant kernel = the time-stepping kernel(s) of the op call.  `achieved` = algorithmic work per launch /
     average launch duration (CUDA events around the op call: the kernels run back to back on one stream)."""
     sec = statistics.median(op_ms) * 1e-3
@@ -420,6 +420,8 @@ def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None):
            "avg_launch_us": sig(sec * 1e6 / max(1, launches)),
            "traffic": tr, "traffic_source": f"ncu dram read+write per launch, profiles/ncu_traffic.json @ {traffic.get('commit')}",
            "hbm_accounting_frac": sig(hbm_acc, 4)}
+    if not verbose:            # per-scheme entries: the sources are those of the headline's roofline
+        out.pop("traffic_source")
     if spec["bound"] == "hbm":
         if spec["op"] == "adjoint":          # every stored forward state is written once and read once
             byt = 2 * (w.n_steps - 1) * w.B * w.N * esz
@@ -430,6 +432,8 @@ def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None):
         ach = byt / sec / 1e9
         out.update({"achieved": sig(ach), "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sig(ach / pk["hbm_gbs"], 4),
                     "peak_source": pk["source"] + " (measured copy bandwidth)", "note": note})
+        if not verbose:
+            out.pop("note"); out["peak_source"] = "measured copy"
         if spec["instr"]:
             out["alu_frac"] = sig(ups * spec["instr"] / (SM_COUNT * spec["lanes"] * pk["sm_max_mhz"] * 1e6), 4)
         return out
@@ -440,13 +444,16 @@ def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None):
         chain = pipe["dfma_chain" if pipe_name == "fp64" else "ffma_chain"]["frac_of_nominal"]
         three = pipe["dfma_3reg" if pipe_name == "fp64" else "ffma_3reg"]["frac_of_nominal"]
         src += f"; measured in this run: FMA chain {chain} of it, FMA with 3 register operands {three}"
+    if not verbose:
+        src = f"nominal {pipe_name} issue rate"
     if spec["instr"] is None:                # 8(f) rows without an instruction-count model: time and accounting only
         out.update({"achieved": None, "peak": sig(peak), "unit": "Ginst/s", "frac": None, "peak_source": src})
         return out
     ach = ups * spec["instr"] / 1e9
     out.update({"achieved": sig(ach), "peak": sig(peak), "unit": "Ginst/s", "frac": sig(ach / peak, 4),
-                "peak_source": src,
-                "note": f"{spec['instr']} algorithmic {pipe_name}-pipe instr/update x updates / kernel time"})
+                "peak_source": src, "instr_per_update": spec["instr"]})
+    if verbose:
+        out["note"] = f"{spec['instr']} algorithmic {pipe_name}-pipe instr/update x updates / kernel time"
     return out
 
 
@@ -461,15 +468,16 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     t0 = time.time()
     step_ms, op_ms = r.timed(steps, 0)
     t1 = time.time()
+    ck = sampler.window(t0, t1)
     rec = {"workload": w.name, "dtype": "f32" if w.dtype == np.float32 else "f64", "n_steps": w.n_steps,
            "plan": int(r.plan), "reps": steps, "ms_median": sig(statistics.median(step_ms)),
-           "ms_min": sig(min(step_ms)), "ms_max": sig(max(step_ms)),
+           "ms_min_max": [sig(min(step_ms)), sig(max(step_ms))],
            "updates_per_s": sig(w.updates / (statistics.median(step_ms) * 1e-3)),
            "gpu_launches_per_step": int(r.launches),
-           "roofline": roofline(name, spec, w, op_ms, pk, traffic, r.op_launches, pipe),
-           "clocks": sampler.window(t0, t1)}
+           "roofline": roofline(name, spec, w, op_ms, pk, traffic, r.op_launches, pipe, verbose=False),
+           "clocks": {"sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons")}}
     cfl_ms = max(1e-6, statistics.median(step_ms) - statistics.median(op_ms))
-    rec["cfl"] = {"ms": sig(cfl_ms, 3), "hbm_frac": sig(w.B * w.N * w.u0.dtype.itemsize / (cfl_ms * 1e-3) / 1e9 / pk["hbm_gbs"], 3)}
+    rec["cfl_ms"] = sig(cfl_ms, 3)
     if r.snaps is not None:
         rec["snapshots"] = int(r.snaps.shape[0]); rec["snapshot_bytes"] = int(r.snaps.numel() * r.snaps.element_size())
     if spec["op"] == "gs":
@@ -479,14 +487,16 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
         rec["tol"] = spec["tol"]; rec["theta"] = spec["theta"]
     if e2e_steps:
         e_ms, h2d, d2h = r.e2e(e2e_steps, 1)
-        rec["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3)), "unit": "updates/s",
+        rec["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3)),
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": sig(statistics.median(e_ms))}
     info = {"w": w, "spec": spec, "launches": int(r.launches), "plan": int(r.plan), "step_ms": step_ms}
     del r
     torch.cuda.empty_cache()
     if cpu[0] > 0:
-        rec["cpu_baseline"] = cpu_baseline(w, spec, cpu[0], cpu[1])
+        c = cpu_baseline(w, spec, cpu[0], cpu[1])
+        rec["cpu_baseline"] = {"value": c["value"], "cores": c["cores"], "sample": c["sample"],
+                               "single_thread": c.get("single_thread", {}).get("value")}
     return rec, info
 
 

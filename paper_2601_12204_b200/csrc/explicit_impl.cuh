@@ -37,10 +37,6 @@
 #pragma once
 #include "common.cuh"
 
-#ifndef BURGERS_F64_SCALED
-#define BURGERS_F64_SCALED 0
-#endif
-
 namespace burgers {
 namespace expl {
 
@@ -194,7 +190,7 @@ explicit_kernel(const Params<T> p) {
 
     // per-trajectory constants, evaluated in fp64 and rounded once (ADAPT: set again below, once the
     // state is loaded)
-    constexpr bool SCALED = (sizeof(T) == 4) || BURGERS_F64_SCALED;
+    constexpr bool SCALED = (sizeof(T) == 4);
     const T nu_b = p.nu[b];
     T dt_cur = ADAPT ? T(0) : p.dt[b];
     T cx, rr;
@@ -374,12 +370,6 @@ explicit_kernel(const Params<T> p) {
                 s[j] = raw ? t_fma(v[j], scale, -base[j]) : T(0);
                 v[j] = base[j];
             }
-        } else if (SCALED) {      // (fp64 built with BURGERS_F64_SCALED) w = scale*u, one rounding
-#pragma unroll
-            for (int j = 0; j < P; ++j) {
-                const bool raw = !p.in_scaled || (j == 0 && fixL) || (j == P - 1 && fixR);
-                v[j] = raw ? v[j] * scale : v[j];
-            }
         }
         // One time step.  Fixed dt: the plain loop over it.  ADAPT: segments of adapt_every steps with a
         // CFL evaluation between them (the first dt was set above).
@@ -442,12 +432,6 @@ explicit_kernel(const Params<T> p) {
                     }
                     v[j] = base[j] + s[j];
                 }
-            } else if (SCALED) {
-#pragma unroll
-                for (int j = 0; j < P; ++j) {
-                    if ((j == 0 && fixL) || (j == P - 1 && fixR)) v[j] = ((j == 0) ? keepL : keepR) * scale;
-                    else v[j] = t_fma(v[j], rho_hi, v[j] * rho_lo);
-                }
             }
             seg_end = (steps - n < p.adapt_every) ? steps : n + p.adapt_every;
         }
@@ -458,9 +442,6 @@ explicit_kernel(const Params<T> p) {
                 const T rem = t_fma(-qn, scale, base[j]) + s[j];
                 v[j] = qn + rem / scale;
             }
-        } else if (SCALED && !p.out_scaled) {
-#pragma unroll
-            for (int j = 0; j < P; ++j) v[j] = v[j] / scale;
         }
     } else {  // classical RK4; K_s = dt*F(y_s) (times scale)
         T y[P], acc[P];
