@@ -469,7 +469,7 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     step_ms, op_ms = r.timed(steps, 0)
     t1 = time.time()
     ck = sampler.window(t0, t1)
-    rec = {"workload": w.name, "dtype": "f32" if w.dtype == np.float32 else "f64", "n_steps": w.n_steps,
+    rec = {"dtype": "f32" if w.dtype == np.float32 else "f64", "B": w.B, "N": w.N, "n_steps": w.n_steps,
            "plan": int(r.plan), "reps": steps, "ms_median": sig(statistics.median(step_ms)),
            "ms_min_max": [sig(min(step_ms)), sig(max(step_ms))],
            "updates_per_s": sig(w.updates / (statistics.median(step_ms) * 1e-3)),
@@ -490,6 +490,8 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
         rec["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3)),
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": sig(statistics.median(e_ms))}
+    rec["roofline"].pop("peak_source", None)                      # (as in the headline's roofline)
+    rec["roofline"] = {k: v for k, v in rec["roofline"].items() if v is not None}
     info = {"w": w, "spec": spec, "launches": int(r.launches), "plan": int(r.plan), "step_ms": step_ms}
     del r
     torch.cuda.empty_cache()
@@ -599,7 +601,7 @@ def run_ours(args):
                 extras[name] = {"error": f"{type(ex).__name__}: {ex}"}
         out["schemes"] = extras
         # the fractions again inside a key the driver keeps whole: [ms, bound, frac]
-        out["roofline"]["other_configs"] = {k: [v.get("ms_median"), v["roofline"]["bound"], v["roofline"]["frac"]]
+        out["roofline"]["other_configs"] = {k: [v.get("ms_median"), v["roofline"]["bound"], v["roofline"].get("frac")]
                                             for k, v in extras.items() if "roofline" in v}
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(w, spec, 12.0, 4.0)

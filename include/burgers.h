@@ -256,6 +256,18 @@ int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *
                        int64_t n_steps, int bc, double theta, double tol, int max_iter,
                        int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream);
 
+/* The same with TRAJECTORY output, semantics as burgers_explicit_traj_* / burgers_btcs_traj_*: one run of the AUTO
+ * plan per snapshot interval followed by a device copy into snaps[k][B][N] (room for floor(n_steps/snap_every)
+ * snapshots); iters_out receives the totals over all intervals.  Workspace as for burgers_newton_* (AUTO plan). */
+int burgers_newton_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                            int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                            int64_t *iters_out, int64_t snap_every, float *snaps, void *ws, size_t ws_bytes,
+                            void *stream);
+int burgers_newton_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt,
+                            int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                            int64_t *iters_out, int64_t snap_every, double *snaps, void *ws, size_t ws_bytes,
+                            void *stream);
+
 /* ---- CFL time step (PAPER.md:116-118 Eq.7-8, :287 Eq.24) -----------------------
  * dt_out[b] = C * min(dx / max_i |u[b][i]|, dx^2 / (2 nu[b])), with x/0 = +inf
  * (u == 0 gives the diffusive bound, nu == 0 the convective one, both: +inf).

@@ -32,7 +32,7 @@ EXPORTS = [
     "burgers_adjoint_workspace_bytes", "burgers_explicit_adjoint_ckpt_f32", "burgers_explicit_adjoint_ckpt_f64",
     "burgers_adjoint_ckpt_workspace_bytes", "burgers_explicit_adjoint_scheme_f32", "burgers_explicit_adjoint_scheme_f64",
     "burgers_adjoint_scheme_workspace_bytes", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
-    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
+    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "burgers_newton_traj_f32", "burgers_newton_traj_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64",
     "burgers_solve_host_f32", "burgers_solve_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
@@ -69,6 +69,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"dt_from_cfl_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _f64, _int, _p, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p, _int, _p, _sz, _p]
     getattr(_lib, f"burgers_newton_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_newton_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p, _i64, _p, _p, _sz, _p]
+    getattr(_lib, f"burgers_newton_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_newton_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int, _p]
     getattr(_lib, f"burgers_newton_host_{_sfx}").restype = _int
     getattr(_lib, f"burgers_explicit_host_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _int]
@@ -354,6 +356,35 @@ def burgers_newton(u, L, nu, dt, n_steps, bc, tol=1e-6, max_iter=50, iters_out=N
                                                 int(plan), wsp, wsb, _stream())
     _check(st, f"burgers_newton_{sfx}")
     return u
+
+
+def burgers_newton_traj(u, L, nu, dt, n_steps, bc, snap_every, tol=1e-6, max_iter=50, iters_out=None, snaps=None, ws=None,
+                        theta=1.0):
+    """Newton / theta-scheme stepping with trajectory output (include/burgers.h: burgers_newton_traj_*).
+    Returns (u, snaps) with snaps [n_steps // snap_every][B][N]."""
+    import torch
+    _dev(u, "u"); sfx = _sfx(u)
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    _check_vecs(B, nu=nu, dt=dt)
+    ns = int(n_steps) // int(snap_every) if snap_every >= 1 else 0
+    if snaps is None:
+        snaps = torch.empty((max(ns, 1), B, N), dtype=u.dtype, device=u.device)
+    _dev(snaps, "snaps", u.dtype)
+    if snaps.numel() < ns * B * N:
+        raise ValueError("snaps is too small")
+    ip = None
+    if iters_out is not None:
+        _dev(iters_out, "iters_out", torch.int64)
+        _check_vecs(B, iters_out=iters_out)
+        ip = ctypes.c_void_p(iters_out.data_ptr())
+    need = workspace_bytes(OP_NEWTON, u.dtype == torch.float64, B, N, bc)
+    wsp, wsb, ws = _ws(ws, need, u.device)
+    st = getattr(_lib, f"burgers_newton_traj_{sfx}")(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(),
+                                                     int(n_steps), int(bc), float(theta), float(tol), int(max_iter), ip,
+                                                     int(snap_every), snaps.data_ptr(), wsp, wsb, _stream())
+    _check(st, f"burgers_newton_traj_{sfx}")
+    return u, snaps[:ns]
 
 
 def dt_from_cfl(u, L, nu, C, bc, out=None):

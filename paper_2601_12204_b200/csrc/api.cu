@@ -259,7 +259,7 @@ int gs_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int6
 template <typename T>
 int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
                 double theta, double tol, int max_iter, int64_t *iters_out, int plan, void *ws, size_t ws_bytes,
-                void *stream) {
+                void *stream, bool accumulate = false) {
     int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
     if (!(tol >= 0.0) || max_iter < 0 || !(theta >= 0.0 && theta <= 1.0)) return BURGERS_ERR_VALUE;
@@ -273,7 +273,35 @@ int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, 
     }
     static_assert(sizeof(long long) == sizeof(int64_t), "iters_out is int64");
     return launch_newton<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, theta, tol, max_iter,
-                            reinterpret_cast<long long *>(iters_out), plan, (T *)ws, (cudaStream_t)stream);
+                            reinterpret_cast<long long *>(iters_out), plan, (T *)ws, (cudaStream_t)stream, accumulate);
+}
+
+// Newton / theta-scheme with trajectory output: one run of the plan per snapshot interval (the state is stored once
+// per interval anyway), a device copy of u into snaps[k]; the iteration totals accumulate over the intervals.
+template <typename T>
+int newton_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc, double theta,
+                     double tol, int max_iter, int64_t *iters_out, int64_t snap_every, T *snaps, void *ws, size_t ws_bytes,
+                     void *stream) {
+    if (!snaps) return BURGERS_ERR_NULL;
+    if (snap_every < 1) return BURGERS_ERR_SHAPE;
+    int st = newton_call<T>(u, B, N, L, nu, dt, 0, bc, theta, tol, max_iter, iters_out, BURGERS_PLAN_AUTO, ws, ws_bytes,
+                            stream);                       // validates everything, zeroes iters_out
+    if (st != BURGERS_OK) return st;
+    int64_t done = 0, k = 0;
+    while (done < n_steps) {
+        const int64_t chunk = (n_steps - done < snap_every) ? n_steps - done : snap_every;
+        st = newton_call<T>(u, B, N, L, nu, dt, chunk, bc, theta, tol, max_iter, iters_out, BURGERS_PLAN_AUTO, ws, ws_bytes,
+                            stream, true);
+        if (st != BURGERS_OK) return st;
+        done += chunk;
+        if (chunk == snap_every) {
+            if (cudaMemcpyAsync(snaps + k * B * N, u, (size_t)B * (size_t)N * sizeof(T), cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)stream) != cudaSuccess)
+                return BURGERS_ERR_CUDA;
+            ++k;
+        }
+    }
+    return BURGERS_OK;
 }
 
 template <typename T>
@@ -627,6 +655,19 @@ int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *
                        int64_t n_steps, int bc, double theta, double tol, int max_iter, int64_t *iters_out,
                        int plan, void *ws, size_t ws_bytes, void *stream) {
     return newton_call<double>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, plan, ws, ws_bytes, stream);
+}
+
+int burgers_newton_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt, int64_t n_steps,
+                            int bc, double theta, double tol, int max_iter, int64_t *iters_out, int64_t snap_every,
+                            float *snaps, void *ws, size_t ws_bytes, void *stream) {
+    return newton_traj_call<float>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, snap_every, snaps, ws,
+                                   ws_bytes, stream);
+}
+int burgers_newton_traj_f64(double *u, int64_t B, int64_t N, double L, const double *nu, const double *dt, int64_t n_steps,
+                            int bc, double theta, double tol, int max_iter, int64_t *iters_out, int64_t snap_every,
+                            double *snaps, void *ws, size_t ws_bytes, void *stream) {
+    return newton_traj_call<double>(u, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, snap_every, snaps, ws,
+                                    ws_bytes, stream);
 }
 
 int dt_from_cfl_f32(const float *u, int64_t B, int64_t N, double L, const float *nu, double C, int bc,

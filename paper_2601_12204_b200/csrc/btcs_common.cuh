@@ -291,8 +291,8 @@ inline bool pick_partition(int64_t N, MaxThreads max_threads, int *P_out, int *T
 // Contains CTA barriers: call from uniform control flow.
 template <typename T>
 __device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T> &last, T *sA, T *sC, T *sD,
-                                                T *sF, T &x0, T &xL) {
-    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+                                                T *sF, T &x0, T &xL, const int t, const int Tn) {
+    const int mask = Tn - 1;
     T *sFA = sF, *sFC = sF + Tn, *sFD = sF + 2 * Tn;
     sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
     __syncthreads();

@@ -39,13 +39,112 @@ constexpr int hybrid_max_threads(int bytes, int P) {
     return t;
 }
 
-// RAGGED = false: N == P * blockDim.x, every thread owns P rows (128-bit loads).  RAGGED = true: any N,
-// thread t owns the q or q + 1 rows partition_of() deals it (btcs_common.cuh), scalar loads -- the state
-// is loaded and stored once per CALL, so the load width does not matter.
-template <typename T, int P, bool RAGGED>
+// N == P * blockDim.x: every thread owns P rows, 128-bit loads.  The interface solve is written out here although
+// btcs::solve_interface is the same code: this instance is C3's kernel and the schedule ptxas finds for the
+// shared-helper form is 3 % slower (measured, C3: 15.70 ms inline, 16.16 ms through solve_interface, same 128
+// registers, 608 / 616 instructions; DESIGN.md 6.1 "Instruction schedule").
+template <typename T, int P>
 __global__ void __launch_bounds__(hybrid_max_threads(sizeof(T), P))
 btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                    double inv_dx, int64_t n_steps, int bc) {
+    constexpr int V = 16 / sizeof(T);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (PCR ping-pong)
+    T *sC = sA + 2 * Tn;
+    T *sD = sC + 2 * Tn;
+    T *sFA = sD + 2 * Tn;                     // [Tn] first interface rows (cyclic-reduction step)
+    T *sFC = sFA + Tn;
+    T *sFD = sFC + Tn;
+    T *row = u + (int64_t)blockIdx.x * N + (int64_t)t * P;
+
+    Coef<T> co;
+    co.init(nu[blockIdx.x], dt[blockIdx.x], inv_dx);
+    const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
+    const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
+
+    T v[P];
+#pragma unroll
+    for (int c = 0; c < P / V; ++c) {
+        int4 q4 = *reinterpret_cast<const int4 *>(row + c * V);
+        const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+        for (int k = 0; k < V; ++k) v[c * V + k] = e[k];
+    }
+
+    for (int64_t n = 0; n < n_steps; ++n) {
+        T f[P], c[P], q[P];
+        // ---- assembly + partition elimination
+        Row<T> first, last;
+        eliminate<T, P>(v, co, [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); },
+                        f, c, q, first, last);
+        // ---- cyclic-reduction step: substitute the x_0 rows of threads t and t+1 into the x_L row
+        // of thread t:  [-f A] x_L(t-1) + [1 - f C - c A'] x_L(t) + [-c C'] x_L(t+1) = q - f D - c D'
+        sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
+        __syncthreads();
+        Row<T> r;
+        {
+            const int tn = (t + 1) & mask;
+            const T nA = sFA[tn], nC = sFC[tn], nD = sFD[tn];
+            const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
+            r.A = -last.A * first.A * m;
+            r.C = -last.C * nC * m;
+            r.D = t_fma(-last.A, first.D, t_fma(-last.C, nD, last.D)) * m;
+        }
+        int cur = 0;
+        sA[t] = r.A; sC[t] = r.C; sD[t] = r.D;
+        __syncthreads();
+        // ---- parallel cyclic reduction over the Tn reduced rows (cyclic chain), early exit
+        bool finished = false;
+        for (int s = 1; s < Tn / 2; s <<= 1) {
+            const int km = (t - s) & mask, kp = (t + s) & mask;
+            const T *pA = sA + cur * Tn, *pC = sC + cur * Tn, *pD = sD + cur * Tn;
+            Row<T> rm, rp;
+            rm.A = pA[km]; rm.C = pC[km]; rm.D = pD[km];
+            rp.A = pA[kp]; rp.C = pC[kp]; rp.D = pD[kp];
+            r = pcr_combine(r, rm, rp);
+            const int o = (cur ^ 1) * Tn + t;
+            sA[o] = r.A; sC[o] = r.C; sD[o] = r.D;
+            const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
+            const int any = __syncthreads_or(flag);
+            cur ^= 1;
+            if (!any) { finished = true; break; }
+        }
+        T xL = r.D, xLprev;
+        if (finished) {
+            xLprev = sD[cur * Tn + ((t - 1) & mask)];
+        } else {  // rows t and t + Tn/2 couple only to each other: exact 2x2 solve
+            const int o = (t + Tn / 2) & mask;
+            const T p1 = r.A + r.C, p2 = sA[cur * Tn + o] + sC[cur * Tn + o];
+            const T D2 = sD[cur * Tn + o];
+            xL = t_fma(-p1, D2, r.D) * rcp(t_fma(-p1, p2, T(1)));
+            sD[(cur ^ 1) * Tn + t] = xL;   // the other PCR buffer is free; its next write follows a barrier
+            __syncthreads();
+            xLprev = sD[(cur ^ 1) * Tn + ((t - 1) & mask)];
+        }
+        // ---- recover x_0 and back-substitute
+        const T x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
+        back_substitute<T, P>(v, f, c, q, x0, xL);
+    }
+
+#pragma unroll
+    for (int c = 0; c < P / V; ++c) {
+        int4 q4;
+        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+        for (int k = 0; k < V; ++k) e[k] = v[c * V + k];
+        *reinterpret_cast<int4 *>(row + c * V) = q4;
+    }
+}
+
+// Any N: thread t owns the P - 1 or P rows partition_of() deals it (btcs_common.cuh), scalar loads -- the state
+// is loaded and stored once per CALL, so the load width does not matter.  Same steps as the kernel above, through
+// the shared helpers (eliminate_general_ragged, solve_interface, back_substitute_ragged).
+template <typename T, int P>
+__global__ void __launch_bounds__(hybrid_max_threads(sizeof(T), P))
+btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
+                   double inv_dx, int64_t n_steps, int bc) {
+    constexpr bool RAGGED = true;
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = blockDim.x;
@@ -98,7 +197,7 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
         }
         // ---- cyclic-reduction step + parallel cyclic reduction over the ring of Tn reduced rows
         T x0, xL;
-        solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL);
+        solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL, t, Tn);
         // ---- back substitution
         if (RAGGED) back_substitute_ragged<T, P>(v, n, f, c, q, x0, xL);
         else back_substitute<T, P>(v, f, c, q, x0, xL);
@@ -131,11 +230,11 @@ int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, in
              int Tn, bool ragged, cudaStream_t s) {
     const size_t smem = (size_t)9 * Tn * sizeof(T);
     if (ragged) {
-        btcs_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        btcs_hybrid_ragged_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
-        btcs_hybrid_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        btcs_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
         return last_launch_status();
     }
     return BURGERS_ERR_PLAN;

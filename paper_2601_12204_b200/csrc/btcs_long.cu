@@ -121,11 +121,9 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
     const unsigned stage0 = smem_u32(&stage[0][0]);
     constexpr unsigned kStageBytes = Tn * P * sizeof(T);
 
-    // (point indices inside a row fit 32 bits: btcs_long_fits() limits N; only b * N needs 64)
-    const int Ni = (int)N;
     auto fetch = [&](int b, int tile, int st) {
-        const int wg0 = tile * kW + (warp * 32 - kHaloL) * P;   // first point of the warp region (may be < 0)
-        const bool edge = (wg0 < 0) || (wg0 + 32 * P > Ni);
+        const int64_t wg0 = (int64_t)tile * kW + (int64_t)(warp * 32 - kHaloL) * P;   // first point of the warp region
+        const bool edge = (wg0 < 0) || (wg0 + 32 * P > N);
         const T *srow = src + (int64_t)b * N;
         const unsigned d0 = stage0 + st * kStageBytes;
         if (!edge) {
@@ -135,10 +133,10 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         } else if (aligned) {
 #pragma unroll
             for (int k = 0; k < CR; ++k) {
-                int g = wg0 + (k * 32 + lane) * V;
+                int64_t g = wg0 + (int64_t)(k * 32 + lane) * V;
                 unsigned bytes = 16;
-                if (dirichlet) { if (g < 0 || g >= Ni) { bytes = 0; g = 0; } }
-                else { if (g < 0) g += Ni; else if (g >= Ni) g -= Ni; }
+                if (dirichlet) { if (g < 0 || g >= N) { bytes = 0; g = 0; } }
+                else { if (g < 0) g += N; else if (g >= N) g -= N; }
                 cp_async16(d0 + f_off(k), srow + g, bytes);
             }
         } else {          // N % V != 0: the wrapped (or cut) chunks are not 16-byte pieces of the row any more
@@ -146,10 +144,10 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
             for (int k = 0; k < CR; ++k) {
 #pragma unroll
                 for (int e = 0; e < V; ++e) {
-                    int g = wg0 + (k * 32 + lane) * V + e;
+                    int64_t g = wg0 + (int64_t)(k * 32 + lane) * V + e;
                     unsigned bytes = sizeof(T);
-                    if (dirichlet) { if (g < 0 || g >= Ni) { bytes = 0; g = 0; } }
-                    else { if (g < 0) g += Ni; else if (g >= Ni) g -= Ni; }
+                    if (dirichlet) { if (g < 0 || g >= N) { bytes = 0; g = 0; } }
+                    else { if (g < 0) g += N; else if (g >= N) g -= N; }
                     cp_async_elem<sizeof(T)>(d0 + f_off(k) + e * sizeof(T), srow + g, bytes);
                 }
             }
@@ -168,7 +166,7 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         else cp_async_wait<0>();
         __syncwarp();
 
-        const int g0 = tile * kW + (t - kHaloL) * P;     // unwrapped index of row 0
+        const int64_t g0 = (int64_t)tile * kW + (int64_t)(t - kHaloL) * P;     // unwrapped index of row 0
         Coef<T> co;
         co.init(nu[b], dt[b], inv_dx);
 
@@ -187,8 +185,8 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         // ---- assembly + partition elimination
         T f[P], c[P], q[P];
         Row<T> first, last;
-        if (dirichlet && (g0 <= 0 || g0 + P >= Ni)) {
-            eliminate<T, P>(v, co, [&](int j) { return g0 + j <= 0 || g0 + j >= Ni - 1; }, f, c, q, first, last);
+        if (dirichlet && (g0 <= 0 || g0 + P >= N)) {
+            eliminate<T, P>(v, co, [&](int j) { return g0 + j <= 0 || g0 + j >= N - 1; }, f, c, q, first, last);
         } else {
             eliminate<T, P>(v, co, [](int) { return false; }, f, c, q, first, last);
         }
@@ -256,35 +254,23 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         }
         __syncwarp();
         {
-            const int wg0 = tile * kW + (warp * 32 - kHaloL) * P;
+            const int64_t wg0 = (int64_t)tile * kW + (int64_t)(warp * 32 - kHaloL) * P;
             T *drow = dst + (int64_t)b * N;
             const unsigned s0 = stage0 + st * kStageBytes;
-            const int lo = kHaloL - warp * 32, hi = Tn - kHaloR - warp * 32;   // owned rows of this warp: [lo, hi)
-            if (lo <= 0 && hi >= 32 && wg0 >= 0 && wg0 + 32 * P <= Ni) {
-                // interior warp of an interior tile: every chunk is owned and inside the row
-                T *g = drow + wg0 + lane * V;
 #pragma unroll
-                for (int k = 0; k < CR; ++k) {
+            for (int k = 0; k < CR; ++k) {
+                const int rt = warp * 32 + (k * 32 + lane) / CR;            // thread that owns this chunk's row
+                const int64_t g = wg0 + (int64_t)(k * 32 + lane) * V;
+                if (rt >= kHaloL && rt < Tn - kHaloR && g < N) {
                     int4 q4;
                     asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(q4.x), "=r"(q4.y), "=r"(q4.z), "=r"(q4.w) : "r"(s0 + f_off(k)));
-                    *reinterpret_cast<int4 *>(g + k * 32 * V) = q4;
-                }
-            } else {
+                    if (g + V <= N) {
+                        *reinterpret_cast<int4 *>(drow + g) = q4;
+                    } else {                   // the chunk that straddles the end of a grid with N % V != 0
+                        const T *e = reinterpret_cast<const T *>(&q4);
 #pragma unroll
-                for (int k = 0; k < CR; ++k) {
-                    const int rl = (k * 32 + lane) / CR;                  // row of this chunk inside the warp region
-                    const int g = wg0 + (k * 32 + lane) * V;
-                    if (rl >= lo && rl < hi && g < Ni) {
-                        int4 q4;
-                        asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(q4.x), "=r"(q4.y), "=r"(q4.z), "=r"(q4.w) : "r"(s0 + f_off(k)));
-                        if (g + V <= Ni) {
-                            *reinterpret_cast<int4 *>(drow + g) = q4;
-                        } else {               // the chunk that straddles the end of a grid with N % V != 0
-                            const T *e = reinterpret_cast<const T *>(&q4);
-#pragma unroll
-                            for (int k2 = 0; k2 < V; ++k2)
-                                if (g + k2 < Ni) drow[g + k2] = e[k2];
-                        }
+                        for (int k2 = 0; k2 < V; ++k2)
+                            if (g + k2 < N) drow[g + k2] = e[k2];
                     }
                 }
             }

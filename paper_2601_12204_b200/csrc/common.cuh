@@ -129,7 +129,8 @@ size_t btcs_gs_ws_elems(int64_t B, int64_t N);
 // ---------------------------------------------------------------- Newton BTCS (newton.cu)
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s);
+                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s,
+                  bool accumulate = false);
 bool newton_hybrid_fits(int is_f64, int64_t N);
 size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc);
 

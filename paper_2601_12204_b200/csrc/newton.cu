@@ -132,7 +132,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             if (RAGGED) eliminate_general_ragged<T, P>(jac, n, q, f, c, first, last);
             else eliminate_general<T, P>(jac, q, f, c, first, last);
             T x0, xL;
-            solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL);
+            solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL, t, Tn);
             T d[P];
 #pragma unroll
             for (int j = 0; j < P; ++j) d[j] = T(0);
@@ -144,7 +144,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             ++iters;
         }
     }
-    if (iters_out && t == 0) iters_out[blockIdx.x] = iters;
+    if (iters_out && t == 0) iters_out[blockIdx.x] += iters;     // (zeroed by launch_newton unless it accumulates)
 
     if (RAGGED) {
 #pragma unroll
@@ -288,7 +288,7 @@ newton_thomas_kernel(T *__restrict__ un, T *__restrict__ w, T *__restrict__ cp, 
         for (int64_t i = 0; i < N; ++i) AT(un, i) = AT(w, i);
     }
 #undef AT
-    if (iters_out) iters_out[b] = iters;
+    if (iters_out) iters_out[b] += iters;
 }
 
 }  // namespace
@@ -304,12 +304,12 @@ size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc) {
 
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s) {
-    if (n_steps == 0) {
-        if (iters_out && cudaMemsetAsync(iters_out, 0, (size_t)B * sizeof(long long), s) != cudaSuccess)
-            return BURGERS_ERR_CUDA;
-        return BURGERS_OK;
-    }
+                  double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s,
+                  bool accumulate) {
+    // the kernels ADD their iteration totals to iters_out (trajectory output calls this once per interval)
+    if (iters_out && !accumulate && cudaMemsetAsync(iters_out, 0, (size_t)B * sizeof(long long), s) != cudaSuccess)
+        return BURGERS_ERR_CUDA;
+    if (n_steps == 0) return BURGERS_OK;
     if (plan == BURGERS_PLAN_HYBRID) {
         int P, Tn;
         bool ragged;
@@ -339,7 +339,7 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
     return launch_transpose<T>(un, u, N, B, s);
 }
 
-template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t);
-template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, double, int, long long *, int, double *, cudaStream_t);
+template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t, bool);
+template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, double, int, long long *, int, double *, cudaStream_t, bool);
 
 }  // namespace burgers

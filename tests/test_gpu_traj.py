@@ -79,3 +79,30 @@ def test_btcs_trajectory(B):
             assert rel_err(snaps[k].cpu().numpy(), ref, w.u0) <= 1e-10, (w.name, k)
         ref = oracle.btcs(ref, w.L, w.nu, dt, n - (n // every) * every, w.bc)
         assert rel_err(u.cpu().numpy(), ref, w.u0) <= 1e-10
+
+
+@pytest.mark.parametrize("theta", [1.0, 0.5])
+def test_newton_trajectory_snapshots(B, theta):
+    """burgers_newton_traj_*: snapshots of the Newton / Crank-Nicolson scheme every m steps equal the oracle's states
+    after m, 2m, ... steps (the oracle called interval by interval: the same composition), the iteration totals are
+    those of the single call, resident ragged (N = 201) and exact (N = 512) plans, Dirichlet and periodic."""
+    import torch
+    for w in (W.c3_periodic_btcs(B=5, N=512, n_steps=0), W.c2_dirichlet_batch(B=4, N=201, dtype=np.float64)):
+        nu = np.full(w.B, 0.1)                                     # cell Peclet number below 2 (D11)
+        dt = oracle.dt_from_cfl(w.u0, w.L, nu, 2.0, w.bc)
+        n, m = 23, 5
+        u = to_dev(w.u0.copy()); it = torch.zeros(w.B, dtype=torch.int64, device="cuda")
+        _, snaps = B.burgers_newton_traj(u, w.L, to_dev(nu), to_dev(dt), n, w.bc, m, tol=1e-12, iters_out=it, theta=theta)
+        assert tuple(snaps.shape) == (4, w.B, w.N)
+        ref = w.u0.copy(); tot = np.zeros(w.B, dtype=np.int64)
+        for k in range(4):
+            ref, itr = oracle.newton_btcs(ref, w.L, nu, dt, m, w.bc, tol=1e-12, theta=theta, return_iters=True)
+            tot += itr
+            assert rel_err(snaps[k].cpu().numpy(), ref, w.u0) <= 1e-10, (w.name, k)
+        ref, itr = oracle.newton_btcs(ref, w.L, nu, dt, n - 4 * m, w.bc, tol=1e-12, theta=theta, return_iters=True)
+        tot += itr
+        assert rel_err(u.cpu().numpy(), ref, w.u0) <= 1e-10
+        u1 = to_dev(w.u0.copy()); it1 = torch.zeros(w.B, dtype=torch.int64, device="cuda")
+        B.burgers_newton(u1, w.L, to_dev(nu), to_dev(dt), n, w.bc, tol=1e-12, iters_out=it1, theta=theta)
+        assert torch.equal(u1, u) and torch.equal(it1, it)          # the composition is bitwise the single call
+        assert np.all(np.abs(it.cpu().numpy() - tot) <= 2)
