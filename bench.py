@@ -51,6 +51,7 @@ BACKEND = "nccl"            # torch.distributed backend of the timing barrier / 
 RUNNER = None               # class with GpuRunner's interface; None -> GpuRunner
 HOT = ("c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5")
 NEXT = ("c3_newton", "c3_cn", "c2_traj", "c3_gs", "c2_adjoint")
+MORE = ("c5_adjoint",)                                                    # --workload only (not in the default table)
 WORKLOADS = HOT + NEXT
 
 
@@ -108,6 +109,11 @@ def make_workload(name, rank=0, world=1, reduced=False):
         w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
                                  n_steps=100 if reduced else 1000)
         return w, dict(op="adjoint", scheme=0, bound="hbm", instr=None, lanes=FP32_LANES)
+    if name == "c5_adjoint":     # adjoint of 100 RK4 steps of 4096 of C5's pulses (D14; streaming backward sweep)
+        Bg = 4096 * world
+        w = W.c5_rk4_ensemble(B=65536 * world, rows=np.arange(0, 65536 * world, 16)[W.shard_rows(Bg, rank, world)],
+                              n_steps=10 if reduced else 100)
+        return w, dict(op="adjoint", scheme=1, bound="hbm", instr=None, lanes=FP32_LANES)
     if name == "c2_traj":        # SURVEY 8(f) NEXT-4b: C2 fp32 with a snapshot of all trajectories every 50 steps
         Bg = 1024 * world
         w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
@@ -199,7 +205,8 @@ def metric_name(spec):
     if spec["op"] == "explicit":
         return base + ("forward Euler upwind/central" if spec["scheme"] == 0 else "RK4")
     return base + {"btcs": "BTCS", "newton": "Newton BTCS (central convection, theta-scheme)",
-                   "gs": "Gauss-Seidel BTCS", "adjoint": "adjoint of forward Euler"}[spec["op"]]
+                   "gs": "Gauss-Seidel BTCS",
+                   "adjoint": "adjoint of forward Euler" if spec["scheme"] == 0 else "adjoint of RK4"}[spec["op"]]
 
 
 # ------------------------------------------------------------------------------- oracle leg
@@ -222,7 +229,7 @@ def oracle_sample_run(w, spec, target_s=12.0, threads=None):
                            threads=threads)
         elif spec["op"] == "adjoint":
             lam = np.random.default_rng(1220404).standard_normal(u0[rows].shape)
-            oracle.explicit_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+            oracle.explicit_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads, scheme=spec["scheme"])
         elif spec["op"] == "newton":
             oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
                                max_iter=spec["max_iter"], threads=threads, theta=spec["theta"])
@@ -277,8 +284,9 @@ class GpuRunner:
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
         elif spec["op"] == "adjoint":
             self.plan = 0
-            need = int(B.raw().burgers_adjoint_workspace_bytes(int(is64), w.B, w.N, w.bc, w.n_steps))
-            self.launches = 2          # forward trajectory kernel + resident backward kernel
+            need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, spec["scheme"], w.n_steps, 0))
+            # Euler: forward trajectory kernel + resident backward kernel; RK4: forward + 7 launches per step
+            self.launches = 2 if spec["scheme"] == 0 else 1 + 7 * w.n_steps
             self.lam0 = torch.randn(self.u0.shape, dtype=self.u0.dtype, device=device,
                                     generator=torch.Generator(device=device).manual_seed(1220404))
         elif spec["op"] == "gs":
@@ -319,7 +327,8 @@ class GpuRunner:
         elif self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
         elif self.spec["op"] == "adjoint":
-            B.burgers_explicit_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
+            B.burgers_explicit_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws,
+                                       scheme=self.spec["scheme"])
         elif self.spec["op"] == "gs":
             B.burgers_btcs_gs(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, tol=self.spec["tol"],
                               max_iter=self.spec["max_iter"], iters_out=self.iters, ws=self.ws)
@@ -364,7 +373,7 @@ class GpuRunner:
                                       max_iter=self.spec["max_iter"], ws=self.ws)
                 else:                                  # (the seed lambda is already on the device)
                     dl = self.lam0.clone()
-                    B.burgers_explicit_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws)
+                    B.burgers_explicit_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws, scheme=self.spec["scheme"])
                     du = dl
                 hu.copy_(du); torch.cuda.synchronize()
             elif self.spec["op"] == "newton":
@@ -689,7 +698,7 @@ def main(argv=None):
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c2_f32", choices=list(WORKLOADS))
+    ap.add_argument("--workload", default="c2_f32", choices=list(WORKLOADS + MORE))
     ap.add_argument("--no-extras", action="store_true", help="skip the per-scheme table of the other configs")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline legs")
     ap.add_argument("--reduced", action="store_true", help="10x fewer time steps per bench step (debug only)")
