@@ -500,13 +500,15 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": sig(statistics.median(e_ms))}
     rec["roofline"].pop("peak_source", None)                      # (as in the headline's roofline)
+    rec["roofline"].pop("kernel_launches", None)                  # (= gpu_launches_per_step minus the CFL launches)
     rec["roofline"] = {k: v for k, v in rec["roofline"].items() if v is not None}
     info = {"w": w, "spec": spec, "launches": int(r.launches), "plan": int(r.plan), "step_ms": step_ms}
     del r
     torch.cuda.empty_cache()
     if cpu[0] > 0:
         c = cpu_baseline(w, spec, cpu[0], cpu[1])
-        rec["cpu_baseline"] = {"value": c["value"], "cores": c["cores"], "sample": c["sample"],
+        rec["cpu_baseline"] = {"value": c["value"], "cores": c["cores"],
+                               "sample": c["sample"].replace("trajectories", "traj").replace(" of the full", " of the"),
                                "single_thread": c.get("single_thread", {}).get("value")}
     return rec, info
 
@@ -577,7 +579,7 @@ def run_ours(args):
                                f"bc={'periodic' if w.bc == 0 else 'dirichlet'}, CFL {w.cfl}",
                    "B_per_gpu": w.B, "N": w.N, "n_steps": w.n_steps, "plan": int(r.plan),
                    "parallelism": f"batch-sharded x{world} (no collective)" if world > 1 else "single GPU",
-                   "l2": "flushed between timed steps (512 MiB memset outside the event pairs)",
+                   "l2": "flushed between timed steps (512 MiB memset)",
                    "input_sha256": w.sha256()[:16]},
         "gpu_launches": int(r.launches * args.steps),
         "clocks": clocks,
@@ -588,7 +590,7 @@ def run_ours(args):
         out["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3), 6), "unit": "updates/s",
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": sig(statistics.median(e_ms)),
-                      "note": "burgers_solve_host_*: pinned host buffers in, one upload, CFL + stepping on the device, one download; rank 0"}
+                      "note": "burgers_solve_host_*: pinned host buffers, upload + CFL + stepping + download; rank 0"}
         cfl_ms = max(1e-6, statistics.median(step_ms) - statistics.median(op_ms))
         out["cfl"] = {"ms": sig(cfl_ms, 3), "hbm_frac": sig(w.B * w.N * w.u0.dtype.itemsize / (cfl_ms * 1e-3) / 1e9 / pk["hbm_gbs"], 3)}
         out["pipe_peaks"] = pipe
