@@ -77,11 +77,19 @@ def peaks():
 def ncu_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of each time-stepping kernel, from the
     `ncu --set full` captures summarised under profiles/ (the file names the commit they were taken at)."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    out = {"commit": None, "bytes_per_launch": {}}
     try:
-        return json.load(open(path))
+        for line in open(path):
+            line = line.strip()
+            if line.startswith("# commit:"):
+                out["commit"] = line.split(":", 1)[1].strip()
+            elif line and not line.startswith("#") and not line.startswith("workload"):
+                k, v = line.split(",")
+                out["bytes_per_launch"][k] = float(v)
     except (OSError, ValueError):
-        return {"commit": None, "bytes_per_launch": {}}
+        pass
+    return out
 
 
 # ------------------------------------------------------------------------------- workloads
@@ -427,7 +435,7 @@ def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None, verbose=Tru
     tr = traffic.get("bytes_per_launch", {}).get(name)
     out = {"bound": spec["bound"], "kernel_launches": int(launches),
            "avg_launch_us": sig(sec * 1e6 / max(1, launches)),
-           "traffic": tr, "traffic_source": f"ncu dram read+write per launch, profiles/ncu_traffic.json @ {traffic.get('commit')}",
+           "traffic": tr, "traffic_source": f"ncu dram read+write per launch, profiles/ncu_traffic.csv @ {traffic.get('commit')}",
            "hbm_accounting_frac": sig(hbm_acc, 4)}
     if not verbose:            # per-scheme entries: the sources are those of the headline's roofline
         out.pop("traffic_source")
