@@ -217,3 +217,20 @@ def test_plain_c_client_compiles_links_and_runs(tmp_path):
     r = subprocess.run([exe], capture_output=True, text=True)
     assert r.returncode == 0, r.stdout + r.stderr
     assert r.stdout.startswith("version ") and r.stdout.strip().endswith("bad 0")
+
+
+def test_binding_rejects_short_per_trajectory_arrays_before_the_library_is_called(B):
+    """ADVICE r01: a nu / dt / iters_out array shorter than B would be read or written out of bounds on the device;
+    every binding entry point checks the lengths first (host entry points can be checked without a GPU)."""
+    import numpy as np
+    u = np.zeros((3, 16)); ok = np.ones(3); short = np.ones(2)
+    for call in (lambda: B.burgers_explicit_host(u, 1.0, short, ok, 1, 0, 0),
+                 lambda: B.burgers_explicit_host(u, 1.0, ok, short, 1, 0, 0),
+                 lambda: B.burgers_btcs_host(u, 1.0, ok, short, 1, 0),
+                 lambda: B.burgers_newton_host(u, 1.0, short, ok, 1, 0),
+                 lambda: B.burgers_solve_host(u, 1.0, short, 0.4, 1, 0),
+                 lambda: B.dt_from_cfl_host(u, 1.0, short, 0.4, 0)):
+        with pytest.raises(ValueError, match="length B"):
+            call()
+    with pytest.raises(TypeError):                       # device entry points refuse host arrays (no CPU fallback)
+        B.burgers_explicit(u, 1.0, ok, ok, 1, 0, 0)

@@ -262,6 +262,26 @@ def test_btcs_any_grid_length_across_ctas(B, dtype, shape):
                 assert rel_err(got, ref, u0) <= TOL[np.dtype(dtype)], (shape, bc, C, plan)
 
 
+@pytest.mark.parametrize("shape", [(1, 5121), (2, 6000), (1, 7001), (5, 4098), (3, 5120)])
+def test_btcs_sizes_around_the_hybrid_long_boundary(B, shape):
+    """fp64 systems just above what one CTA holds (HYBRID: N <= 5120 on 512 threads x 10 slots) run LONG with only
+    three or four tiles, whose halos wrap around the ring; just below, HYBRID with 512 threads."""
+    Bn, N = shape
+    rng = np.random.default_rng(N)
+    for bc, L in ((B.BC_PERIODIC, 2 * math.pi), (B.BC_DIRICHLET, 1.0)):
+        plan = B.plan_query(B.OP_BTCS, True, Bn, N, bc)
+        assert plan == (B.PLAN_HYBRID if N <= 5120 else B.PLAN_LONG), (shape, plan)
+        x = np.arange(N) / N
+        u0 = np.stack([a * np.sin(2 * math.pi * k * x + p) + m for a, k, p, m in
+                       zip(rng.uniform(0.5, 2, Bn), (1, 3, 7, 2, 5), rng.uniform(0, 6, Bn), (-0.4, 0.0, 1.0, 0.3, -1.0))])
+        nu = rng.uniform(0.01, 0.1, Bn)
+        for C in (10.0, 3000.0):
+            dt = oracle_dt(u0, L, nu, C, bc, np.float64)
+            ref = oracle.btcs(u0, L, nu, dt, 5, bc)
+            got = run_btcs(B, u0, L, nu, dt, 5, bc)
+            assert rel_err(got, ref, u0) <= 1e-10, (shape, bc, C)
+
+
 def test_btcs_long_grid_of_four_million_and_forty_points(B):
     """N = 2^22 + 40 (the size VERDICT r01 names), fp64, periodic, C4b's profile and time step: the whole grid
     against the oracle after 6 steps."""
