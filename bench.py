@@ -413,7 +413,7 @@ def measure_pipe_peaks(device, pk):
     out = {}
     for k, name in enumerate(B.PEAK_KINDS):
         nominal = SM_COUNT * (FP32_LANES if k < 3 else FP64_LANES) * pk["sm_max_mhz"] * 1e6
-        iters = 2000 if k < 3 else 1000
+        iters = 2000 if k < 3 else 1000          # (kind 6, DFMA + select mix: fraction of the FP64 rate left to the DFMAs)
         B.pipe_peak(k, 50, sink)
         torch.cuda.synchronize()
         best = 0.0

@@ -332,14 +332,16 @@ int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int
  *   BURGERS_PEAK_FFMA_CHAIN  a = fma(a, x, y), shared constant operands (operand-reuse cache): issue rate
  *   BURGERS_PEAK_FFMA_3REG   a = fma(a, b, c), three distinct registers: register-operand bandwidth
  *   BURGERS_PEAK_FADD_2REG   a = a + b
- *   BURGERS_PEAK_DFMA_CHAIN / _DFMA_3REG / _DADD_2REG: the same in fp64.
+ *   BURGERS_PEAK_DFMA_CHAIN / _DFMA_3REG / _DADD_2REG: the same in fp64;
+ *   BURGERS_PEAK_DFMA_SELECT_MIX  5 DFMA chains and one FSETP + 2 FSEL per round (the mix of the fp64
+ *                            upwind stencil); only the DFMAs are counted.
  * The caller times the launch (CUDA events on `stream`); *lane_instr_out (HOST pointer, may be NULL)
  * receives the lane-instructions executed = threads x 64 x iters.  sink: DEVICE pointer to 8 writable
  * bytes (never written in practice).  Computes nothing of the method. */
 enum {
     BURGERS_PEAK_FFMA_CHAIN = 0, BURGERS_PEAK_FFMA_3REG = 1, BURGERS_PEAK_FADD_2REG = 2,
     BURGERS_PEAK_DFMA_CHAIN = 3, BURGERS_PEAK_DFMA_3REG = 4, BURGERS_PEAK_DADD_2REG = 5,
-    BURGERS_PEAK_KINDS = 6
+    BURGERS_PEAK_DFMA_SELECT_MIX = 6, BURGERS_PEAK_KINDS = 7
 };
 int burgers_pipe_peak(int kind, int64_t iters, void *sink, void *stream, double *lane_instr_out);
 

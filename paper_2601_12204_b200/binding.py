@@ -403,7 +403,7 @@ def dt_from_cfl(u, L, nu, C, bc, out=None):
     return out
 
 
-PEAK_KINDS = ("ffma_chain", "ffma_3reg", "fadd_2reg", "dfma_chain", "dfma_3reg", "dadd_2reg")
+PEAK_KINDS = ("ffma_chain", "ffma_3reg", "fadd_2reg", "dfma_chain", "dfma_3reg", "dadd_2reg", "dfma_select_mix")
 
 
 def pipe_peak(kind, iters, sink):

@@ -12,6 +12,9 @@
 //                reads per instruction -- what register-operand bandwidth allows
 //   FADD_2REG    a_k = a_k + b_k: two register reads per instruction
 //   DFMA_CHAIN / DFMA_3REG / DADD_2REG: the same on the FP64 pipe
+//   DFMA_SELECT_MIX  per round 5 independent DFMA chains and one "64-bit select" (FSETP + 2 FSEL), the instruction
+//                mix of the fp64 upwind stencil per update: how much of the FP64 rate is left when ALU-pipe
+//                instructions are issued in between (only the DFMAs are counted)
 #include "common.cuh"
 
 namespace burgers {
@@ -45,6 +48,33 @@ __global__ void __launch_bounds__(kBlock) pipe_peak_kernel(T *sink, long long it
     if (s == T(-123.456)) *sink = s;       // never true for the finite chains above; keeps the loop alive
 }
 
+__global__ void __launch_bounds__(kBlock) pipe_mix_kernel(double *sink, long long iters, double x, double y, float fx) {
+    double a[5];
+    float f[4], g[3];
+#pragma unroll
+    for (int k = 0; k < 5; ++k) a[k] = x + double(threadIdx.x + k);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) f[k] = fx + float(k);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) g[k] = fx - float(threadIdx.x + k);
+    for (long long i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int r = 0; r < kUnroll; ++r) {
+#pragma unroll
+            for (int k = 0; k < 5; ++k) a[k] = fma(a[k], x, y);
+            // one "64-bit select": a predicate from the sign test and the two 32-bit halves (FSETP + 2 FSEL)
+            const bool p = f[0] > fx;
+            const float lo = p ? f[1] : g[0], hi = p ? f[2] : g[1];
+            f[0] = lo; f[1] = hi;
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 5; ++k) s += a[k];
+    s += f[0] + f[1] + f[2];
+    if (s == -123.456) *sink = s;
+}
+
 template <typename T>
 int launch_kind(int kind, T *sink, long long iters, int grid, cudaStream_t s) {
     // x slightly below 1 and y tiny: |a| decays towards y/(1-x), no overflow, no denormals
@@ -71,8 +101,13 @@ extern "C" int burgers_pipe_peak(int kind, int64_t iters, void *sink, void *stre
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return BURGERS_ERR_CUDA;
     const int grid = sms * (2048 / kBlock);            // every SM at full occupancy, one wave
-    if (lane_instr_out) *lane_instr_out = (double)grid * kBlock * kAcc * kUnroll * (double)iters;
     cudaStream_t s = (cudaStream_t)stream;
+    if (kind == BURGERS_PEAK_DFMA_SELECT_MIX) {
+        if (lane_instr_out) *lane_instr_out = (double)grid * kBlock * 5 * kUnroll * (double)iters;
+        pipe_mix_kernel<<<grid, kBlock, 0, s>>>((double *)sink, iters, 0.999, 1e-3, 1.0001f);
+        return last_launch_status();
+    }
+    if (lane_instr_out) *lane_instr_out = (double)grid * kBlock * kAcc * kUnroll * (double)iters;
     return kind < 3 ? launch_kind<float>(kind, (float *)sink, iters, grid, s)
                     : launch_kind<double>(kind - 3, (double *)sink, iters, grid, s);
 }
