@@ -265,6 +265,25 @@ def test_guard_bands_other_entry_points(B, dtype):
             assert rel_err(got, direct, w.u0) <= 30 * gtol
             first = got if first is None else first
             np.testing.assert_array_equal(got, first)
+    # ---- adjoint of RK4: resident backward kernel (eight single-barrier exchanges per step), checkpointed, streaming
+    for w, seg in ((W.c5_rk4_ensemble(B=3, N=1024, dtype=dtype), 0), (W.c2_dirichlet_batch(B=3, N=1000, dtype=dtype), 4),
+                   (W.c4a_long_explicit(N=40000, dtype=dtype), 0)):
+        dt = _dt(w, 0.8)
+        lam_T = rng.standard_normal(w.u0.shape).astype(dtype)
+        need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, 1, 10, seg))
+        ref = oracle.explicit_adjoint(_f64(w.u0), _f64(lam_T), w.L, _f64(w.nu), _f64(dt), 10, w.bc, scheme=oracle.RK4)
+        first = None
+        for _ in range(3):
+            gu, u = guarded_from(w.u0); gl, lam = guarded_from(lam_T); gw, ws = guarded_empty(need)
+            B.burgers_explicit_adjoint(u, lam, w.L, torch.from_numpy(w.nu).cuda(), torch.from_numpy(dt).cuda(), 10, w.bc,
+                                       ws=ws, segment=seg, scheme=B.SCHEME_RK4)
+            torch.cuda.synchronize()
+            assert gu.intact() and gl.intact() and gw.intact()
+            np.testing.assert_array_equal(u.cpu().numpy(), w.u0)
+            got = lam.cpu().numpy()
+            assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
+            first = got if first is None else first
+            np.testing.assert_array_equal(got, first)
     # ---- adjoint of forward Euler
     for w, seg in ((W.c2_dirichlet_batch(B=3, N=4096, dtype=dtype), 0), (W.c3_periodic_btcs(B=3, N=1024, dtype=dtype), 5),
                    (W.c4a_long_explicit(N=40000, dtype=dtype), 0)):
