@@ -493,6 +493,8 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
            "gpu_launches_per_step": int(r.launches),
            "roofline": roofline(name, spec, w, op_ms, pk, traffic, r.op_launches, pipe, verbose=False),
            "clocks": {"sm_mhz": ck.get("sm_mhz"), "reasons": ck.get("reasons")}}
+    if not rec["clocks"]["reasons"]:
+        rec["clocks"] = {"sm_mhz": ck.get("sm_mhz")}            # (no throttle reason in this config's window)
     cfl_ms = max(1e-6, statistics.median(step_ms) - statistics.median(op_ms))
     rec["cfl_ms"] = sig(cfl_ms, 3)
     if r.snaps is not None:
@@ -509,6 +511,8 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
                       "ms_per_step": sig(statistics.median(e_ms))}
     rec["roofline"].pop("peak_source", None)                      # (as in the headline's roofline)
     rec["roofline"].pop("kernel_launches", None)                  # (= gpu_launches_per_step minus the CFL launches)
+    if rec["roofline"].get("bound") == "hbm":
+        rec["roofline"].pop("hbm_accounting_frac", None)          # (= frac)
     rec["roofline"] = {k: v for k, v in rec["roofline"].items() if v is not None}
     info = {"w": w, "spec": spec, "launches": int(r.launches), "plan": int(r.plan), "step_ms": step_ms}
     del r
