@@ -502,8 +502,14 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     if spec["op"] == "gs":
         rec["gs_sweeps_per_step"] = sig(float(r.iters.double().mean().item()) / w.n_steps, 4); rec["tol"] = spec["tol"]
     if spec["op"] == "newton":
-        rec["newton_iterations_per_step"] = sig(float(r.iters.double().mean().item()) / w.n_steps, 4)
+        its = float(r.iters.double().mean().item()) / w.n_steps
+        rec["newton_iterations_per_step"] = sig(its, 4)
         rec["tol"] = spec["tol"]; rec["theta"] = spec["theta"]
+        # FP64 instructions per update, counted from newton.cu for the measured iteration count: one
+        # residual pass per iteration + one final (10 per row), per iteration Jacobian rows 4 + elimination 9 +
+        # backward recurrence 3 + back substitution 2 + update 1, + the interface solve (23 + 12 x 4 levels) / 16 rows
+        spec = dict(spec, instr=round(its * (10 + 19 + 71.0 / 16) + 10, 1))
+        rec["roofline"] = roofline(name, spec, w, op_ms, pk, traffic, r.op_launches, pipe, verbose=False)
     if e2e_steps:
         e_ms, h2d, d2h = r.e2e(e2e_steps, 1)
         rec["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3)),
