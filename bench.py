@@ -602,6 +602,10 @@ def run_ours(args):
         "gpu_launches": int(r.launches * args.steps),
         "clocks": clocks,
     }
+    if spec["op"] == "newton" and hasattr(r, "iters"):          # instruction count for the measured iteration count (see measure())
+        its = float(r.iters.double().mean().item()) / w.n_steps
+        spec = dict(spec, instr=round(its * (10 + 19 + 71.0 / 16) + 10, 1))
+        out["newton_iterations_per_step"] = sig(its, 4)
     if rank == 0:
         out["roofline"] = roofline(args.workload, spec, w, op_ms, pk, traffic, r.op_launches, pipe)
         e_ms, h2d, d2h = r.e2e(max(1, min(args.steps, 5)), 1)
