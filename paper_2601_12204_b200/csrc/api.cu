@@ -86,12 +86,9 @@ template <typename T>
 int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out, void *stream);
 
 // Adaptive time step (SURVEY 8(f) NEXT-4a): n_outer times { dt = dt_from_cfl(u); m explicit steps with it;
-// t += m dt }, all enqueued on the stream, no host synchronisation.
-template <typename T>
-__global__ void accumulate_time_kernel(double *__restrict__ t, const T *__restrict__ dt, int64_t B, double m) {
-    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b < B) t[b] += m * (double)dt[b];
-}
+// t += m dt }, all enqueued on the stream, no host synchronisation; the CFL evaluation is fused into the kernels
+// of both explicit plans.
+inline size_t tiled_adapt_slot_bytes(int64_t B) { return align_up((size_t)3 * (size_t)B * sizeof(unsigned long long), 256); }
 
 template <typename T>
 int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, int64_t n_outer, int64_t m_steps,
@@ -114,17 +111,22 @@ int adaptive_call(T *u, int64_t B, int64_t N, double L, const T *nu, double C, i
         return launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt_scratch, n_outer * m_steps, bc, scheme, g, (T *)ws,
                                   nullptr, 0, s, &ad);
     }
+    // TILED plan: the CFL reduction rides on the launches themselves (explicit_impl.cuh, TADAPT): the last launch of a
+    // segment leaves max |u| of the state it stores in one of three rotating slots behind the ping-pong buffer, the
+    // launches of the next segment evaluate dt from it.  Only the first dt comes from the CFL kernel.
+    if (n_outer == 0) return BURGERS_OK;
+    const size_t state_b = align_up((size_t)B * (size_t)N * sizeof(T), 256);
+    if (!ws || ws_bytes < state_b + tiled_adapt_slot_bytes(B)) return BURGERS_ERR_WORKSPACE;
+    unsigned long long *slots = reinterpret_cast<unsigned long long *>(static_cast<unsigned char *>(ws) + state_b);
+    st = cfl_call<T>(u, B, N, L, nu, C, bc, dt_scratch, stream);
+    if (st != BURGERS_OK) return st;
+    if (cudaMemsetAsync(slots, 0, tiled_adapt_slot_bytes(B), s) != cudaSuccess) return BURGERS_ERR_CUDA;
     for (int64_t k = 0; k < n_outer; ++k) {
-        st = cfl_call<T>(u, B, N, L, nu, C, bc, dt_scratch, stream);
+        const ExplicitTiledAdapt<T> ta{slots, k == 0 ? -1 : (int)((k - 1) % 3), (int)(k % 3), (int)((k + 1) % 3), C, t_out,
+                                       dt_scratch};
+        st = launch_explicit<T>(u, B, N, grid_dx(N, L, bc), nu, dt_scratch, m_steps, bc, scheme, g, (T *)ws, nullptr, 0, s,
+                                nullptr, &ta);
         if (st != BURGERS_OK) return st;
-        st = explicit_call<T>(u, B, N, L, nu, dt_scratch, m_steps, bc, scheme, BURGERS_PLAN_AUTO, 0, 0, ws, ws_bytes,
-                              stream);
-        if (st != BURGERS_OK) return st;
-        if (t_out) {
-            accumulate_time_kernel<T><<<(unsigned)((B + 255) / 256), 256, 0, s>>>(t_out, dt_scratch, B, (double)m_steps);
-            st = last_launch_status();
-            if (st != BURGERS_OK) return st;
-        }
     }
     return BURGERS_OK;
 }
@@ -731,7 +733,8 @@ size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, i
     if (op == BURGERS_OP_EXPLICIT) {
         ExplicitGeom g;
         if (explicit_geometry(dtype_is_f64, B, N, bc, scheme, plan, 0, 0, &g) != BURGERS_OK) return 0;
-        return g.plan == BURGERS_PLAN_TILED ? align_up((size_t)B * (size_t)N * esz, 256) : 0;
+        // TILED: the ping-pong buffer, + the three maximum slots of the adaptive call (a few bytes per trajectory)
+        return g.plan == BURGERS_PLAN_TILED ? align_up((size_t)B * (size_t)N * esz, 256) + tiled_adapt_slot_bytes(B) : 0;
     }
     if (op == BURGERS_OP_NEWTON) {
         if (plan == BURGERS_PLAN_AUTO) plan = newton_hybrid_fits(dtype_is_f64, N) ? BURGERS_PLAN_HYBRID : BURGERS_PLAN_THOMAS;

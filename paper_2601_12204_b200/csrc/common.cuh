@@ -68,10 +68,22 @@ struct ExplicitAdapt {
     double *t_out;   // [B] simulated time, sum of m*dt (may be nullptr)
     T *dt_out;       // [B] the last dt used
 };
+// The same for TILED grids, one call per segment of n_steps steps (explicit_impl.cuh, Params::umax): the last
+// launch of the segment leaves max |u| in slot seg_write of umax[3][B], the launches of the next segment compute
+// their dt from slot seg_read (< 0: from `dt`), its first launch clears slot seg_zero and records dt / time.
+template <typename T>
+struct ExplicitTiledAdapt {
+    unsigned long long *umax;
+    int seg_read, seg_write, seg_zero;
+    double C;
+    double *t_out;
+    T *dt_out;
+};
 template <typename T>
 int launch_explicit(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                     int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                    T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt = nullptr);
+                    T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt = nullptr,
+                    const ExplicitTiledAdapt<T> *tadapt = nullptr);
 // Register budget -> launch bound of explicit_kernel<T, P, scheme> (the one definition: the kernel's
 // __launch_bounds__ and the host-side geometry both use it).  State registers per thread: P points x
 // words x arrays (fp32 Euler: base, s, v; other Euler: v; RK4: v, y, acc) plus ~40 for addressing and

@@ -70,7 +70,22 @@ struct Params {
     double adapt_C, dx;
     double *t_out;         // [B] sum of adapt_every*dt over the evaluations, or nullptr
     T *dt_out;             // [B] the last dt
+    // Adaptive time step on TILED grids (kernel template TADAPT): the CFL reduction is fused into the launches of a
+    // segment of adapt_every steps.  The LAST launch of segment k takes the maximum |u| of what it stores into slot
+    // seg_write of umax[3][B] (bit patterns of non-negative values, atomicMax); every launch of segment k+1 evaluates
+    // dt = cfl_dt(that maximum) itself (seg_read); its first launch (seg_first) records dt and the elapsed time and
+    // clears the slot the segment after it will use (seg_zero).  seg_read < 0: dt comes from p.dt (segment 0).
+    unsigned long long *umax;
+    int64_t Bn;
+    int seg_read, seg_write, seg_zero, seg_first;
 };
+
+template <typename T> __device__ __forceinline__ unsigned long long to_bits(T x);
+template <> __device__ __forceinline__ unsigned long long to_bits<float>(float x) { return (unsigned long long)__float_as_uint(x); }
+template <> __device__ __forceinline__ unsigned long long to_bits<double>(double x) { return (unsigned long long)__double_as_longlong(x); }
+template <typename T> __device__ __forceinline__ T from_bits(unsigned long long b);
+template <> __device__ __forceinline__ float from_bits<float>(unsigned long long b) { return __uint_as_float((unsigned)b); }
+template <> __device__ __forceinline__ double from_bits<double>(unsigned long long b) { return __longlong_as_double((long long)b); }
 
 // max over the CTA of a non-negative value (NaN operands are ignored, as in cfl.cu)
 template <typename T, bool WARP>
@@ -162,13 +177,14 @@ constexpr int adapt_min_ctas(int bytes, int P, int scheme) {
     return n > 0 ? n : 1;
 }
 
-template <typename T, int P, int SCHEME, bool TILED, bool WARP, bool SNAP = false, bool ADAPT = false>
+template <typename T, int P, int SCHEME, bool TILED, bool WARP, bool SNAP = false, bool ADAPT = false, bool TADAPT = false>
 __global__ void __launch_bounds__(WARP ? 32 : max_threads_for(sizeof(T), P, SCHEME),
                                   (ADAPT && !WARP) ? adapt_min_ctas(sizeof(T), P, SCHEME)
                                                    : (WARP && sizeof(T) == 4 && SCHEME == BURGERS_SCHEME_RK4 && P == 32 && !SNAP && !ADAPT) ? 12 : 0)   // (0 = unspecified)
 explicit_kernel(const Params<T> p) {
     static_assert(!(SNAP && TILED), "snapshots are fused into the RESIDENT plan only");
-    static_assert(!(ADAPT && TILED), "the CFL evaluation is fused into the RESIDENT plan only");
+    static_assert(!(ADAPT && TILED), "ADAPT is the RESIDENT form of the fused CFL evaluation, TADAPT the TILED one");
+    static_assert(!TADAPT || TILED, "TADAPT is the TILED form");
     constexpr bool SPLIT = (sizeof(T) == 4) && (SCHEME == BURGERS_SCHEME_EULER);
     constexpr bool RK4_DESC = WARP && (sizeof(T) == 4);
     constexpr bool EULER_DESC = !SNAP;
@@ -193,6 +209,13 @@ explicit_kernel(const Params<T> p) {
     constexpr bool SCALED = (sizeof(T) == 4);
     const T nu_b = p.nu[b];
     T dt_cur = ADAPT ? T(0) : p.dt[b];
+    if (TADAPT && p.seg_read >= 0)      // the maximum the previous segment's last launch left, the formula of cfl.cu
+        dt_cur = cfl_dt<T>(from_bits<T>(p.umax[(int64_t)p.seg_read * p.Bn + b]), nu_b, p.dx, p.adapt_C);
+    if (TADAPT && p.seg_first && tile == 0 && t == 0) {
+        if (p.seg_read >= 0) p.dt_out[b] = dt_cur;             // (segment 0: dt_out already holds it -- it IS p.dt)
+        if (p.t_out) p.t_out[b] += (double)p.adapt_every * (double)dt_cur;
+        if (p.seg_zero >= 0) p.umax[(int64_t)p.seg_zero * p.Bn + b] = 0ull;
+    }
     T cx, rr;
     auto set_dt = [&](T dt_new) {
         const double dtb = (double)dt_new;
@@ -243,7 +266,7 @@ explicit_kernel(const Params<T> p) {
     }
 
     // ADAPT: the first dt comes from the loaded state (the same max and the same formula as dt_from_cfl_*)
-    __shared__ T red[ADAPT ? 32 : 1];
+    __shared__ T red[(ADAPT || TADAPT) ? 32 : 1];
     if (ADAPT) {
         T m = T(0);
 #pragma unroll
@@ -512,6 +535,7 @@ explicit_kernel(const Params<T> p) {
     }
 
     // ---------------- store
+    T mloc = T(0);                     // TADAPT: max |u| of what this thread stores
     if (active) {
         if (vec_ok) {
 #pragma unroll
@@ -526,7 +550,10 @@ explicit_kernel(const Params<T> p) {
                     int4 q;
                     T *e = reinterpret_cast<T *>(&q);
 #pragma unroll
-                    for (int k = 0; k < V; ++k) e[k] = v[c * V + k];
+                    for (int k = 0; k < V; ++k) {
+                        e[k] = v[c * V + k];
+                        if (TADAPT) mloc = fmax(mloc, t_abs(v[c * V + k]));
+                    }
                     *reinterpret_cast<int4 *>(drow + g) = q;
                 }
             }
@@ -539,9 +566,16 @@ explicit_kernel(const Params<T> p) {
                     const int64_t li = (int64_t)t * P + j;
                     ok = (li >= p.halo) && (li < p.halo + p.W) && (g < N);
                 }
-                if (ok) drow[g] = v[j];
+                if (ok) {
+                    drow[g] = v[j];
+                    if (TADAPT) mloc = fmax(mloc, t_abs(v[j]));
+                }
             }
         }
+    }
+    if (TADAPT && p.seg_write >= 0) {      // (uniform over the grid: every CTA takes part in the reduction)
+        const T m = cta_max<T, false>(mloc, red);
+        if (t == 0) atomicMax(p.umax + (int64_t)p.seg_write * p.Bn + b, to_bits<T>(m));
     }
 }
 
@@ -552,7 +586,9 @@ int launch_P(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStream_t 
     const int64_t grid = tiled ? B * g.tiles : B;
     if (grid > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
     const size_t smem = (size_t)4 * g.block * sizeof(T);
-    if (tiled) {
+    if (tiled && p.umax) {
+        explicit_kernel<T, P, SCHEME, true, false, false, false, true><<<(unsigned)grid, g.block, smem, s>>>(p);
+    } else if (tiled) {
         explicit_kernel<T, P, SCHEME, true, false><<<(unsigned)grid, g.block, smem, s>>>(p);
     } else if (p.adapt_every > 0) {
         if (g.block == 32) explicit_kernel<T, P, SCHEME, false, true, false, true><<<(unsigned)grid, 32, 0, s>>>(p);
@@ -591,9 +627,11 @@ int launch_scheme(const Params<T> &p, const ExplicitGeom &g, int64_t B, cudaStre
 template <typename T>
 int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                          int64_t n_steps, int bc, int scheme, const ExplicitGeom &g, T *ws,
-                         T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt) {
+                         T *snaps, int64_t snap_every, cudaStream_t s, const ExplicitAdapt<T> *adapt,
+                         const ExplicitTiledAdapt<T> *tadapt) {
     if (n_steps == 0) return BURGERS_OK;
-    if (adapt && g.plan != BURGERS_PLAN_RESIDENT) return BURGERS_ERR_PLAN;   // (the caller falls back)
+    if (adapt && g.plan != BURGERS_PLAN_RESIDENT) return BURGERS_ERR_PLAN;   // (the caller uses tadapt for TILED)
+    if (tadapt && g.plan != BURGERS_PLAN_TILED) return BURGERS_ERR_PLAN;
     Params<T> p;
     p.nu = nu; p.dt = dt; p.N = N; p.inv_dx = 1.0 / dx; p.nth = g.nth; p.bc = bc;
     p.halo = g.halo; p.W = g.W; p.tiles = g.tiles;
@@ -601,6 +639,11 @@ int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, con
     p.snaps = nullptr; p.snap_every = 0; p.snap_stride = B * N;
     p.adapt_every = adapt ? adapt->every : 0; p.adapt_C = adapt ? adapt->C : 0.0; p.dx = dx;
     p.t_out = adapt ? adapt->t_out : nullptr; p.dt_out = adapt ? adapt->dt_out : nullptr;
+    p.umax = nullptr; p.Bn = B; p.seg_read = p.seg_write = p.seg_zero = -1; p.seg_first = 0;
+    if (tadapt) {
+        p.umax = tadapt->umax; p.adapt_every = n_steps; p.adapt_C = tadapt->C;
+        p.t_out = tadapt->t_out; p.dt_out = tadapt->dt_out;
+    }
     auto launch = [&]() {
         return scheme == BURGERS_SCHEME_EULER ? launch_scheme<T, BURGERS_SCHEME_EULER>(p, g, B, s)
                                               : launch_scheme<T, BURGERS_SCHEME_RK4>(p, g, B, s);
@@ -619,6 +662,12 @@ int launch_explicit_impl(T *u, int64_t B, int64_t N, double dx, const T *nu, con
             const int64_t k = (steps - done < g.tblock) ? steps - done : g.tblock;
             p.src = cur; p.dst = nxt; p.steps = k;
             p.in_scaled = (done > 0); p.out_scaled = (done + k < steps);
+            if (tadapt) {          // one segment: dt from the previous segment's maximum, this one's maximum at the end
+                p.seg_read = tadapt->seg_read;
+                p.seg_first = (done == 0);
+                p.seg_zero = (done == 0) ? tadapt->seg_zero : -1;
+                p.seg_write = (done + k == steps) ? tadapt->seg_write : -1;
+            }
             int st = launch();
             if (st != BURGERS_OK) return st;
             T *tmp = cur; cur = nxt; nxt = tmp;

@@ -139,7 +139,7 @@ def test_plan_queries(B):
     assert B.plan_query(B.OP_EXPLICIT, False, 1, 1 << 24, B.BC_PERIODIC, B.SCHEME_EULER) == B.PLAN_TILED
     assert B.plan_query(B.OP_EXPLICIT, True, 1, 3001, B.BC_PERIODIC, B.SCHEME_EULER) == B.PLAN_TILED
     assert B.workspace_bytes(B.OP_EXPLICIT, False, 1024, 4096, B.BC_DIRICHLET, 0) == 0
-    assert B.workspace_bytes(B.OP_EXPLICIT, False, 1, 1 << 24, B.BC_PERIODIC, 0) == 4 << 24
+    assert 4 << 24 <= B.workspace_bytes(B.OP_EXPLICIT, False, 1, 1 << 24, B.BC_PERIODIC, 0) <= (4 << 24) + 512   # + adaptive slots
     assert B.workspace_bytes(B.OP_BTCS, True, 8, 100, B.BC_PERIODIC, 0, B.PLAN_THOMAS) >= 4 * 8 * 100 * 8
     assert B.workspace_bytes(B.OP_BTCS, True, 8, 100, B.BC_DIRICHLET, 0, B.PLAN_THOMAS) >= 3 * 8 * 100 * 8
     assert B.launch_count(B.OP_EXPLICIT, False, 1024, 4096, 1, 0, n_steps=10000) == 1

@@ -101,3 +101,37 @@ def test_zero_state_and_single_warp_shapes(B):
             _, t, _ = B.burgers_explicit_adaptive(u, w.L, to_dev(w.nu), 0.4, 7, 9, w.bc, scheme)
             assert rel_err(u.cpu().numpy(), ref_u, w.u0) <= tol
             np.testing.assert_allclose(t.cpu().numpy(), ref_t, rtol=1e-5 if dtype == np.float32 else 1e-12)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("scheme,m", [(0, 300), (0, 70), (1, 90)])
+def test_fused_tiled_path_equals_separate_calls_bitwise(B, dtype, scheme, m):
+    """TILED grids: the CFL reduction rides on the launches of the time stepping (the last launch of a segment leaves
+    max |u| of what it stores in a slot, the next segment's launches evaluate dt from it).  Same maximum, same dt
+    formula, same launches otherwise: the bits of dt_from_cfl -> m explicit steps -> ... made of separate library
+    calls, in fp32 too (the state is unscaled in HBM at every segment boundary in both).  m = 300 / 90: two launches
+    per segment (256 Euler / 64 RK4 steps per launch); batches of two long rows, periodic and Dirichlet."""
+    import torch
+    n_outer = 4
+    for bc in (0, 1):
+        N = 40000
+        x = np.arange(N) / N
+        u0 = np.stack([np.sin(2 * np.pi * x) + 0.3, 0.8 * np.cos(6 * np.pi * x) - 0.2]).astype(dtype)
+        nu_h = np.array([2e-4, 5e-4], dtype=dtype)
+        L = 1.0
+        C = 0.4 if scheme == 0 else 0.7
+        assert B.plan_query(B.OP_EXPLICIT, dtype == np.float64, 2, N, bc, scheme) == B.PLAN_TILED
+        nu = to_dev(nu_h)
+        u1 = to_dev(u0.copy())
+        _, t1, dt1 = B.burgers_explicit_adaptive(u1, L, nu, C, n_outer, m, bc, scheme)
+        u2 = to_dev(u0.copy())
+        t2 = torch.zeros(2, dtype=torch.float64, device="cuda")
+        for _ in range(n_outer):
+            dt2 = B.dt_from_cfl(u2, L, nu, C, bc)
+            B.burgers_explicit(u2, L, nu, dt2, m, bc, scheme)
+            t2 += m * dt2.double()
+        assert torch.equal(u1, u2), (bc, "state")
+        assert torch.equal(dt1, dt2) and torch.equal(t1, t2), (bc, "dt / t")
+        ref_u, ref_t = oracle.explicit_adaptive(u0.astype(np.float64), L, nu_h.astype(np.float64), C, n_outer, m, bc, scheme,
+                                                dtype=dtype)
+        assert rel_err(u1.cpu().numpy(), ref_u, u0) <= (1e-4 if dtype == np.float32 else 1e-10)
