@@ -213,7 +213,8 @@ explicit_kernel(const Params<T> p) {
         dt_cur = cfl_dt<T>(from_bits<T>(p.umax[(int64_t)p.seg_read * p.Bn + b]), nu_b, p.dx, p.adapt_C);
     if (TADAPT && p.seg_first && tile == 0 && t == 0) {
         if (p.seg_read >= 0) p.dt_out[b] = dt_cur;             // (segment 0: dt_out already holds it -- it IS p.dt)
-        if (p.t_out) p.t_out[b] += (double)p.adapt_every * (double)dt_cur;
+        // (product and sum rounded separately, as the accumulation of the separate-call sequence does)
+        if (p.t_out) p.t_out[b] = __dadd_rn(p.t_out[b], __dmul_rn((double)p.adapt_every, (double)dt_cur));
         if (p.seg_zero >= 0) p.umax[(int64_t)p.seg_zero * p.Bn + b] = 0ull;
     }
     T cx, rr;
