@@ -138,7 +138,9 @@ int burgers_explicit_traj_f64(double *u, int64_t B, int64_t N, double L, const d
  * satisfy the CFL criteria"): n_outer times { dt_b = C min(dx/max|u_b|, dx^2/(2 nu_b)) from the current
  * state (dt_from_cfl_*); m_steps steps of the scheme with it }.  Shapes of the RESIDENT plan run as ONE
  * kernel with the CFL evaluation inside its time loop (fp64: the bits of the separate calls; fp32: the
- * state is not rounded to fp32 between the segments); longer grids as a sequence of launches.  Everything is
+ * state is not rounded to fp32 between the segments); longer grids (TILED) as the launches of the time stepping
+ * alone, the last launch of a segment leaving max|u| for the next segment's dt (the bits of the separate calls);
+ * their workspace is that of burgers_workspace_bytes(BURGERS_OP_EXPLICIT, ...).  Everything is
  * enqueued on the stream; nothing synchronises with the host.  dt_scratch: DEVICE [B] (holds the last dt on return);
  * t_out: DEVICE double [B] receiving the simulated time sum m_steps*dt_b, or NULL. */
 int burgers_explicit_adaptive_f32(float *u, int64_t B, int64_t N, double L, const float *nu, double C,
