@@ -75,6 +75,8 @@ def _load():
     lib.oracle_explicit_adjoint.restype = ci
     lib.oracle_rk4_adjoint.argtypes = [p, p, i64, i64, f64, p, p, i64, ci, ci, f64, ci]
     lib.oracle_rk4_adjoint.restype = ci
+    lib.oracle_btcs_adjoint.argtypes = [p, p, i64, i64, f64, p, p, i64, ci, ci, f64, ci]
+    lib.oracle_btcs_adjoint.restype = ci
     lib.oracle_max_threads.argtypes = []
     lib.oracle_max_threads.restype = ci
     _lib = lib
@@ -282,6 +284,21 @@ def explicit_adaptive(u0, L, nu, C, n_outer, m_steps, bc, scheme, dtype=np.float
         u2 = explicit(u2, L, nu, dt, m_steps, bc, scheme, threads=threads)
         t += m_steps * dt
     return u2.reshape(u.shape), t
+
+
+def btcs_adjoint(u0, lam_T, L, nu, dt, n_steps, bc, adv=None, threads=None) -> np.ndarray:
+    """Discrete adjoint of n_steps lagged-upwind BTCS steps (D15): dJ/du^0 from lam_T = dJ/du^N."""
+    u = _f64(u0)
+    shape = u.shape
+    u = np.ascontiguousarray(u.reshape(-1, shape[-1]))
+    lam = np.ascontiguousarray(_f64(lam_T).reshape(u.shape).copy())
+    B, N = u.shape
+    nu_a, dt_a = _per_traj(nu, B), _per_traj(dt, B)
+    rc = _load().oracle_btcs_adjoint(_ptr(u), _ptr(lam), B, N, float(L), _ptr(nu_a), _ptr(dt_a), int(n_steps),
+                                     int(bc), int(adv is not None), float(adv or 0.0), int(threads or default_threads()))
+    if rc != 0:
+        raise ValueError("oracle_btcs_adjoint: bad arguments")
+    return lam.reshape(shape)
 
 
 def explicit_adjoint(u0, lam_T, L, nu, dt, n_steps, bc, adv=None, threads=None, scheme=EULER) -> np.ndarray:

@@ -733,6 +733,83 @@ int oracle_rk4_adjoint(const double *u0, double *lam, int64_t B, int64_t N, doub
     return fail ? -1 : 0;
 }
 
+/* ---------------------------------------------------------------------------
+ * D15: DISCRETE ADJOINT of the lagged upwind BTCS scheme of D4-D6 ("gradients of the
+ * numerical solution"; VERDICT r01 "missing" item 6).  One step solves A(u) u' = u, where row i of A depends on
+ * u_i alone (D4).  Differentiating,  A du' + diag(D) du = du  with
+ *   D_i = d/du_i [ sub_i(u_i) u'_{i-1} + diag_i(u_i) u'_i + sup_i(u_i) u'_{i+1} ]
+ *       = (dt/dx) (u'_i - u'_{i-1})   if u_i > 0,      (dt/dx) (u'_{i+1} - u'_i)   otherwise
+ * (sub' = -dt/dx [u>0], diag' = dt/dx sign(u), sup' = dt/dx [u<=0]; the upwind switch held fixed), so
+ * du' = A^{-1} (I - D) du and the reverse step is   mu = A^{-T} lam',   lam_i = (1 - D_i) mu_i.
+ * Dirichlet: the system is written on all N nodes with identity rows at the two end nodes (x_0 = u_0), D = 0
+ * there; A^T mu = lam' then reads: interior j:  sup_{j-1} mu_{j-1} + diag_j mu_j + sub_{j+1} mu_{j+1} = lam'_j
+ * (neighbours that are end nodes drop out), and mu_0 = lam'_0 - sub_1 mu_1, mu_{N-1} = lam'_{N-1} - sup_{N-2} mu_{N-2}.
+ * Periodic: the transposed cyclic system (Sherman-Morrison, D6, on the transposed rows).
+ * Test hook use_adv: A is then constant, D = 0, and the adjoint is the exact transpose of the linear step.
+ */
+int oracle_btcs_adjoint(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                        const double *dt, int64_t n_steps, int bc, int use_adv, double adv, int nthreads)
+{
+    if (!u0 || !lam || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 1)
+    for (int64_t b = 0; b < B; ++b) {
+        /* states u^0..u^{n_steps}, 11N for btcs_one, then 4N rows + 3N transposed + N mu + 6N cyclic scratch */
+        double *st = (double *)malloc((size_t)(n_steps + 1 + 11 + 14) * (size_t)N * sizeof(double));
+        if (!st) {
+#pragma omp atomic write
+            fail = 1;
+            continue;
+        }
+        double *wk = st + (size_t)(n_steps + 1) * N;
+        double *sub = wk + 11 * N, *diag = sub + N, *sup = diag + N, *rhs = sup + N;
+        double *subT = rhs + N, *supT = subT + N, *mu = supT + N, *wk2 = mu + N; /* wk2: 6N */
+        for (int64_t i = 0; i < N; ++i) st[i] = u0[b * N + i];
+        for (int64_t n = 0; n < n_steps; ++n) {      /* forward, storing u^0..u^{n_steps} */
+            double *cur = st + (size_t)(n + 1) * N;
+            for (int64_t i = 0; i < N; ++i) cur[i] = st[(size_t)n * N + i];
+            btcs_one(cur, N, dx, nu[b], dt[b], 1, bc, use_adv, adv, wk);
+        }
+        double cx = dt[b] / dx;
+        double *l = lam + b * N;
+        for (int64_t n = n_steps - 1; n >= 0; --n) {
+            const double *u = st + (size_t)n * N, *up = st + (size_t)(n + 1) * N;
+            btcs_rows(u, N, dx, nu[b], dt[b], use_adv, adv, sub, diag, sup, rhs);
+            if (bc == BC_PERIODIC) {
+                for (int64_t j = 0; j < N; ++j) {      /* rows of A^T, cyclic indexing */
+                    subT[j] = sup[(j == 0) ? N - 1 : j - 1];
+                    supT[j] = sub[(j == N - 1) ? 0 : j + 1];
+                }
+                cyclic_sm(N, subT, diag, supT, l, mu, wk2);
+            } else {
+                int64_t m = N - 2;                      /* interior unknowns 1..N-2 */
+                for (int64_t j = 1; j <= N - 2; ++j) {
+                    subT[j] = sup[j - 1];               /* not referenced for j = 1 */
+                    supT[j] = sub[j + 1];               /* not referenced for j = N-2 */
+                }
+                thomas(m, subT + 1, diag + 1, supT + 1, l + 1, mu + 1, wk2, wk2 + N);
+                mu[0] = l[0] - sub[1] * mu[1];
+                mu[N - 1] = l[N - 1] - sup[N - 2] * mu[N - 2];
+            }
+            for (int64_t i = 0; i < N; ++i) {
+                double D = 0.0;
+                if (!use_adv && !(bc == BC_DIRICHLET && (i == 0 || i == N - 1))) {
+                    int64_t im = (i == 0) ? N - 1 : i - 1;
+                    int64_t ip = (i == N - 1) ? 0 : i + 1;
+                    D = (u[i] > 0.0) ? cx * (up[i] - up[im]) : cx * (up[ip] - up[i]);
+                }
+                l[i] = (1.0 - D) * mu[i];
+            }
+        }
+        free(st);
+    }
+    return fail ? -1 : 0;
+}
+
 int oracle_max_threads(void)
 {
 #ifdef _OPENMP

@@ -73,3 +73,70 @@ def test_rk4_adjoint_of_one_step_is_the_transposed_step_matrix():
     np.testing.assert_allclose(got, R.T @ lam, rtol=0, atol=1e-14)
     got3 = oracle.explicit_adjoint(rng.standard_normal(N), lam, L, nu, dt, 3, P, adv=adv, scheme=oracle.RK4)
     np.testing.assert_allclose(got3, np.linalg.matrix_power(R.T, 3) @ lam, rtol=0, atol=1e-14)
+
+
+# ---------------------------------------------------------------- D15: adjoint of the lagged upwind BTCS scheme
+@pytest.mark.parametrize("bc", [P, D])
+@pytest.mark.parametrize("adv", [0.9, -0.6])
+def test_btcs_adjoint_linear_case_is_the_exact_transpose(bc, adv):
+    # constant advection speed: u^N = M u^0 with M = (A^{-1})^n; the adjoint must be M^T
+    rng = np.random.default_rng(3)
+    N, L, nu, dt, n = 33, 1.0, 0.02, 0.03, 9          # dt far above the explicit limit (r = nu dt/dx^2 ~ 0.65, c ~ 0.9)
+    v, lam = rng.standard_normal(N), rng.standard_normal(N)
+    Mv = oracle.btcs(v, L, nu, dt, n, bc, adv=adv)
+    Mt_lam = oracle.btcs_adjoint(v, lam, L, nu, dt, n, bc, adv=adv)
+    assert abs(lam @ Mv - Mt_lam @ v) <= 1e-13 * (np.abs(lam) @ np.abs(Mv) + 1)
+
+
+@pytest.mark.parametrize("bc", [P, D])
+def test_btcs_adjoint_of_one_step_against_the_dense_formula(bc):
+    """One step: du' = A^{-1} (I - D) du with A from the pinned oracle.btcs_rows and D written out here in numpy (dense
+    matrices, numpy.linalg): the adjoint must be (I - D) A^{-T} lam."""
+    rng = np.random.default_rng(5)
+    N, L, nu, dt = 12, 1.0, 0.05, 0.04
+    u = rng.uniform(-1.0, 1.5, N)
+    u[np.abs(u) < 0.1] += 0.3
+    lam = rng.standard_normal(N)
+    sub, diag, sup, _ = oracle.btcs_rows(u, L, nu, dt, bc)
+    dx = L / N if bc == P else L / (N - 1)
+    A = np.diag(diag) + np.diag(sub[1:], -1) + np.diag(sup[:-1], 1)
+    if bc == P:
+        A[0, N - 1] = sub[0]; A[N - 1, 0] = sup[N - 1]
+    else:
+        A[0, :] = 0; A[0, 0] = 1; A[N - 1, :] = 0; A[N - 1, N - 1] = 1
+    up = oracle.btcs(u, L, nu, dt, 1, bc)
+    np.testing.assert_allclose(A @ up, u, atol=1e-13)                 # (the step itself, for the record)
+    Dv = np.where(u > 0, up - np.roll(up, 1), np.roll(up, -1) - up) * dt / dx
+    if bc == D:
+        Dv[0] = Dv[-1] = 0.0
+    want = (1.0 - Dv) * np.linalg.solve(A.T, lam)
+    got = oracle.btcs_adjoint(u, lam, L, nu, dt, 1, bc)
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("bc", [P, D])
+def test_btcs_adjoint_matches_finite_differences(bc):
+    rng = np.random.default_rng(8)
+    N, L, nu, n = 24, 1.0, 0.03, 12
+    x = np.arange(N) / N
+    u0 = 0.8 + 0.5 * np.sin(2 * np.pi * x) - 1.6 * (x > 0.6)       # both signs, away from zero at the nodes
+    dt = 10 * oracle.dt_from_cfl(u0, L, nu, 0.4, bc)[0]            # the hot path's "10x the explicit limit"
+    lam = rng.standard_normal(N)
+    grad = oracle.btcs_adjoint(u0, lam, L, nu, dt, n, bc)
+    eps = 1e-6
+    for j in range(N):
+        e = np.zeros(N); e[j] = eps
+        Jp = lam @ oracle.btcs(u0 + e, L, nu, dt, n, bc)
+        Jm = lam @ oracle.btcs(u0 - e, L, nu, dt, n, bc)
+        fd = (Jp - Jm) / (2 * eps)
+        assert abs(fd - grad[j]) <= 2e-7 * (1 + np.abs(grad).max()), (j, fd, grad[j])
+
+
+def test_btcs_adjoint_zero_steps_and_batches():
+    rng = np.random.default_rng(2)
+    u0 = rng.uniform(0.2, 1.0, (3, 16)); lam = rng.standard_normal((3, 16))
+    np.testing.assert_array_equal(oracle.btcs_adjoint(u0, lam, 1.0, 0.1, 0.01, 0, P), lam)
+    nu = np.array([0.05, 0.1, 0.2]); dt = np.array([1e-2, 2e-2, 5e-3])
+    g = oracle.btcs_adjoint(u0, lam, 1.0, nu, dt, 5, P)
+    for b in range(3):
+        np.testing.assert_array_equal(g[b], oracle.btcs_adjoint(u0[b], lam[b], 1.0, nu[b], dt[b], 5, P))
