@@ -221,6 +221,19 @@ int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const doubl
                           int64_t n_steps, int bc, int64_t snap_every, double *snaps, void *ws,
                           size_t ws_bytes, void *stream);
 
+/* Discrete ADJOINT of n_steps BTCS steps (D15; gradients of the numerical solution).
+ * One step solves A(u) u' = u; reverse mode:  mu = A(u^n)^{-T} lam,  lam_i <- (1 - D_i) mu_i,
+ * D_i = (dt/dx) (u'_i - u'_{i-1}) if u_i > 0 else (dt/dx) (u'_{i+1} - u'_i)  (identity rows, D = 0 at Dirichlet ends).
+ * u0: initial state (not modified); lam: in dJ/du^N, out dJ/du^0.  The forward sweep stores every state in the
+ * workspace (burgers_btcs_adjoint_workspace_bytes: (n_steps + 1) B N elements + the BTCS workspace; no
+ * checkpointing); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
+ * otherwise). */
+int burgers_btcs_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                             const float *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream);
+int burgers_btcs_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                             const double *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream);
+size_t burgers_btcs_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+
 /* ---- BTCS with a Gauss-Seidel inner solver -----------
  * The system of burgers_btcs_* solved per step by lexicographic Gauss-Seidel sweeps from x = u^n until
  * max_i |rhs_i - (A x)_i| < tol or max_iter sweeps were done (D12) -- the paper's iterative

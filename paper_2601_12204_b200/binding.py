@@ -32,7 +32,8 @@ EXPORTS = [
     "burgers_adjoint_workspace_bytes", "burgers_explicit_adjoint_ckpt_f32", "burgers_explicit_adjoint_ckpt_f64",
     "burgers_adjoint_ckpt_workspace_bytes", "burgers_explicit_adjoint_scheme_f32", "burgers_explicit_adjoint_scheme_f64",
     "burgers_adjoint_scheme_workspace_bytes", "burgers_btcs_f32", "burgers_btcs_f64", "burgers_btcs_plan_f32",
-    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "burgers_newton_traj_f32", "burgers_newton_traj_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
+    "burgers_btcs_plan_f64", "burgers_btcs_traj_f32", "burgers_btcs_traj_f64", "burgers_btcs_adjoint_f32", "burgers_btcs_adjoint_f64",
+    "burgers_btcs_adjoint_workspace_bytes", "burgers_btcs_gs_f32", "burgers_btcs_gs_f64", "burgers_newton_f32", "burgers_newton_f64", "burgers_newton_traj_f32", "burgers_newton_traj_f64", "dt_from_cfl_f32", "dt_from_cfl_f64", "burgers_explicit_host_f32",
     "burgers_explicit_host_f64", "burgers_btcs_host_f32", "burgers_btcs_host_f64",
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64",
     "burgers_solve_host_f32", "burgers_solve_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
@@ -61,6 +62,8 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_explicit_adjoint_ckpt_{_sfx}").restype = _int
     getattr(_lib, f"burgers_explicit_adjoint_scheme_{_sfx}").argtypes = [_p, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _int, _i64, _p, _sz, _p]
     getattr(_lib, f"burgers_explicit_adjoint_scheme_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_btcs_adjoint_{_sfx}").argtypes = [_p, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_adjoint_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_gs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _p, _sz, _p]
@@ -89,6 +92,8 @@ _lib.burgers_adjoint_ckpt_workspace_bytes.argtypes = [_int, _i64, _i64, _int, _i
 _lib.burgers_adjoint_ckpt_workspace_bytes.restype = _sz
 _lib.burgers_adjoint_scheme_workspace_bytes.argtypes = [_int, _i64, _i64, _int, _int, _i64, _i64]
 _lib.burgers_adjoint_scheme_workspace_bytes.restype = _sz
+_lib.burgers_btcs_adjoint_workspace_bytes.argtypes = [_int, _i64, _i64, _int, _i64]
+_lib.burgers_btcs_adjoint_workspace_bytes.restype = _sz
 _lib.burgers_plan_query.argtypes = [_int, _int, _i64, _i64, _int, _int]
 _lib.burgers_plan_query.restype = _int
 _lib.burgers_launch_count.argtypes = [_int, _int, _i64, _i64, _int, _int, _int, _int, _i64]
@@ -272,6 +277,23 @@ def burgers_explicit_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None, segment=0
                                                                  nu.data_ptr(), dt.data_ptr(), int(n_steps), int(bc),
                                                                  int(scheme), int(segment), wsp, wsb, _stream())
     _check(st, f"burgers_explicit_adjoint_{sfx}")
+    return lam
+
+
+def burgers_btcs_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None):
+    """lam <- (du^N/du^0)^T lam for n_steps BTCS steps from u0 (include/burgers.h: burgers_btcs_adjoint_*)."""
+    import torch
+    _dev(u0, "u0"); sfx = _sfx(u0)
+    _dev(lam, "lam", u0.dtype); _dev(nu, "nu", u0.dtype); _dev(dt, "dt", u0.dtype)
+    B, N = _shape(u0)
+    _check_vecs(B, nu=nu, dt=dt)
+    if lam.numel() != u0.numel():
+        raise ValueError("lam must have the shape of u0")
+    need = int(_lib.burgers_btcs_adjoint_workspace_bytes(int(u0.dtype == torch.float64), B, N, int(bc), int(n_steps)))
+    wsp, wsb, ws = _ws(ws, need, u0.device)
+    st = getattr(_lib, f"burgers_btcs_adjoint_{sfx}")(u0.data_ptr(), lam.data_ptr(), B, N, float(L), nu.data_ptr(),
+                                                      dt.data_ptr(), int(n_steps), int(bc), wsp, wsb, _stream())
+    _check(st, f"burgers_btcs_adjoint_{sfx}")
     return lam
 
 

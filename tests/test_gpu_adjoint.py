@@ -139,3 +139,52 @@ def test_rk4_adjoint_dot_product_identity_with_the_gpu_forward_path(B):
     np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
     with pytest.raises(B.BurgersError):
         B.burgers_explicit_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 3, w.bc, scheme=7)
+
+
+# ---------------------------------------------------------------- adjoint of the lagged upwind BTCS scheme (D15)
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-10), (np.float32, 1e-4)])
+def test_btcs_adjoint_matches_oracle(B, dtype, tol):
+    """PAPER.md:231 "gradients of the numerical solution" for the implicit scheme of the hot path: against the oracle's
+    adjoint (pinned by the transpose identity, the dense (I - D) A^{-T} formula and finite differences).  Shapes:
+    C3-like periodic with mixed signs (resident, exact partitions), the paper's N = 201 and N = 1000 Dirichlet
+    (ragged partitions), a long grid (thread-per-system fallback), at the hot path's C = 10."""
+    rng = np.random.default_rng(26)
+    for w, n in ((W.c3_periodic_btcs(B=5, N=2048, n_steps=0, dtype=dtype), 12),
+                 (W.c3_periodic_btcs(B=6, N=201, n_steps=0, dtype=dtype), 15),
+                 (W.c2_dirichlet_batch(B=4, N=1000, dtype=dtype), 10),
+                 (W.c4b_long_btcs(N=20000, n_steps=0, dtype=dtype), 4)):
+        u0 = w.u0.copy()
+        if w.bc == 1:
+            u0[:, 0] = dtype(0.3); u0[:, -1] = dtype(-0.2)
+        dt = oracle_dt(u0, w.L, w.nu, 10.0, w.bc, dtype)
+        lam_T = rng.standard_normal(u0.shape).astype(dtype)
+        ref = oracle.btcs_adjoint(u0.astype(np.float64), lam_T.astype(np.float64), w.L, w.nu.astype(np.float64),
+                                  dt.astype(np.float64), n, w.bc)
+        d_u0 = to_dev(u0.copy()); lam = to_dev(lam_T.copy())
+        B.burgers_btcs_adjoint(d_u0, lam, w.L, to_dev(w.nu), to_dev(dt), n, w.bc)
+        got = lam.cpu().numpy().astype(np.float64)
+        scale = np.abs(ref).max(axis=1, keepdims=True)
+        assert (np.abs(got - ref) / scale).max() <= tol, w.name
+        np.testing.assert_array_equal(d_u0.cpu().numpy(), u0)          # u0 untouched
+
+
+def test_btcs_adjoint_against_finite_differences_of_the_gpu_forward_path(B):
+    rng = np.random.default_rng(29)
+    w = W.c3_periodic_btcs(B=2, N=256, n_steps=0)
+    dt = oracle_dt(w.u0, w.L, w.nu, 10.0, w.bc, np.float64)
+    n = 8
+    lam_T = rng.standard_normal(w.u0.shape); v = rng.standard_normal(w.u0.shape)
+    lam = to_dev(lam_T.copy())
+    B.burgers_btcs_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), n, w.bc)
+    g = lam.cpu().numpy()
+    eps = 1e-6
+
+    def J(u0):
+        u = to_dev(u0.copy()); B.burgers_btcs(u, w.L, to_dev(w.nu), to_dev(dt), n, w.bc)
+        return (lam_T * u.cpu().numpy()).sum(axis=1)
+    fd = (J(w.u0 + eps * v) - J(w.u0 - eps * v)) / (2 * eps)
+    an = (g * v).sum(axis=1)
+    assert np.all(np.abs(fd - an) <= 1e-6 * (1 + np.abs(an)))
+    lam = to_dev(lam_T.copy())
+    B.burgers_btcs_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 0, w.bc)
+    np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
