@@ -284,6 +284,24 @@ def test_guard_bands_other_entry_points(B, dtype):
             assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
             first = got if first is None else first
             np.testing.assert_array_equal(got, first)
+    # ---- adjoint of BTCS: resident transposed solve (exact and ragged partitions), thread-per-system fallback
+    for w in (W.c3_periodic_btcs(B=3, N=2048, dtype=dtype), W.c2_dirichlet_batch(B=3, N=201, dtype=dtype),
+              W.c4b_long_btcs(N=20000, dtype=dtype)):
+        dt = _dt(w, 10.0)
+        lam_T = rng.standard_normal(w.u0.shape).astype(dtype)
+        need = int(B.raw().burgers_btcs_adjoint_workspace_bytes(int(is64), w.B, w.N, w.bc, 5))
+        ref = oracle.btcs_adjoint(_f64(w.u0), _f64(lam_T), w.L, _f64(w.nu), _f64(dt), 5, w.bc)
+        first = None
+        for _ in range(3):
+            gu, u = guarded_from(w.u0); gl, lam = guarded_from(lam_T); gw, ws = guarded_empty(need)
+            B.burgers_btcs_adjoint(u, lam, w.L, torch.from_numpy(w.nu).cuda(), torch.from_numpy(dt).cuda(), 5, w.bc, ws=ws)
+            torch.cuda.synchronize()
+            assert gu.intact() and gl.intact() and gw.intact()
+            np.testing.assert_array_equal(u.cpu().numpy(), w.u0)
+            got = lam.cpu().numpy()
+            assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
+            first = got if first is None else first
+            np.testing.assert_array_equal(got, first)
     # ---- adjoint of forward Euler
     for w, seg in ((W.c2_dirichlet_batch(B=3, N=4096, dtype=dtype), 0), (W.c3_periodic_btcs(B=3, N=1024, dtype=dtype), 5),
                    (W.c4a_long_explicit(N=40000, dtype=dtype), 0)):
