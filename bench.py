@@ -435,7 +435,7 @@ def roofline(name, spec, w, op_ms, pk, traffic, launches, pipe=None, verbose=Tru
     tr = traffic.get("bytes_per_launch", {}).get(name)
     out = {"bound": spec["bound"], "kernel_launches": int(launches),
            "avg_launch_us": sig(sec * 1e6 / max(1, launches)),
-           "traffic": tr, "traffic_source": f"ncu dram read+write per launch, profiles/ncu_traffic.csv @ {traffic.get('commit')}",
+           "traffic": tr, "traffic_source": f"ncu dram rd+wr per launch, profiles/ncu_traffic.csv @ {str(traffic.get('commit'))[:7]}",
            "hbm_accounting_frac": sig(hbm_acc, 4)}
     if not verbose:            # per-scheme entries: the sources are those of the headline's roofline
         out.pop("traffic_source")
@@ -516,6 +516,8 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": sig(statistics.median(e_ms))}
     rec["roofline"].pop("peak_source", None)                      # (as in the headline's roofline)
+    rec["roofline"].pop("unit", None)                             # (Ginst/s for "alu", GB/s for "hbm")
+    rec.pop("cfl_ms", None)
     rec["roofline"].pop("kernel_launches", None)                  # (= gpu_launches_per_step minus the CFL launches)
     if rec["roofline"].get("bound") == "hbm":
         rec["roofline"].pop("hbm_accounting_frac", None)          # (= frac)
@@ -526,7 +528,7 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     if cpu[0] > 0:
         c = cpu_baseline(w, spec, cpu[0], cpu[1])
         rec["cpu_baseline"] = {"value": c["value"], "cores": c["cores"],
-                               "sample": c["sample"].replace("trajectories", "traj").replace(" of the full", " of the"),
+                               "sample": c["sample"].split(",")[0].replace("trajectories", "traj").replace(" of the full", ""),
                                "single_thread": c.get("single_thread", {}).get("value")}
     return rec, info
 
