@@ -831,7 +831,7 @@ int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int
         if (plan == BURGERS_PLAN_THOMAS) return btcs_thomas_launch_count(n_steps);
         if (plan == BURGERS_PLAN_HYBRID) return 1;
         if (plan == BURGERS_PLAN_LONG || plan == BURGERS_PLAN_LONG_GENERAL)
-            return btcs_long_launch_count(n_steps, plan == BURGERS_PLAN_LONG_GENERAL);
+            return btcs_long_launch_count(B, N, n_steps, plan == BURGERS_PLAN_LONG_GENERAL);
     }
     return 0;
 }

@@ -44,9 +44,15 @@ constexpr int kP = 8;          // rows per thread partition of the GENERAL kerne
 constexpr int kTP = 16;
 constexpr int kTn = 128;
 constexpr int kLevels = 3;
-constexpr int kHaloR = 1 << kLevels;          // threads
-constexpr int kHaloL = kHaloR + 1;
-constexpr int kW = (kTn - kHaloL - kHaloR) * kTP;   // owned points per tile
+// Contaminated threads at the open ends of a tile after s steps in registers: one step spoils 2^kLevels reduced
+// rows per end; the next step starts from partitions that are wrong there, so the band grows by 2^kLevels per
+// step, plus one thread on the left (x_0 of a partition needs the reduced unknown of its left neighbour).
+__host__ __device__ constexpr int tile_halo_r(int s) { return s << kLevels; }
+__host__ __device__ constexpr int tile_halo_l(int s) { return (s << kLevels) + 1; }
+__host__ __device__ constexpr int tile_width(int tn, int s) { return (tn - tile_halo_l(s) - tile_halo_r(s)) * kTP; }   // owned points
+constexpr int kHaloR = tile_halo_r(1);        // threads; the one-step tile of kTn threads
+constexpr int kHaloL = tile_halo_l(1);
+constexpr int kW = tile_width(kTn, 1);
 constexpr int kGenThreads = 256;
 constexpr int kStatusBytes = 1024;            // status word + 2 x 64 level flags
 
@@ -82,18 +88,21 @@ __device__ __forceinline__ void cp_async_elem(unsigned dst, const void *src, uns
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N_> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
 
-template <typename T>
-__global__ void __launch_bounds__(kTn, 4)
+// TN threads per CTA, S time steps per launch (S = 2: the tile is solved twice in registers before it is stored;
+// the contaminated band at each open end grows by 2^kLevels threads per step, tile_halo_l/r below).
+template <typename T, int TN, int S>
+__global__ void __launch_bounds__(TN, 512 / TN)
 btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *__restrict__ nu,
                        const T *__restrict__ dt, int64_t N, int tiles, int B, double inv_dx,
                        int bc, int step, int *__restrict__ status) {
-    constexpr int P = kTP, Tn = kTn;
+    constexpr int P = kTP, Tn = TN;
+    constexpr int kHaloL = tile_halo_l(S), kHaloR = tile_halo_r(S), kW = tile_width(TN, S);
     constexpr int V = 16 / sizeof(T);
     constexpr int CR = P / V;                 // 16-byte chunks per thread row (8 fp64, 4 fp32)
     constexpr int SW = 8 / CR;                // rows sharing one 128-byte line
     constexpr int RB = CR * 16;               // bytes per thread row
     constexpr int WB = 32 * RB;               // bytes per warp region of a stage
-    __shared__ __align__(128) T stage[2][Tn * P];
+    extern __shared__ __align__(128) unsigned char stage_dyn[];    // [2][Tn * P] of T
     __shared__ T sA[2][Tn], sC[2][Tn], sD[2][Tn];
     __shared__ T sFA[Tn], sFC[Tn], sFD[Tn];   // first interface rows (own arrays: the PCR buffers of the
                                               // previous tile may still be read when these are written)
@@ -118,7 +127,7 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         return (unsigned)(warp * WB + r * RB + ((fc ^ ((r / SW) % CR)) * 16));
     };
     const unsigned r_off = (unsigned)(t * RB) | (unsigned)((((t / SW) % CR)) * 16);   // XOR with c*16 per chunk
-    const unsigned stage0 = smem_u32(&stage[0][0]);
+    const unsigned stage0 = smem_u32(stage_dyn);
     constexpr unsigned kStageBytes = Tn * P * sizeof(T);
 
     auto fetch = [&](int b, int tile, int st) {
@@ -182,6 +191,9 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
             for (int k = 0; k < V; ++k) v[c * V + k] = e[k];
         }
 
+        bool failed = false;
+#pragma unroll
+        for (int sub = 0; sub < S; ++sub) {
         // ---- assembly + partition elimination
         T f[P], c[P], q[P];
         Row<T> first, last;
@@ -209,8 +221,8 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         __syncthreads();
 
         // ---- PCR on the open chain of Tn rows, at most kLevels levels.  Rows that must be
-        // finished: the owned threads and the left neighbour of the first owned thread.
-        const bool needed = (t >= kHaloL - 1) && (t < Tn - kHaloR);
+        // finished: the threads still valid after this step and the left neighbour of the first of them.
+        const bool needed = (t >= tile_halo_l(sub + 1) - 1) && (t < Tn - tile_halo_r(sub + 1));
         int cur = 0;
         bool finished = false;
 #pragma unroll
@@ -232,11 +244,21 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
         }
         if (!finished) {                       // the halo was too short for these coefficients
             if (t == 0) atomicCAS(status, 0, step + 1);
+            failed = true;
             break;                             // uniform over the CTA
         }
 
-        // ---- recover x_0, back substitution; the warp's rows go back through its stage region so
-        // that the global stores are 512 contiguous bytes per request
+        // ---- recover x_0, back substitution
+        if (sub + 1 < S) {
+            // another step follows in registers: every thread advances (the threads of the contaminated band
+            // compute values nobody uses; what they touch is bounded by the reach of the PCR levels)
+            const T xL = row.D;
+            const T xLprev = sD[cur][t > 0 ? t - 1 : 0];
+            const T x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
+            back_substitute<T, P>(v, f, c, q, x0, xL);
+        } else {
+        // the warp's rows go back through its stage region so that the global stores are 512 contiguous
+        // bytes per request
         const bool owned = (t >= kHaloL) && (t < Tn - kHaloR);
         if (owned) {
             const T xL = row.D;
@@ -252,6 +274,9 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
                 asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(rbase ^ (unsigned)(cc * 16)), "r"(q4.x), "r"(q4.y), "r"(q4.z), "r"(q4.w) : "memory");
             }
         }
+        }
+        }
+        if (failed) break;
         __syncwarp();
         {
             const int64_t wg0 = (int64_t)tile * kW + (int64_t)(warp * 32 - kHaloL) * P;
@@ -281,14 +306,16 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
     cp_async_wait<0>();
 }
 
-// After the TILED launches: move the newest valid state into u when it sits in ws.
-//   no failure: u^{n_steps} is in ws iff n_steps is odd;  failure at step n: u^n is in ws iff n odd.
+// After the TILED launches: move the newest valid state into u when it sits in ws.  The first n_multi launches made
+// S steps each, the others one; the state after L launches is in ws iff L is odd.  No failure: the final state;
+// failure in the launch that starts at step n: u^n.
 template <typename T>
 __global__ void btcs_long_fixup_kernel(T *__restrict__ u, const T *__restrict__ ws, int64_t elems,
-                                       int64_t n_steps, const int *__restrict__ status) {
+                                       int64_t n_steps, int64_t n_multi, int S, const int *__restrict__ status) {
     const int fail = *status;
     const int64_t n = fail ? (int64_t)(fail - 1) : n_steps;
-    if ((n & 1) == 0) return;
+    const int64_t launches = (n < S * n_multi) ? n / S : n_multi + (n - S * n_multi);
+    if ((launches & 1) == 0) return;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < elems; i += stride) u[i] = ws[i];
 }
@@ -481,10 +508,51 @@ size_t btcs_long_ws_bytes(int esz, int64_t B, int64_t N) {
     return state + rows + kStatusBytes;
 }
 
-// memset + n_steps TILED + fixup + GENERAL (PLAN_LONG); GENERAL alone for PLAN_LONG_GENERAL
-int64_t btcs_long_launch_count(int64_t n_steps, int general_only) {
+namespace {
+
+// TILED shapes: threads per CTA, steps per launch, and the measured time of one tile round of the persistent grid
+// (us, fp64, B200, C4b's coefficients).  More steps per launch amortise the launch, the stage fill
+// and the store over S solves in registers, wider tiles keep the growing halo (16 S + 1 threads) a small part of
+// the tile; what decides between them for a given grid is how evenly its tiles fill the rounds.
+struct TileShape { int tn, S; double round_us; };
+constexpr TileShape kTileShapes[] = {{128, 1, 3.3}, {256, 2, 5.9}, {256, 4, 10.4}, {512, 4, 11.3}, {512, 5, 13.7}, {512, 6, 16.0}};
+constexpr double kLaunchUs = 2.2;
+
+int sm_count() {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        (void)cudaGetLastError();
+        return 148;                      // plan queries without a device: B200
+    }
+    return sms;
+}
+
+// The shape with the lowest modelled time per step: (launch + rounds x round time) / S, rounds = tiles of the
+// call / CTAs of the persistent grid (512 / tn per SM), rounded up.
+TileShape long_tile_shape(int64_t B, int64_t N, int64_t n_steps) {
+    const int sms = sm_count();
+    TileShape best = kTileShapes[0];
+    double best_cost = 0;
+    for (const TileShape &c : kTileShapes) {
+        if (c.S > n_steps || N <= 2 * (int64_t)c.tn * kTP) continue;
+        const int64_t width = tile_width(c.tn, c.S);
+        const int64_t items = B * ((N + width - 1) / width);
+        const int64_t grid = (int64_t)sms * (512 / c.tn);
+        const double cost = (kLaunchUs + (double)((items + grid - 1) / grid) * c.round_us) / c.S;
+        if (best_cost == 0 || cost < best_cost) { best = c; best_cost = cost; }
+    }
+    return best;
+}
+
+}  // namespace
+
+// memset + TILED launches + fixup + GENERAL (PLAN_LONG); GENERAL alone for PLAN_LONG_GENERAL
+int64_t btcs_long_launch_count(int64_t B, int64_t N, int64_t n_steps, int general_only) {
     if (n_steps <= 0) return 0;
-    return general_only ? 1 : n_steps + 2;
+    if (general_only) return 1;
+    const int S = long_tile_shape(B, N, n_steps).S;
+    return n_steps / S + n_steps % S + 2;
 }
 
 template <typename T>
@@ -504,33 +572,54 @@ int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T
     if (cudaMemsetAsync(status, 0, kStatusBytes, s) != cudaSuccess) return BURGERS_ERR_CUDA;
 
     if (!general_only) {
-        const int64_t tiles = (N + kW - 1) / kW;
-        const int64_t items = B * tiles;
-        int dev0 = 0, sms0 = 0, occ0 = 0;
+        int dev0 = 0, sms0 = 0;
         if (cudaGetDevice(&dev0) != cudaSuccess ||
-            cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, btcs_long_tiled_kernel<T>, kTn, 0) != cudaSuccess ||
-            occ0 < 1)
+            cudaDeviceGetAttribute(&sms0, cudaDevAttrMultiProcessorCount, dev0) != cudaSuccess)
             return BURGERS_ERR_CUDA;
-        // persistent grid: every SM gets the same number of CTAs, every CTA about the same number of tiles
-        int64_t grid_t = (int64_t)sms0 * occ0;
-        if (grid_t > items) grid_t = items;
+        const TileShape shape = long_tile_shape(B, N, n_steps);
+        const int64_t n_multi = n_steps / shape.S;                 // launches of shape.S steps, then single steps
         T *cur = u, *nxt = pong;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)grid_t); cfg.blockDim = dim3(kTn); cfg.dynamicSmemBytes = 0; cfg.stream = s;
-        cfg.attrs = attr; cfg.numAttrs = 1;
-        for (int64_t n = 0; n < n_steps; ++n) {
-            if (cudaLaunchKernelEx(&cfg, btcs_long_tiled_kernel<T>, (const T *)cur, nxt, nu, dt, N, (int)tiles, (int)B,
-                                   inv_dx, bc, (int)n, status) != cudaSuccess)
+        // one persistent grid per launch: every SM gets the same number of CTAs, every CTA about the same number
+        // of tiles; programmatic dependent launch lets the next grid become resident as this one retires
+        auto run = [&](auto kernel, int tn, int width, int64_t first_step, int64_t launches, int steps_each) -> int {
+            if (launches <= 0) return BURGERS_OK;
+            const size_t dyn = 2 * (size_t)tn * kTP * sizeof(T);
+            int occ0 = 0;
+            if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn) != cudaSuccess ||
+                cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ0, kernel, tn, dyn) != cudaSuccess || occ0 < 1)
                 return BURGERS_ERR_CUDA;
-            T *tmp = cur; cur = nxt; nxt = tmp;
+            const int64_t tiles = (N + width - 1) / width;
+            const int64_t items = B * tiles;
+            int64_t grid_t = (int64_t)sms0 * occ0;
+            if (grid_t > items) grid_t = items;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)grid_t); cfg.blockDim = dim3(tn); cfg.dynamicSmemBytes = dyn; cfg.stream = s;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            for (int64_t l = 0; l < launches; ++l) {
+                if (cudaLaunchKernelEx(&cfg, kernel, (const T *)cur, nxt, nu, dt, N, (int)tiles, (int)B, inv_dx, bc,
+                                       (int)(first_step + l * steps_each), status) != cudaSuccess)
+                    return BURGERS_ERR_CUDA;
+                T *tmp = cur; cur = nxt; nxt = tmp;
+            }
+            return last_launch_status();
+        };
+        int st = BURGERS_OK;
+        switch (shape.tn * 16 + shape.S) {
+#define BURGERS_CASE(TN, S_) \
+    case TN * 16 + S_: st = run(btcs_long_tiled_kernel<T, TN, S_>, TN, tile_width(TN, S_), 0, n_multi, S_); break;
+            BURGERS_CASE(256, 2) BURGERS_CASE(256, 4) BURGERS_CASE(512, 4) BURGERS_CASE(512, 5) BURGERS_CASE(512, 6)
+#undef BURGERS_CASE
+            default: break;                                        // (128, 1): everything goes to the loop below
         }
-        int st = last_launch_status();
         if (st != BURGERS_OK) return st;
-        btcs_long_fixup_kernel<T><<<(unsigned)(sms0 * 4), 256, 0, s>>>(u, pong, B * N, n_steps, status);
+        const int64_t done = (shape.S > 1) ? shape.S * n_multi : 0;
+        st = run(btcs_long_tiled_kernel<T, kTn, 1>, kTn, kW, done, n_steps - done, 1);
+        if (st != BURGERS_OK) return st;
+        btcs_long_fixup_kernel<T><<<(unsigned)(sms0 * 4), 256, 0, s>>>(u, pong, B * N, n_steps,
+                                                                      shape.S > 1 ? n_multi : 0, shape.S, status);
         st = last_launch_status();
         if (st != BURGERS_OK) return st;
     }

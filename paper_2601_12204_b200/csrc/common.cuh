@@ -118,7 +118,7 @@ template <typename T>
 int launch_btcs_long(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                      int64_t n_steps, int bc, void *ws, int general_only, cudaStream_t s);
 size_t btcs_long_ws_bytes(int esz, int64_t B, int64_t N);
-int64_t btcs_long_launch_count(int64_t n_steps, int general_only);
+int64_t btcs_long_launch_count(int64_t B, int64_t N, int64_t n_steps, int general_only);
 bool btcs_long_fits(int is_f64, int64_t B, int64_t N, int bc);
 
 // ---------------------------------------------------------------- adjoint of explicit Euler (adjoint.cu)

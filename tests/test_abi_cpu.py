@@ -163,7 +163,11 @@ def test_plan_queries(B):
             assert B.plan_query(B.OP_BTCS, is64, 4, 5, bc) == B.PLAN_THOMAS
     assert B.plan_query(B.OP_BTCS, True, 3, 6000, 0) == B.PLAN_LONG and B.plan_query(B.OP_BTCS, False, 3, 8192, 0) == B.PLAN_HYBRID
     assert B.launch_count(B.OP_BTCS, True, 4096, 2048, 0, n_steps=1000) == 1
-    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=200) == 202
+    # LONG: 50 launches of four steps on 512-thread tiles + fixup + GENERAL; 203 steps: + 3 single steps
+    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=200) == 52
+    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=203) == 55
+    assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, n_steps=1) == 3
+    assert B.launch_count(B.OP_BTCS, True, 1, 6000, 0, n_steps=10) == 12     # too short for the wide tiles
     assert B.launch_count(B.OP_BTCS, True, 1, 1 << 22, 0, plan=B.PLAN_LONG_GENERAL, n_steps=200) == 1
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1 << 22, 0) >= int(2.5 * 8 * (1 << 22))
     assert B.workspace_bytes(B.OP_BTCS, True, 1, 1000, 0, 0, B.PLAN_LONG) == 0      # does not fit

@@ -290,6 +290,27 @@ def test_btcs_long_grid_of_four_million_and_forty_points(B):
     check_btcs(B, w, 6)
 
 
+@pytest.mark.parametrize("case", [(600_000, 3, 4), (600_000, 13, 5), (1 << 20, 9, 5), (3_000_000, 11, 5),
+                                  (3_600_000, 9, 5), (6_000, 5, 7)])
+def test_btcs_long_every_tile_shape(B, case):
+    """LONG makes S steps per launch on tiles of 128 / 256 / 512 threads, whichever its cost model finds cheapest
+    for the grid (btcs_long.cu: long_tile_shape).  One grid per shape -- (256, 2), (512, 6), (512, 4), (512, 5),
+    (256, 4), (128, 1) in this order, identified by the launch count: multi-step launches + single-step
+    remainder + fixup + GENERAL -- whole grid against the oracle, both boundary types, step counts that are not
+    multiples of S (remainder launches, result ending in the workspace or in u)."""
+    N, n_steps, launches = case
+    for bc in (B.BC_PERIODIC, B.BC_DIRICHLET):
+        w = W.c4b_long_btcs(N=N, n_steps=n_steps)
+        assert B.plan_query(B.OP_BTCS, True, 1, N, bc) == B.PLAN_LONG
+        assert B.launch_count(B.OP_BTCS, True, 1, N, bc, n_steps=n_steps) == launches
+        dt = oracle_dt(w.u0, w.L, w.nu, w.cfl, bc, np.float64)
+        ref = oracle.btcs(w.u0, w.L, w.nu, dt, n_steps, bc)
+        got = run_btcs(B, w.u0, w.L, w.nu, dt, n_steps, bc)
+        assert rel_err(got, ref, w.u0) <= 1e-10, (case, bc)
+        general = run_btcs(B, w.u0, w.L, w.nu, dt, n_steps, bc, plan=B.PLAN_LONG_GENERAL)
+        assert rel_err(got, general, w.u0) <= 1e-12, (case, bc)
+
+
 def test_btcs_dirichlet_and_fp32(B):
     w = W.c2_dirichlet_batch(B=9, N=1000, dtype=np.float64)
     check_btcs(B, w, 40, cfl=10.0)
