@@ -86,7 +86,7 @@ enum {
     /* BTCS: */
     BURGERS_PLAN_THOMAS = 3,   /* one thread per system, interleaved [N][B] ws  */
     BURGERS_PLAN_HYBRID = 4,   /* one CTA per system: partitions + PCR, resident*/
-    BURGERS_PLAN_LONG = 5,     /* one system across many CTAs: overlapped tiles with a
+    BURGERS_PLAN_LONG = 5,     /* one system across many CTAs: overlapped tiles (1-6 steps per launch) with a
                                   checked truncated PCR, cooperative fallback     */
     BURGERS_PLAN_LONG_GENERAL = 6 /* the cooperative global-PCR kernel alone       */
 };

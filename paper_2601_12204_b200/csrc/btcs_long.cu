@@ -5,18 +5,20 @@
 // is solved exactly (to rounding) by partition elimination + parallel cyclic reduction, as in
 // btcs_hybrid.cu, with the interface system now spanning CTAs.  Two device paths:
 //
-//  TILED (fast path, one launch per time step, ping-pong u <-> ws): every tile of kW consecutive
-//    points of one system is loaded with a halo of kHaloL / kHaloR threads (x kTP points) per side.
+//  TILED (fast path, S = 1..6 time steps per launch, ping-pong u <-> ws): every tile of consecutive points of
+//    one system is loaded with a halo of 8 S + 1 / 8 S threads (x kTP points) per side.
 //    Its threads eliminate their kTP-row partitions, one in-CTA cyclic-reduction step leaves ONE
 //    reduced row per thread, and the CTA runs PCR on these rows as an OPEN chain (the couplings
 //    leaving the tile are dropped).  The wrong rows at the two tile ends contaminate, after j PCR
 //    levels, only the 2^j outermost threads; the matrix is strictly diagonally dominant, so the
-//    off-diagonals of the reduced rows decay (quadratically per level) and the owned rows are
+//    off-diagonals of the reduced rows decay (quadratically per level) and the needed rows are
 //    normally finished (all |A|,|C| < 2^-70 fp64 / 2^-40 fp32) before the contamination has
 //    crossed the halo.  The CTA CHECKS this: if after the kLevels levels the halo allows some
-//    needed row is not finished, it records the failing step in the status word and every later
-//    TILED launch returns at once, leaving u^n of the failing step intact.  The kernel is
-//    persistent within a step (grid = SMs x resident CTAs) and software-pipelined with cp.async.
+//    needed row is not finished, it records the first step of its launch in the status word and every
+//    later TILED launch returns at once, leaving the state that launch started from intact.  The row
+//    coefficients depend on the row's own u only, so the next step is solved from the registers: S solves
+//    per tile, the band of wrong threads growing by 2^kLevels per step, then one store.  The kernel is
+//    persistent within a launch (grid = SMs x resident CTAs) and software-pipelined with cp.async.
 //  GENERAL (cooperative persistent kernel, exact for any coefficients): partitions eliminated by
 //    all threads of the grid, interface rows in global memory (L2 resident), global PCR with one
 //    grid-wide barrier per level and early exit as soon as every off-diagonal is below the
