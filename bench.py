@@ -499,6 +499,8 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     rec["cfl_ms"] = sig(cfl_ms, 3)
     if r.snaps is not None:
         rec["snapshots"] = int(r.snaps.shape[0]); rec["snapshot_bytes"] = int(r.snaps.numel() * r.snaps.element_size())
+    if spec["op"] == "btcs" and r.plan == r.B.PLAN_LONG and r.op_launches > 2:
+        rec["steps_per_launch"] = sig(w.n_steps / (r.op_launches - 2), 3)       # LONG: S steps per HBM round trip
     if spec["op"] == "gs":
         rec["gs_sweeps_per_step"] = sig(float(r.iters.double().mean().item()) / w.n_steps, 4); rec["tol"] = spec["tol"]
     if spec["op"] == "newton":
@@ -610,6 +612,8 @@ def run_ours(args):
         out["newton_iterations_per_step"] = sig(its, 4)
     if rank == 0:
         out["roofline"] = roofline(args.workload, spec, w, op_ms, pk, traffic, r.op_launches, pipe)
+        if spec["op"] == "btcs" and r.plan == r.B.PLAN_LONG and r.op_launches > 2:
+            out["roofline"]["steps_per_launch"] = sig(w.n_steps / (r.op_launches - 2), 3)
         e_ms, h2d, d2h = r.e2e(max(1, min(args.steps, 5)), 1)
         out["e2e"] = {"value": sig(w.updates * world / (statistics.median(e_ms) * 1e-3), 6), "unit": "updates/s",
                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
