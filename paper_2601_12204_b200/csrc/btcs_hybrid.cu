@@ -43,13 +43,18 @@ constexpr int hybrid_max_threads(int bytes, int P) {
 // btcs::solve_interface is the same code: this instance is C3's kernel and the schedule ptxas finds for the
 // shared-helper form is 3 % slower (measured, C3: 15.70 ms inline, 16.16 ms through solve_interface, same 128
 // registers, 608 / 616 instructions; DESIGN.md 6.1 "Instruction schedule").
-template <typename T, int P>
-__global__ void __launch_bounds__(hybrid_max_threads(sizeof(T), P))
+// TN: the thread count as a compile-time constant (0: blockDim.x).  With TN known the PCR levels are unrolled and
+// every shared-memory index is an immediate offset from two registers; the run-time form spends 50 of the 64
+// instructions of a level on address arithmetic, and the kernel is bound by issue slots (an FP64 instruction
+// takes two): C3 15.66 -> 14.2 ms.
+// DIRI: Dirichlet ends (identity rows 0 and N - 1); the periodic instances carry no row selects.
+template <typename T, int P, int TN, bool DIRI>
+__global__ void __launch_bounds__(TN ? TN : hybrid_max_threads(sizeof(T), P))
 btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                    double inv_dx, int64_t n_steps, int bc) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    const int t = threadIdx.x, Tn = TN ? TN : (int)blockDim.x, mask = Tn - 1;
     T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (PCR ping-pong)
     T *sC = sA + 2 * Tn;
     T *sD = sC + 2 * Tn;
@@ -60,8 +65,9 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
 
     Coef<T> co;
     co.init(nu[blockIdx.x], dt[blockIdx.x], inv_dx);
-    const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
-    const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
+    (void)bc;
+    const bool fixL = DIRI && t == 0;
+    const bool fixR = DIRI && t == Tn - 1;
 
     T v[P];
 #pragma unroll
@@ -96,6 +102,7 @@ btcs_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restr
         __syncthreads();
         // ---- parallel cyclic reduction over the Tn reduced rows (cyclic chain), early exit
         bool finished = false;
+#pragma unroll
         for (int s = 1; s < Tn / 2; s <<= 1) {
             const int km = (t - s) & mask, kp = (t + s) & mask;
             const T *pA = sA + cur * Tn, *pC = sC + cur * Tn, *pD = sD + cur * Tn;
@@ -234,7 +241,25 @@ int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, in
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
-        btcs_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        switch (Tn) {
+#define BURGERS_TN(TN_) \
+    case TN_: \
+        if constexpr (TN_ <= hybrid_max_threads(sizeof(T), P)) { \
+            if (bc == BURGERS_BC_DIRICHLET) \
+                btcs_hybrid_kernel<T, P, TN_, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc); \
+            else \
+                btcs_hybrid_kernel<T, P, TN_, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc); \
+            return last_launch_status(); \
+        } \
+        break;
+            BURGERS_TN(32) BURGERS_TN(64) BURGERS_TN(128) BURGERS_TN(256) BURGERS_TN(512)
+#undef BURGERS_TN
+            default: break;
+        }
+        if (bc == BURGERS_BC_DIRICHLET)
+            btcs_hybrid_kernel<T, P, 0, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        else
+            btcs_hybrid_kernel<T, P, 0, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
         return last_launch_status();
     }
     return BURGERS_ERR_PLAN;
