@@ -36,10 +36,8 @@ adjoint_btcs_resident_kernel(const T *__restrict__ u0, const T *__restrict__ sta
                              int64_t n_steps, int bc) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
-    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn]
-    T *sC = sA + 2 * Tn;
-    T *sD = sC + 2 * Tn;
-    T *sF = sD + 2 * Tn;                      // [3][Tn]
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
     T *sE = sF + 3 * Tn;                      // [4][Tn] partition edge values of u^n and u^{n+1}
     Part part;
     part.r0 = t * P; part.n = P;
@@ -98,7 +96,7 @@ adjoint_btcs_resident_kernel(const T *__restrict__ u0, const T *__restrict__ sta
         if (RAGGED) eliminate_general_ragged<T, P>(rowT, n, l, f, c, first, last);
         else eliminate_general<T, P>(rowT, l, f, c, first, last);
         T x0, xL;
-        solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL, t, Tn);
+        solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
         T mu[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) mu[j] = T(0);

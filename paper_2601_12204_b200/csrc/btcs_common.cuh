@@ -287,54 +287,62 @@ inline bool pick_partition(int64_t N, MaxThreads max_threads, int *P_out, int *T
 // Solve the cyclic interface system of one CTA (Tn = blockDim.x threads, a power of two >= 2) given
 // every thread's two interface rows: one cyclic-reduction step (one reduced row per thread in the
 // unknowns x_L), parallel cyclic reduction with early exit, exact 2x2 ending; returns this thread's
-// x_0 and x_L.  smem: sA, sC, sD of 2*Tn entries each (PCR ping-pong), sF of 3*Tn entries.
+// x_0 and x_L.  smem: sR = two buffers of Tn rows (A, C, D) each (PCR ping-pong), sF = Tn rows.  The rows
+// are stored as (A, C, D) triples -- ONE address per neighbour row, its three values at immediate offsets,
+// and 24-byte (fp64) / 12-byte strides are conflict-free for 64- / 32-bit shared loads: with a run-time Tn
+// the three-array layout spent 50 of the 64 instructions of a PCR level on address arithmetic, and these
+// kernels are bound by issue slots (c3_newton 54.0 -> 49.6 ms).
 // Contains CTA barriers: call from uniform control flow.
 template <typename T>
-__device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T> &last, T *sA, T *sC, T *sD,
-                                                T *sF, T &x0, T &xL, const int t, const int Tn) {
+__device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T> &last, T *sR, T *sF,
+                                                T &x0, T &xL, const int t, const int Tn) {
     const int mask = Tn - 1;
-    T *sFA = sF, *sFC = sF + Tn, *sFD = sF + 2 * Tn;
-    sFA[t] = first.A; sFC[t] = first.C; sFD[t] = first.D;
+    {
+        T *mine = sF + 3 * t;
+        mine[0] = first.A; mine[1] = first.C; mine[2] = first.D;
+    }
     __syncthreads();
     Row<T> r;
     {
-        const int tn = (t + 1) & mask;
-        const T nA = sFA[tn], nC = sFC[tn], nD = sFD[tn];
+        const T *nx = sF + 3 * ((t + 1) & mask);
+        const T nA = nx[0], nC = nx[1], nD = nx[2];
         const T m = rcp(t_fma(-last.A, first.C, t_fma(-last.C, nA, T(1))));
         r.A = -last.A * first.A * m;
         r.C = -last.C * nC * m;
         r.D = t_fma(-last.A, first.D, t_fma(-last.C, nD, last.D)) * m;
     }
-    int cur = 0;
-    sA[t] = r.A; sC[t] = r.C; sD[t] = r.D;
+    T *rd = sR, *wr = sR + 3 * Tn;          // the buffer the next level reads / writes
+    {
+        T *mine = rd + 3 * t;
+        mine[0] = r.A; mine[1] = r.C; mine[2] = r.D;
+    }
     __syncthreads();
     bool finished = false;
     for (int s = 1; s < Tn / 2; s <<= 1) {
-        const int km = (t - s) & mask, kp = (t + s) & mask;
-        const T *pA = sA + cur * Tn, *pC = sC + cur * Tn, *pD = sD + cur * Tn;
+        const T *pm = rd + 3 * ((t - s) & mask), *pp = rd + 3 * ((t + s) & mask);
         Row<T> rm, rp;
-        rm.A = pA[km]; rm.C = pC[km]; rm.D = pD[km];
-        rp.A = pA[kp]; rp.C = pC[kp]; rp.D = pD[kp];
+        rm.A = pm[0]; rm.C = pm[1]; rm.D = pm[2];
+        rp.A = pp[0]; rp.C = pp[1]; rp.D = pp[2];
         r = pcr_combine(r, rm, rp);
-        const int o = (cur ^ 1) * Tn + t;
-        sA[o] = r.A; sC[o] = r.C; sD[o] = r.D;
+        T *mine = wr + 3 * t;
+        mine[0] = r.A; mine[1] = r.C; mine[2] = r.D;
         const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
         const int any = __syncthreads_or(flag);
-        cur ^= 1;
+        T *tmp = rd; rd = wr; wr = tmp;
         if (!any) { finished = true; break; }
     }
     T xLprev;
     xL = r.D;
     if (finished) {
-        xLprev = sD[cur * Tn + ((t - 1) & mask)];
+        xLprev = rd[3 * ((t - 1) & mask) + 2];
     } else {  // rows t and t + Tn/2 couple only to each other: exact 2x2 solve
-        const int o = (t + Tn / 2) & mask;
-        const T p1 = r.A + r.C, p2 = sA[cur * Tn + o] + sC[cur * Tn + o];
-        const T D2 = sD[cur * Tn + o];
+        const T *po = rd + 3 * ((t + Tn / 2) & mask);
+        const T p1 = r.A + r.C, p2 = po[0] + po[1];
+        const T D2 = po[2];
         xL = t_fma(-p1, D2, r.D) * rcp(t_fma(-p1, p2, T(1)));
-        sD[(cur ^ 1) * Tn + t] = xL;   // the other PCR buffer is free; the next write to it follows a barrier
+        wr[3 * t + 2] = xL;                 // the other PCR buffer is free; the next write to it follows a barrier
         __syncthreads();
-        xLprev = sD[(cur ^ 1) * Tn + ((t - 1) & mask)];
+        xLprev = wr[3 * ((t - 1) & mask) + 2];
     }
     x0 = t_fma(-first.A, xLprev, t_fma(-first.C, xL, first.D));
 }

@@ -155,10 +155,8 @@ btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = blockDim.x;
-    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (PCR ping-pong)
-    T *sC = sA + 2 * Tn;
-    T *sD = sC + 2 * Tn;
-    T *sF = sD + 2 * Tn;                      // [3][Tn] first interface rows (cyclic-reduction step)
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
     Part part;
     part.r0 = t * P; part.n = P;
     if (RAGGED) part = partition_of(t, N, Tn);
@@ -204,7 +202,7 @@ btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *
         }
         // ---- cyclic-reduction step + parallel cyclic reduction over the ring of Tn reduced rows
         T x0, xL;
-        solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL, t, Tn);
+        solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
         // ---- back substitution
         if (RAGGED) back_substitute_ragged<T, P>(v, n, f, c, q, x0, xL);
         else back_substitute<T, P>(v, f, c, q, x0, xL);

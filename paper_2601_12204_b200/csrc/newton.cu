@@ -49,10 +49,8 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
-    T *sA = reinterpret_cast<T *>(smem_raw);  // [2][Tn]
-    T *sC = sA + 2 * Tn;
-    T *sD = sC + 2 * Tn;
-    T *sF = sD + 2 * Tn;                      // [3][Tn]
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
     T *sE = sF + 3 * Tn;                      // [2][Tn] partition edge values of w
     Part part;
     part.r0 = t * P; part.n = P;
@@ -132,7 +130,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             if (RAGGED) eliminate_general_ragged<T, P>(jac, n, q, f, c, first, last);
             else eliminate_general<T, P>(jac, q, f, c, first, last);
             T x0, xL;
-            solve_interface<T>(first, last, sA, sC, sD, sF, x0, xL, t, Tn);
+            solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
             T d[P];
 #pragma unroll
             for (int j = 0; j < P; ++j) d[j] = T(0);
