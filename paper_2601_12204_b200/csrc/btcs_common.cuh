@@ -326,10 +326,13 @@ __device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T
         r = pcr_combine(r, rm, rp);
         T *mine = wr + 3 * t;
         mine[0] = r.A; mine[1] = r.C; mine[2] = r.D;
-        const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
-        const int any = __syncthreads_or(flag);
         T *tmp = rd; rd = wr; wr = tmp;
-        if (!any) { finished = true; break; }
+        if (s >= 4) {       // the vote starts at the third level (see btcs_hybrid.cu)
+            const int flag = !((t_abs(r.A) <= Lim<T>::tiny()) & (t_abs(r.C) <= Lim<T>::tiny()));
+            if (!__syncthreads_or(flag)) { finished = true; break; }
+        } else {
+            __syncthreads();
+        }
     }
     T xLprev;
     xL = r.D;
