@@ -239,11 +239,16 @@ btcs_long_tiled_kernel(const T *__restrict__ src, T *__restrict__ dst, const T *
             else { rp.A = T(0); rp.C = T(0); rp.D = T(0); }
             row = pcr_combine(row, rm, rp);
             sA[cur ^ 1][t] = row.A; sC[cur ^ 1][t] = row.C; sD[cur ^ 1][t] = row.D;
-            // NaN-safe: a row that is not provably finished counts as unfinished
-            const int flag = needed & !((t_abs(row.A) <= Lim<T>::tiny()) & (t_abs(row.C) <= Lim<T>::tiny()));
-            const int any = __syncthreads_or(flag);
             cur ^= 1;
-            if (!any) { finished = true; break; }
+            // The check is made once, after the last level the halo allows (a vote per level costs the read-back
+            // of the barrier's result and a dependent branch; levels past the decoupling change nothing that is
+            // stored).  NaN-safe: a row that is not provably finished counts as unfinished.
+            if (l == kLevels - 1) {
+                const int flag = needed & !((t_abs(row.A) <= Lim<T>::tiny()) & (t_abs(row.C) <= Lim<T>::tiny()));
+                finished = !__syncthreads_or(flag);
+            } else {
+                __syncthreads();
+            }
         }
         if (!finished) {                       // the halo was too short for these coefficients
             if (t == 0) atomicCAS(status, 0, step + 1);
