@@ -293,9 +293,11 @@ inline bool pick_partition(int64_t N, MaxThreads max_threads, int *P_out, int *T
 // the three-array layout spent 50 of the 64 instructions of a PCR level on address arithmetic, and these
 // kernels are bound by issue slots (c3_newton 54.0 -> 49.6 ms).
 // Contains CTA barriers: call from uniform control flow.
-template <typename T>
+// TN: the thread count when it is known at compile time (the PCR levels are unrolled), else 0.
+template <typename T, int TN = 0>
 __device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T> &last, T *sR, T *sF,
-                                                T &x0, T &xL, const int t, const int Tn) {
+                                                T &x0, T &xL, const int t, const int Tn_rt) {
+    const int Tn = TN ? TN : Tn_rt;
     const int mask = Tn - 1;
     {
         T *mine = sF + 3 * t;
@@ -318,6 +320,7 @@ __device__ __forceinline__ void solve_interface(const Row<T> &first, const Row<T
     }
     __syncthreads();
     bool finished = false;
+#pragma unroll
     for (int s = 1; s < Tn / 2; s <<= 1) {
         const T *pm = rd + 3 * ((t - s) & mask), *pp = rd + 3 * ((t + s) & mask);
         Row<T> rm, rp;

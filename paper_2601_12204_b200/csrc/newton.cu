@@ -41,14 +41,16 @@ constexpr int newton_max_threads(int bytes, int P) {
 // warps per SM, measured 11 % faster.  Everything else keeps the budget newton_max_threads() assumes.
 // RAGGED: any N on a power-of-two number of threads, thread t owning the q or q + 1 rows partition_of() deals
 // it (btcs_common.cuh) in the first n of its P register slots; otherwise N == P * blockDim.x.
-template <typename T, int P, bool SMALL = false, bool RAGGED = false>
+// TN: the thread count as a compile-time constant for the SMALL instances (PCR levels unrolled), else 0.
+// PERIODIC: the boundary type is known to be periodic (no identity-row selects); false: decided by `bc`.
+template <typename T, int P, bool SMALL = false, bool RAGGED = false, int TN = 0, bool PERIODIC = false>
 __global__ void __launch_bounds__(SMALL ? 128 : newton_max_threads(sizeof(T), P), SMALL ? 3 : 1)
 newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                      double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
                      long long *__restrict__ iters_out) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    const int t = threadIdx.x, Tn = TN ? TN : (int)blockDim.x, mask = Tn - 1;
     T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
     T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
     T *sE = sF + 3 * Tn;                      // [2][Tn] partition edge values of w
@@ -64,8 +66,8 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
     const T r = (T)((double)nu[blockIdx.x] * dtb * inv_dx * inv_dx);
     const T th = theta * h, tr = theta * r, omt = T(1) - theta;     // Jacobian: I + theta dG/dw
     const T b0 = T(1) + T(2) * tr;
-    const bool fixL = (bc == BURGERS_BC_DIRICHLET) && t == 0;
-    const bool fixR = (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
+    const bool fixL = !PERIODIC && (bc == BURGERS_BC_DIRICHLET) && t == 0;
+    const bool fixR = !PERIODIC && (bc == BURGERS_BC_DIRICHLET) && t == Tn - 1;
 
     T w[P], un[P];       // un holds k_i = (1-theta) G_i(u^n) - u_i^n once the first residual of a step is done
     if (RAGGED) {
@@ -130,7 +132,7 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
             if (RAGGED) eliminate_general_ragged<T, P>(jac, n, q, f, c, first, last);
             else eliminate_general<T, P>(jac, q, f, c, first, last);
             T x0, xL;
-            solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
+            solve_interface<T, TN>(first, last, sR, sF, x0, xL, t, Tn);
             T d[P];
 #pragma unroll
             for (int j = 0; j < P; ++j) d[j] = T(0);
@@ -175,7 +177,13 @@ int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T 
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
-        if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+        if (sizeof(T) == 8 && P == 16 && Tn == 128 && bc == BURGERS_BC_PERIODIC)
+            newton_hybrid_kernel<T, P, true, false, 128, true><<<(unsigned)B, Tn, smem, s>>>(
+                u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta, (T)tol, max_iter, iters_out);
+        else if (sizeof(T) == 8 && P == 16 && Tn == 128)
+            newton_hybrid_kernel<T, P, true, false, 128><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                                      (T)theta, (T)tol, max_iter, iters_out);
+        else if (sizeof(T) == 8 && P == 16 && Tn <= 128)
             newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
                                                                           (T)theta, (T)tol, max_iter, iters_out);
         else
