@@ -68,7 +68,8 @@ enum {
     BURGERS_ERR_VALUE = -4,
     BURGERS_ERR_WORKSPACE = -5,
     BURGERS_ERR_CUDA = -6,
-    BURGERS_ERR_PLAN = -7
+    BURGERS_ERR_PLAN = -7,
+    BURGERS_ERR_LIMIT = -8     /* burgers_btcs_noalloc: the problem needs more than the built-in scratch */
 };
 enum { BURGERS_BC_PERIODIC = 0, BURGERS_BC_DIRICHLET = 1 };
 enum { BURGERS_SCHEME_EULER = 0, BURGERS_SCHEME_RK4 = 1 };
@@ -338,6 +339,26 @@ size_t burgers_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, i
  * Needs a CUDA device only for the resident-fit check of the explicit op. */
 int burgers_plan_query(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
                        int scheme);
+/* ---- BTCS without any allocation ----------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): burgers_btcs_f32 / _f64 (above; plan AUTO, same kernels, same bits) with the workspace
+ * taken from a device array built into the library instead of from the caller.  u, nu, dt: DEVICE pointers
+ * of the element type dtype_is_f64 selects, caller-owned as in burgers_btcs_*; stream: cudaStream_t.
+ * The call, like burgers_btcs_*, is asynchronous and calls no cudaMalloc / cudaFree / allocating routine.
+ *  - Limit: burgers_noalloc_scratch_bytes() = 32 MiB per GPU, held by every GPU that loads the library from
+ *    module load until the process exits.  A problem whose burgers_workspace_bytes(BURGERS_OP_BTCS, ...,
+ *    BURGERS_PLAN_AUTO) exceeds it (a single fp64 grid of more than 2^20 points, say) is rejected with
+ *    BURGERS_ERR_LIMIT before anything is launched; the other errors are those of burgers_btcs_*.
+ *  - Set-up: the array's device address is looked up once per device, on the first call made with that
+ *    device current (or by burgers_noalloc_init(), which does only that: call it before a graph capture).
+ *  - Sharing: every call on a device uses the same array, which keeps the last call's contents; what must
+ *    start at zero is cleared on `stream` by the call itself.  Calls that OVERLAP on the GPU (two streams,
+ *    two host threads, two graphs replayed concurrently) race on it: serialise them. */
+size_t burgers_noalloc_scratch_bytes(void);
+int burgers_noalloc_init(void);
+int burgers_btcs_noalloc(int dtype_is_f64, void *u, int64_t B, int64_t N, double L, const void *nu,
+                         const void *dt, int64_t n_steps, int bc, void *stream);
+
 /* Number of kernel launches (memset/memcpy nodes excluded) the op enqueues. */
 int64_t burgers_launch_count(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
                              int scheme, int plan, int tblock, int64_t n_steps);

@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(_HERE, "libburgers.so")
 
 OK = 0
 ERR_NULL, ERR_SHAPE, ERR_ENUM, ERR_VALUE, ERR_WORKSPACE, ERR_CUDA, ERR_PLAN = -1, -2, -3, -4, -5, -6, -7
+ERR_LIMIT = -8
 BC_PERIODIC, BC_DIRICHLET = 0, 1
 SCHEME_EULER, SCHEME_RK4 = 0, 1
 OP_EXPLICIT, OP_BTCS, OP_CFL, OP_NEWTON, OP_GS = 0, 1, 2, 3, 4
@@ -38,6 +39,7 @@ EXPORTS = [
     "burgers_newton_host_f32", "burgers_newton_host_f64", "dt_from_cfl_host_f32", "dt_from_cfl_host_f64",
     "burgers_solve_host_f32", "burgers_solve_host_f64", "burgers_workspace_bytes", "burgers_plan_query",
     "burgers_launch_count", "burgers_pipe_peak", "burgers_strerror", "burgers_version",
+    "burgers_noalloc_scratch_bytes", "burgers_noalloc_init", "burgers_btcs_noalloc",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -100,6 +102,12 @@ _lib.burgers_launch_count.argtypes = [_int, _int, _i64, _i64, _int, _int, _int, 
 _lib.burgers_launch_count.restype = _i64
 _lib.burgers_pipe_peak.argtypes = [_int, _i64, _p, _p, ctypes.POINTER(ctypes.c_double)]
 _lib.burgers_pipe_peak.restype = _int
+_lib.burgers_noalloc_scratch_bytes.argtypes = []
+_lib.burgers_noalloc_scratch_bytes.restype = _sz
+_lib.burgers_noalloc_init.argtypes = []
+_lib.burgers_noalloc_init.restype = _int
+_lib.burgers_btcs_noalloc.argtypes = [_int, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _p]
+_lib.burgers_btcs_noalloc.restype = _int
 _lib.burgers_strerror.argtypes = [_int]
 _lib.burgers_strerror.restype = ctypes.c_char_p
 _lib.burgers_version.argtypes = []
@@ -332,6 +340,24 @@ def burgers_btcs(u, L, nu, dt, n_steps, bc, ws=None, plan=PLAN_AUTO):
     st = fn(u.data_ptr(), B, N, float(L), nu.data_ptr(), dt.data_ptr(), int(n_steps), int(bc),
             int(plan), wsp, wsb, _stream())
     _check(st, f"burgers_btcs_{sfx}")
+    return u
+
+
+def noalloc_scratch_bytes() -> int:
+    return int(_lib.burgers_noalloc_scratch_bytes())
+
+
+def burgers_btcs_noalloc(u, L, nu, dt, n_steps, bc):
+    """In-place BTCS time stepping with the library's built-in scratch array: no allocation anywhere
+    (include/burgers.h: burgers_btcs_noalloc; BurgersError(ERR_LIMIT) beyond noalloc_scratch_bytes())."""
+    import torch
+    _dev(u, "u")
+    _dev(nu, "nu", u.dtype); _dev(dt, "dt", u.dtype)
+    B, N = _shape(u)
+    _check_vecs(B, nu=nu, dt=dt)
+    st = _lib.burgers_btcs_noalloc(int(u.dtype == torch.float64), u.data_ptr(), B, N, float(L), nu.data_ptr(),
+                                   dt.data_ptr(), int(n_steps), int(bc), _stream())
+    _check(st, "burgers_btcs_noalloc")
     return u
 
 

@@ -846,6 +846,7 @@ const char *burgers_strerror(int status) {
         case BURGERS_ERR_WORKSPACE: return "workspace missing or too small (see burgers_workspace_bytes)";
         case BURGERS_ERR_CUDA: return "CUDA runtime / launch failure";
         case BURGERS_ERR_PLAN: return "requested plan cannot run this shape";
+        case BURGERS_ERR_LIMIT: return "problem needs more scratch than the no-allocation entry point holds (see burgers_noalloc_scratch_bytes)";
     }
     return "unknown status";
 }
