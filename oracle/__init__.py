@@ -77,6 +77,8 @@ def _load():
     lib.oracle_rk4_adjoint.restype = ci
     lib.oracle_btcs_adjoint.argtypes = [p, p, i64, i64, f64, p, p, i64, ci, ci, f64, ci]
     lib.oracle_btcs_adjoint.restype = ci
+    lib.oracle_newton_adjoint.argtypes = [p, p, i64, i64, f64, p, p, f64, i64, ci, f64, ci, ci, f64, ci]
+    lib.oracle_newton_adjoint.restype = ci
     lib.oracle_max_threads.argtypes = []
     lib.oracle_max_threads.restype = ci
     _lib = lib
@@ -298,6 +300,24 @@ def btcs_adjoint(u0, lam_T, L, nu, dt, n_steps, bc, adv=None, threads=None) -> n
                                      int(bc), int(adv is not None), float(adv or 0.0), int(threads or default_threads()))
     if rc != 0:
         raise ValueError("oracle_btcs_adjoint: bad arguments")
+    return lam.reshape(shape)
+
+
+def newton_adjoint(u0, lam_T, L, nu, dt, n_steps, bc, tol=1e-13, max_iter=50, adv=None, threads=None,
+                   theta=1.0) -> np.ndarray:
+    """Reverse mode of n_steps Newton / theta-scheme steps (D16; implicit-function theorem at the converged
+    states): dJ/du^0 from lam_T = dJ/du^N."""
+    u = _f64(u0)
+    shape = u.shape
+    u = np.ascontiguousarray(u.reshape(-1, shape[-1]))
+    lam = np.ascontiguousarray(_f64(lam_T).reshape(u.shape).copy())
+    B, N = u.shape
+    nu_a, dt_a = _per_traj(nu, B), _per_traj(dt, B)
+    rc = _load().oracle_newton_adjoint(_ptr(u), _ptr(lam), B, N, float(L), _ptr(nu_a), _ptr(dt_a), float(theta),
+                                       int(n_steps), int(bc), float(tol), int(max_iter), int(adv is not None),
+                                       float(adv or 0.0), int(threads or default_threads()))
+    if rc != 0:
+        raise ValueError("oracle_newton_adjoint: bad arguments")
     return lam.reshape(shape)
 
 

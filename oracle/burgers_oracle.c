@@ -25,7 +25,9 @@
  * rational arithmetic (G1,G4), Cole-Hopf closed form (R1/G2), exact Fourier
  * amplification factors (R2/G3), dense Gaussian elimination for N<=16 (R3),
  * CFL limit closed form (R4/G5), invariants (G6), textbook special cases (G7),
- * travelling viscous shock (G8).  No function here is "parity unpinned".
+ * travelling viscous shock (G8); the adjoints (D13-D16): exact transpose in the linear case, dense one-step
+ * formulas in numpy, central finite differences of the pinned forward functions.  No function here is
+ * "parity unpinned".
  *
  * Notation follows the paper / SURVEY.md 8(c): c_i = u_i dt/dx, r = nu dt/dx^2.
  */
@@ -803,6 +805,79 @@ int oracle_btcs_adjoint(const double *u0, double *lam, int64_t B, int64_t N, dou
                     D = (u[i] > 0.0) ? cx * (up[i] - up[im]) : cx * (up[ip] - up[i]);
                 }
                 l[i] = (1.0 - D) * mu[i];
+            }
+        }
+        free(st);
+    }
+    return fail ? -1 : 0;
+}
+
+/* ---------------------------------------------------------------------------
+ * D16: reverse mode of the Newton / theta-scheme of D11 (PAPER.md:137-159 Eq.10-15 for the scheme; :231, :261 for
+ * the purpose: "gradients of the numerical solution").  One step maps u = u^n to the root w = u^{n+1} of
+ *   F_i(w; u) = w_i - u_i + theta G_i(w) + (1 - theta) G_i(u)   (interior / periodic rows; F_i = w_i - u_i at
+ * Dirichlet end nodes), so by the implicit-function theorem dw/du = -(dF/dw)^{-1} dF/du with
+ *   dF/dw = J(w)                                   (newton_jacobian at the root: identity rows at Dirichlet ends),
+ *   dF/du = -I + (1 - theta) M G'(u)               (M: zero rows at Dirichlet end nodes),
+ *   G'(v) row i = (-h v_i - r,  h (v_{i+1} - v_{i-1}) + 2 r,  h v_i - r)   on columns (i-1, i, i+1), cyclic.
+ * Reverse mode, given lam' = dJ/du^{n+1}:
+ *   J(u^{n+1})^T mu = lam',        lam_i = mu_i - (1 - theta) (G'(u^n)^T M mu)_i,
+ *   (G'(v)^T x)_i = (h v_{i-1} - r) x_{i-1} + (h (v_{i+1} - v_{i-1}) + 2 r) x_i + (-h v_{i+1} - r) x_{i+1}.
+ * This differentiates the map the CONVERGED iteration defines; the forward sweep below is newton_one with the
+ * caller's tol and max_iter (use a tol near rounding for gradients), all states stored.
+ * J^T: row j = (sup_{j-1}, diag_j, sub_{j+1}); with identity rows at Dirichlet ends sub_0 = sup_{N-1} = 0, so the
+ * wrap entries vanish and the plain Thomas solve of all N rows applies; periodic: Sherman-Morrison (D6).
+ * Test hook use_adv: G is linear (multiplier adv), the step is u' = S u and the adjoint is S^T.
+ */
+int oracle_newton_adjoint(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                          const double *dt, double theta, int64_t n_steps, int bc, double tol, int max_iter,
+                          int use_adv, double adv, int nthreads)
+{
+    if (!u0 || !lam || !nu || !dt || B < 1 || N < 3 || n_steps < 0 || !(L > 0.0) || max_iter < 0) return -1;
+    if (!(theta >= 0.0 && theta <= 1.0)) return -1;
+    if (bc != BC_PERIODIC && bc != BC_DIRICHLET) return -1;
+    double dx = grid_dx(N, L, bc);
+    int fail = 0;
+    if (nthreads < 1) nthreads = 1;
+    (void)nthreads;
+#pragma omp parallel for num_threads(nthreads) schedule(dynamic, 1)
+    for (int64_t b = 0; b < B; ++b) {
+        /* states u^0..u^{n_steps}, 13N for newton_one, 3N rows, 2N transposed, 2N mu / masked mu, 6N cyclic scratch */
+        double *st = (double *)malloc((size_t)(n_steps + 1 + 13 + 13) * (size_t)N * sizeof(double));
+        if (!st) {
+#pragma omp atomic write
+            fail = 1;
+            continue;
+        }
+        double *wk = st + (size_t)(n_steps + 1) * N;
+        double *sub = wk + 13 * N, *diag = sub + N, *sup = diag + N;
+        double *subT = sup + N, *supT = subT + N, *mu = supT + N, *mm = mu + N, *wk2 = mm + N; /* wk2: 6N */
+        double h = dt[b] / (2.0 * dx), r = nu[b] * dt[b] / (dx * dx);
+        for (int64_t i = 0; i < N; ++i) st[i] = u0[b * N + i];
+        for (int64_t n = 0; n < n_steps; ++n) {      /* forward, storing u^0..u^{n_steps} */
+            double *cur = st + (size_t)(n + 1) * N;
+            for (int64_t i = 0; i < N; ++i) cur[i] = st[(size_t)n * N + i];
+            newton_one(cur, N, dx, nu[b], dt[b], theta, 1, bc, tol, max_iter, use_adv, adv, wk);
+        }
+        double *l = lam + b * N;
+        for (int64_t n = n_steps - 1; n >= 0; --n) {
+            const double *u = st + (size_t)n * N, *up = st + (size_t)(n + 1) * N;
+            newton_jacobian(up, N, h, r, theta, bc, use_adv, adv, sub, diag, sup);
+            for (int64_t j = 0; j < N; ++j) {        /* rows of J^T, cyclic indexing (zero wrap for Dirichlet) */
+                subT[j] = sup[(j == 0) ? N - 1 : j - 1];
+                supT[j] = sub[(j == N - 1) ? 0 : j + 1];
+            }
+            if (bc == BC_PERIODIC) cyclic_sm(N, subT, diag, supT, l, mu, wk2);
+            else thomas(N, subT, diag, supT, l, mu, wk2, wk2 + N);
+            for (int64_t i = 0; i < N; ++i)
+                mm[i] = (bc == BC_DIRICHLET && (i == 0 || i == N - 1)) ? 0.0 : mu[i];     /* M mu */
+            for (int64_t i = 0; i < N; ++i) {
+                int64_t im = (i == 0) ? N - 1 : i - 1;
+                int64_t ip = (i == N - 1) ? 0 : i + 1;
+                double am = use_adv ? adv : u[im], ap = use_adv ? adv : u[ip];
+                double dg = use_adv ? 0.0 : h * (u[ip] - u[im]);
+                double gt = (h * am - r) * mm[im] + (dg + 2.0 * r) * mm[i] + (-h * ap - r) * mm[ip];
+                l[i] = mu[i] - (1.0 - theta) * gt;
             }
         }
         free(st);

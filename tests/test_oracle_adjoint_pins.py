@@ -140,3 +140,94 @@ def test_btcs_adjoint_zero_steps_and_batches():
     g = oracle.btcs_adjoint(u0, lam, 1.0, nu, dt, 5, P)
     for b in range(3):
         np.testing.assert_array_equal(g[b], oracle.btcs_adjoint(u0[b], lam[b], 1.0, nu[b], dt[b], 5, P))
+
+
+# ---------------------------------------------------------------- D16: reverse mode of the Newton / theta-scheme
+THETAS = [1.0, 0.5, 0.3]
+
+
+def _dense_G_prime(v, h, r, bc, adv=None):
+    """d G / d v written out densely (numpy): G_i(v) = h a_i (v_{i+1} - v_{i-1}) - r (v_{i+1} - 2 v_i + v_{i-1}),
+    a_i = v_i (or the constant adv), cyclic neighbours; rows of Dirichlet end nodes are zero (M G')."""
+    N = len(v)
+    Gp = np.zeros((N, N))
+    for i in range(N):
+        if bc == D and i in (0, N - 1):
+            continue
+        im, ip = (i - 1) % N, (i + 1) % N
+        a = v[i] if adv is None else adv
+        Gp[i, im] += -h * a - r
+        Gp[i, ip] += h * a - r
+        Gp[i, i] += 2 * r + (h * (v[ip] - v[im]) if adv is None else 0.0)
+    return Gp
+
+
+@pytest.mark.parametrize("theta", THETAS)
+@pytest.mark.parametrize("bc", [P, D])
+@pytest.mark.parametrize("adv", [0.9, -0.6])
+def test_newton_adjoint_linear_case_is_the_exact_transpose(bc, adv, theta):
+    # constant multiplier: u^N = S^n u^0 with S = (I + theta G')^{-1} (I - (1 - theta) G'); the adjoint must be S^T
+    rng = np.random.default_rng(13)
+    N, L, nu, dt, n = 21, 1.0, 0.02, 0.01, 7
+    v, lam = rng.standard_normal(N), rng.standard_normal(N)
+    Sv = oracle.newton_btcs(v, L, nu, dt, n, bc, tol=1e-14, adv=adv, theta=theta)
+    St_lam = oracle.newton_adjoint(v, lam, L, nu, dt, n, bc, tol=1e-14, adv=adv, theta=theta)
+    assert abs(lam @ Sv - St_lam @ v) <= 1e-12 * (np.abs(lam) @ np.abs(Sv) + 1)
+    dx = L / N if bc == P else L / (N - 1)
+    Gp = _dense_G_prime(v, dt / (2 * dx), nu * dt / dx**2, bc, adv)
+    S = np.linalg.solve(np.eye(N) + theta * Gp, np.eye(N) - (1 - theta) * Gp)
+    np.testing.assert_allclose(St_lam, np.linalg.matrix_power(S.T, n) @ lam, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("theta", THETAS)
+@pytest.mark.parametrize("bc", [P, D])
+def test_newton_adjoint_of_one_step_against_the_dense_formula(bc, theta):
+    """One step from u to the root w (pinned forward oracle): dw/du = (I + theta M G'(w))^{-1} (I - (1 - theta) M G'(u))
+    with G' written out densely here; the adjoint must be the transpose applied to lam (numpy.linalg)."""
+    rng = np.random.default_rng(17)
+    N, L, nu, dt = 14, 1.0, 0.05, 0.004
+    u = rng.uniform(-1.0, 1.5, N)
+    lam = rng.standard_normal(N)
+    dx = L / N if bc == P else L / (N - 1)
+    h, r = dt / (2 * dx), nu * dt / dx**2
+    w = oracle.newton_btcs(u, L, nu, dt, 1, bc, tol=1e-14, theta=theta)
+    Jw = np.eye(N) + theta * _dense_G_prime(w, h, r, bc)
+    Ku = np.eye(N) - (1 - theta) * _dense_G_prime(u, h, r, bc)
+    want = Ku.T @ np.linalg.solve(Jw.T, lam)
+    got = oracle.newton_adjoint(u, lam, L, nu, dt, 1, bc, tol=1e-14, theta=theta)
+    np.testing.assert_allclose(got, want, rtol=0, atol=1e-12)
+
+
+@pytest.mark.parametrize("theta", [1.0, 0.5])
+@pytest.mark.parametrize("bc", [P, D])
+def test_newton_adjoint_matches_finite_differences(bc, theta):
+    rng = np.random.default_rng(19)
+    N, L, nu, n = 24, 1.0, 0.03, 10
+    x = np.arange(N) / N
+    u0 = 0.8 + 0.5 * np.sin(2 * np.pi * x) - 1.6 * (x > 0.6)       # both signs, a jump
+    dt = 4 * oracle.dt_from_cfl(u0, L, nu, 0.4, bc)[0]             # implicit step, cell Peclet number < 2
+    lam = rng.standard_normal(N)
+    grad = oracle.newton_adjoint(u0, lam, L, nu, dt, n, bc, tol=1e-14, theta=theta)
+    eps = 1e-6
+    for j in range(N):
+        e = np.zeros(N); e[j] = eps
+        Jp = lam @ oracle.newton_btcs(u0 + e, L, nu, dt, n, bc, tol=1e-14, theta=theta)
+        Jm = lam @ oracle.newton_btcs(u0 - e, L, nu, dt, n, bc, tol=1e-14, theta=theta)
+        fd = (Jp - Jm) / (2 * eps)
+        assert abs(fd - grad[j]) <= 2e-7 * (1 + np.abs(grad).max()), (j, fd, grad[j])
+
+
+def test_newton_adjoint_theta_zero_is_the_explicit_central_transpose_and_batches():
+    rng = np.random.default_rng(23)
+    u0 = rng.uniform(0.2, 1.0, (3, 16)); lam = rng.standard_normal((3, 16))
+    np.testing.assert_array_equal(oracle.newton_adjoint(u0, lam, 1.0, 0.1, 0.01, 0, P), lam)
+    # theta = 0: w = u - G(u) explicitly, J = I, so one step's adjoint is (I - G'(u))^T lam
+    N, L, nu, dt = 16, 1.0, 0.1, 1e-3
+    dx = L / N
+    Gp = _dense_G_prime(u0[0], dt / (2 * dx), nu * dt / dx**2, P)
+    np.testing.assert_allclose(oracle.newton_adjoint(u0[0], lam[0], L, nu, dt, 1, P, theta=0.0),
+                               (np.eye(N) - Gp).T @ lam[0], rtol=0, atol=1e-14)
+    nu = np.array([0.05, 0.1, 0.2]); dt = np.array([1e-3, 2e-3, 5e-4])
+    g = oracle.newton_adjoint(u0, lam, 1.0, nu, dt, 5, P, theta=0.5)
+    for b in range(3):
+        np.testing.assert_array_equal(g[b], oracle.newton_adjoint(u0[b], lam[b], 1.0, nu[b], dt[b], 5, P, theta=0.5))
