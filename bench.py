@@ -51,7 +51,7 @@ BACKEND = "nccl"            # torch.distributed backend of the timing barrier / 
 RUNNER = None               # class with GpuRunner's interface; None -> GpuRunner
 HOT = ("c2_f32", "c2_f64", "c3", "c4a", "c4b", "c5")
 NEXT = ("c3_newton", "c3_cn", "c2_traj", "c3_gs", "c2_adjoint")
-MORE = ("c5_adjoint",)                                                    # --workload only (not in the default table)
+MORE = ("c5_adjoint", "c3_btcs_adjoint", "c3_newton_adjoint")        # --workload only (not in the default table)
 WORKLOADS = HOT + NEXT
 
 
@@ -122,6 +122,12 @@ def make_workload(name, rank=0, world=1, reduced=False):
         w = W.c5_rk4_ensemble(B=65536 * world, rows=np.arange(0, 65536 * world, 16)[W.shard_rows(Bg, rank, world)],
                               n_steps=10 if reduced else 100)
         return w, dict(op="adjoint", scheme=1, bound="hbm", instr=None, lanes=FP32_LANES)
+    if name in ("c3_btcs_adjoint", "c3_newton_adjoint"):   # reverse mode of 100 implicit steps of 256 C3 trajectories (D15 / D16)
+        Bg = 256 * world
+        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=10 if reduced else 100)
+        if name == "c3_newton_adjoint":
+            w.cfl = 4.0
+        return w, dict(op="adjoint", scheme=2 if name == "c3_btcs_adjoint" else 3, bound="hbm", instr=None, lanes=FP64_LANES)
     if name == "c2_traj":        # SURVEY 8(f) NEXT-4b: C2 fp32 with a snapshot of all trajectories every 50 steps
         Bg = 1024 * world
         w = W.c2_dirichlet_batch(B=Bg, dtype=np.float32, rows=W.shard_rows(Bg, rank, world),
@@ -214,7 +220,8 @@ def metric_name(spec):
         return base + ("forward Euler upwind/central" if spec["scheme"] == 0 else "RK4")
     return base + {"btcs": "BTCS", "newton": "Newton BTCS (central convection, theta-scheme)",
                    "gs": "Gauss-Seidel BTCS",
-                   "adjoint": "adjoint of forward Euler" if spec["scheme"] == 0 else "adjoint of RK4"}[spec["op"]]
+                   "adjoint": ("adjoint of forward Euler", "adjoint of RK4", "adjoint of BTCS",
+                               "reverse mode of Newton BTCS")[spec["scheme"] or 0]}[spec["op"]]
 
 
 # ------------------------------------------------------------------------------- oracle leg
@@ -237,7 +244,12 @@ def oracle_sample_run(w, spec, target_s=12.0, threads=None):
                            threads=threads)
         elif spec["op"] == "adjoint":
             lam = np.random.default_rng(1220404).standard_normal(u0[rows].shape)
-            oracle.explicit_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads, scheme=spec["scheme"])
+            if spec["scheme"] == 2:
+                oracle.btcs_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+            elif spec["scheme"] == 3:
+                oracle.newton_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads)
+            else:
+                oracle.explicit_adjoint(u0[rows], lam, w.L, nu[rows], dt[rows], n, w.bc, threads=threads, scheme=spec["scheme"])
         elif spec["op"] == "newton":
             oracle.newton_btcs(u0[rows], w.L, nu[rows], dt[rows], n, w.bc, tol=spec["tol"],
                                max_iter=spec["max_iter"], threads=threads, theta=spec["theta"])
@@ -292,9 +304,14 @@ class GpuRunner:
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
         elif spec["op"] == "adjoint":
             self.plan = 0
-            need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, spec["scheme"], w.n_steps, 0))
-            # Euler: forward trajectory kernel + resident backward kernel; RK4: forward + 7 launches per step
-            self.launches = 2 if spec["scheme"] == 0 else 1 + 7 * w.n_steps
+            if spec["scheme"] >= 2:      # implicit schemes: one forward launch per step (+ its copy), one backward launch
+                q = B.raw().burgers_btcs_adjoint_workspace_bytes if spec["scheme"] == 2 else B.raw().burgers_newton_adjoint_workspace_bytes
+                need = int(q(int(is64), w.B, w.N, w.bc, w.n_steps))
+                self.launches = w.n_steps + 1
+            else:
+                need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, spec["scheme"], w.n_steps, 0))
+                # Euler: forward trajectory kernel + resident backward kernel; RK4: forward + 7 launches per step
+                self.launches = 2 if spec["scheme"] == 0 else 1 + 7 * w.n_steps
             self.lam0 = torch.randn(self.u0.shape, dtype=self.u0.dtype, device=device,
                                     generator=torch.Generator(device=device).manual_seed(1220404))
         elif spec["op"] == "gs":
@@ -334,6 +351,10 @@ class GpuRunner:
                                     self.spec["snap_every"], snaps=self.snaps, ws=self.ws)
         elif self.spec["op"] == "explicit":
             B.burgers_explicit(self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, self.spec["scheme"], ws=self.ws)
+        elif self.spec["op"] == "adjoint" and self.spec["scheme"] == 2:
+            B.burgers_btcs_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
+        elif self.spec["op"] == "adjoint" and self.spec["scheme"] == 3:
+            B.burgers_newton_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws)
         elif self.spec["op"] == "adjoint":
             B.burgers_explicit_adjoint(self.u0, self.u, w.L, self.nu, self.dt, w.n_steps, w.bc, ws=self.ws,
                                        scheme=self.spec["scheme"])
@@ -381,7 +402,12 @@ class GpuRunner:
                                       max_iter=self.spec["max_iter"], ws=self.ws)
                 else:                                  # (the seed lambda is already on the device)
                     dl = self.lam0.clone()
-                    B.burgers_explicit_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws, scheme=self.spec["scheme"])
+                    if self.spec["scheme"] == 2:
+                        B.burgers_btcs_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws)
+                    elif self.spec["scheme"] == 3:
+                        B.burgers_newton_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws)
+                    else:
+                        B.burgers_explicit_adjoint(du, dl, w.L, dnu, ddt, w.n_steps, w.bc, ws=self.ws, scheme=self.spec["scheme"])
                     du = dl
                 hu.copy_(du); torch.cuda.synchronize()
             elif self.spec["op"] == "newton":

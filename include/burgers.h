@@ -284,6 +284,25 @@ int burgers_newton_traj_f64(double *u, int64_t B, int64_t N, double L, const dou
                             int64_t *iters_out, int64_t snap_every, double *snaps, void *ws, size_t ws_bytes,
                             void *stream);
 
+/* REVERSE MODE of n_steps Newton / theta-scheme steps (D16; the scheme: Eq.10-15; the
+ * purpose: PAPER.md:231, :261).  One step maps u = u^n to the root w = u^{n+1} of
+ *   F(w; u) = w - u + theta G(w) + (1 - theta) G(u),   G_i(v) = h v_i (v_{i+1} - v_{i-1}) - r (v_{i+1} - 2 v_i + v_{i-1}),
+ * h = dt/(2 dx), r = nu dt/dx^2 (identity rows at Dirichlet end nodes).  Implicit-function theorem:
+ *   J(u^{n+1})^T mu = lam,   lam <- mu - (1 - theta) G'(u^n)^T M mu     (J: the Newton Jacobian, Eq.14; M: zero rows at
+ * Dirichlet ends) -- the derivative of the map the CONVERGED iteration defines: pass a tol near rounding
+ * (e.g. 1e-13 in fp64); tol and max_iter drive the forward sweep exactly as in burgers_newton_*.
+ * u0: initial state (not modified); lam: in dJ/du^N, out dJ/du^0.  The forward sweep stores every state in the
+ * workspace (burgers_newton_adjoint_workspace_bytes: (n_steps + 1) B N elements + the Newton workspace; no
+ * checkpointing); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
+ * otherwise).  Errors as burgers_newton_*. */
+int burgers_newton_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                               const float *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                               void *ws, size_t ws_bytes, void *stream);
+int burgers_newton_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                               const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                               void *ws, size_t ws_bytes, void *stream);
+size_t burgers_newton_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+
 /* ---- CFL time step (PAPER.md:116-118 Eq.7-8, :287 Eq.24) -----------------------
  * dt_out[b] = C * min(dx / max_i |u[b][i]|, dx^2 / (2 nu[b])), with x/0 = +inf
  * (u == 0 gives the diffusive bound, nu == 0 the convective one, both: +inf).

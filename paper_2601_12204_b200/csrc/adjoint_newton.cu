@@ -1,0 +1,251 @@
+// adjoint_newton.cu -- reverse mode of the Newton / theta-scheme of newton.cu (D16; the scheme:
+// PAPER.md:137-159 Eq.10-15; the purpose: "gradients of the numerical solution").
+//
+// One forward step maps u = u^n to the root w = u^{n+1} of F(w; u) = w - u + theta G(w) + (1 - theta) G(u) (identity
+// rows at Dirichlet end nodes), G_i(v) = h v_i (v_{i+1} - v_{i-1}) - r (v_{i+1} - 2 v_i + v_{i-1}), h = dt/(2 dx),
+// r = nu dt/dx^2.  By the implicit-function theorem (dF/dw = J(w), dF/du = -I + (1 - theta) M G'(u), M = zero rows at
+// Dirichlet ends) the reverse step is
+//     J(u^{n+1})^T mu = lam^{n+1},
+//     lam^n_i = mu_i - (1 - theta) [ (h u_{i-1} - r) m_{i-1} + (h (u_{i+1} - u_{i-1}) + 2 r) m_i + (-h u_{i+1} - r) m_{i+1} ],
+// m = M mu, u = u^n, neighbours cyclic.  Row j of J^T is (sup_{j-1}, diag_j, sub_{j+1}) with J's rows
+//     sub_i = theta (-h w_i - r),  diag_i = 1 + theta (h (w_{i+1} - w_{i-1}) + 2 r),  sup_i = theta (h w_i - r)
+// (Eq.14 / reading Q5) at w = u^{n+1}; identity rows of J at Dirichlet ends make the wrap entries of J^T zero, so
+// the cyclic form serves both boundary types.  Like J itself, J^T is eliminated without pivoting (cell Peclet
+// number <= 2, D11) with the machinery of the forward solver (btcs_common.cuh).
+//
+// This is the derivative of the map the CONVERGED iteration defines: run the forward sweep with a tolerance
+// near rounding.  The forward states u^1 .. u^n come from burgers_newton_traj_* (one snapshot per step).  Plans:
+//   RESIDENT  one CTA per system, lam and u^{n+1} in registers across the steps, u^n streamed in, any N that fits
+//             one CTA (exact or ragged partitions as btcs_hybrid.cu);
+//   THOMAS    one thread per system on [B][N] as it lies (the general-shape fallback), Sherman-Morrison for
+//             periodic systems; scratch 3 B N.
+#include "btcs_common.cuh"
+
+namespace burgers {
+namespace {
+
+using namespace btcs;
+
+constexpr int adjn_max_threads(int bytes, int P) {
+    int regs = P * (bytes / 4) * 6 + 56;
+    int t = 1024;
+    while (t > 32 && t * regs > 65536) t /= 2;
+    return t;
+}
+
+template <typename T, int P, bool RAGGED>
+__global__ void __launch_bounds__(adjn_max_threads(sizeof(T), P))
+adjoint_newton_resident_kernel(const T *__restrict__ u0, const T *__restrict__ states, T *__restrict__ lam,
+                               const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int N, double inv_dx,
+                               int64_t n_steps, int bc, T theta) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1;
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
+    T *sE = sF + 3 * Tn;                      // [6][Tn] partition edge values of u^n, u^{n+1} and M mu
+    Part part;
+    part.r0 = t * P; part.n = P;
+    if (RAGGED) part = partition_of(t, N, Tn);
+    const int n = part.n;
+    __builtin_assume(n >= P - 1 && n <= P);
+    const int64_t b = blockIdx.x, BN = B * (int64_t)N, off = b * N + part.r0;
+
+    const double dtb = (double)dt[b];
+    const T h = (T)(0.5 * dtb * inv_dx);
+    const T r = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
+    const T th = theta * h, tr = theta * r, omt = T(1) - theta;
+    const T b0 = T(1) + T(2) * tr;
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    const bool fixL = dirichlet && t == 0, fixR = dirichlet && t == Tn - 1;
+    auto state = [&](int64_t k) { return (k == 0) ? u0 : states + (size_t)(k - 1) * (size_t)BN; };
+    auto load = [&](const T *src, T (&dst)[P]) {
+#pragma unroll
+        for (int j = 0; j < P; ++j) dst[j] = (j < n) ? src[off + j] : T(0);
+    };
+    auto last_of = [&](const T (&a)[P]) {          // value of slot n - 1 without a run-time register index
+        T x = a[0];
+#pragma unroll
+        for (int j = 1; j < P; ++j)
+            if (j < n) x = a[j];
+        return x;
+    };
+    auto frozen_at = [&](int j) { return (j == 0 && fixL) || (j >= n - 1 && fixR); };
+    const bool frozL = dirichlet && t == 0;        // the row left of this partition (wrap: row N-1) is an end node
+    const bool frozR = dirichlet && t == Tn - 1;   // the row right of it (wrap: row 0)
+
+    T l[P], u[P], up[P];
+    load(lam, l);
+    load(state(n_steps), up);
+    for (int64_t k = n_steps - 1; k >= 0; --k) {
+        load(state(k), u);
+        sE[t] = u[0]; sE[Tn + t] = last_of(u); sE[2 * Tn + t] = up[0]; sE[3 * Tn + t] = last_of(up);
+        __syncthreads();
+        const int tl = (t - 1) & mask, tr_ = (t + 1) & mask;
+        const T uL = sE[Tn + tl], uR = sE[tr_], upL = sE[3 * Tn + tl], upR = sE[2 * Tn + tr_];
+        // ---- J(u^{n+1})^T mu = lam
+        T f[P], c[P];
+        Row<T> first, last;
+        auto rowT = [&](int j, T &a, T &bb, T &e) {        // row j of J^T: (sup_{j-1}, diag_j, sub_{j+1})
+            const bool lastrow = (j >= n - 1);
+            const T wm = j ? up[j - 1] : upL, wp = lastrow ? upR : up[(j + 1 < P) ? j + 1 : j];
+            const bool fm = j ? frozen_at(j - 1) : frozL, fp = lastrow ? frozR : frozen_at(j + 1);
+            a = fm ? T(0) : t_fma(th, wm, -tr);             // sup_{j-1} = theta (h w_{j-1} - r)
+            e = fp ? T(0) : t_fma(-th, wp, -tr);            // sub_{j+1} = theta (-h w_{j+1} - r)
+            bb = frozen_at(j) ? T(1) : t_fma(th, wp - wm, b0);
+        };
+        if (RAGGED) eliminate_general_ragged<T, P>(rowT, n, l, f, c, first, last);
+        else eliminate_general<T, P>(rowT, l, f, c, first, last);
+        T x0, xL;
+        solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
+        T mu[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) mu[j] = T(0);
+        if (RAGGED) back_substitute_ragged<T, P>(mu, n, f, c, l, x0, xL);
+        else back_substitute<T, P>(mu, f, c, l, x0, xL);
+        // ---- lam^n = mu - (1 - theta) G'(u^n)^T (M mu)
+        T m[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) m[j] = frozen_at(j) ? T(0) : mu[j];
+        sE[4 * Tn + t] = m[0]; sE[5 * Tn + t] = last_of(m);
+        __syncthreads();
+        const T mL = sE[5 * Tn + tl], mR = sE[4 * Tn + tr_];
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            if (j < n) {
+                const bool lastrow = (j >= n - 1);
+                const T vm = j ? u[j - 1] : uL, vp = lastrow ? uR : u[(j + 1 < P) ? j + 1 : j];
+                const T mm = j ? m[j - 1] : mL, mp = lastrow ? mR : m[(j + 1 < P) ? j + 1 : j];
+                T g = t_fma(h, vm, -r) * mm;
+                g = t_fma(t_fma(h, vp - vm, T(2) * r), m[j], g);
+                g = t_fma(t_fma(-h, vp, -r), mp, g);
+                l[j] = t_fma(-omt, g, mu[j]);
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < P; ++j) up[j] = u[j];
+        __syncthreads();                                   // sE is rewritten by the next step
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j)
+        if (j < n) lam[off + j] = l[j];
+}
+
+// ---- thread-per-system fallback on the caller's [B][N] layout.  ws: cp, dp, wp ([B][N] each).
+template <typename T>
+__global__ void __launch_bounds__(64)
+adjoint_newton_thomas_kernel(const T *__restrict__ u0, const T *__restrict__ states, T *__restrict__ lam,
+                             T *__restrict__ ws, const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int64_t N,
+                             double inv_dx, int64_t n_steps, int bc, T theta) {
+    const int64_t b = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= B) return;
+    const int64_t BN = B * N;
+    const double dtb = (double)dt[b];
+    const T h = (T)(0.5 * dtb * inv_dx);
+    const T r = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
+    const T th = theta * h, tr = theta * r, omt = T(1) - theta;
+    const T b0 = T(1) + T(2) * tr;
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    T *cp = ws + b * N, *dp = ws + BN + b * N, *wp = ws + 2 * BN + b * N, *l = lam + b * N;
+    auto frozen = [&](int64_t i) { return dirichlet && (i == 0 || i == N - 1); };
+    auto rowT = [&](const T *w, int64_t j, T &a, T &bb, T &e) {      // row j of J(w)^T, cyclic neighbours
+        const int64_t jm = (j == 0) ? N - 1 : j - 1, jp = (j == N - 1) ? 0 : j + 1;
+        a = frozen(jm) ? T(0) : t_fma(th, w[jm], -tr);
+        e = frozen(jp) ? T(0) : t_fma(-th, w[jp], -tr);
+        bb = frozen(j) ? T(1) : t_fma(th, w[jp] - w[jm], b0);
+    };
+    for (int64_t k = n_steps - 1; k >= 0; --k) {
+        const T *u = ((k == 0) ? u0 : states + (size_t)(k - 1) * (size_t)BN) + b * N;
+        const T *up = states + (size_t)k * (size_t)BN + b * N;
+        // cyclic Thomas by Sherman-Morrison (D6) on the transposed rows; for Dirichlet the corner entries are zero,
+        // the correction term vanishes and the plain solve remains
+        T a, bb, e;
+        rowT(up, 0, a, bb, e);
+        const T alpha = a;                       // corner (0, N-1)
+        T aN, bN, eN;
+        rowT(up, N - 1, aN, bN, eN);
+        const T beta = eN;                       // corner (N-1, 0)
+        const T gamma = -bb;
+        T m = bb - gamma;
+        cp[0] = e / m; dp[0] = l[0] / m; wp[0] = gamma / m;
+        for (int64_t j = 1; j < N; ++j) {
+            rowT(up, j, a, bb, e);
+            if (j == N - 1) bb = bb - alpha * beta / gamma;
+            m = bb - a * cp[j - 1];
+            cp[j] = e / m;
+            dp[j] = (l[j] - a * dp[j - 1]) / m;
+            wp[j] = (((j == N - 1) ? beta : T(0)) - a * wp[j - 1]) / m;
+        }
+        for (int64_t j = N - 2; j >= 0; --j) {
+            dp[j] = dp[j] - cp[j] * dp[j + 1];
+            wp[j] = wp[j] - cp[j] * wp[j + 1];
+        }
+        const T fact = (dp[0] + alpha / gamma * dp[N - 1]) / (T(1) + wp[0] + alpha / gamma * wp[N - 1]);
+        for (int64_t j = 0; j < N; ++j) dp[j] = dp[j] - fact * wp[j];            // mu
+        auto masked = [&](int64_t i) { return frozen(i) ? T(0) : dp[i]; };
+        for (int64_t j = 0; j < N; ++j) {
+            const int64_t jm = (j == 0) ? N - 1 : j - 1, jp = (j == N - 1) ? 0 : j + 1;
+            T g = t_fma(h, u[jm], -r) * masked(jm);
+            g = t_fma(t_fma(h, u[jp] - u[jm], T(2) * r), masked(j), g);
+            g = t_fma(t_fma(-h, u[jp], -r), masked(jp), g);
+            l[j] = t_fma(-omt, g, dp[j]);
+        }
+    }
+}
+
+bool adjn_geometry(int is_f64, int64_t N, int *P_out, int *T_out, bool *ragged) {
+    const int bytes = is_f64 ? 8 : 4;
+    return pick_partition(N, [bytes](int P) { return adjn_max_threads(bytes, P); }, P_out, T_out, ragged);
+}
+
+template <typename T, int P>
+int launch_resident_P(const T *u0, const T *states, T *lam, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
+                      int64_t n_steps, int bc, double theta, int Tn, bool ragged, cudaStream_t s) {
+    const size_t smem = (size_t)15 * Tn * sizeof(T);
+    if (ragged) {
+        adjoint_newton_resident_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u0, states, lam, nu, dt, B, (int)N,
+                                                                               1.0 / dx, n_steps, bc, (T)theta);
+        return last_launch_status();
+    }
+    if constexpr (P == 4 || P == 8 || P == 16) {
+        adjoint_newton_resident_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u0, states, lam, nu, dt, B, (int)N,
+                                                                                1.0 / dx, n_steps, bc, (T)theta);
+        return last_launch_status();
+    }
+    return BURGERS_ERR_PLAN;
+}
+
+}  // namespace
+
+size_t adjoint_newton_ws_elems(int is_f64, int64_t B, int64_t N) {
+    int P, Tn;
+    bool ragged;
+    return adjn_geometry(is_f64, N, &P, &Tn, &ragged) ? 0 : (size_t)3 * (size_t)B * (size_t)N;
+}
+
+template <typename T>
+int launch_adjoint_newton_steps(const T *u0, const T *states, T *lam, T *ws, int64_t B, int64_t N, double dx,
+                                const T *nu, const T *dt, int64_t n_steps, int bc, double theta, cudaStream_t s) {
+    if (n_steps == 0) return BURGERS_OK;
+    if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+    int P, Tn;
+    bool ragged;
+    if (adjn_geometry(sizeof(T) == 8, N, &P, &Tn, &ragged)) {
+        switch (P) {
+#define BURGERS_CASE(PP) \
+    case PP: return launch_resident_P<T, PP>(u0, states, lam, B, N, dx, nu, dt, n_steps, bc, theta, Tn, ragged, s);
+            BURGERS_CASE(4) BURGERS_CASE(5) BURGERS_CASE(6) BURGERS_CASE(7) BURGERS_CASE(8) BURGERS_CASE(9)
+            BURGERS_CASE(10) BURGERS_CASE(11) BURGERS_CASE(12) BURGERS_CASE(13) BURGERS_CASE(14) BURGERS_CASE(15)
+            BURGERS_CASE(16)
+#undef BURGERS_CASE
+        }
+        return BURGERS_ERR_PLAN;
+    }
+    adjoint_newton_thomas_kernel<T><<<(unsigned)((B + 63) / 64), 64, 0, s>>>(u0, states, lam, ws, nu, dt, B, N, 1.0 / dx,
+                                                                           n_steps, bc, (T)theta);
+    return last_launch_status();
+}
+
+template int launch_adjoint_newton_steps<float>(const float *, const float *, float *, float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, cudaStream_t);
+template int launch_adjoint_newton_steps<double>(const double *, const double *, double *, double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, cudaStream_t);
+
+}  // namespace burgers

@@ -339,6 +339,41 @@ int newton_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T 
     return BURGERS_OK;
 }
 
+// Reverse mode of the Newton / theta-scheme: forward sweep with one snapshot per step (newton_traj_call), then the
+// backward sweep of adjoint_newton.cu.  ws: [work state B N][states n_steps B N][backward scratch][Newton workspace].
+template <typename T>
+size_t newton_adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps) {
+    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
+    const size_t st = align_up((size_t)n_steps * (size_t)B * (size_t)N * sizeof(T), 256);
+    const size_t sc = align_up(adjoint_newton_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
+    return bn + st + sc + burgers_workspace_bytes(BURGERS_OP_NEWTON, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
+}
+
+template <typename T>
+int newton_adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
+                        int bc, double theta, double tol, int max_iter, void *ws, size_t ws_bytes, void *stream) {
+    if (!lam) return BURGERS_ERR_NULL;
+    int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
+    if (st != BURGERS_OK) return st;
+    if (!(tol >= 0.0) || max_iter < 0 || !(theta >= 0.0 && theta <= 1.0)) return BURGERS_ERR_VALUE;
+    if (n_steps == 0) return BURGERS_OK;
+    if (!ws || ws_bytes < newton_adjoint_ws_bytes<T>(B, N, bc, n_steps)) return BURGERS_ERR_WORKSPACE;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t BN = (size_t)B * (size_t)N;
+    const size_t bn = align_up(BN * sizeof(T), 256), stb = align_up((size_t)n_steps * BN * sizeof(T), 256);
+    const size_t scb = align_up(adjoint_newton_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
+    unsigned char *base = static_cast<unsigned char *>(ws);
+    T *work = reinterpret_cast<T *>(base);
+    T *states = reinterpret_cast<T *>(base + bn);
+    T *scratch = reinterpret_cast<T *>(base + bn + stb);
+    void *nws = base + bn + stb + scb;
+    if (cudaMemcpyAsync(work, u0, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
+    st = newton_traj_call<T>(work, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, nullptr, 1, states, nws,
+                             ws_bytes - (bn + stb + scb), stream);
+    if (st != BURGERS_OK) return st;
+    return launch_adjoint_newton_steps<T>(u0, states, lam, scratch, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, theta, s);
+}
+
 template <typename T>
 int cfl_call(const T *u, int64_t B, int64_t N, double L, const T *nu, double C, int bc, T *dt_out,
              void *stream) {
@@ -681,6 +716,21 @@ int burgers_btcs_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N
 size_t burgers_btcs_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
     if (B < 1 || N < 3 || n_steps < 0) return 0;
     return dtype_is_f64 ? btcs_adjoint_ws_bytes<double>(B, N, bc, n_steps) : btcs_adjoint_ws_bytes<float>(B, N, bc, n_steps);
+}
+
+int burgers_newton_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu, const float *dt,
+                               int64_t n_steps, int bc, double theta, double tol, int max_iter, void *ws, size_t ws_bytes,
+                               void *stream) {
+    return newton_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, ws, ws_bytes, stream);
+}
+int burgers_newton_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                               const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter, void *ws,
+                               size_t ws_bytes, void *stream) {
+    return newton_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, ws, ws_bytes, stream);
+}
+size_t burgers_newton_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
+    if (B < 1 || N < 3 || n_steps < 0) return 0;
+    return dtype_is_f64 ? newton_adjoint_ws_bytes<double>(B, N, bc, n_steps) : newton_adjoint_ws_bytes<float>(B, N, bc, n_steps);
 }
 
 int burgers_btcs_gs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

@@ -132,6 +132,13 @@ int launch_adjoint_rk4_steps(const T *start, const T *states, T *lam, T *ws, int
                              const T *dt, int64_t len, int bc, cudaStream_t s);
 size_t adjoint_rk4_ws_elems(int64_t B, int64_t N);
 
+// ---------------------------------------------------------------- reverse mode of the Newton / theta-scheme (adjoint_newton.cu)
+// states: u^1 .. u^{n_steps} ([n_steps][B][N]); ws: adjoint_newton_ws_elems elements (0 when the resident plan runs)
+template <typename T>
+int launch_adjoint_newton_steps(const T *u0, const T *states, T *lam, T *ws, int64_t B, int64_t N, double dx,
+                                const T *nu, const T *dt, int64_t n_steps, int bc, double theta, cudaStream_t s);
+size_t adjoint_newton_ws_elems(int is_f64, int64_t B, int64_t N);
+
 // ---------------------------------------------------------------- adjoint of BTCS (adjoint_btcs.cu)
 // states: u^1 .. u^{n_steps} ([n_steps][B][N]); ws: adjoint_btcs_ws_elems elements (0 when the resident plan runs)
 template <typename T>

@@ -188,3 +188,64 @@ def test_btcs_adjoint_against_finite_differences_of_the_gpu_forward_path(B):
     lam = to_dev(lam_T.copy())
     B.burgers_btcs_adjoint(to_dev(w.u0), lam, w.L, to_dev(w.nu), to_dev(dt), 0, w.bc)
     np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
+
+
+# ---------------------------------------------------------------- D16: reverse mode of the Newton / theta-scheme
+def _newton_adjoint_cases(dtype):
+    """(workload, u0, nu, n_steps): cell Peclet number |u| dx / nu < 2 everywhere (the Jacobian needs no pivoting)."""
+    out = []
+    w = W.c3_periodic_btcs(B=5, N=2048, n_steps=0, dtype=dtype)          # resident, exact partitions, mixed signs
+    out.append((w, w.u0.copy(), w.nu.copy(), 10))
+    w = W.c3_periodic_btcs(B=6, N=201, n_steps=0, dtype=dtype)           # the paper's grid: ragged partitions
+    out.append((w, w.u0.copy(), np.full(6, 0.1, dtype), 12))
+    w = W.c2_dirichlet_batch(B=4, N=1000, dtype=dtype)                   # Dirichlet, ragged
+    u0 = w.u0.copy(); u0[:, 0] = dtype(0.3); u0[:, -1] = dtype(-0.2)
+    out.append((w, u0, np.maximum(w.nu, dtype(5e-3)), 8))
+    w = W.c4b_long_btcs(N=20000, n_steps=0, dtype=dtype)                 # a long grid: thread-per-system fallback
+    out.append((w, w.u0.copy(), np.full(1, 1e-3, dtype), 4))
+    return out
+
+
+@pytest.mark.parametrize("theta", [1.0, 0.5])
+@pytest.mark.parametrize("dtype,tol", [(np.float64, 1e-10), (np.float32, 1e-4)])
+def test_newton_adjoint_matches_oracle(B, dtype, tol, theta):
+    """Reverse mode of the paper's fully implicit scheme (Eq.10-15) and of Crank-Nicolson against the oracle's (D16:
+    pinned by the exact transpose of the linear case, the dense one-step formula and finite differences)."""
+    rng = np.random.default_rng(31)
+    newton_tol = 1e-13 if dtype == np.float64 else 2e-6
+    for w, u0, nu, n in _newton_adjoint_cases(dtype):
+        dt = oracle_dt(u0, w.L, nu, 4.0, w.bc, dtype)
+        lam_T = rng.standard_normal(u0.shape).astype(dtype)
+        ref = oracle.newton_adjoint(u0.astype(np.float64), lam_T.astype(np.float64), w.L, nu.astype(np.float64),
+                                    dt.astype(np.float64), n, w.bc, tol=1e-13, theta=theta)
+        d_u0 = to_dev(u0.copy()); lam = to_dev(lam_T.copy())
+        B.burgers_newton_adjoint(d_u0, lam, w.L, to_dev(nu), to_dev(dt), n, w.bc, theta=theta, tol=newton_tol)
+        got = lam.cpu().numpy().astype(np.float64)
+        scale = np.abs(ref).max(axis=1, keepdims=True)
+        assert np.isfinite(got).all(), w.name
+        assert (np.abs(got - ref) / scale).max() <= tol, (w.name, theta)
+        np.testing.assert_array_equal(d_u0.cpu().numpy(), u0)          # u0 untouched
+
+
+def test_newton_adjoint_against_finite_differences_of_the_gpu_forward_path(B):
+    rng = np.random.default_rng(37)
+    w = W.c3_periodic_btcs(B=2, N=256, n_steps=0)
+    nu = np.full(2, 0.05)
+    dt = oracle_dt(w.u0, w.L, nu, 4.0, w.bc, np.float64)
+    n = 6
+    lam_T = rng.standard_normal(w.u0.shape); v = rng.standard_normal(w.u0.shape)
+    for theta in (1.0, 0.5):
+        lam = to_dev(lam_T.copy())
+        B.burgers_newton_adjoint(to_dev(w.u0), lam, w.L, to_dev(nu), to_dev(dt), n, w.bc, theta=theta)
+        g = lam.cpu().numpy()
+        eps = 1e-6
+
+        def J(u0):
+            u = to_dev(u0.copy()); B.burgers_newton(u, w.L, to_dev(nu), to_dev(dt), n, w.bc, tol=1e-13, theta=theta)
+            return (lam_T * u.cpu().numpy()).sum(axis=1)
+        fd = (J(w.u0 + eps * v) - J(w.u0 - eps * v)) / (2 * eps)
+        an = (g * v).sum(axis=1)
+        assert np.all(np.abs(fd - an) <= 1e-6 * (1 + np.abs(an))), theta
+    lam = to_dev(lam_T.copy())
+    B.burgers_newton_adjoint(to_dev(w.u0), lam, w.L, to_dev(nu), to_dev(dt), 0, w.bc)
+    np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
