@@ -304,10 +304,12 @@ class GpuRunner:
             self.launches = B.launch_count(B.OP_EXPLICIT, is64, w.B, w.N, w.bc, spec["scheme"], n_steps=w.n_steps)
         elif spec["op"] == "adjoint":
             self.plan = 0
-            if spec["scheme"] >= 2:      # implicit schemes: one forward launch per step (+ its copy), one backward launch
+            if spec["scheme"] >= 2:      # implicit schemes: forward sweep (one launch when the system fits one CTA: the
+                #                          kernel writes the states; else one per step) + one backward launch
                 q = B.raw().burgers_btcs_adjoint_workspace_bytes if spec["scheme"] == 2 else B.raw().burgers_newton_adjoint_workspace_bytes
                 need = int(q(int(is64), w.B, w.N, w.bc, w.n_steps))
-                self.launches = w.n_steps + 1
+                fits = B.plan_query(B.OP_BTCS if spec["scheme"] == 2 else B.OP_NEWTON, is64, w.B, w.N, w.bc) == B.PLAN_HYBRID
+                self.launches = 2 if fits else w.n_steps + 1
             else:
                 need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, spec["scheme"], w.n_steps, 0))
                 # Euler: forward trajectory kernel + resident backward kernel; RK4: forward + 7 launches per step

@@ -213,8 +213,9 @@ int burgers_btcs_plan_f64(double *u, int64_t B, int64_t N, double L, const doubl
                           const double *dt, int64_t n_steps, int bc, int plan, void *ws,
                           size_t ws_bytes, void *stream);
 
-/* BTCS with trajectory output, semantics as burgers_explicit_traj_*: one run of the AUTO plan per
- * snapshot interval followed by a device copy (workspace as for burgers_btcs_*). */
+/* BTCS with trajectory output, semantics as burgers_explicit_traj_*.  Systems that fit one CTA (plan HYBRID):
+ * ONE launch, the kernel stores the state after every snap_every-th step; longer grids: one run of the AUTO
+ * plan per snapshot interval followed by a device copy (workspace as for burgers_btcs_*). */
 int burgers_btcs_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                           int64_t n_steps, int bc, int64_t snap_every, float *snaps, void *ws,
                           size_t ws_bytes, void *stream);
@@ -272,9 +273,10 @@ int burgers_newton_f64(double *u, int64_t B, int64_t N, double L, const double *
                        int64_t n_steps, int bc, double theta, double tol, int max_iter,
                        int64_t *iters_out, int plan, void *ws, size_t ws_bytes, void *stream);
 
-/* The same with TRAJECTORY output, semantics as burgers_explicit_traj_* / burgers_btcs_traj_*: one run of the AUTO
- * plan per snapshot interval followed by a device copy into snaps[k][B][N] (room for floor(n_steps/snap_every)
- * snapshots); iters_out receives the totals over all intervals.  Workspace as for burgers_newton_* (AUTO plan). */
+/* The same with TRAJECTORY output, semantics as burgers_explicit_traj_* / burgers_btcs_traj_*: one launch that
+ * stores snaps[k][B][N] from inside the kernel when the system fits one CTA, else one run of the AUTO plan per
+ * snapshot interval followed by a device copy (room for floor(n_steps/snap_every) snapshots); iters_out receives
+ * the totals over all intervals.  Workspace as for burgers_newton_* (AUTO plan). */
 int burgers_newton_traj_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                             int64_t n_steps, int bc, double theta, double tol, int max_iter,
                             int64_t *iters_out, int64_t snap_every, float *snaps, void *ws, size_t ws_bytes,

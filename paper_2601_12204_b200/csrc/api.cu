@@ -230,6 +230,9 @@ int btcs_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *d
     if (snap_every < 1) return BURGERS_ERR_SHAPE;
     int st = check_common(u, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
+    if (btcs_auto_plan(sizeof(T) == 8, B, N, bc) == BURGERS_PLAN_HYBRID)       // snapshots written by the kernel: one launch
+        return launch_btcs_hybrid_traj<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, snap_every, snaps,
+                                          (cudaStream_t)stream);
     int64_t done = 0, k = 0;
     while (done < n_steps) {
         const int64_t chunk = (n_steps - done < snap_every) ? n_steps - done : snap_every;
@@ -311,8 +314,9 @@ int newton_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, 
                             reinterpret_cast<long long *>(iters_out), plan, (T *)ws, (cudaStream_t)stream, accumulate);
 }
 
-// Newton / theta-scheme with trajectory output: one run of the plan per snapshot interval (the state is stored once
-// per interval anyway), a device copy of u into snaps[k]; the iteration totals accumulate over the intervals.
+// Newton / theta-scheme with trajectory output: shapes of the HYBRID plan write the snapshots from inside the kernel
+// (one launch); otherwise one run of the plan per snapshot interval and a device copy of u into snaps[k], the
+// iteration totals accumulating over the intervals.
 template <typename T>
 int newton_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc, double theta,
                      double tol, int max_iter, int64_t *iters_out, int64_t snap_every, T *snaps, void *ws, size_t ws_bytes,
@@ -322,6 +326,10 @@ int newton_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T 
     int st = newton_call<T>(u, B, N, L, nu, dt, 0, bc, theta, tol, max_iter, iters_out, BURGERS_PLAN_AUTO, ws, ws_bytes,
                             stream);                       // validates everything, zeroes iters_out
     if (st != BURGERS_OK) return st;
+    if (newton_hybrid_fits(sizeof(T) == 8, N))       // snapshots written by the kernel: one launch
+        return launch_newton<T>(u, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, theta, tol, max_iter,
+                                reinterpret_cast<long long *>(iters_out), BURGERS_PLAN_HYBRID, (T *)ws, (cudaStream_t)stream,
+                                true, snaps, snap_every);
     int64_t done = 0, k = 0;
     while (done < n_steps) {
         const int64_t chunk = (n_steps - done < snap_every) ? n_steps - done : snap_every;

@@ -62,11 +62,15 @@ constexpr int hybrid_max_threads(int bytes, int P) {
 // Any N: thread t owns the P - 1 or P rows partition_of() deals it (btcs_common.cuh), scalar loads -- the state
 // is loaded and stored once per CALL, so the load width does not matter.  Same steps as the kernel above, through
 // the shared helpers (eliminate_general_ragged, solve_interface, back_substitute_ragged).
-template <typename T, int P>
+// SNAP: trajectory output from inside the time loop -- after every snap_every-th step the state goes to
+// snaps[k][b][:] (k = 0, 1, ...; BN = B N elements per snapshot), so that burgers_btcs_traj_* and the forward sweep
+// of the BTCS adjoint are ONE launch instead of one launch + one copy per snapshot (RAGGED = false: the exact
+// partitions of the kernel above, through the helpers).
+template <typename T, int P, bool RAGGED, bool SNAP>
 __global__ void __launch_bounds__(hybrid_max_threads(sizeof(T), P))
-btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
-                   double inv_dx, int64_t n_steps, int bc) {
-    constexpr bool RAGGED = true;
+btcs_hybrid_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
+                           double inv_dx, int64_t n_steps, int bc, T *__restrict__ snaps, int64_t snap_every,
+                           int64_t BN) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = blockDim.x;
@@ -98,6 +102,8 @@ btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *
         }
     }
 
+    int64_t until_snap = snap_every;
+    T *snap_row = SNAP ? snaps + (int64_t)blockIdx.x * N + part.r0 : nullptr;
     for (int64_t step = 0; step < n_steps; ++step) {
         T f[P], c[P], q[P];
         // ---- assembly + partition elimination
@@ -121,6 +127,27 @@ btcs_hybrid_ragged_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *
         // ---- back substitution
         if (RAGGED) back_substitute_ragged<T, P>(v, n, f, c, q, x0, xL);
         else back_substitute<T, P>(v, f, c, q, x0, xL);
+        if (SNAP) {
+            if (--until_snap == 0) {
+                until_snap = snap_every;
+                T *srow = snap_row;
+                snap_row += BN;
+                if (RAGGED) {
+#pragma unroll
+                    for (int j = 0; j < P; ++j)
+                        if (j < n) srow[j] = v[j];
+                } else {
+#pragma unroll
+                    for (int c2 = 0; c2 < P / V; ++c2) {
+                        int4 q4;
+                        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+                        for (int k = 0; k < V; ++k) e[k] = v[c2 * V + k];
+                        *reinterpret_cast<int4 *>(srow + c2 * V) = q4;
+                    }
+                }
+            }
+        }
     }
 
     if (RAGGED) {
@@ -150,7 +177,8 @@ int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, in
              int Tn, bool ragged, cudaStream_t s) {
     const size_t smem = (size_t)9 * Tn * sizeof(T);
     if (ragged) {
-        btcs_hybrid_ragged_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc);
+        btcs_hybrid_general_kernel<T, P, true, false><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                                  nullptr, 0, 0);
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
@@ -185,6 +213,23 @@ int launch_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, in
     return BURGERS_ERR_PLAN;
 }
 
+template <typename T, int P>
+int launch_traj_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                  int64_t snap_every, T *snaps, int Tn, bool ragged, cudaStream_t s) {
+    const size_t smem = (size_t)9 * Tn * sizeof(T);
+    if (ragged) {
+        btcs_hybrid_general_kernel<T, P, true, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                                 snaps, snap_every, B * N);
+        return last_launch_status();
+    }
+    if constexpr (P == 4 || P == 8 || P == 16) {
+        btcs_hybrid_general_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                                  snaps, snap_every, B * N);
+        return last_launch_status();
+    }
+    return BURGERS_ERR_PLAN;
+}
+
 }  // namespace
 
 bool btcs_hybrid_fits(int is_f64, int64_t N, int bc) {
@@ -211,6 +256,27 @@ int launch_btcs_hybrid(T *u, int64_t B, int64_t N, double dx, const T *nu, const
     return BURGERS_ERR_PLAN;
 }
 
+// n_steps steps with a snapshot after every snap_every-th one (snaps: [n_steps / snap_every][B][N]); one launch.
+template <typename T>
+int launch_btcs_hybrid_traj(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                            int64_t snap_every, T *snaps, cudaStream_t s) {
+    if (n_steps == 0) return BURGERS_OK;
+    int P, Tn;
+    bool ragged;
+    if (!hybrid_geometry(sizeof(T) == 8, N, &P, &Tn, &ragged)) return BURGERS_ERR_PLAN;
+    if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
+    switch (P) {
+#define BURGERS_CASE(PP) \
+    case PP: return launch_traj_P<T, PP>(u, B, N, dx, nu, dt, n_steps, bc, snap_every, snaps, Tn, ragged, s);
+        BURGERS_CASE(4) BURGERS_CASE(5) BURGERS_CASE(6) BURGERS_CASE(7) BURGERS_CASE(8) BURGERS_CASE(9) BURGERS_CASE(10)
+        BURGERS_CASE(11) BURGERS_CASE(12) BURGERS_CASE(13) BURGERS_CASE(14) BURGERS_CASE(15) BURGERS_CASE(16)
+#undef BURGERS_CASE
+    }
+    return BURGERS_ERR_PLAN;
+}
+
+template int launch_btcs_hybrid_traj<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, int64_t, float *, cudaStream_t);
+template int launch_btcs_hybrid_traj<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, int64_t, double *, cudaStream_t);
 template int launch_btcs_hybrid<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, cudaStream_t);
 template int launch_btcs_hybrid<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, cudaStream_t);
 

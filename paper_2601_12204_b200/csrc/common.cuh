@@ -110,6 +110,10 @@ template <typename T>
 int launch_btcs_hybrid(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt,
                        int64_t n_steps, int bc, cudaStream_t s);
 bool btcs_hybrid_fits(int is_f64, int64_t N, int bc);
+// the same with trajectory output from inside the kernel (one launch): snaps[k] after every snap_every-th step
+template <typename T>
+int launch_btcs_hybrid_traj(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
+                            int64_t snap_every, T *snaps, cudaStream_t s);
 
 // LONG: one system across many CTAs.  `ws` holds the ping-pong state, the global interface rows
 // and the status word (btcs_long_ws_bytes).  general_only != 0 runs the cooperative GENERAL
@@ -156,7 +160,7 @@ size_t btcs_gs_ws_elems(int64_t B, int64_t N);
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
                   double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s,
-                  bool accumulate = false);
+                  bool accumulate = false, T *snaps = nullptr, int64_t snap_every = 0);   // snaps: HYBRID plan only
 bool newton_hybrid_fits(int is_f64, int64_t N);
 size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc);
 

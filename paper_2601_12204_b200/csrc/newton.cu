@@ -43,11 +43,14 @@ constexpr int newton_max_threads(int bytes, int P) {
 // it (btcs_common.cuh) in the first n of its P register slots; otherwise N == P * blockDim.x.
 // TN: the thread count as a compile-time constant for the SMALL instances (PCR levels unrolled), else 0.
 // PERIODIC: the boundary type is known to be periodic (no identity-row selects); false: decided by `bc`.
-template <typename T, int P, bool SMALL = false, bool RAGGED = false, int TN = 0, bool PERIODIC = false>
+// SNAP: trajectory output from inside the time loop: after every snap_every-th step the state goes to
+// snaps[k][b][:] (BN = B N elements per snapshot) -- burgers_newton_traj_* and the forward sweep of the reverse
+// mode are then one launch (the three trailing parameters are unused otherwise).
+template <typename T, int P, bool SMALL = false, bool RAGGED = false, int TN = 0, bool PERIODIC = false, bool SNAP = false>
 __global__ void __launch_bounds__(SMALL ? 128 : newton_max_threads(sizeof(T), P), SMALL ? 3 : 1)
 newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__restrict__ dt, int N,
                      double inv_dx, int64_t n_steps, int bc, T theta, T tol, int max_iter,
-                     long long *__restrict__ iters_out) {
+                     long long *__restrict__ iters_out, T *__restrict__ snaps, int64_t snap_every, int64_t BN) {
     constexpr int V = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int t = threadIdx.x, Tn = TN ? TN : (int)blockDim.x, mask = Tn - 1;
@@ -83,6 +86,8 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
         }
     }
     long long iters = 0;
+    int64_t until_snap = snap_every;
+    T *snap_row = SNAP ? snaps + (int64_t)blockIdx.x * N + part.r0 : nullptr;
     for (int64_t step = 0; step < n_steps; ++step) {
 #pragma unroll
         for (int j = 0; j < P; ++j) un[j] = w[j];
@@ -143,6 +148,16 @@ newton_hybrid_kernel(T *__restrict__ u, const T *__restrict__ nu, const T *__res
                 if (!RAGGED || j < n) w[j] += d[j];      // Eq.13
             ++iters;
         }
+        if (SNAP) {
+            if (--until_snap == 0) {
+                until_snap = snap_every;
+                T *srow = snap_row;
+                snap_row += BN;
+#pragma unroll
+                for (int j = 0; j < P; ++j)
+                    if (!RAGGED || j < n) srow[j] = w[j];
+            }
+        }
     }
     if (iters_out && t == 0) iters_out[blockIdx.x] += iters;     // (zeroed by launch_newton unless it accumulates)
 
@@ -169,28 +184,41 @@ bool newton_geometry(int is_f64, int64_t N, int *P_out, int *T_out, bool *ragged
 
 template <typename T, int P>
 int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
-                    double theta, double tol, int max_iter, long long *iters_out, int Tn, bool ragged, cudaStream_t s) {
+                    double theta, double tol, int max_iter, long long *iters_out, int Tn, bool ragged, cudaStream_t s,
+                    T *snaps, int64_t snap_every) {
     const size_t smem = (size_t)11 * Tn * sizeof(T);
+    const int64_t BN = B * N;
+#define BURGERS_NEWTON_ARGS u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta, (T)tol, max_iter, iters_out, snaps, snap_every, BN
+    if (snaps) {            // trajectory output: the generic instances, snapshots written by the kernel
+        if (ragged) {
+            newton_hybrid_kernel<T, P, false, true, 0, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
+            return last_launch_status();
+        }
+        if constexpr (P == 4 || P == 8 || P == 16) {
+            if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+                newton_hybrid_kernel<T, P, true, false, 0, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
+            else
+                newton_hybrid_kernel<T, P, false, false, 0, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
+            return last_launch_status();
+        }
+        return BURGERS_ERR_PLAN;
+    }
     if (ragged) {
-        newton_hybrid_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
-                                                                             (T)theta, (T)tol, max_iter, iters_out);
+        newton_hybrid_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
         if (sizeof(T) == 8 && P == 16 && Tn == 128 && bc == BURGERS_BC_PERIODIC)
-            newton_hybrid_kernel<T, P, true, false, 128, true><<<(unsigned)B, Tn, smem, s>>>(
-                u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta, (T)tol, max_iter, iters_out);
+            newton_hybrid_kernel<T, P, true, false, 128, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
         else if (sizeof(T) == 8 && P == 16 && Tn == 128)
-            newton_hybrid_kernel<T, P, true, false, 128><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
-                                                                                      (T)theta, (T)tol, max_iter, iters_out);
+            newton_hybrid_kernel<T, P, true, false, 128><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
         else if (sizeof(T) == 8 && P == 16 && Tn <= 128)
-            newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
-                                                                          (T)theta, (T)tol, max_iter, iters_out);
+            newton_hybrid_kernel<T, P, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
         else
-            newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc, (T)theta,
-                                                                    (T)tol, max_iter, iters_out);
+            newton_hybrid_kernel<T, P><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
         return last_launch_status();
     }
+#undef BURGERS_NEWTON_ARGS
     return BURGERS_ERR_PLAN;
 }
 
@@ -311,7 +339,7 @@ size_t newton_thomas_ws_elems(int64_t B, int64_t N, int bc) {
 template <typename T>
 int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *dt, int64_t n_steps, int bc,
                   double theta, double tol, int max_iter, long long *iters_out, int plan, T *ws, cudaStream_t s,
-                  bool accumulate) {
+                  bool accumulate, T *snaps, int64_t snap_every) {
     // the kernels ADD their iteration totals to iters_out (trajectory output calls this once per interval)
     if (iters_out && !accumulate && cudaMemsetAsync(iters_out, 0, (size_t)B * sizeof(long long), s) != cudaSuccess)
         return BURGERS_ERR_CUDA;
@@ -323,7 +351,9 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
         if (B > 0x7fffffffLL) return BURGERS_ERR_SHAPE;
         switch (P) {
 #define BURGERS_CASE(PP) \
-    case PP: return launch_hybrid_P<T, PP>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s);
+    case PP: \
+        return launch_hybrid_P<T, PP>(u, B, N, dx, nu, dt, n_steps, bc, theta, tol, max_iter, iters_out, Tn, ragged, s, snaps, \
+                                      snap_every);
             BURGERS_CASE(4) BURGERS_CASE(5) BURGERS_CASE(6) BURGERS_CASE(7) BURGERS_CASE(8) BURGERS_CASE(9)
             BURGERS_CASE(10) BURGERS_CASE(11) BURGERS_CASE(12) BURGERS_CASE(13) BURGERS_CASE(14) BURGERS_CASE(15)
             BURGERS_CASE(16)
@@ -332,6 +362,7 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
         return BURGERS_ERR_PLAN;
     }
     // THOMAS
+    if (snaps) return BURGERS_ERR_PLAN;          // (trajectory output through this plan: one call per interval, api.cu)
     const size_t BN = (size_t)B * (size_t)N;
     T *un = ws, *w = ws + BN, *cp = ws + 2 * BN, *dp = ws + 3 * BN, *kn = ws + 4 * BN;
     T *wp = (bc == BURGERS_BC_PERIODIC) ? ws + 5 * BN : nullptr;
@@ -345,7 +376,7 @@ int launch_newton(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
     return launch_transpose<T>(un, u, N, B, s);
 }
 
-template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t, bool);
-template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, double, int, long long *, int, double *, cudaStream_t, bool);
+template int launch_newton<float>(float *, int64_t, int64_t, double, const float *, const float *, int64_t, int, double, double, int, long long *, int, float *, cudaStream_t, bool, float *, int64_t);
+template int launch_newton<double>(double *, int64_t, int64_t, double, const double *, const double *, int64_t, int, double, double, int, long long *, int, double *, cudaStream_t, bool, double *, int64_t);
 
 }  // namespace burgers
