@@ -22,6 +22,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import socket
 import statistics
@@ -122,9 +123,9 @@ def make_workload(name, rank=0, world=1, reduced=False):
         w = W.c5_rk4_ensemble(B=65536 * world, rows=np.arange(0, 65536 * world, 16)[W.shard_rows(Bg, rank, world)],
                               n_steps=10 if reduced else 100)
         return w, dict(op="adjoint", scheme=1, bound="hbm", instr=None, lanes=FP32_LANES)
-    if name in ("c3_btcs_adjoint", "c3_newton_adjoint"):   # reverse mode of 100 implicit steps of 256 C3 trajectories (D15 / D16)
-        Bg = 256 * world
-        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=10 if reduced else 100)
+    if name in ("c3_btcs_adjoint", "c3_newton_adjoint"):   # reverse mode of ALL of C3 (D15 / D16): 4096 trajectories, 1000
+        Bg = 4096 * world                                  # implicit steps; 67 GB of states -> checkpointed (32-step segments)
+        w = W.c3_periodic_btcs(B=Bg, rows=W.shard_rows(Bg, rank, world), n_steps=100 if reduced else 1000)
         if name == "c3_newton_adjoint":
             w.cfl = 4.0
         return w, dict(op="adjoint", scheme=2 if name == "c3_btcs_adjoint" else 3, bound="hbm", instr=None, lanes=FP64_LANES)
@@ -309,7 +310,11 @@ class GpuRunner:
                 q = B.raw().burgers_btcs_adjoint_workspace_bytes if spec["scheme"] == 2 else B.raw().burgers_newton_adjoint_workspace_bytes
                 need = int(q(int(is64), w.B, w.N, w.bc, w.n_steps))
                 fits = B.plan_query(B.OP_BTCS if spec["scheme"] == 2 else B.OP_NEWTON, is64, w.B, w.N, w.bc) == B.PLAN_HYBRID
-                self.launches = 2 if fits else w.n_steps + 1
+                one = w.n_steps * w.B * w.N * w.u0.dtype.itemsize <= (8 << 30)       # one segment (binding: segment = 0)
+                m = w.n_steps if one else math.ceil(math.sqrt(w.n_steps))
+                K = -(-w.n_steps // m)
+                # per segment: forward (one launch if the kernel writes the states, else one per step) + backward
+                self.launches = (1 if K > 1 and fits else 0) + K * ((1 if fits else m) + 1)
             else:
                 need = int(B.raw().burgers_adjoint_scheme_workspace_bytes(int(is64), w.B, w.N, w.bc, spec["scheme"], w.n_steps, 0))
                 # Euler: forward trajectory kernel + resident backward kernel; RK4: forward + 7 launches per step

@@ -227,14 +227,28 @@ int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const doubl
  * One step solves A(u) u' = u; reverse mode:  mu = A(u^n)^{-T} lam,  lam_i <- (1 - D_i) mu_i,
  * D_i = (dt/dx) (u'_i - u'_{i-1}) if u_i > 0 else (dt/dx) (u'_{i+1} - u'_i)  (identity rows, D = 0 at Dirichlet ends).
  * u0: initial state (not modified); lam: in dJ/du^N, out dJ/du^0.  The forward sweep stores every state in the
- * workspace (burgers_btcs_adjoint_workspace_bytes: (n_steps + 1) B N elements + the BTCS workspace; no
- * checkpointing); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
+ * workspace (burgers_btcs_adjoint_workspace_bytes: (n_steps + 1) B N elements + the BTCS workspace while that is
+ * below 8 GiB, checkpointed beyond -- see burgers_btcs_adjoint_ckpt_*); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
  * otherwise). */
 int burgers_btcs_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
                              const float *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream);
 int burgers_btcs_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
                              const double *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream);
 size_t burgers_btcs_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+/* The same with an explicit checkpoint segment, as burgers_explicit_adjoint_ckpt_*: checkpoints every `segment`
+ * steps from a first forward sweep, each segment recomputed (one state per step, written by the forward kernel) and
+ * swept backwards; memory (n_steps/segment + segment + 1) states.  segment = 0: automatic (one segment while all
+ * states fit 8 GiB, else ceil(sqrt(n_steps))) -- what burgers_btcs_adjoint_* / burgers_newton_adjoint_* use, so the
+ * reverse sweep of a full-size config (C3: 1000 steps of 4096 x 2048 = 67 GB of states) fits in 4.5 GB.
+ * op: BURGERS_OP_BTCS or BURGERS_OP_NEWTON (the workspace query serves both schemes). */
+int burgers_btcs_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                  const float *dt, int64_t n_steps, int bc, int64_t segment, void *ws,
+                                  size_t ws_bytes, void *stream);
+int burgers_btcs_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                  const double *dt, int64_t n_steps, int bc, int64_t segment, void *ws,
+                                  size_t ws_bytes, void *stream);
+size_t burgers_implicit_adjoint_ckpt_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, int bc,
+                                                     int64_t n_steps, int64_t segment);
 
 /* ---- BTCS with a Gauss-Seidel inner solver -----------
  * The system of burgers_btcs_* solved per step by lexicographic Gauss-Seidel sweeps from x = u^n until
@@ -294,8 +308,8 @@ int burgers_newton_traj_f64(double *u, int64_t B, int64_t N, double L, const dou
  * Dirichlet ends) -- the derivative of the map the CONVERGED iteration defines: pass a tol near rounding
  * (e.g. 1e-13 in fp64); tol and max_iter drive the forward sweep exactly as in burgers_newton_*.
  * u0: initial state (not modified); lam: in dJ/du^N, out dJ/du^0.  The forward sweep stores every state in the
- * workspace (burgers_newton_adjoint_workspace_bytes: (n_steps + 1) B N elements + the Newton workspace; no
- * checkpointing); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
+ * workspace (burgers_newton_adjoint_workspace_bytes: (n_steps + 1) B N elements + the Newton workspace while that
+ * is below 8 GiB, checkpointed beyond); the backward sweep keeps lam resident per CTA for every N that fits one CTA (thread per system
  * otherwise).  Errors as burgers_newton_*. */
 int burgers_newton_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
                                const float *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
@@ -304,6 +318,14 @@ int burgers_newton_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t
                                const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
                                void *ws, size_t ws_bytes, void *stream);
 size_t burgers_newton_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps);
+/* With an explicit checkpoint segment (see burgers_btcs_adjoint_ckpt_*; workspace:
+ * burgers_implicit_adjoint_ckpt_workspace_bytes(BURGERS_OP_NEWTON, ...)). */
+int burgers_newton_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                    const float *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                                    int64_t segment, void *ws, size_t ws_bytes, void *stream);
+int burgers_newton_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                    const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                                    int64_t segment, void *ws, size_t ws_bytes, void *stream);
 
 /* ---- CFL time step (PAPER.md:116-118 Eq.7-8, :287 Eq.24) -----------------------
  * dt_out[b] = C * min(dx / max_i |u[b][i]|, dx^2 / (2 nu[b])), with x/0 = +inf

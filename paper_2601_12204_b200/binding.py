@@ -41,6 +41,8 @@ EXPORTS = [
     "burgers_launch_count", "burgers_pipe_peak", "burgers_strerror", "burgers_version",
     "burgers_noalloc_scratch_bytes", "burgers_noalloc_init", "burgers_btcs_noalloc",
     "burgers_newton_adjoint_f32", "burgers_newton_adjoint_f64", "burgers_newton_adjoint_workspace_bytes",
+    "burgers_btcs_adjoint_ckpt_f32", "burgers_btcs_adjoint_ckpt_f64", "burgers_newton_adjoint_ckpt_f32",
+    "burgers_newton_adjoint_ckpt_f64", "burgers_implicit_adjoint_ckpt_workspace_bytes",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -70,6 +72,11 @@ for _sfx in ("f32", "f64"):
     getattr(_lib, f"burgers_newton_adjoint_{_sfx}").argtypes = [_p, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64, _int,
                                                                _p, _sz, _p]
     getattr(_lib, f"burgers_newton_adjoint_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_btcs_adjoint_ckpt_{_sfx}").argtypes = [_p, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _sz, _p]
+    getattr(_lib, f"burgers_btcs_adjoint_ckpt_{_sfx}").restype = _int
+    getattr(_lib, f"burgers_newton_adjoint_ckpt_{_sfx}").argtypes = [_p, _p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _f64,
+                                                                    _int, _i64, _p, _sz, _p]
+    getattr(_lib, f"burgers_newton_adjoint_ckpt_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _i64, _p, _p, _sz, _p]
     getattr(_lib, f"burgers_btcs_traj_{_sfx}").restype = _int
     getattr(_lib, f"burgers_btcs_gs_{_sfx}").argtypes = [_p, _i64, _i64, _f64, _p, _p, _i64, _int, _f64, _int, _p, _p, _sz, _p]
@@ -102,6 +109,8 @@ _lib.burgers_btcs_adjoint_workspace_bytes.argtypes = [_int, _i64, _i64, _int, _i
 _lib.burgers_btcs_adjoint_workspace_bytes.restype = _sz
 _lib.burgers_newton_adjoint_workspace_bytes.argtypes = [_int, _i64, _i64, _int, _i64]
 _lib.burgers_newton_adjoint_workspace_bytes.restype = _sz
+_lib.burgers_implicit_adjoint_ckpt_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _int, _i64, _i64]
+_lib.burgers_implicit_adjoint_ckpt_workspace_bytes.restype = _sz
 _lib.burgers_plan_query.argtypes = [_int, _int, _i64, _i64, _int, _int]
 _lib.burgers_plan_query.restype = _int
 _lib.burgers_launch_count.argtypes = [_int, _int, _i64, _i64, _int, _int, _int, _int, _i64]
@@ -294,8 +303,9 @@ def burgers_explicit_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None, segment=0
     return lam
 
 
-def burgers_btcs_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None):
-    """lam <- (du^N/du^0)^T lam for n_steps BTCS steps from u0 (include/burgers.h: burgers_btcs_adjoint_*)."""
+def burgers_btcs_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None, segment=0):
+    """lam <- (du^N/du^0)^T lam for n_steps BTCS steps from u0 (include/burgers.h: burgers_btcs_adjoint_ckpt_*;
+    segment = 0: automatic checkpointing)."""
     import torch
     _dev(u0, "u0"); sfx = _sfx(u0)
     _dev(lam, "lam", u0.dtype); _dev(nu, "nu", u0.dtype); _dev(dt, "dt", u0.dtype)
@@ -303,15 +313,17 @@ def burgers_btcs_adjoint(u0, lam, L, nu, dt, n_steps, bc, ws=None):
     _check_vecs(B, nu=nu, dt=dt)
     if lam.numel() != u0.numel():
         raise ValueError("lam must have the shape of u0")
-    need = int(_lib.burgers_btcs_adjoint_workspace_bytes(int(u0.dtype == torch.float64), B, N, int(bc), int(n_steps)))
+    need = int(_lib.burgers_implicit_adjoint_ckpt_workspace_bytes(OP_BTCS, int(u0.dtype == torch.float64), B, N, int(bc),
+                                                                  int(n_steps), int(segment)))
     wsp, wsb, ws = _ws(ws, need, u0.device)
-    st = getattr(_lib, f"burgers_btcs_adjoint_{sfx}")(u0.data_ptr(), lam.data_ptr(), B, N, float(L), nu.data_ptr(),
-                                                      dt.data_ptr(), int(n_steps), int(bc), wsp, wsb, _stream())
+    st = getattr(_lib, f"burgers_btcs_adjoint_ckpt_{sfx}")(u0.data_ptr(), lam.data_ptr(), B, N, float(L), nu.data_ptr(),
+                                                           dt.data_ptr(), int(n_steps), int(bc), int(segment), wsp, wsb,
+                                                           _stream())
     _check(st, f"burgers_btcs_adjoint_{sfx}")
     return lam
 
 
-def burgers_newton_adjoint(u0, lam, L, nu, dt, n_steps, bc, theta=1.0, tol=1e-13, max_iter=50, ws=None):
+def burgers_newton_adjoint(u0, lam, L, nu, dt, n_steps, bc, theta=1.0, tol=1e-13, max_iter=50, ws=None, segment=0):
     """lam <- (du^N/du^0)^T lam for n_steps Newton / theta-scheme steps from u0 (include/burgers.h:
     burgers_newton_adjoint_*; the forward sweep is iterated to tol)."""
     import torch
@@ -321,11 +333,12 @@ def burgers_newton_adjoint(u0, lam, L, nu, dt, n_steps, bc, theta=1.0, tol=1e-13
     _check_vecs(B, nu=nu, dt=dt)
     if lam.numel() != u0.numel():
         raise ValueError("lam must have the shape of u0")
-    need = int(_lib.burgers_newton_adjoint_workspace_bytes(int(u0.dtype == torch.float64), B, N, int(bc), int(n_steps)))
+    need = int(_lib.burgers_implicit_adjoint_ckpt_workspace_bytes(OP_NEWTON, int(u0.dtype == torch.float64), B, N, int(bc),
+                                                                  int(n_steps), int(segment)))
     wsp, wsb, ws = _ws(ws, need, u0.device)
-    st = getattr(_lib, f"burgers_newton_adjoint_{sfx}")(u0.data_ptr(), lam.data_ptr(), B, N, float(L), nu.data_ptr(),
-                                                        dt.data_ptr(), int(n_steps), int(bc), float(theta), float(tol),
-                                                        int(max_iter), wsp, wsb, _stream())
+    st = getattr(_lib, f"burgers_newton_adjoint_ckpt_{sfx}")(u0.data_ptr(), lam.data_ptr(), B, N, float(L), nu.data_ptr(),
+                                                             dt.data_ptr(), int(n_steps), int(bc), float(theta), float(tol),
+                                                             int(max_iter), int(segment), wsp, wsb, _stream())
     _check(st, f"burgers_newton_adjoint_{sfx}")
     return lam
 

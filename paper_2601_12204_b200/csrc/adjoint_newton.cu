@@ -76,8 +76,12 @@ adjoint_newton_resident_kernel(const T *__restrict__ u0, const T *__restrict__ s
     T l[P], u[P], up[P];
     load(lam, l);
     load(state(n_steps), up);
+    load(state(n_steps - 1), u);
     for (int64_t k = n_steps - 1; k >= 0; --k) {
-        load(state(k), u);
+        // the state of the NEXT backward step is fetched now and consumed at the end of this one: its DRAM latency
+        // (the states are read once, in reverse order, nothing is in cache) hides behind the solve
+        T nx[P];
+        if (k > 0) load(state(k - 1), nx);
         sE[t] = u[0]; sE[Tn + t] = last_of(u); sE[2 * Tn + t] = up[0]; sE[3 * Tn + t] = last_of(up);
         __syncthreads();
         const int tl = (t - 1) & mask, tr_ = (t + 1) & mask;
@@ -97,15 +101,14 @@ adjoint_newton_resident_kernel(const T *__restrict__ u0, const T *__restrict__ s
         else eliminate_general<T, P>(rowT, l, f, c, first, last);
         T x0, xL;
         solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
-        T mu[P];
-#pragma unroll
-        for (int j = 0; j < P; ++j) mu[j] = T(0);
+        // (mu overwrites lam in place: slot j of the right-hand side is read before slot j of the solution is written)
+        T (&mu)[P] = l;
         if (RAGGED) back_substitute_ragged<T, P>(mu, n, f, c, l, x0, xL);
         else back_substitute<T, P>(mu, f, c, l, x0, xL);
         // ---- lam^n = mu - (1 - theta) G'(u^n)^T (M mu)
         T m[P];
 #pragma unroll
-        for (int j = 0; j < P; ++j) m[j] = frozen_at(j) ? T(0) : mu[j];
+        for (int j = 0; j < P; ++j) m[j] = (frozen_at(j) || j >= n) ? T(0) : mu[j];
         sE[4 * Tn + t] = m[0]; sE[5 * Tn + t] = last_of(m);
         __syncthreads();
         const T mL = sE[5 * Tn + tl], mR = sE[4 * Tn + tr_];
@@ -119,10 +122,12 @@ adjoint_newton_resident_kernel(const T *__restrict__ u0, const T *__restrict__ s
                 g = t_fma(t_fma(h, vp - vm, T(2) * r), m[j], g);
                 g = t_fma(t_fma(-h, vp, -r), mp, g);
                 l[j] = t_fma(-omt, g, mu[j]);
+            } else {
+                l[j] = T(0);                               // (the unused slot of a ragged partition stays zero)
             }
         }
 #pragma unroll
-        for (int j = 0; j < P; ++j) up[j] = u[j];
+        for (int j = 0; j < P; ++j) { up[j] = u[j]; u[j] = nx[j]; }
         __syncthreads();                                   // sE is rewritten by the next step
     }
 #pragma unroll

@@ -249,37 +249,86 @@ int btcs_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T *d
     return BURGERS_OK;
 }
 
-// Discrete adjoint of n_steps BTCS steps (D15): forward sweep with one snapshot per step (burgers_btcs_traj), then the
-// backward sweep of adjoint_btcs.cu.  ws: [work state B N][states n_steps B N][backward scratch][BTCS workspace].
+// ---- checkpointed reverse sweeps of the two implicit schemes (D15, D16) -----------------------------------
+// As adjoint_call above: segments of m steps (adjoint_segment: one segment while all states fit 8 GiB, else
+// ceil(sqrt(n_steps)), or the caller's), checkpoints at the segment starts from a first forward sweep, each
+// segment recomputed with one snapshot per step and swept backwards.  Unlike the explicit schemes the backward step
+// needs the state at BOTH ends of a step (D_i of D15 and the Jacobian of D16 are taken at u^{n+1}), so a segment
+// stores its len states u^{km+1} .. u^{km+len}.
+// ws layout: [u work B*N][checkpoints (K-1)*B*N][segment states m*B*N][backward scratch][workspace of the forward op].
 template <typename T>
-size_t btcs_adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps) {
-    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t st = align_up((size_t)n_steps * (size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t sc = align_up(adjoint_btcs_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
-    return bn + st + sc + burgers_workspace_bytes(BURGERS_OP_BTCS, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
+size_t implicit_adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps, int64_t segment, int op) {
+    const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
+    const int64_t K = (n_steps + m - 1) / m;
+    const size_t BN = (size_t)B * (size_t)N;
+    const size_t bn = align_up(BN * sizeof(T), 256);
+    const size_t ck = align_up((size_t)(K > 1 ? K - 1 : 0) * BN * sizeof(T), 256);
+    const size_t st = align_up((size_t)m * BN * sizeof(T), 256);
+    const size_t sc = align_up((op == BURGERS_OP_BTCS ? adjoint_btcs_ws_elems(sizeof(T) == 8, B, N)
+                                                      : adjoint_newton_ws_elems(sizeof(T) == 8, B, N)) * sizeof(T), 256);
+    return bn + ck + st + sc + burgers_workspace_bytes(op, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
+}
+
+// forward(work, steps, snaps, every): `steps` steps from the state in `work`, snapshots as the *_traj_* calls;
+// backward(start, states, scratch, len): lam through the len steps that start at `start` (states: the len states after it)
+template <typename T, typename Fwd, typename Bwd>
+int implicit_adjoint_sweep(const T *u0, int64_t B, int64_t N, int bc, int64_t n_steps, int64_t segment, int op, void *ws,
+                           size_t ws_bytes, cudaStream_t s, Fwd forward, Bwd backward) {
+    if (segment < 0) return BURGERS_ERR_SHAPE;
+    if (n_steps == 0) return BURGERS_OK;
+    if (!ws || ws_bytes < implicit_adjoint_ws_bytes<T>(B, N, bc, n_steps, segment, op)) return BURGERS_ERR_WORKSPACE;
+    const int64_t m = adjoint_segment(sizeof(T), B, N, n_steps, segment);
+    const int64_t K = (n_steps + m - 1) / m;
+    const size_t BN = (size_t)B * (size_t)N;
+    const size_t bn = align_up(BN * sizeof(T), 256);
+    const size_t ckb = align_up((size_t)(K > 1 ? K - 1 : 0) * BN * sizeof(T), 256);
+    const size_t stb = align_up((size_t)m * BN * sizeof(T), 256);
+    const size_t scb = align_up((op == BURGERS_OP_BTCS ? adjoint_btcs_ws_elems(sizeof(T) == 8, B, N)
+                                                       : adjoint_newton_ws_elems(sizeof(T) == 8, B, N)) * sizeof(T), 256);
+    unsigned char *base = static_cast<unsigned char *>(ws);
+    T *work = reinterpret_cast<T *>(base);
+    T *ckpt = reinterpret_cast<T *>(base + bn);
+    T *seg = reinterpret_cast<T *>(base + bn + ckb);
+    T *scratch = reinterpret_cast<T *>(base + bn + ckb + stb);
+    void *ows = base + bn + ckb + stb + scb;
+    const size_t ows_bytes = ws_bytes - (bn + ckb + stb + scb);
+    auto run_forward = [&](const T *from, int64_t steps, T *snaps, int64_t every) {
+        if (cudaMemcpyAsync(work, from, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess)
+            return (int)BURGERS_ERR_CUDA;
+        return forward(work, steps, snaps, every, ows, ows_bytes);
+    };
+    int st = BURGERS_OK;
+    if (K > 1) {            // checkpoints u^{m}, u^{2m}, ..., u^{(K-1)m}
+        st = run_forward(u0, (K - 1) * m, ckpt, m);
+        if (st != BURGERS_OK) return st;
+    }
+    for (int64_t k = K - 1; k >= 0; --k) {
+        const T *start = (k == 0) ? u0 : ckpt + (size_t)(k - 1) * BN;
+        const int64_t len = (k == K - 1) ? n_steps - k * m : m;
+        st = run_forward(start, len, seg, 1);
+        if (st != BURGERS_OK) return st;
+        st = backward(start, seg, scratch, len);
+        if (st != BURGERS_OK) return st;
+    }
+    return BURGERS_OK;
 }
 
 template <typename T>
 int btcs_adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps, int bc,
-                      void *ws, size_t ws_bytes, void *stream) {
+                      int64_t segment, void *ws, size_t ws_bytes, void *stream) {
     if (!lam) return BURGERS_ERR_NULL;
     int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
-    if (n_steps == 0) return BURGERS_OK;
-    if (!ws || ws_bytes < btcs_adjoint_ws_bytes<T>(B, N, bc, n_steps)) return BURGERS_ERR_WORKSPACE;
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t BN = (size_t)B * (size_t)N;
-    const size_t bn = align_up(BN * sizeof(T), 256), stb = align_up((size_t)n_steps * BN * sizeof(T), 256);
-    const size_t scb = align_up(adjoint_btcs_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
-    unsigned char *base = static_cast<unsigned char *>(ws);
-    T *work = reinterpret_cast<T *>(base);
-    T *states = reinterpret_cast<T *>(base + bn);
-    T *scratch = reinterpret_cast<T *>(base + bn + stb);
-    void *bws = base + bn + stb + scb;
-    if (cudaMemcpyAsync(work, u0, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
-    st = btcs_traj_call<T>(work, B, N, L, nu, dt, n_steps, bc, 1, states, bws, ws_bytes - (bn + stb + scb), stream);
-    if (st != BURGERS_OK) return st;
-    return launch_adjoint_btcs_steps<T>(u0, states, lam, scratch, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, s);
+    const double dx = grid_dx(N, L, bc);
+    return implicit_adjoint_sweep<T>(
+        u0, B, N, bc, n_steps, segment, BURGERS_OP_BTCS, ws, ws_bytes, s,
+        [&](T *work, int64_t steps, T *snaps, int64_t every, void *ows, size_t ows_bytes) {
+            return btcs_traj_call<T>(work, B, N, L, nu, dt, steps, bc, every, snaps, ows, ows_bytes, stream);
+        },
+        [&](const T *start, const T *states, T *scratch, int64_t len) {
+            return launch_adjoint_btcs_steps<T>(start, states, lam, scratch, B, N, dx, nu, dt, len, bc, s);
+        });
 }
 
 template <typename T>
@@ -347,39 +396,27 @@ int newton_traj_call(T *u, int64_t B, int64_t N, double L, const T *nu, const T 
     return BURGERS_OK;
 }
 
-// Reverse mode of the Newton / theta-scheme: forward sweep with one snapshot per step (newton_traj_call), then the
-// backward sweep of adjoint_newton.cu.  ws: [work state B N][states n_steps B N][backward scratch][Newton workspace].
-template <typename T>
-size_t newton_adjoint_ws_bytes(int64_t B, int64_t N, int bc, int64_t n_steps) {
-    const size_t bn = align_up((size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t st = align_up((size_t)n_steps * (size_t)B * (size_t)N * sizeof(T), 256);
-    const size_t sc = align_up(adjoint_newton_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
-    return bn + st + sc + burgers_workspace_bytes(BURGERS_OP_NEWTON, sizeof(T) == 8, B, N, bc, 0, BURGERS_PLAN_AUTO);
-}
-
+// Reverse mode of the Newton / theta-scheme (D16): the checkpointed sweep above with newton_traj_call forward and the
+// backward kernels of adjoint_newton.cu.
 template <typename T>
 int newton_adjoint_call(const T *u0, T *lam, int64_t B, int64_t N, double L, const T *nu, const T *dt, int64_t n_steps,
-                        int bc, double theta, double tol, int max_iter, void *ws, size_t ws_bytes, void *stream) {
+                        int bc, double theta, double tol, int max_iter, int64_t segment, void *ws, size_t ws_bytes,
+                        void *stream) {
     if (!lam) return BURGERS_ERR_NULL;
     int st = check_common(u0, nu, dt, B, N, L, n_steps, bc);
     if (st != BURGERS_OK) return st;
     if (!(tol >= 0.0) || max_iter < 0 || !(theta >= 0.0 && theta <= 1.0)) return BURGERS_ERR_VALUE;
-    if (n_steps == 0) return BURGERS_OK;
-    if (!ws || ws_bytes < newton_adjoint_ws_bytes<T>(B, N, bc, n_steps)) return BURGERS_ERR_WORKSPACE;
     cudaStream_t s = (cudaStream_t)stream;
-    const size_t BN = (size_t)B * (size_t)N;
-    const size_t bn = align_up(BN * sizeof(T), 256), stb = align_up((size_t)n_steps * BN * sizeof(T), 256);
-    const size_t scb = align_up(adjoint_newton_ws_elems(sizeof(T) == 8, B, N) * sizeof(T), 256);
-    unsigned char *base = static_cast<unsigned char *>(ws);
-    T *work = reinterpret_cast<T *>(base);
-    T *states = reinterpret_cast<T *>(base + bn);
-    T *scratch = reinterpret_cast<T *>(base + bn + stb);
-    void *nws = base + bn + stb + scb;
-    if (cudaMemcpyAsync(work, u0, BN * sizeof(T), cudaMemcpyDeviceToDevice, s) != cudaSuccess) return BURGERS_ERR_CUDA;
-    st = newton_traj_call<T>(work, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, nullptr, 1, states, nws,
-                             ws_bytes - (bn + stb + scb), stream);
-    if (st != BURGERS_OK) return st;
-    return launch_adjoint_newton_steps<T>(u0, states, lam, scratch, B, N, grid_dx(N, L, bc), nu, dt, n_steps, bc, theta, s);
+    const double dx = grid_dx(N, L, bc);
+    return implicit_adjoint_sweep<T>(
+        u0, B, N, bc, n_steps, segment, BURGERS_OP_NEWTON, ws, ws_bytes, s,
+        [&](T *work, int64_t steps, T *snaps, int64_t every, void *ows, size_t ows_bytes) {
+            return newton_traj_call<T>(work, B, N, L, nu, dt, steps, bc, theta, tol, max_iter, nullptr, every, snaps, ows,
+                                       ows_bytes, stream);
+        },
+        [&](const T *start, const T *states, T *scratch, int64_t len) {
+            return launch_adjoint_newton_steps<T>(start, states, lam, scratch, B, N, dx, nu, dt, len, bc, theta, s);
+        });
 }
 
 template <typename T>
@@ -715,30 +752,57 @@ int burgers_btcs_traj_f64(double *u, int64_t B, int64_t N, double L, const doubl
 
 int burgers_btcs_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                              int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
-    return btcs_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+    return btcs_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, 0, ws, ws_bytes, stream);
 }
 int burgers_btcs_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
                              const double *dt, int64_t n_steps, int bc, void *ws, size_t ws_bytes, void *stream) {
-    return btcs_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, ws, ws_bytes, stream);
+    return btcs_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, 0, ws, ws_bytes, stream);
 }
 size_t burgers_btcs_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
-    if (B < 1 || N < 3 || n_steps < 0) return 0;
-    return dtype_is_f64 ? btcs_adjoint_ws_bytes<double>(B, N, bc, n_steps) : btcs_adjoint_ws_bytes<float>(B, N, bc, n_steps);
+    return burgers_implicit_adjoint_ckpt_workspace_bytes(BURGERS_OP_BTCS, dtype_is_f64, B, N, bc, n_steps, 0);
+}
+int burgers_btcs_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                  const float *dt, int64_t n_steps, int bc, int64_t segment, void *ws, size_t ws_bytes,
+                                  void *stream) {
+    return btcs_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream);
+}
+int burgers_btcs_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                  const double *dt, int64_t n_steps, int bc, int64_t segment, void *ws, size_t ws_bytes,
+                                  void *stream) {
+    return btcs_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, segment, ws, ws_bytes, stream);
+}
+size_t burgers_implicit_adjoint_ckpt_workspace_bytes(int op, int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps,
+                                                     int64_t segment) {
+    if (B < 1 || N < 3 || n_steps < 0 || segment < 0) return 0;
+    if (op != BURGERS_OP_BTCS && op != BURGERS_OP_NEWTON) return 0;
+    return dtype_is_f64 ? implicit_adjoint_ws_bytes<double>(B, N, bc, n_steps, segment, op)
+                        : implicit_adjoint_ws_bytes<float>(B, N, bc, n_steps, segment, op);
 }
 
 int burgers_newton_adjoint_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu, const float *dt,
                                int64_t n_steps, int bc, double theta, double tol, int max_iter, void *ws, size_t ws_bytes,
                                void *stream) {
-    return newton_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, ws, ws_bytes, stream);
+    return newton_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, 0, ws, ws_bytes, stream);
 }
 int burgers_newton_adjoint_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
                                const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter, void *ws,
                                size_t ws_bytes, void *stream) {
-    return newton_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, ws, ws_bytes, stream);
+    return newton_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, 0, ws, ws_bytes, stream);
 }
 size_t burgers_newton_adjoint_workspace_bytes(int dtype_is_f64, int64_t B, int64_t N, int bc, int64_t n_steps) {
-    if (B < 1 || N < 3 || n_steps < 0) return 0;
-    return dtype_is_f64 ? newton_adjoint_ws_bytes<double>(B, N, bc, n_steps) : newton_adjoint_ws_bytes<float>(B, N, bc, n_steps);
+    return burgers_implicit_adjoint_ckpt_workspace_bytes(BURGERS_OP_NEWTON, dtype_is_f64, B, N, bc, n_steps, 0);
+}
+int burgers_newton_adjoint_ckpt_f32(const float *u0, float *lam, int64_t B, int64_t N, double L, const float *nu,
+                                    const float *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                                    int64_t segment, void *ws, size_t ws_bytes, void *stream) {
+    return newton_adjoint_call<float>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, segment, ws, ws_bytes,
+                                      stream);
+}
+int burgers_newton_adjoint_ckpt_f64(const double *u0, double *lam, int64_t B, int64_t N, double L, const double *nu,
+                                    const double *dt, int64_t n_steps, int bc, double theta, double tol, int max_iter,
+                                    int64_t segment, void *ws, size_t ws_bytes, void *stream) {
+    return newton_adjoint_call<double>(u0, lam, B, N, L, nu, dt, n_steps, bc, theta, tol, max_iter, segment, ws, ws_bytes,
+                                       stream);
 }
 
 int burgers_btcs_gs_f32(float *u, int64_t B, int64_t N, double L, const float *nu, const float *dt,

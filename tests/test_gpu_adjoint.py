@@ -249,3 +249,37 @@ def test_newton_adjoint_against_finite_differences_of_the_gpu_forward_path(B):
     lam = to_dev(lam_T.copy())
     B.burgers_newton_adjoint(to_dev(w.u0), lam, w.L, to_dev(nu), to_dev(dt), 0, w.bc)
     np.testing.assert_array_equal(lam.cpu().numpy(), lam_T)
+
+
+@pytest.mark.parametrize("scheme", ["btcs", "newton"])
+def test_implicit_adjoints_checkpointed(B, scheme):
+    """Checkpoint segments of the implicit adjoints (burgers_*_adjoint_ckpt_*): any segment length gives the bits of
+    the one-segment sweep (the recomputed states are those of the first sweep: p then q steps == p + q steps), the
+    workspace shrinks as n/m + m, and a long grid (thread-per-system backward sweep) goes the same way."""
+    rng = np.random.default_rng(41)
+    for w, nu, n in ((W.c3_periodic_btcs(B=3, N=512, n_steps=0), np.full(3, 0.05), 17),
+                     (W.c4b_long_btcs(N=12000, n_steps=0), np.full(1, 1e-3), 7)):
+        dt = oracle_dt(w.u0, w.L, nu, 4.0, w.bc, np.float64)
+        lam_T = rng.standard_normal(w.u0.shape)
+        is_btcs = scheme == "btcs"
+        fn = B.burgers_btcs_adjoint if is_btcs else B.burgers_newton_adjoint
+        ref = (oracle.btcs_adjoint if is_btcs else oracle.newton_adjoint)(w.u0, lam_T, w.L, nu, dt, n, w.bc)
+        want = None
+        sizes = []
+        for seg in (n, 1, 3, 5, n + 7, 0):
+            lam = to_dev(lam_T.copy())
+            fn(to_dev(w.u0), lam, w.L, to_dev(nu), to_dev(dt), n, w.bc, segment=seg)
+            got = lam.cpu().numpy()
+            if want is None:
+                want = got
+                assert (np.abs(got - ref) / np.abs(ref).max(axis=1, keepdims=True)).max() <= 1e-10, (w.name, seg)
+            np.testing.assert_array_equal(got, want, err_msg=f"{w.name} segment {seg}")
+            sizes.append(int(B.raw().burgers_implicit_adjoint_ckpt_workspace_bytes(
+                B.OP_BTCS if is_btcs else B.OP_NEWTON, 1, w.u0.shape[0], w.u0.shape[1], w.bc, n, seg)))
+        assert sizes[3] < sizes[0] and sizes[4] == sizes[0] and sizes[5] == sizes[0]     # 5-step segments < one segment
+    # error paths
+    one = to_dev(np.ones((1, 64)))
+    with pytest.raises(B.BurgersError) as e:
+        (B.burgers_btcs_adjoint if scheme == "btcs" else B.burgers_newton_adjoint)(
+            one, one.clone(), 1.0, to_dev(np.array([0.1])), to_dev(np.array([1e-3])), 4, 0, segment=-1)
+    assert e.value.status in (B.ERR_SHAPE, B.ERR_WORKSPACE)
