@@ -195,7 +195,9 @@ int launch_hybrid_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T 
             return last_launch_status();
         }
         if constexpr (P == 4 || P == 8 || P == 16) {
-            if (sizeof(T) == 8 && P == 16 && Tn <= 128)
+            if (sizeof(T) == 8 && P == 16 && Tn == 128 && bc == BURGERS_BC_PERIODIC)      // C3's shape
+                newton_hybrid_kernel<T, P, true, false, 128, true, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
+            else if (sizeof(T) == 8 && P == 16 && Tn <= 128)
                 newton_hybrid_kernel<T, P, true, false, 0, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
             else
                 newton_hybrid_kernel<T, P, false, false, 0, false, true><<<(unsigned)B, Tn, smem, s>>>(BURGERS_NEWTON_ARGS);
