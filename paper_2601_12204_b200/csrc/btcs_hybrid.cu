@@ -76,6 +76,7 @@ btcs_hybrid_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T 
     const int t = threadIdx.x, Tn = blockDim.x;
     T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
     T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
+    T *sS = sF + 3 * Tn;                      // SNAP, exact partitions: [Tn * P] staging of a snapshot
     Part part;
     part.r0 = t * P; part.n = P;
     if (RAGGED) part = partition_of(t, N, Tn);
@@ -136,7 +137,7 @@ btcs_hybrid_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T 
 #pragma unroll
                     for (int j = 0; j < P; ++j)
                         if (j < n) srow[j] = v[j];
-                } else {
+                } else if (Tn < 32) {                  // (a partial warp: straight from the registers)
 #pragma unroll
                     for (int c2 = 0; c2 < P / V; ++c2) {
                         int4 q4;
@@ -145,6 +146,33 @@ btcs_hybrid_general_kernel(T *__restrict__ u, const T *__restrict__ nu, const T 
                         for (int k = 0; k < V; ++k) e[k] = v[c2 * V + k];
                         *reinterpret_cast<int4 *>(srow + c2 * V) = q4;
                     }
+                } else {
+                    // Coalesced stores through a warp-private stage: the 32 rows of a warp are 32 * P contiguous
+                    // elements of the snapshot.  Every lane puts its row into shared memory (16-byte chunk c of row
+                    // r at r * CR + (c ^ ((r / SW) % CR)): conflict-free for the row-wise stores and for the
+                    // chunk-wise loads), then the warp writes CR requests of 512 contiguous bytes.  Straight from
+                    // the registers a store instruction touches 32 different 128-byte lines (27 -> 17 us per step
+                    // of C3 with a snapshot after every step).
+                    constexpr int CR = P / V;             // 16-byte chunks per row
+                    constexpr int SW = (CR >= 8) ? 1 : 8 / CR;
+                    const int lane = t & 31;
+                    int4 *wst = reinterpret_cast<int4 *>(sS) + (t - lane) * CR;      // this warp's 32 * CR chunks
+#pragma unroll
+                    for (int c2 = 0; c2 < CR; ++c2) {
+                        int4 q4;
+                        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+                        for (int k = 0; k < V; ++k) e[k] = v[c2 * V + k];
+                        wst[lane * CR + (c2 ^ ((lane / SW) % CR))] = q4;
+                    }
+                    __syncwarp();
+                    int4 *wdst = reinterpret_cast<int4 *>(srow - lane * P);          // first element of the warp's rows
+#pragma unroll
+                    for (int k = 0; k < CR; ++k) {
+                        const int g = k * 32 + lane, r = g / CR, c2 = g % CR;
+                        wdst[g] = wst[r * CR + (c2 ^ ((r / SW) % CR))];
+                    }
+                    __syncwarp();
                 }
             }
         }
@@ -223,8 +251,13 @@ int launch_traj_P(T *u, int64_t B, int64_t N, double dx, const T *nu, const T *d
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
-        btcs_hybrid_general_kernel<T, P, false, true><<<(unsigned)B, Tn, smem, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
-                                                                                  snaps, snap_every, B * N);
+        const size_t smem_s = smem + (size_t)Tn * P * sizeof(T);                  // + the snapshot stage
+        if (smem_s > 48 * 1024 &&
+            cudaFuncSetAttribute(btcs_hybrid_general_kernel<T, P, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem_s) != cudaSuccess)
+            return BURGERS_ERR_CUDA;
+        btcs_hybrid_general_kernel<T, P, false, true><<<(unsigned)B, Tn, smem_s, s>>>(u, nu, dt, (int)N, 1.0 / dx, n_steps, bc,
+                                                                                    snaps, snap_every, B * N);
         return last_launch_status();
     }
     return BURGERS_ERR_PLAN;
