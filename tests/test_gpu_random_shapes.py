@@ -84,3 +84,39 @@ def test_newton_random_shapes(B, case):
         u = to_dev(u0.copy())
         B.burgers_newton(u, L, to_dev(nu), to_dev(dt), 3, bc, tol=2e-6 if dtype == np.float32 else 1e-13, max_iter=30, theta=theta)
         assert rel_err(u.cpu().numpy(), ref, u0) <= TOL[np.dtype(dtype)], (case, theta)
+
+
+@pytest.mark.parametrize("case", _shapes(14, 24, 7000), ids=lambda c: f"B{c[0]}-N{c[1]}-bc{c[2]}-{np.dtype(c[3]).name}")
+def test_implicit_adjoints_random_shapes(B, case):
+    """Reverse mode of the two implicit schemes (D15, D16) on random shapes: every register-slot count of the
+    resident backward kernels (P = 4 .. 16, exact and ragged), the thread-per-system fallback beyond one CTA,
+    both boundary types and dtypes, with a checkpoint segment that does not divide the step count."""
+    Bn, N, bc, dtype = case
+    rng = np.random.default_rng(N * 11 + Bn)
+    u0, _ = _data(rng, Bn, N, dtype)
+    L = 2 * math.pi if bc == 0 else 1.0
+    dx = L / N if bc == 0 else L / (N - 1)
+    nu = np.maximum(0.05, 0.75 * np.abs(u0).max(axis=1) * dx).astype(dtype)       # cell Peclet number < 2 (D11)
+    lam_T = rng.standard_normal(u0.shape).astype(dtype)
+    n = 5
+    tol = TOL[np.dtype(dtype)]
+
+    def check(got, ref, what):
+        scale = np.abs(ref).max(axis=1, keepdims=True)
+        assert np.isfinite(got).all(), (case, what)
+        assert (np.abs(got.astype(np.float64) - ref) / scale).max() <= tol, (case, what)
+
+    f64 = lambda a: a.astype(np.float64)
+    dt = oracle_dt(u0, L, nu, 10.0, bc, dtype)
+    ref = oracle.btcs_adjoint(f64(u0), f64(lam_T), L, f64(nu), f64(dt), n, bc)
+    for seg in (0, 2):
+        lam = to_dev(lam_T.copy())
+        B.burgers_btcs_adjoint(to_dev(u0), lam, L, to_dev(nu), to_dev(dt), n, bc, segment=seg)
+        check(lam.cpu().numpy(), ref, ("btcs", seg))
+    dt = oracle_dt(u0, L, nu, 2.0, bc, dtype)
+    for theta in (1.0, 0.5):
+        ref = oracle.newton_adjoint(f64(u0), f64(lam_T), L, f64(nu), f64(dt), n, bc, tol=1e-13, theta=theta)
+        lam = to_dev(lam_T.copy())
+        B.burgers_newton_adjoint(to_dev(u0), lam, L, to_dev(nu), to_dev(dt), n, bc, theta=theta,
+                                 tol=2e-6 if dtype == np.float32 else 1e-13, max_iter=30, segment=2)
+        check(lam.cpu().numpy(), ref, ("newton", theta))
