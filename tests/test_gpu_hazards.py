@@ -321,3 +321,48 @@ def test_guard_bands_other_entry_points(B, dtype):
             assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
             first = got if first is None else first
             np.testing.assert_array_equal(got, first)
+    # ---- reverse mode of the Newton scheme (resident exact / ragged, thread-per-system), checkpoint segments of both
+    #      implicit adjoints, and the trajectory kernels of the implicit schemes (snapshots staged per warp)
+    wn = W.c3_periodic_btcs(B=3, N=2048, dtype=dtype)
+    wd = W.c2_dirichlet_batch(B=3, N=201, dtype=dtype); wd.nu[:] = 0.05
+    wl = W.c4b_long_btcs(N=20000, dtype=dtype); wl.nu[:] = 1e-3
+    ntol = 2e-6 if dtype == np.float32 else 1e-13
+    for w, seg in ((wn, 0), (wd, 2), (wl, 3)):
+        dt = _dt(w, 4.0)
+        lam_T = rng.standard_normal(w.u0.shape).astype(dtype)
+        for op, fn, ofn, kw in ((B.OP_NEWTON, B.burgers_newton_adjoint, oracle.newton_adjoint, dict(tol=ntol)),
+                                (B.OP_BTCS, B.burgers_btcs_adjoint, oracle.btcs_adjoint, {})):
+            need = int(B.raw().burgers_implicit_adjoint_ckpt_workspace_bytes(op, int(is64), w.B, w.N, w.bc, 5, seg))
+            ref = ofn(_f64(w.u0), _f64(lam_T), w.L, _f64(w.nu), _f64(dt), 5, w.bc)
+            first = None
+            for _ in range(3):
+                gu, u = guarded_from(w.u0); gl, lam = guarded_from(lam_T); gw, ws = guarded_empty(need)
+                fn(u, lam, w.L, torch.from_numpy(w.nu).cuda(), torch.from_numpy(dt).cuda(), 5, w.bc, ws=ws, segment=seg, **kw)
+                torch.cuda.synchronize()
+                assert gu.intact() and gl.intact() and gw.intact(), (w.name, op, seg)
+                np.testing.assert_array_equal(u.cpu().numpy(), w.u0)
+                got = lam.cpu().numpy()
+                assert np.abs(got - ref).max() / np.abs(ref).max() <= tol, (w.name, op, seg)
+                first = got if first is None else first
+                np.testing.assert_array_equal(got, first)
+    w96 = W.c3_periodic_btcs(B=2, N=96, dtype=dtype); w96.nu[:] = 0.2       # (cell Peclet number < 2 for the Newton scheme)
+    for w in (wn, wd, w96):
+        dt = _dt(w, 4.0)
+        for which in ("btcs", "newton"):
+            first = None
+            for _ in range(3):
+                gu, u = guarded_from(w.u0); gs, sraw = guarded_empty(3 * w.u0.size * w.u0.itemsize)
+                snaps = sraw.view(u.dtype).view(3, w.B, w.N)
+                dnu, ddt = torch.from_numpy(w.nu).cuda(), torch.from_numpy(dt).cuda()
+                if which == "btcs":
+                    B.burgers_btcs_traj(u, w.L, dnu, ddt, 7, w.bc, 2, snaps=snaps)
+                    ref = oracle.btcs(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), 6, w.bc)
+                else:
+                    B.burgers_newton_traj(u, w.L, dnu, ddt, 7, w.bc, 2, snaps=snaps, tol=ntol)
+                    ref = oracle.newton_btcs(_f64(w.u0), w.L, _f64(w.nu), _f64(dt), 6, w.bc, tol=1e-13)
+                torch.cuda.synchronize()
+                assert gu.intact() and gs.intact(), (w.name, which)
+                got = snaps.cpu().numpy()
+                assert rel_err(got[2], ref, w.u0) <= tol, (w.name, which)      # third snapshot = state after 6 steps
+                first = got if first is None else first
+                np.testing.assert_array_equal(got, first)
