@@ -535,7 +535,13 @@ def measure(name, device, args, pk, traffic, sampler, pipe, steps, warmup, rank=
     if spec["op"] == "btcs" and r.plan == r.B.PLAN_LONG and r.op_launches > 2:
         rec["steps_per_launch"] = sig(w.n_steps / (r.op_launches - 2), 3)       # LONG: S steps per HBM round trip
     if spec["op"] == "gs":
-        rec["gs_sweeps_per_step"] = sig(float(r.iters.double().mean().item()) / w.n_steps, 4); rec["tol"] = spec["tol"]
+        sw = float(r.iters.double().mean().item()) / w.n_steps
+        rec["gs_sweeps_per_step"] = sig(sw, 4); rec["tol"] = spec["tol"]
+        # FP64 instructions per update, counted from btcs_gs.cu (CTA plan, 16 rows per thread) for the measured sweep count:
+        # per step rows + reciprocal + scaled coefficients 12; per residual pass (one more than sweeps) 6 + the scan of
+        # the thread maps 14/16; per sweep the second pass 1
+        spec = dict(spec, instr=round(12 + (sw + 1) * (6 + 14.0 / 16) + sw, 1))
+        rec["roofline"] = roofline(name, spec, w, op_ms, pk, traffic, r.op_launches, pipe, verbose=False)
     if spec["op"] == "newton":
         its = float(r.iters.double().mean().item()) / w.n_steps
         rec["newton_iterations_per_step"] = sig(its, 4)
@@ -639,6 +645,10 @@ def run_ours(args):
         "gpu_launches": int(r.launches * args.steps),
         "clocks": clocks,
     }
+    if spec["op"] == "gs" and hasattr(r, "iters"):              # instruction count for the measured sweep count (see measure())
+        sw = float(r.iters.double().mean().item()) / w.n_steps
+        spec = dict(spec, instr=round(12 + (sw + 1) * (6 + 14.0 / 16) + sw, 1))
+        out["gs_sweeps_per_step"] = sig(sw, 4)
     if spec["op"] == "newton" and hasattr(r, "iters"):          # instruction count for the measured iteration count (see measure())
         its = float(r.iters.double().mean().item()) / w.n_steps
         spec = dict(spec, instr=round(its * (10 + 19 + 71.0 / 16) + 10, 1))
