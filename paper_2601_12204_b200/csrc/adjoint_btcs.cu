@@ -11,8 +11,10 @@
 // (btcs_common.cuh: partition elimination, cyclic-reduction step, PCR, back substitution).
 //
 // The forward states u^1 .. u^n come from burgers_btcs_traj_* (one snapshot per step).  Two plans:
-//   RESIDENT  one CTA per system, lam and u^{n+1} in registers across the steps, u^n streamed in, any N that fits
-//             one CTA (exact or ragged partitions as btcs_hybrid.cu);
+//   RESIDENT  one CTA per system, lam in registers across the steps, any N that fits one CTA.  Exact partitions
+//             (N == P * threads): the STAGED kernel -- the stored states pass through a ring of three
+//             shared-memory stages (cp.async), 168 registers, three CTAs per SM; ragged partitions: u^{n+1}
+//             in registers, u^n streamed in one step ahead;
 //   THOMAS    one thread per system on [B][N] as it lies (strided accesses; the general-shape fallback), transposed
 //             rows eliminated by the Thomas recurrences, Sherman-Morrison for periodic systems; scratch 3 B N.
 #include "btcs_common.cuh"
@@ -127,6 +129,126 @@ adjoint_btcs_resident_kernel(const T *__restrict__ u0, const T *__restrict__ sta
         if (j < n) lam[off + j] = l[j];
 }
 
+// ---- STAGED variant of the resident kernel for exact partitions (N == P * threads, at least one warp).
+// The stored states go through a ring of three shared-memory stages instead of through registers: while step k is
+// solved, u^{k-1} is in flight (cp.async, warp-private: the 32 rows of a warp are 32 P contiguous elements, copied
+// with P/V requests of 512 contiguous bytes), u^k and u^{k+1} sit in the other two stages.  Registers hold lam, u^k
+// and the two coefficient arrays of the elimination only (u^{k+1} is read back from its stage for the D_i at the
+// end, the prefetched state never passes through registers): 168 instead of 249 registers, three CTAs per SM
+// instead of two.  16-byte chunk c of row r lives at r CR + (c ^ ((r / SW) % CR)) of a stage (CR chunks per row, SW
+// rows per 128-byte line): conflict-free for the copy and for every thread reading its own row.
+__device__ __forceinline__ unsigned adj_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <typename T, int P, bool SMALL>
+__global__ void __launch_bounds__(SMALL ? 128 : adj_max_threads(sizeof(T), P), SMALL ? 3 : 1)
+adjoint_btcs_staged_kernel(const T *__restrict__ u0, const T *__restrict__ states, T *__restrict__ lam,
+                           const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int N, double inv_dx,
+                           int64_t n_steps, int bc) {
+    constexpr int V = 16 / sizeof(T);
+    constexpr int CR = P / V;
+    constexpr int SW = (CR >= 8) ? 1 : 8 / CR;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1, lane = t & 31, warp0 = t - lane;
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
+    int4 *sS = reinterpret_cast<int4 *>(sF + 3 * Tn);      // [3][Tn * CR] chunks: ring of stages
+    const int64_t b = blockIdx.x, BN = B * (int64_t)N;
+    const int64_t off = b * N + (int64_t)t * P, woff = b * N + (int64_t)warp0 * P;
+
+    Coef<T> co;
+    co.init(nu[b], dt[b], inv_dx);
+    const T cx = T(2) * co.hcx;
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    const bool fixL = dirichlet && t == 0, fixR = dirichlet && t == Tn - 1;
+    auto state = [&](int64_t k) { return (k == 0) ? u0 : states + (size_t)(k - 1) * (size_t)BN; };
+    auto chunk_of = [&](int r, int c) { return r * CR + (c ^ ((r / SW) % CR)); };
+    auto fetch = [&](int64_t k) {              // this warp's rows of u^k -> stage k % 3
+        const int4 *src = reinterpret_cast<const int4 *>(state(k) + woff);
+        int4 *dst = sS + (int)(k % 3) * Tn * CR;
+#pragma unroll
+        for (int i = 0; i < CR; ++i) {
+            const int g = i * 32 + lane, r = warp0 + g / CR, c = g % CR;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(adj_smem_u32(dst + chunk_of(r, c))), "l"(src + g)
+                         : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto own_row = [&](int64_t k, T (&dst)[P]) {
+        const int4 *st = sS + (int)(k % 3) * Tn * CR;
+#pragma unroll
+        for (int c = 0; c < CR; ++c) {
+            const int4 q4 = st[chunk_of(t, c)];
+            const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+            for (int i = 0; i < V; ++i) dst[c * V + i] = e[i];
+        }
+    };
+    auto elem = [&](int64_t k, int r, int j) {  // element j of row r of u^k
+        const T *st = reinterpret_cast<const T *>(sS + (int)(k % 3) * Tn * CR);
+        return st[chunk_of(r, j / V) * V + (j % V)];
+    };
+    const bool frozL = dirichlet && t == 0;            // row N-1 (wrap): a Dirichlet end node
+    const bool frozR = dirichlet && t == Tn - 1;       // row 0 (wrap)
+    auto frozen_at = [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); };
+
+    T l[P], u[P];
+#pragma unroll
+    for (int c = 0; c < CR; ++c) {
+        const int4 q4 = *reinterpret_cast<const int4 *>(lam + off + c * V);
+        const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+        for (int i = 0; i < V; ++i) l[c * V + i] = e[i];
+    }
+    fetch(n_steps);
+    fetch(n_steps - 1);
+    for (int64_t k = n_steps - 1; k >= 0; --k) {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                       // u^k and u^{k+1} staged by every warp; the reads of step k + 1 are done
+        if (k > 0) fetch(k - 1);               // into the stage that held u^{k+2}
+        own_row(k, u);
+        const int tl = (t - 1) & mask, tr = (t + 1) & mask;
+        const T uL = elem(k, tl, P - 1), uR = elem(k, tr, 0);
+        auto rowA = [&](T uk, bool frozen, T &a, T &bb, T &e) {
+            co.at(uk, a, bb, e);
+            if (frozen) { a = T(0); bb = T(1); e = T(0); }
+        };
+        T f[P], c[P];
+        Row<T> first, last;
+        auto rowT = [&](int j, T &a, T &bb, T &e) {        // row j of A^T: (sup_{j-1}, diag_j, sub_{j+1})
+            T a1, b1, e1;
+            rowA(j ? u[j - 1] : uL, j ? frozen_at(j - 1) : frozL, a1, b1, e1);
+            a = e1;
+            rowA(u[j], frozen_at(j), a1, bb, e1);
+            rowA((j == P - 1) ? uR : u[(j + 1 < P) ? j + 1 : j], (j == P - 1) ? frozR : frozen_at(j + 1), a1, b1, e1);
+            e = a1;
+        };
+        eliminate_general<T, P>(rowT, l, f, c, first, last);
+        T x0, xL;
+        solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
+        T (&mu)[P] = l;                                     // in place (see the kernel above)
+        back_substitute<T, P>(mu, f, c, l, x0, xL);
+        // lam^n_i = (1 - D_i) mu_i, u^{k+1} from its stage
+        T up[P];
+        own_row(k + 1, up);
+        const T upL = elem(k + 1, tl, P - 1), upR = elem(k + 1, tr, 0);
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            const T pm = j ? up[j - 1] : upL, pj = up[j], pp = (j == P - 1) ? upR : up[(j + 1 < P) ? j + 1 : j];
+            T Dj = (u[j] > T(0)) ? cx * (pj - pm) : cx * (pp - pj);
+            if (frozen_at(j)) Dj = T(0);
+            l[j] = t_fma(-Dj, mu[j], mu[j]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < CR; ++c) {
+        int4 q4;
+        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+        for (int i = 0; i < V; ++i) e[i] = l[c * V + i];
+        *reinterpret_cast<int4 *>(lam + off + c * V) = q4;
+    }
+}
+
 // ---- thread-per-system fallback on the caller's [B][N] layout.  ws: cp, dp, wp ([B][N] each).
 template <typename T>
 __global__ void __launch_bounds__(64)
@@ -205,6 +327,17 @@ int launch_resident_P(const T *u0, const T *states, T *lam, int64_t B, int64_t N
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
+        if (Tn >= 32) {                                     // states through the shared-memory ring
+            const size_t smem_s = (size_t)(9 + 3 * P) * Tn * sizeof(T);
+            auto go = [&](auto kernel) {
+                if (smem_s > 48 * 1024 &&
+                    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s) != cudaSuccess)
+                    return (int)BURGERS_ERR_CUDA;
+                kernel<<<(unsigned)B, Tn, smem_s, s>>>(u0, states, lam, nu, dt, B, (int)N, 1.0 / dx, n_steps, bc);
+                return last_launch_status();
+            };
+            return Tn <= 128 ? go(adjoint_btcs_staged_kernel<T, P, true>) : go(adjoint_btcs_staged_kernel<T, P, false>);
+        }
         adjoint_btcs_resident_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u0, states, lam, nu, dt, B, (int)N, 1.0 / dx,
                                                                               n_steps, bc);
         return last_launch_status();

@@ -15,8 +15,9 @@
 //
 // This is the derivative of the map the CONVERGED iteration defines: run the forward sweep with a tolerance
 // near rounding.  The forward states u^1 .. u^n come from burgers_newton_traj_* (one snapshot per step).  Plans:
-//   RESIDENT  one CTA per system, lam and u^{n+1} in registers across the steps, u^n streamed in, any N that fits
-//             one CTA (exact or ragged partitions as btcs_hybrid.cu);
+//   RESIDENT  one CTA per system, lam in registers across the steps, any N that fits one CTA.  Exact partitions
+//             (N == P * threads): the STAGED kernel (states through a ring of three shared-memory stages); ragged
+//             partitions: u^{n+1} in registers, u^n streamed in one step ahead;
 //   THOMAS    one thread per system on [B][N] as it lies (the general-shape fallback), Sherman-Morrison for
 //             periodic systems; scratch 3 B N.
 #include "btcs_common.cuh"
@@ -135,6 +136,130 @@ adjoint_newton_resident_kernel(const T *__restrict__ u0, const T *__restrict__ s
         if (j < n) lam[off + j] = l[j];
 }
 
+// ---- STAGED variant of the resident kernel for exact partitions (N == P * threads, at least one warp): as
+// adjoint_btcs_staged_kernel (adjoint_btcs.cu) -- the stored states go through a ring of three shared-memory stages
+// (cp.async, warp-private, swizzled) instead of through registers; lam, u^{k+1} (the Jacobian's state) and the two
+// coefficient arrays are what the registers hold, u^k is read back from its stage for the G'(u^k)^T product.
+__device__ __forceinline__ unsigned adjn_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+template <typename T, int P, bool SMALL>
+__global__ void __launch_bounds__(SMALL ? 128 : adjn_max_threads(sizeof(T), P), SMALL ? 3 : 1)
+adjoint_newton_staged_kernel(const T *__restrict__ u0, const T *__restrict__ states, T *__restrict__ lam,
+                             const T *__restrict__ nu, const T *__restrict__ dt, int64_t B, int N, double inv_dx,
+                             int64_t n_steps, int bc, T theta) {
+    constexpr int V = 16 / sizeof(T);
+    constexpr int CR = P / V;
+    constexpr int SW = (CR >= 8) ? 1 : 8 / CR;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int t = threadIdx.x, Tn = blockDim.x, mask = Tn - 1, lane = t & 31, warp0 = t - lane;
+    T *sR = reinterpret_cast<T *>(smem_raw);  // [2][Tn] reduced rows (A, C, D): PCR ping-pong
+    T *sF = sR + 6 * Tn;                      // [Tn] first interface rows (A, C, D)
+    T *sE = sF + 3 * Tn;                      // [2][Tn] partition edge values of M mu
+    int4 *sS = reinterpret_cast<int4 *>(sE + 2 * Tn + (Tn & 1));   // [3][Tn * CR] chunks: ring of stages (Tn is even)
+    const int64_t b = blockIdx.x, BN = B * (int64_t)N;
+    const int64_t off = b * N + (int64_t)t * P, woff = b * N + (int64_t)warp0 * P;
+
+    const double dtb = (double)dt[b];
+    const T h = (T)(0.5 * dtb * inv_dx);
+    const T r = (T)((double)nu[b] * dtb * inv_dx * inv_dx);
+    const T th = theta * h, tr = theta * r, omt = T(1) - theta;
+    const T b0 = T(1) + T(2) * tr;
+    const bool dirichlet = (bc == BURGERS_BC_DIRICHLET);
+    const bool fixL = dirichlet && t == 0, fixR = dirichlet && t == Tn - 1;
+    auto state = [&](int64_t k) { return (k == 0) ? u0 : states + (size_t)(k - 1) * (size_t)BN; };
+    auto chunk_of = [&](int rr, int c) { return rr * CR + (c ^ ((rr / SW) % CR)); };
+    auto fetch = [&](int64_t k) {              // this warp's rows of u^k -> stage k % 3
+        const int4 *src = reinterpret_cast<const int4 *>(state(k) + woff);
+        int4 *dst = sS + (int)(k % 3) * Tn * CR;
+#pragma unroll
+        for (int i = 0; i < CR; ++i) {
+            const int g = i * 32 + lane, rr = warp0 + g / CR, c = g % CR;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(adjn_smem_u32(dst + chunk_of(rr, c))), "l"(src + g)
+                         : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    auto own_row = [&](int64_t k, T (&dst)[P]) {
+        const int4 *st = sS + (int)(k % 3) * Tn * CR;
+#pragma unroll
+        for (int c = 0; c < CR; ++c) {
+            const int4 q4 = st[chunk_of(t, c)];
+            const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+            for (int i = 0; i < V; ++i) dst[c * V + i] = e[i];
+        }
+    };
+    auto elem = [&](int64_t k, int rr, int j) {  // element j of row rr of u^k
+        const T *st = reinterpret_cast<const T *>(sS + (int)(k % 3) * Tn * CR);
+        return st[chunk_of(rr, j / V) * V + (j % V)];
+    };
+    const bool frozL = dirichlet && t == 0;        // the row left of this partition (wrap: row N-1) is an end node
+    const bool frozR = dirichlet && t == Tn - 1;   // the row right of it (wrap: row 0)
+    auto frozen_at = [&](int j) { return (j == 0 && fixL) || (j == P - 1 && fixR); };
+
+    T l[P], w[P];
+#pragma unroll
+    for (int c = 0; c < CR; ++c) {
+        const int4 q4 = *reinterpret_cast<const int4 *>(lam + off + c * V);
+        const T *e = reinterpret_cast<const T *>(&q4);
+#pragma unroll
+        for (int i = 0; i < V; ++i) l[c * V + i] = e[i];
+    }
+    fetch(n_steps);
+    fetch(n_steps - 1);
+    for (int64_t k = n_steps - 1; k >= 0; --k) {
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncthreads();                       // u^k and u^{k+1} staged by every warp; the reads of step k + 1 are done
+        if (k > 0) fetch(k - 1);               // into the stage that held u^{k+2}
+        own_row(k + 1, w);                     // the Jacobian is taken at w = u^{k+1}
+        const int tl = (t - 1) & mask, tr_ = (t + 1) & mask;
+        const T wL = elem(k + 1, tl, P - 1), wR = elem(k + 1, tr_, 0);
+        // ---- J(u^{k+1})^T mu = lam
+        T f[P], c[P];
+        Row<T> first, last;
+        auto rowT = [&](int j, T &a, T &bb, T &e) {        // row j of J^T: (sup_{j-1}, diag_j, sub_{j+1})
+            const T wm = j ? w[j - 1] : wL, wp = (j == P - 1) ? wR : w[(j + 1 < P) ? j + 1 : j];
+            const bool fm = j ? frozen_at(j - 1) : frozL, fp = (j == P - 1) ? frozR : frozen_at(j + 1);
+            a = fm ? T(0) : t_fma(th, wm, -tr);
+            e = fp ? T(0) : t_fma(-th, wp, -tr);
+            bb = frozen_at(j) ? T(1) : t_fma(th, wp - wm, b0);
+        };
+        eliminate_general<T, P>(rowT, l, f, c, first, last);
+        T x0, xL;
+        solve_interface<T>(first, last, sR, sF, x0, xL, t, Tn);
+        T (&mu)[P] = l;                                     // in place
+        back_substitute<T, P>(mu, f, c, l, x0, xL);
+        // ---- lam^k = mu - (1 - theta) G'(u^k)^T (M mu), u^k from its stage
+        const T m0 = frozen_at(0) ? T(0) : mu[0], mP = frozen_at(P - 1) ? T(0) : mu[P - 1];
+        sE[t] = m0; sE[Tn + t] = mP;
+        __syncthreads();
+        const T mL = sE[Tn + tl], mR = sE[tr_];
+        T u[P];
+        own_row(k, u);
+        const T uL = elem(k, tl, P - 1), uR = elem(k, tr_, 0);
+        T mprev = mL;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            const T vm = j ? u[j - 1] : uL, vp = (j == P - 1) ? uR : u[(j + 1 < P) ? j + 1 : j];
+            const T mj = frozen_at(j) ? T(0) : mu[j];
+            const T mp = (j == P - 1) ? mR : (frozen_at(j + 1) ? T(0) : mu[(j + 1 < P) ? j + 1 : j]);
+            T g = t_fma(h, vm, -r) * mprev;
+            g = t_fma(t_fma(h, vp - vm, T(2) * r), mj, g);
+            g = t_fma(t_fma(-h, vp, -r), mp, g);
+            l[j] = t_fma(-omt, g, mu[j]);                   // (mu[j] is l[j]: read, then written; mu[j + 1] is still mu)
+            mprev = mj;
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < CR; ++c) {
+        int4 q4;
+        T *e = reinterpret_cast<T *>(&q4);
+#pragma unroll
+        for (int i = 0; i < V; ++i) e[i] = l[c * V + i];
+        *reinterpret_cast<int4 *>(lam + off + c * V) = q4;
+    }
+}
+
 // ---- thread-per-system fallback on the caller's [B][N] layout.  ws: cp, dp, wp ([B][N] each).
 template <typename T>
 __global__ void __launch_bounds__(64)
@@ -212,6 +337,17 @@ int launch_resident_P(const T *u0, const T *states, T *lam, int64_t B, int64_t N
         return last_launch_status();
     }
     if constexpr (P == 4 || P == 8 || P == 16) {
+        if (Tn >= 32) {                                     // states through the shared-memory ring
+            const size_t smem_s = (size_t)(11 + 3 * P) * Tn * sizeof(T) + 16;
+            auto go = [&](auto kernel) {
+                if (smem_s > 48 * 1024 &&
+                    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_s) != cudaSuccess)
+                    return (int)BURGERS_ERR_CUDA;
+                kernel<<<(unsigned)B, Tn, smem_s, s>>>(u0, states, lam, nu, dt, B, (int)N, 1.0 / dx, n_steps, bc, (T)theta);
+                return last_launch_status();
+            };
+            return Tn <= 128 ? go(adjoint_newton_staged_kernel<T, P, true>) : go(adjoint_newton_staged_kernel<T, P, false>);
+        }
         adjoint_newton_resident_kernel<T, P, false><<<(unsigned)B, Tn, smem, s>>>(u0, states, lam, nu, dt, B, (int)N,
                                                                                 1.0 / dx, n_steps, bc, (T)theta);
         return last_launch_status();
